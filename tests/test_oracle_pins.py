@@ -1,0 +1,278 @@
+"""Pins for the CPU oracle (run with -m "not gpu").
+
+The oracle is checked against things OTHER than itself: LAPACK's
+eigendecomposition, first-order perturbation theory, finite differences,
+algebraic invariants of a projector, exact closed forms on tiny matrices
+(tests/golden/closed_forms.txt) and exact rational arithmetic.  Each pin is
+chosen so that a plausible slip (dropped term, wrong sign / branch, transposed
+operand, wrong bound, spin factor 2) fails at least one of them.
+"""
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2107_02737_b200 import inputs
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "closed_forms.txt")
+
+
+def _golden():
+    out = {}
+    with open(GOLDEN) as f:
+        for line in f:
+            line = line.split("#", 1)[0].strip()
+            if not line or "=" not in line:
+                continue
+            k, v = (s.strip() for s in line.split("=", 1))
+            out[k] = v
+    return out
+
+
+def _vec(s):
+    return np.array([float(x) for x in s.split()])
+
+
+G = _golden()
+
+
+@pytest.fixture(scope="module")
+def cfg1():
+    return inputs.make_problem(inputs.CONFIGS[1])
+
+
+@pytest.fixture(scope="module")
+def cfg2():
+    p = inputs.make_problem(inputs.CONFIGS[2])
+    p["sp2"] = oracle.sp2_density(p["H"], p["n_occ"], H1=p["H1"])
+    return p
+
+
+# ----------------------------------------------------------------- bounds (a1)
+def test_gershgorin_textbook_and_diagonal():
+    H = _vec(G["C.H"]).reshape(3, 3)
+    lo, hi = oracle.gershgorin_bounds(H)
+    assert (lo, hi) == (float(G["C.eps_min"]), float(G["C.eps_max"]))
+    d = np.array([-2.0, -1.0, 1.0, 2.0])
+    assert oracle.gershgorin_bounds(np.diag(d)) == (-2.0, 2.0)   # exact for diagonal H
+
+
+def test_gershgorin_encloses_spectrum_and_uses_offdiag_abs():
+    rng = np.random.default_rng(1)
+    A = rng.standard_normal((40, 40))
+    H = A + A.T
+    lo, hi = oracle.gershgorin_bounds(H)
+    w = np.linalg.eigvalsh(H)
+    assert lo <= w[0] and w[-1] <= hi
+    # brute force, element loops (catches a missing abs() or an included diagonal)
+    lo2 = min(H[i, i] - sum(abs(H[i, j]) for j in range(40) if j != i) for i in range(40))
+    hi2 = max(H[i, i] + sum(abs(H[i, j]) for j in range(40) if j != i) for i in range(40))
+    assert lo == pytest.approx(lo2, rel=1e-14) and hi == pytest.approx(hi2, rel=1e-14)
+
+
+def test_rescale_reverses_spectrum_into_unit_interval(cfg1):
+    H = cfg1["H"]
+    lo, hi = oracle.gershgorin_bounds(H)
+    X0 = oracle.rescale_to_unit_interval(H, lo, hi)
+    w = np.linalg.eigvalsh(H)
+    x = np.linalg.eigvalsh(X0)
+    assert x[0] >= 0.0 and x[-1] <= 1.0
+    # lowest H eigenvalue -> closest to 1, highest -> closest to 0
+    np.testing.assert_allclose(x[::-1], (hi - w) / (hi - lo), atol=1e-13)
+    with pytest.raises(ValueError):
+        oracle.rescale_to_unit_interval(np.eye(3), 1.0, 1.0)
+
+
+# ------------------------------------------------------- closed forms (golden)
+def test_case_A_diagonal_hand_example():
+    H = np.diag(_vec(G["A.diag_H"]))
+    r = oracle.sp2_density(H, int(G["A.n_occ"]))
+    assert (r["eps_min"], r["eps_max"]) == (float(G["A.eps_min"]), float(G["A.eps_max"]))
+    np.testing.assert_allclose(np.diag(r["D"]), _vec(G["A.D_diag"]), atol=1e-13)
+    assert np.abs(r["D"] - np.diag(np.diag(r["D"]))).max() == 0.0
+    assert r["tr_dh"] == pytest.approx(float(G["A.tr_DH"]), abs=1e-12)
+    assert r["signs"].startswith(G["A.signs_prefix"])            # tie at n=0 -> '-'
+    np.testing.assert_array_equal(r["tr_x"][:3], _vec(G["A.tr_X"]))   # exact dyadics
+    t2 = [r["tr_x"][k] - r["e"][k] for k in range(2)]
+    np.testing.assert_array_equal(t2, _vec(G["A.tr_X2"]))
+
+
+def test_case_A_against_exact_rational_arithmetic():
+    """Every trace of the float64 loop equals the exact rational value while
+    the dyadic numbers still fit in 53 bits (first 4 layers)."""
+    H = np.diag(_vec(G["A.diag_H"]))
+    r = oracle.sp2_density(H, 2)
+    x = [Fraction(2 - int(v), 4) for v in _vec(G["A.diag_H"])]
+    for n in range(4):
+        t = sum(x)
+        t2 = sum(v * v for v in x)
+        assert Fraction(r["tr_x"][n]) == t
+        plus = abs(t2 - 2) < abs(2 * t - t2 - 2)
+        assert r["signs"][n] == ("+" if plus else "-")
+        x = [v * v if plus else 2 * v - v * v for v in x]
+
+
+def test_case_B_2x2_converged_on_entry_and_response():
+    H = _vec(G["B.H"]).reshape(2, 2)
+    H1 = _vec(G["B.H1"]).reshape(2, 2)
+    r = oracle.sp2_density(H, 1, H1=H1)
+    assert (r["eps_min"], r["eps_max"]) == (-1.0, 1.0)
+    np.testing.assert_allclose(r["D"], _vec(G["B.D"]).reshape(2, 2), atol=1e-15)
+    np.testing.assert_allclose(r["D1"], _vec(G["B.D1"]).reshape(2, 2), atol=1e-15)
+    assert r["tr_dh"] == pytest.approx(float(G["B.tr_DH"]))
+    assert r["layers"] == 0 and r["stop"] == "idempotent"
+    # the independent routes agree with the hand value too
+    D, _ = oracle.density_eigh(H, 1)
+    np.testing.assert_allclose(D, _vec(G["B.D"]).reshape(2, 2), atol=1e-15)
+    Q = np.array([[1.0, 1.0], [-1.0, 1.0]]) / np.sqrt(2.0)
+    D1 = oracle.response_closed_form(Q, np.array([-1.0, 1.0]), 1, H1)
+    np.testing.assert_allclose(D1, _vec(G["B.D1"]).reshape(2, 2), atol=1e-15)
+
+
+# ---------------------------------------------- definition vs algorithm (O-1/O-2)
+def test_config1_sp2_equals_eigh_projector(cfg1):
+    H, n_occ = cfg1["H"], cfg1["n_occ"]
+    r = oracle.sp2_density(H, n_occ)
+    D_eig, w = oracle.density_eigh(H, n_occ)
+    assert np.abs(r["D"] - D_eig).max() < 1e-12
+    D_gen = oracle.density_from_eigenpairs(cfg1["Q"], cfg1["lam"], n_occ)
+    assert np.abs(D_eig - D_gen).max() < 1e-12
+    assert r["stop"] == "floor" and 13 <= r["layers"] <= 40
+    # band energy: sum of the lowest eigenvalues (closed form of the generator)
+    assert r["tr_dh"] == pytest.approx(inputs.band_energy_closed_form(cfg1["lam"], n_occ), rel=1e-12)
+    assert r["tr_dh"] == pytest.approx(w[:n_occ].sum(), rel=1e-12)
+
+
+def test_projector_invariants(cfg1):
+    H, n_occ = cfg1["H"], cfg1["n_occ"]
+    D = oracle.sp2_density(H, n_occ)["D"]
+    assert abs(np.trace(D) - n_occ) < 1e-10                       # no spin factor (Eq. 17)
+    assert np.linalg.norm(D @ D - D) < 1e-11                      # idempotent
+    assert np.linalg.norm(H @ D - D @ H) < 1e-11                  # same eigenvectors as H
+    assert np.abs(D - D.T).max() < 1e-13
+    assert np.linalg.matrix_rank(D, tol=1e-8) == n_occ
+
+
+def test_particle_hole_symmetry(cfg1):
+    H, n_occ, N = cfg1["H"], cfg1["n_occ"], cfg1["n"]
+    D = oracle.sp2_density(H, n_occ)["D"]
+    Dm = oracle.sp2_density(-H, N - n_occ)["D"]
+    assert np.abs(Dm - (np.eye(N) - D)).max() < 1e-12
+
+
+def test_uneven_occupation_and_sampled_entries():
+    cfg = inputs.scaled_config(inputs.CONFIGS[3], 96)             # n_occ/N = 2/3
+    cfg = inputs.Sp2Config(cfg.name, 3, 96, 64, cfg.occ, cfg.unocc, "f64", False)
+    p = inputs.make_problem(cfg)
+    r = oracle.sp2_density(p["H"], 64)
+    D_eig, _ = oracle.density_eigh(p["H"], 64)
+    assert np.abs(r["D"] - D_eig).max() < 1e-12
+    rows = np.array([0, 5, 95, 17])
+    cols = np.array([0, 77, 95, 3])
+    np.testing.assert_allclose(oracle.density_from_eigenpairs(p["Q"], p["lam"], 64, rows, cols),
+                               D_eig[rows, cols], atol=1e-13)
+
+
+def test_trivial_occupations(cfg1):
+    H, N = cfg1["H"], cfg1["n"]
+    assert np.array_equal(oracle.sp2_density(H, 0)["D"], np.zeros((N, N)))
+    r = oracle.sp2_density(H, N)
+    assert np.array_equal(r["D"], np.eye(N)) and r["tr_dh"] == pytest.approx(np.trace(H))
+    with pytest.raises(ValueError):
+        oracle.sp2_density(H, N + 1)
+    with pytest.raises(ValueError):
+        oracle.sp2_density(H + np.triu(np.ones((N, N)), 1), 3)    # not symmetric
+
+
+def test_user_bounds_give_same_projector_fewer_layers(cfg1):
+    H, n_occ = cfg1["H"], cfg1["n_occ"]
+    w = np.linalg.eigvalsh(H)
+    r_g = oracle.sp2_density(H, n_occ)
+    r_t = oracle.sp2_density(H, n_occ, bounds=(w[0], w[-1]))
+    assert np.abs(r_g["D"] - r_t["D"]).max() < 1e-12
+    assert r_t["layers"] < r_g["layers"]
+
+
+def test_tol_stop_rule(cfg1):
+    H, n_occ = cfg1["H"], cfg1["n_occ"]
+    r = oracle.sp2_density(H, n_occ, tol=1e-3)
+    assert r["stop"] == "tol" and 0.0 <= r["e"][-1] <= 1e-3
+    full = oracle.sp2_density(H, n_occ)
+    assert r["layers"] < full["layers"]
+    assert np.abs(r["D"] - full["D"]).max() < 1e-2
+    r3 = oracle.sp2_density(H, n_occ, max_layers=5)
+    assert r3["stop"] == "max_layers" and r3["layers"] == 5
+
+
+# ----------------------------------------------------- spectrum-only simulator
+def test_spectrum_simulator_matches_matrix_loop(cfg1):
+    H, n_occ = cfg1["H"], cfg1["n_occ"]
+    r = oracle.sp2_density(H, n_occ)
+    w = np.linalg.eigvalsh(H)
+    s = oracle.sp2_spectrum_simulator(w, n_occ, r["eps_min"], r["eps_max"])
+    k = min(len(s["signs"]), len(r["signs"])) - 3                 # last layers are noise-driven
+    assert s["signs"][:k] == r["signs"][:k]
+    np.testing.assert_allclose(s["tr_x"][:k], r["tr_x"][:k], rtol=0, atol=1e-9)
+    assert abs(s["layers"] - r["layers"]) <= 3
+    occ = np.sort(s["x"])[::-1]
+    np.testing.assert_allclose(occ[:n_occ], 1.0, atol=1e-12)
+    np.testing.assert_allclose(occ[n_occ:], 0.0, atol=1e-12)
+
+
+def test_diagonal_matrix_is_the_scalar_map():
+    lam = np.array([-1.3, -0.2, 0.05, 0.4, 0.9, 1.7])
+    r = oracle.sp2_density(np.diag(lam), 3)
+    s = oracle.sp2_spectrum_simulator(lam, 3, r["eps_min"], r["eps_max"])
+    assert s["signs"] == r["signs"] and s["layers"] == r["layers"]
+    np.testing.assert_allclose(np.diag(r["D"]), s["x"], atol=0)
+    np.testing.assert_allclose(np.diag(r["D"]), [1, 1, 1, 0, 0, 0], atol=1e-12)
+
+
+def test_layer_count_estimates_for_big_configs():
+    """Configs 4/5 at full size via the O(N L) simulator with Gershgorin-like
+    bounds ~ +-sqrt(2/pi) sqrt(N <lam^2>): BASELINE.json expects ~35-45 layers."""
+    for k in (4, 5):
+        cfg = inputs.CONFIGS[k]
+        rng = np.random.default_rng(0)
+        lam = np.concatenate([rng.uniform(*cfg.occ, cfg.n_occ), rng.uniform(*cfg.unocc, cfg.n - cfg.n_occ)])
+        half = np.sqrt(2 / np.pi) * np.sqrt(cfg.n * np.mean(lam ** 2))
+        s = oracle.sp2_spectrum_simulator(lam, cfg.n_occ, -half, half)
+        assert 30 <= s["layers"] <= 50 and s["stop"] == "floor"
+
+
+# ------------------------------------------------------------- response (O-3)
+def test_response_recursion_vs_perturbation_theory_vs_finite_difference(cfg2):
+    H, H1, n_occ = cfg2["H"], cfg2["H1"], cfg2["n_occ"]
+    r = cfg2["sp2"]
+    D_eig, w = oracle.density_eigh(H, n_occ)
+    assert np.abs(r["D"] - D_eig).max() < 1e-12
+    D1_pt = oracle.response_closed_form(cfg2["Q"], cfg2["lam"], n_occ, H1)
+    scale = np.abs(D1_pt).max()
+    assert np.abs(r["D1"] - D1_pt).max() < 1e-10 * scale
+    D1_fd = oracle.response_finite_difference(H, H1, n_occ, eps=1e-5)
+    assert np.abs(D1_fd - D1_pt).max() < 1e-6 * scale
+    assert r["tr_dh"] == pytest.approx(w[:n_occ].sum(), rel=1e-12)
+
+
+def test_response_invariants(cfg2):
+    D, D1 = cfg2["sp2"]["D"], cfg2["sp2"]["D1"]
+    s = np.abs(D1).max()
+    assert abs(np.trace(D1)) < 1e-10 * s * len(D)                # particle number conserved
+    assert np.abs(D1 - D1.T).max() < 1e-13 * s
+    assert np.abs(D @ D1 + D1 @ D - D1).max() < 1e-10 * s        # derivative of D^2 = D
+    assert np.abs(D @ D1 @ D).max() < 1e-10 * s                  # no occ-occ block
+
+
+def test_response_is_linear_and_sign_sensitive(cfg2):
+    """A transposed/dropped term in X Z + Z X or a wrong branch sign breaks this
+    on a small non-commuting case (H1 does not commute with H)."""
+    cfg = inputs.Sp2Config("t", 2, 48, 20, (-1.5, -0.25), (0.25, 1.5), "f64", True)
+    p = inputs.make_problem(cfg)
+    r = oracle.sp2_density(p["H"], 20, H1=p["H1"])
+    D1_pt = oracle.response_closed_form(p["Q"], p["lam"], 20, p["H1"])
+    assert np.abs(r["D1"] - D1_pt).max() < 1e-11 * np.abs(D1_pt).max()
+    r2 = oracle.sp2_density(p["H"], 20, H1=-3.0 * p["H1"])
+    np.testing.assert_allclose(r2["D1"], -3.0 * r["D1"], atol=1e-12)
+    assert np.abs(p["H"] @ p["H1"] - p["H1"] @ p["H"]).max() > 1e-3
