@@ -1,0 +1,159 @@
+/* sp2.h -- C ABI of the B200-native (sm_100a) SP2 / DNN-SP2 density-matrix library.
+ *
+ * What the calls compute (arXiv 2107.02737; PAPER.md = /root/reference/PAPER.md at build time):
+ *
+ *   D = theta(mu*I - H)                                   PAPER.md:127-135, Eq. 17-18
+ *     = the orthogonal projector onto the N_occ lowest eigenvectors of the symmetric,
+ *       orthogonalised Hamiltonian H, obtained by the DNN-SP2 recursion
+ *       X_0 = (eps_max*I - H)/(eps_max - eps_min),        PAPER.md:145   (input layer W0, B0)
+ *       X_{n+1} = X_n^2   or   2 X_n - X_n^2,              PAPER.md:149   (Fig. 1: S_n = S_{n-1}^2 or 2S_{n-1} - S_{n-1}^2)
+ *     the branch chosen by trace so that tr X moves toward N_occ, repeated until
+ *     the idempotency estimate tr X - tr X^2 stops improving.
+ *   D1 = first-order response of D to H -> H + eps*H1, carried through the same layers with the
+ *     same branches (BASELINE.json north_star; not printed in the paper, which only names its
+ *     consumer):  Z_0 = -H1/(eps_max - eps_min),
+ *       Z_{n+1} = X_n Z_n + Z_n X_n   or   2 Z_n - (X_n Z_n + Z_n X_n).
+ *   tr(DH) = sum_ij D_ij H_ij with the caller's unscaled H (band energy).
+ *
+ * Conventions
+ *   - Matrices are dense, row-major, symmetric, `ld` = row pitch in ELEMENTS (ld >= N).
+ *     Input symmetry: the library uses (H_ij + H_ji)/2, which is H itself when H is exactly symmetric.
+ *   - sp2_density / sp2_response / sp2_sequence_*: every matrix pointer is a DEVICE pointer owned
+ *     by the caller; H, H1 are never written; D, D1 must not alias H, H1 or the workspace.
+ *     sp2_density_host / sp2_response_host: every matrix pointer is a HOST pointer (pinned memory
+ *     is faster, pageable works); the copies to and from the device are part of the call.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - The library allocates NO device memory: the caller passes a device workspace of at least
+ *     sp2_workspace_bytes() bytes (e.g. a torch uint8 tensor), 1024-byte aligned, which the handle
+ *     uses until sp2_destroy.  One handle = one call in flight (not re-entrant).
+ *   - Every call returns an sp2_status_t; nothing throws, nothing prints.  The blocking calls
+ *     enqueue all kernels on `stream`, synchronise that stream once, and fill *out (a HOST struct).
+ *   - There is no CPU fallback: on a device that is not compute capability 10.x the calls return
+ *     SP2_ERR_ARCH.
+ */
+#ifndef SP2_B200_H
+#define SP2_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define SP2_API __attribute__((visibility("default")))
+#else
+#define SP2_API
+#endif
+
+typedef struct sp2_handle_s* sp2_handle_t;
+
+typedef enum {
+  SP2_OK = 0,
+  SP2_ERR_INVALID_ARG = 1,   /* null pointer, N <= 0, N > n_max, N_occ outside [0,N], ld < N, bad dtype */
+  SP2_ERR_WORKSPACE = 2,     /* workspace null, misaligned or too small */
+  SP2_ERR_CUDA = 3,          /* a CUDA runtime / driver call failed (sp2_last_cuda_error) */
+  SP2_ERR_ARCH = 4,          /* device is not sm_100 */
+  SP2_ERR_NONFINITE = 5,     /* H (or H1) holds NaN/Inf, or the iterate became non-finite */
+  SP2_ERR_DEGENERATE = 6,    /* eps_max == eps_min (H = c*I): no spectral width to rescale */
+  SP2_WARN_NOT_CONVERGED = 7 /* max_layers reached; D (and D1) are still written */
+} sp2_status_t;
+
+typedef enum { SP2_F32 = 0, SP2_F64 = 1 } sp2_dtype_t;
+
+/* flags of sp2_workspace_bytes / sp2_create */
+#define SP2_WITH_RESPONSE 1     /* room for the first-order iterate Z (sp2_response) */
+#define SP2_WITH_HOST_STAGING 2 /* room for device copies of H, H1, D, D1 (the *_host calls), f64-sized */
+
+/* layer engines (sp2_options_t.engine) */
+#define SP2_ENGINE_TCGEN05 0 /* product path: TMA + tcgen05.mma + TMEM */
+#define SP2_ENGINE_SIMT_DEBUG 1 /* slow FP32-FMA scaffold on the same planes/epilogue; tests only, N <= 4096 */
+
+typedef struct {
+  int max_layers;   /* default 100, capped at 126 */
+  int user_bounds;  /* 0: Gershgorin discs (default); 1: use eps_min/eps_max below (must enclose the spectrum) */
+  double eps_min, eps_max;
+  int engine;       /* SP2_ENGINE_* (default SP2_ENGINE_TCGEN05) */
+  int forced_layers;      /* debug: > 0 runs exactly this many layers, no stop test */
+  unsigned long long forced_signs; /* debug: with forced_layers, bit n = 1 -> layer n is X^2, else 2X - X^2 */
+  int cta_group;    /* 0 = auto; 1 = 128x128 tiles, one CTA; 2 = 256x256 tiles on a CTA pair (cta_group::2) */
+} sp2_options_t;
+
+typedef struct {
+  int status;                        /* sp2_status_t of the solve */
+  int layers;                        /* number of layers applied (paper: 14-16 for water) */
+  unsigned long long sign_mask[2];   /* bit n = 1 if layer n was X^2 ('+'), 0 if 2X - X^2 ('-') */
+  int stop_reason;                   /* 1 tol, 2 floor (parameter-free), 3 idempotent on entry, 4 max_layers, 5 trivial N_occ, 6 forced */
+  int reserved;
+  double tr_d;                       /* tr D (should be N_occ) */
+  double tr_dh;                      /* sum_ij D_ij H_ij */
+  double tr_d1;                      /* tr D1 (should be 0); 0 when no response */
+  double idem_est;                   /* last idempotency estimate e_L = tr X_L - tr X_L^2 */
+  double eps_min, eps_max;           /* spectral bounds used by the input layer */
+  float gpu_ms;                      /* device time of the call (CUDA events on `stream`), blocking calls only */
+  int kernel_launches;               /* kernels of this library launched by the call */
+} sp2_result_t;
+
+/* Bytes of device workspace needed for problems up to n_max (flags: SP2_WITH_*). 0 if n_max <= 0. */
+SP2_API size_t sp2_workspace_bytes(int n_max, int flags);
+
+/* Create a handle on the CURRENT device over caller-owned device memory. */
+SP2_API sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_workspace, size_t bytes);
+SP2_API sp2_status_t sp2_destroy(sp2_handle_t handle);
+
+/* NULL restores the defaults. */
+SP2_API sp2_status_t sp2_set_options(sp2_handle_t handle, const sp2_options_t* opt);
+SP2_API sp2_status_t sp2_get_options(sp2_handle_t handle, sp2_options_t* opt);
+
+/* H (N x N, in_dtype, pitch ldh) -> D (N x N, out_dtype, pitch ldd).  tol > 0: stop as soon as
+ * 0 <= tr X - tr X^2 <= tol with |tr X - N_occ| < 0.5; tol <= 0: parameter-free stop only.
+ * N_occ = 0 -> D = 0; N_occ = N -> D = I.  Blocking (one stream synchronise). */
+SP2_API sp2_status_t sp2_density(sp2_handle_t handle, const void* dH, sp2_dtype_t in_dtype, long ldh,
+                         int N, int N_occ, double tol,
+                         void* dD, sp2_dtype_t out_dtype, long ldd,
+                         sp2_result_t* out, void* stream);
+
+/* As sp2_density, plus H1 -> D1 (same dtypes and pitches as H / D).  Needs SP2_WITH_RESPONSE. */
+SP2_API sp2_status_t sp2_response(sp2_handle_t handle, const void* dH, const void* dH1, sp2_dtype_t in_dtype, long ld,
+                          int N, int N_occ, double tol,
+                          void* dD, void* dD1, sp2_dtype_t out_dtype, long ldo,
+                          sp2_result_t* out, void* stream);
+
+/* Host-buffer twins: hH/hH1/hD/hD1 are HOST pointers; H2D and D2H copies run on `stream` inside the
+ * call.  Need SP2_WITH_HOST_STAGING (and SP2_WITH_RESPONSE for the response twin). */
+SP2_API sp2_status_t sp2_density_host(sp2_handle_t handle, const void* hH, sp2_dtype_t in_dtype, long ldh,
+                              int N, int N_occ, double tol,
+                              void* hD, sp2_dtype_t out_dtype, long ldd,
+                              sp2_result_t* out, void* stream);
+SP2_API sp2_status_t sp2_response_host(sp2_handle_t handle, const void* hH, const void* hH1, sp2_dtype_t in_dtype, long ld,
+                               int N, int N_occ, double tol,
+                               void* hD, void* hD1, sp2_dtype_t out_dtype, long ldo,
+                               sp2_result_t* out, void* stream);
+
+/* Consecutive MD-step Hamiltonians (one density-matrix construction per time step).
+ * begin fixes N, N_occ, tol and the stream; each step enqueues one density solve and returns
+ * without synchronising (per-step results land in a device ring of n_steps_hint entries, at most
+ * 4096); end synchronises once and copies the results of the steps issued since begin. */
+SP2_API sp2_status_t sp2_sequence_begin(sp2_handle_t handle, int N, int N_occ, double tol, int n_steps_hint, void* stream);
+SP2_API sp2_status_t sp2_sequence_step(sp2_handle_t handle, const void* dH_t, sp2_dtype_t in_dtype, long ldh,
+                               void* dD_t, sp2_dtype_t out_dtype, long ldd);
+SP2_API sp2_status_t sp2_sequence_end(sp2_handle_t handle, sp2_result_t* results, int* n_steps);
+
+/* Diagnostics. */
+SP2_API const char* sp2_status_string(sp2_status_t status);
+SP2_API int sp2_last_cuda_error(sp2_handle_t handle);            /* cudaError_t of the last failing CUDA call, 0 if none */
+SP2_API unsigned long long sp2_launch_count(sp2_handle_t handle); /* kernels launched through this handle so far */
+
+/* Test hooks (used by tests/ only; stable but not part of the paper's problem statement).
+ * Per-layer trace history of the last solve: tr X_n and e_n = tr X_n - tr X_n^2, n = 0..layers. Returns count. */
+SP2_API int sp2_debug_history(sp2_handle_t handle, double* tr_x, double* e, int capacity);
+/* Byte offset inside the workspace, pitch (elements) and power-of-two exponent of an internal
+ * 16-bit plane after the last solve: which = 0 Y.hi, 1 Y.lo, 2 Z.hi, 3 Z.lo of the FINAL iterate
+ * (X_L = c*I + (hi+lo)*2^-exp); which + 4 = the same plane of the previous iterate X_{L-1} (other
+ * ping-pong buffer; exponent and shift are still those of X_L).  c is returned in *shift. */
+SP2_API sp2_status_t sp2_debug_plane(sp2_handle_t handle, int which, size_t* offset, long* pitch, int* exponent, double* shift);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SP2_B200_H */

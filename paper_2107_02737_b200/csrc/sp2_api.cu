@@ -1,0 +1,484 @@
+// sp2_api.cu -- host side of the C ABI declared in include/sp2.h: workspace carving, TMA descriptor
+// encoding, the launch sequence of one solve and result retrieval.
+//
+// One solve = k_init, k_bounds (H [, H1]), k_setup, k_rescale ([H1,] H), k_ctrl0,
+//             max_layers x layer kernel (early-exit once the device controller sets `done`),
+//             k_finalise, k_finalise_reduce   -- all on the caller's stream, no host round trip
+// in between (the paper's design crosses to the CPU every layer).
+#include <cuda.h>
+#include <cudaTypedefs.h>
+#include <cuda_runtime.h>
+#include <new>
+#include <string.h>
+#include <vector>
+
+#include "sp2.h"
+#include "sp2_internal.cuh"
+#include "sp2_layer.h"
+
+// launchers defined in sp2_prologue.cu
+void sp2_launch_init(Sp2Ctrl* c, int N, int n_occ, int npad, int with_response, int max_layers, int user_bounds,
+                     double eps_min, double eps_max, double tol, int forced_layers, unsigned long long forced_signs,
+                     cudaStream_t s);
+int sp2_bounds_blocks(int N);
+void sp2_launch_bounds(const void* H, sp2_dtype_t dt, long ld, int N, int mode, Sp2BoundSlot* slots, cudaStream_t s);
+void sp2_launch_setup(Sp2Ctrl* c, const Sp2BoundSlot* sh, int n_h, const Sp2BoundSlot* s1, int n_h1, cudaStream_t s);
+int sp2_rescale_blocks(int npad);
+void sp2_launch_rescale(const void* H, sp2_dtype_t dt, long ld, const Sp2Ctrl* c, int which, __half* Ph, __half* Pm,
+                        int npad, Sp2Slot* slots, cudaStream_t s);
+void sp2_launch_ctrl0(Sp2Ctrl* c, const Sp2Slot* ys, const Sp2Slot* zs, int count, cudaStream_t s);
+int sp2_finalise_blocks(int N);
+void sp2_launch_finalise(Sp2Ctrl* c, __half* const planes[8], int npad, const void* H, sp2_dtype_t in_dt, long ldh,
+                         void* D, void* D1, sp2_dtype_t out_dt, long ldo, int N, double* slots,
+                         sp2_result_t* ring_entry, cudaStream_t s);
+void sp2_launch_trivial(Sp2Ctrl* c, void* D, void* D1, sp2_dtype_t out_dt, long ldo, int N, sp2_result_t* ring_entry,
+                        cudaStream_t s);
+
+namespace {
+
+constexpr int kRingCap = 4096;
+constexpr int kPadTo = 256;          // npad is a multiple of the largest tile edge
+constexpr int kSimtMaxN = 4096;
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+inline int pad_n(int n) { return (int)align_up((size_t)n, kPadTo); }
+
+struct Layout {
+  size_t plane_bytes;     // one FP16 plane at n_max
+  size_t off_planes;      // 4 or 8 planes: [buf][Yh, Ym] then [buf][Zh, Zm]
+  size_t off_slots, slots_count;
+  size_t off_slots2;      // second slot array (Z partials of the prologue)
+  size_t off_bslots, bslots_count;
+  size_t off_fslots;
+  size_t off_tiles, tiles_count;
+  size_t off_ctrl, off_ring;
+  size_t off_staging, staging_each;
+  size_t total;
+};
+
+Layout make_layout(int n_max, int flags) {
+  Layout L;
+  memset(&L, 0, sizeof(L));
+  const size_t npad = (size_t)pad_n(n_max);
+  const bool resp = flags & SP2_WITH_RESPONSE;
+  L.plane_bytes = align_up(npad * npad * 2, 1024);
+  size_t off = 0;
+  L.off_planes = off; off += L.plane_bytes * (resp ? 8 : 4);
+  size_t s_tc = (size_t)sp2_layer_slots((int)npad, 1, resp, SP2_ENGINE_TCGEN05);
+  size_t s_tc2 = (size_t)sp2_layer_slots((int)npad, 2, resp, SP2_ENGINE_TCGEN05);
+  size_t s_simt = npad <= (size_t)kSimtMaxN ? (size_t)sp2_layer_slots((int)npad, 1, resp, SP2_ENGINE_SIMT_DEBUG) : 0;
+  size_t s_resc = (size_t)sp2_rescale_blocks((int)npad);
+  L.slots_count = s_tc;
+  if (s_tc2 > L.slots_count) L.slots_count = s_tc2;
+  if (s_simt > L.slots_count) L.slots_count = s_simt;
+  if (s_resc > L.slots_count) L.slots_count = s_resc;
+  L.off_slots = off; off += align_up(L.slots_count * sizeof(Sp2Slot), 1024);
+  L.off_slots2 = off; off += align_up(s_resc * sizeof(Sp2Slot), 1024);
+  L.bslots_count = (size_t)sp2_bounds_blocks(n_max);
+  L.off_bslots = off; off += align_up(2 * L.bslots_count * sizeof(Sp2BoundSlot), 1024);
+  L.off_fslots = off; off += align_up(3 * (size_t)sp2_finalise_blocks(n_max) * sizeof(double), 1024);
+  const size_t nt1 = npad / 128;
+  L.tiles_count = nt1 * (nt1 + 1) / 2;
+  L.off_tiles = off; off += align_up(L.tiles_count * sizeof(int2), 1024);
+  L.off_ctrl = off; off += align_up(sizeof(Sp2Ctrl), 1024);
+  L.off_ring = off; off += align_up((size_t)kRingCap * sizeof(sp2_result_t), 1024);
+  if (flags & SP2_WITH_HOST_STAGING) {
+    L.staging_each = align_up((size_t)n_max * (size_t)n_max * 8, 1024);
+    L.off_staging = off; off += L.staging_each * (resp ? 4 : 2);
+  }
+  L.total = off;
+  return L;
+}
+
+void default_options(sp2_options_t* o) {
+  memset(o, 0, sizeof(*o));
+  o->max_layers = 100;
+  o->engine = SP2_ENGINE_TCGEN05;
+  o->cta_group = 0;
+}
+
+}  // namespace
+
+struct sp2_handle_s {
+  int n_max, flags, device, num_sms;
+  uint8_t* ws;
+  size_t ws_bytes;
+  Layout L;
+  sp2_options_t opt;
+  PFN_cuTensorMapEncodeTiled_v12000 encode;
+  // per-(N, cta_group) cache
+  int cur_npad, cur_cg, cur_resp;
+  Sp2LayerArgs args[2];          // parity 0: buffer 0 -> 1, parity 1: buffer 1 -> 0
+  std::vector<int2> tiles_host;
+  cudaEvent_t ev0, ev1;
+  sp2_result_t* h_result;        // pinned
+  int last_cuda_error;
+  unsigned long long launches;
+  // sequence state
+  int seq_active, seq_N, seq_nocc, seq_steps;
+  double seq_tol;
+  cudaStream_t seq_stream;
+
+  __half* plane(int which /*0 Yh,1 Ym,2 Zh,3 Zm*/, int buf) const {
+    const int idx = (which < 2) ? (buf * 2 + which) : (4 + buf * 2 + (which - 2));
+    return reinterpret_cast<__half*>(ws + L.off_planes + (size_t)idx * L.plane_bytes);
+  }
+  Sp2Slot* slots() const { return reinterpret_cast<Sp2Slot*>(ws + L.off_slots); }
+  Sp2Slot* slots2() const { return reinterpret_cast<Sp2Slot*>(ws + L.off_slots2); }
+  Sp2BoundSlot* bslots(int i) const { return reinterpret_cast<Sp2BoundSlot*>(ws + L.off_bslots) + (size_t)i * L.bslots_count; }
+  double* fslots() const { return reinterpret_cast<double*>(ws + L.off_fslots); }
+  int2* tiles() const { return reinterpret_cast<int2*>(ws + L.off_tiles); }
+  Sp2Ctrl* ctrl() const { return reinterpret_cast<Sp2Ctrl*>(ws + L.off_ctrl); }
+  sp2_result_t* ring() const { return reinterpret_cast<sp2_result_t*>(ws + L.off_ring); }
+  void* staging(int i) const { return ws + L.off_staging + (size_t)i * L.staging_each; }
+};
+
+namespace {
+
+#define SP2_CUDA(h, expr)                                   \
+  do {                                                      \
+    cudaError_t e_ = (expr);                                \
+    if (e_ != cudaSuccess) { (h)->last_cuda_error = (int)e_; return SP2_ERR_CUDA; } \
+  } while (0)
+
+// Upper-triangular tile list in an L2-friendly order: G x G groups of tiles, so that the tiles that
+// run concurrently (consecutive list entries) share row panels of the operand planes.
+void build_tiles(int nt, std::vector<int2>& out) {
+  out.clear();
+  const int G = 8;
+  const int ng = (nt + G - 1) / G;
+  for (int gi = 0; gi < ng; ++gi)
+    for (int gj = gi; gj < ng; ++gj)
+      for (int ti = gi * G; ti < (gi + 1) * G && ti < nt; ++ti)
+        for (int tj = gj * G; tj < (gj + 1) * G && tj < nt; ++tj)
+          if (tj >= ti) out.push_back(make_int2(ti, tj));
+}
+
+sp2_status_t encode_plane_map(sp2_handle_t h, CUtensorMap* map, const __half* base, int npad) {
+  cuuint64_t gdim[2] = {(cuuint64_t)npad, (cuuint64_t)npad};
+  cuuint64_t gstride[1] = {(cuuint64_t)npad * 2};
+  cuuint32_t box[2] = {64, 128};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = h->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<__half*>(base), gdim, gstride, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { h->last_cuda_error = 100000 + (int)r; return SP2_ERR_CUDA; }
+  return SP2_OK;
+}
+
+int pick_cta_group(sp2_handle_t h, int npad) {
+  if (h->opt.cta_group == 1 || h->opt.cta_group == 2) return h->opt.cta_group;
+  const int nt2 = npad / 256;
+  return (nt2 * (nt2 + 1) / 2 >= h->num_sms / 2) ? 2 : 1;
+}
+
+// (re)build the per-problem launch state: tile list, TMA descriptors, ping-pong argument blocks
+sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
+  const int npad = pad_n(N);
+  const int cg = pick_cta_group(h, npad);
+  if (h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp) return SP2_OK;
+  const int nt = npad / (128 * cg);
+  build_tiles(nt, h->tiles_host);
+  SP2_CUDA(h, cudaMemcpyAsync(h->tiles(), h->tiles_host.data(), h->tiles_host.size() * sizeof(int2),
+                              cudaMemcpyHostToDevice, s));
+  SP2_CUDA(h, cudaStreamSynchronize(s));     // tiles_host may be rebuilt by the next prepare
+  for (int par = 0; par < 2; ++par) {
+    Sp2LayerArgs& a = h->args[par];
+    memset(&a, 0, sizeof(a));
+    for (int w = 0; w < 4; ++w) {
+      const bool have = (w < 2) || (h->flags & SP2_WITH_RESPONSE);
+      const __half* in = have ? h->plane(w, par) : h->plane(w & 1, par);
+      __half* out = have ? h->plane(w, par ^ 1) : h->plane(w & 1, par ^ 1);
+      a.in[w] = in; a.out[w] = out;
+      sp2_status_t st = encode_plane_map(h, &a.tm[w], in, npad);
+      if (st != SP2_OK) return st;
+    }
+    a.ctrl = h->ctrl(); a.slots = h->slots(); a.tiles = h->tiles();
+    a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = resp; a.pad = 0;
+  }
+  h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp;
+  return SP2_OK;
+}
+
+sp2_status_t check_args(sp2_handle_t h, const void* H, const void* H1, int want_resp, sp2_dtype_t in_dt, long ldh, int N,
+                        int N_occ, void* D, void* D1, sp2_dtype_t out_dt, long ldd) {
+  if (!h) return SP2_ERR_INVALID_ARG;
+  if (!H || !D) return SP2_ERR_INVALID_ARG;
+  if (want_resp && (!H1 || !D1)) return SP2_ERR_INVALID_ARG;
+  if (want_resp && !(h->flags & SP2_WITH_RESPONSE)) return SP2_ERR_INVALID_ARG;
+  if (N <= 0 || N > h->n_max) return SP2_ERR_INVALID_ARG;
+  if (N_occ < 0 || N_occ > N) return SP2_ERR_INVALID_ARG;
+  if (ldh < N || ldd < N) return SP2_ERR_INVALID_ARG;
+  if ((in_dt != SP2_F32 && in_dt != SP2_F64) || (out_dt != SP2_F32 && out_dt != SP2_F64)) return SP2_ERR_INVALID_ARG;
+  if (h->opt.engine == SP2_ENGINE_SIMT_DEBUG && pad_n(N) > kSimtMaxN) return SP2_ERR_INVALID_ARG;
+  return SP2_OK;
+}
+
+// enqueue one whole solve on `s`; the result struct lands in ring[ring_idx]
+sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const void* H1, sp2_dtype_t in_dt, long ldh, int N, int N_occ,
+                           double tol, void* D, void* D1, sp2_dtype_t out_dt, long ldd, int ring_idx, cudaStream_t s,
+                           int* launches_out) {
+  const int resp = (H1 != nullptr) ? 1 : 0;
+  sp2_status_t st = prepare(h, N, resp, s);
+  if (st != SP2_OK) return st;
+  const int npad = h->cur_npad;
+  const sp2_options_t& o = h->opt;
+  int max_layers = o.max_layers <= 0 ? 100 : (o.max_layers > 126 ? 126 : o.max_layers);
+  int forced = o.forced_layers > 0 ? (o.forced_layers > 64 ? 64 : o.forced_layers) : 0;
+  if (forced) max_layers = forced;
+  int launches = 0;
+  Sp2Ctrl* c = h->ctrl();
+  sp2_launch_init(c, N, N_occ, npad, resp, max_layers, o.user_bounds, o.eps_min, o.eps_max, tol, forced, o.forced_signs, s);
+  ++launches;
+  sp2_launch_bounds(H, in_dt, ldh, N, 0, h->bslots(0), s); ++launches;
+  if (resp) { sp2_launch_bounds(H1, in_dt, ldh, N, 1, h->bslots(1), s); ++launches; }
+  sp2_launch_setup(c, h->bslots(0), sp2_bounds_blocks(N), h->bslots(1), resp ? sp2_bounds_blocks(N) : 0, s); ++launches;
+  if (N_occ == 0 || N_occ == N) {
+    sp2_launch_trivial(c, D, D1, out_dt, ldd, N, h->ring() + ring_idx, s); ++launches;
+  } else {
+    if (resp) { sp2_launch_rescale(H1, in_dt, ldh, c, 1, h->plane(2, 0), h->plane(3, 0), npad, h->slots2(), s); ++launches; }
+    sp2_launch_rescale(H, in_dt, ldh, c, 0, h->plane(0, 0), h->plane(1, 0), npad, h->slots(), s); ++launches;
+    sp2_launch_ctrl0(c, h->slots(), h->slots2(), sp2_rescale_blocks(npad), s); ++launches;
+    for (int n = 0; n < max_layers; ++n) {
+      cudaError_t e = sp2_launch_layer(h->args[n & 1], o.engine, h->cur_cg, h->num_sms, s);
+      if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
+      ++launches;
+    }
+    __half* planes[8] = {h->plane(0, 0), h->plane(1, 0), h->plane(0, 1), h->plane(1, 1),
+                         h->plane(resp ? 2 : 0, 0), h->plane(resp ? 3 : 1, 0), h->plane(resp ? 2 : 0, 1), h->plane(resp ? 3 : 1, 1)};
+    sp2_launch_finalise(c, planes, npad, H, in_dt, ldh, D, resp ? D1 : nullptr, out_dt, ldd, N, h->fslots(),
+                        h->ring() + ring_idx, s);
+    launches += 2;
+  }
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
+  h->launches += (unsigned long long)launches;
+  if (launches_out) *launches_out = launches;
+  return SP2_OK;
+}
+
+sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const void* H1, sp2_dtype_t in_dt, long ldh, int N, int N_occ,
+                            double tol, void* D, void* D1, sp2_dtype_t out_dt, long ldd, sp2_result_t* out, cudaStream_t s,
+                            bool host_buffers) {
+  const int want_resp = (H1 != nullptr || D1 != nullptr) ? 1 : 0;
+  sp2_status_t st = check_args(h, H, H1, want_resp, in_dt, ldh, N, N_occ, D, D1, out_dt, ldd);
+  if (st != SP2_OK) return st;
+  if (h->seq_active) return SP2_ERR_INVALID_ARG;
+  const void* dH = H; const void* dH1 = H1; void* dD = D; void* dD1 = D1;
+  long dld_in = ldh, dld_out = ldd;
+  const size_t in_sz = in_dt == SP2_F32 ? 4 : 8, out_sz = out_dt == SP2_F32 ? 4 : 8;
+  // make sure the launch state is ready before the timed region starts
+  st = prepare(h, N, want_resp, s);
+  if (st != SP2_OK) return st;
+  SP2_CUDA(h, cudaEventRecord(h->ev0, s));
+  if (host_buffers) {
+    if (!(h->flags & SP2_WITH_HOST_STAGING)) return SP2_ERR_WORKSPACE;
+    dH = h->staging(0); dD = h->staging(1);
+    dld_in = N; dld_out = N;
+    SP2_CUDA(h, cudaMemcpy2DAsync(h->staging(0), (size_t)N * in_sz, H, (size_t)ldh * in_sz, (size_t)N * in_sz, N,
+                                  cudaMemcpyHostToDevice, s));
+    if (want_resp) {
+      dH1 = h->staging(2); dD1 = h->staging(3);
+      SP2_CUDA(h, cudaMemcpy2DAsync(h->staging(2), (size_t)N * in_sz, H1, (size_t)ldh * in_sz, (size_t)N * in_sz, N,
+                                    cudaMemcpyHostToDevice, s));
+    }
+  }
+  int launches = 0;
+  st = enqueue_solve(h, dH, dH1, in_dt, dld_in, N, N_occ, tol, dD, dD1, out_dt, dld_out, 0, s, &launches);
+  if (st != SP2_OK) return st;
+  if (host_buffers) {
+    SP2_CUDA(h, cudaMemcpy2DAsync(D, (size_t)ldd * out_sz, dD, (size_t)N * out_sz, (size_t)N * out_sz, N,
+                                  cudaMemcpyDeviceToHost, s));
+    if (want_resp)
+      SP2_CUDA(h, cudaMemcpy2DAsync(D1, (size_t)ldd * out_sz, dD1, (size_t)N * out_sz, (size_t)N * out_sz, N,
+                                    cudaMemcpyDeviceToHost, s));
+  }
+  SP2_CUDA(h, cudaMemcpyAsync(h->h_result, h->ring(), sizeof(sp2_result_t), cudaMemcpyDeviceToHost, s));
+  SP2_CUDA(h, cudaEventRecord(h->ev1, s));
+  SP2_CUDA(h, cudaStreamSynchronize(s));
+  float ms = 0.f;
+  SP2_CUDA(h, cudaEventElapsedTime(&ms, h->ev0, h->ev1));
+  sp2_result_t r = *h->h_result;
+  r.gpu_ms = ms;
+  r.kernel_launches = launches;
+  if (out) *out = r;
+  return (sp2_status_t)r.status;
+}
+
+}  // namespace
+
+// ================================================================================================
+extern "C" {
+
+size_t sp2_workspace_bytes(int n_max, int flags) {
+  if (n_max <= 0) return 0;
+  return make_layout(n_max, flags).total;
+}
+
+sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_workspace, size_t bytes) {
+  if (!handle || n_max <= 0) return SP2_ERR_INVALID_ARG;
+  *handle = nullptr;
+  Layout L = make_layout(n_max, flags);
+  if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 1023) || bytes < L.total) return SP2_ERR_WORKSPACE;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return SP2_ERR_CUDA;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return SP2_ERR_CUDA;
+  if (prop.major != 10) return SP2_ERR_ARCH;
+  sp2_handle_s* h = new (std::nothrow) sp2_handle_s();
+  if (!h) return SP2_ERR_INVALID_ARG;
+  h->n_max = n_max; h->flags = flags; h->device = dev; h->num_sms = prop.multiProcessorCount;
+  h->ws = static_cast<uint8_t*>(d_workspace); h->ws_bytes = bytes; h->L = L;
+  default_options(&h->opt);
+  h->cur_npad = -1; h->cur_cg = -1; h->cur_resp = -1;
+  h->last_cuda_error = 0; h->launches = 0; h->seq_active = 0;
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+  if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) { delete h; return SP2_ERR_CUDA; }
+  h->encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(fn);
+  if (sp2_layer_configure() != cudaSuccess) { delete h; return SP2_ERR_CUDA; }
+  if (cudaEventCreate(&h->ev0) != cudaSuccess || cudaEventCreate(&h->ev1) != cudaSuccess) { delete h; return SP2_ERR_CUDA; }
+  if (cudaMallocHost(reinterpret_cast<void**>(&h->h_result), sizeof(sp2_result_t) * kRingCap) != cudaSuccess) {
+    delete h; return SP2_ERR_CUDA;
+  }
+  *handle = h;
+  return SP2_OK;
+}
+
+sp2_status_t sp2_destroy(sp2_handle_t h) {
+  if (!h) return SP2_ERR_INVALID_ARG;
+  cudaEventDestroy(h->ev0);
+  cudaEventDestroy(h->ev1);
+  cudaFreeHost(h->h_result);
+  delete h;
+  return SP2_OK;
+}
+
+sp2_status_t sp2_set_options(sp2_handle_t h, const sp2_options_t* opt) {
+  if (!h) return SP2_ERR_INVALID_ARG;
+  if (!opt) { default_options(&h->opt); return SP2_OK; }
+  if (opt->engine != SP2_ENGINE_TCGEN05 && opt->engine != SP2_ENGINE_SIMT_DEBUG) return SP2_ERR_INVALID_ARG;
+  if (opt->cta_group < 0 || opt->cta_group > 2) return SP2_ERR_INVALID_ARG;
+  if (opt->user_bounds && !(opt->eps_max > opt->eps_min)) return SP2_ERR_INVALID_ARG;
+  h->opt = *opt;
+  return SP2_OK;
+}
+
+sp2_status_t sp2_get_options(sp2_handle_t h, sp2_options_t* opt) {
+  if (!h || !opt) return SP2_ERR_INVALID_ARG;
+  *opt = h->opt;
+  return SP2_OK;
+}
+
+sp2_status_t sp2_density(sp2_handle_t h, const void* dH, sp2_dtype_t in_dtype, long ldh, int N, int N_occ, double tol,
+                         void* dD, sp2_dtype_t out_dtype, long ldd, sp2_result_t* out, void* stream) {
+  return blocking_solve(h, dH, nullptr, in_dtype, ldh, N, N_occ, tol, dD, nullptr, out_dtype, ldd, out,
+                        static_cast<cudaStream_t>(stream), false);
+}
+
+sp2_status_t sp2_response(sp2_handle_t h, const void* dH, const void* dH1, sp2_dtype_t in_dtype, long ld, int N, int N_occ,
+                          double tol, void* dD, void* dD1, sp2_dtype_t out_dtype, long ldo, sp2_result_t* out, void* stream) {
+  if (!dH1 || !dD1) return SP2_ERR_INVALID_ARG;
+  return blocking_solve(h, dH, dH1, in_dtype, ld, N, N_occ, tol, dD, dD1, out_dtype, ldo, out,
+                        static_cast<cudaStream_t>(stream), false);
+}
+
+sp2_status_t sp2_density_host(sp2_handle_t h, const void* hH, sp2_dtype_t in_dtype, long ldh, int N, int N_occ, double tol,
+                              void* hD, sp2_dtype_t out_dtype, long ldd, sp2_result_t* out, void* stream) {
+  return blocking_solve(h, hH, nullptr, in_dtype, ldh, N, N_occ, tol, hD, nullptr, out_dtype, ldd, out,
+                        static_cast<cudaStream_t>(stream), true);
+}
+
+sp2_status_t sp2_response_host(sp2_handle_t h, const void* hH, const void* hH1, sp2_dtype_t in_dtype, long ld, int N,
+                               int N_occ, double tol, void* hD, void* hD1, sp2_dtype_t out_dtype, long ldo,
+                               sp2_result_t* out, void* stream) {
+  if (!hH1 || !hD1) return SP2_ERR_INVALID_ARG;
+  return blocking_solve(h, hH, hH1, in_dtype, ld, N, N_occ, tol, hD, hD1, out_dtype, ldo, out,
+                        static_cast<cudaStream_t>(stream), true);
+}
+
+sp2_status_t sp2_sequence_begin(sp2_handle_t h, int N, int N_occ, double tol, int n_steps_hint, void* stream) {
+  if (!h || N <= 0 || N > h->n_max || N_occ < 0 || N_occ > N) return SP2_ERR_INVALID_ARG;
+  if (n_steps_hint > kRingCap) return SP2_ERR_INVALID_ARG;
+  if (h->seq_active) return SP2_ERR_INVALID_ARG;
+  h->seq_active = 1; h->seq_N = N; h->seq_nocc = N_occ; h->seq_tol = tol; h->seq_steps = 0;
+  h->seq_stream = static_cast<cudaStream_t>(stream);
+  return prepare(h, N, 0, h->seq_stream);
+}
+
+sp2_status_t sp2_sequence_step(sp2_handle_t h, const void* dH_t, sp2_dtype_t in_dtype, long ldh, void* dD_t,
+                               sp2_dtype_t out_dtype, long ldd) {
+  if (!h || !h->seq_active) return SP2_ERR_INVALID_ARG;
+  if (h->seq_steps >= kRingCap) return SP2_ERR_INVALID_ARG;
+  sp2_status_t st = check_args(h, dH_t, nullptr, 0, in_dtype, ldh, h->seq_N, h->seq_nocc, dD_t, nullptr, out_dtype, ldd);
+  if (st != SP2_OK) return st;
+  st = enqueue_solve(h, dH_t, nullptr, in_dtype, ldh, h->seq_N, h->seq_nocc, h->seq_tol, dD_t, nullptr, out_dtype, ldd,
+                     h->seq_steps, h->seq_stream, nullptr);
+  if (st == SP2_OK) ++h->seq_steps;
+  return st;
+}
+
+sp2_status_t sp2_sequence_end(sp2_handle_t h, sp2_result_t* results, int* n_steps) {
+  if (!h || !h->seq_active) return SP2_ERR_INVALID_ARG;
+  h->seq_active = 0;
+  const int n = h->seq_steps;
+  if (n_steps) *n_steps = n;
+  if (n > 0)
+    SP2_CUDA(h, cudaMemcpyAsync(h->h_result, h->ring(), sizeof(sp2_result_t) * (size_t)n, cudaMemcpyDeviceToHost,
+                                h->seq_stream));
+  SP2_CUDA(h, cudaStreamSynchronize(h->seq_stream));
+  sp2_status_t worst = SP2_OK;
+  for (int i = 0; i < n; ++i) {
+    if (results) results[i] = h->h_result[i];
+    if (h->h_result[i].status != SP2_OK && worst == SP2_OK) worst = (sp2_status_t)h->h_result[i].status;
+  }
+  return worst;
+}
+
+const char* sp2_status_string(sp2_status_t s) {
+  switch (s) {
+    case SP2_OK: return "ok";
+    case SP2_ERR_INVALID_ARG: return "invalid argument";
+    case SP2_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+    case SP2_ERR_CUDA: return "CUDA call failed";
+    case SP2_ERR_ARCH: return "device is not sm_100";
+    case SP2_ERR_NONFINITE: return "non-finite input or iterate";
+    case SP2_ERR_DEGENERATE: return "degenerate spectral bounds (eps_max == eps_min)";
+    case SP2_WARN_NOT_CONVERGED: return "not converged within max_layers";
+  }
+  return "unknown status";
+}
+
+int sp2_last_cuda_error(sp2_handle_t h) { return h ? h->last_cuda_error : 0; }
+unsigned long long sp2_launch_count(sp2_handle_t h) { return h ? h->launches : 0ull; }
+
+int sp2_debug_history(sp2_handle_t h, double* tr_x, double* e, int capacity) {
+  if (!h) return -1;
+  static Sp2Ctrl host_ctrl;
+  if (cudaMemcpy(&host_ctrl, h->ctrl(), sizeof(Sp2Ctrl), cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
+  int cnt = host_ctrl.n + 1;
+  if (cnt > SP2_LAYER_CAP) cnt = SP2_LAYER_CAP;
+  for (int i = 0; i < cnt && i < capacity; ++i) {
+    if (tr_x) tr_x[i] = host_ctrl.tr_x[i];
+    if (e) e[i] = host_ctrl.e[i];
+  }
+  return cnt;
+}
+
+sp2_status_t sp2_debug_plane(sp2_handle_t h, int which, size_t* offset, long* pitch, int* exponent, double* shift) {
+  if (!h || which < 0 || which > 7) return SP2_ERR_INVALID_ARG;
+  const int prev = which >> 2;      // 4..7: the same planes of the PREVIOUS iterate (other ping-pong buffer)
+  which &= 3;
+  if (which >= 2 && !(h->flags & SP2_WITH_RESPONSE)) return SP2_ERR_INVALID_ARG;
+  static Sp2Ctrl host_ctrl;
+  if (cudaMemcpy(&host_ctrl, h->ctrl(), sizeof(Sp2Ctrl), cudaMemcpyDeviceToHost) != cudaSuccess) return SP2_ERR_CUDA;
+  const int buf = (host_ctrl.n & 1) ^ prev;
+  if (offset) *offset = (size_t)(reinterpret_cast<uint8_t*>(h->plane(which, buf)) - h->ws);
+  if (pitch) *pitch = host_ctrl.npad;
+  if (exponent) *exponent = which < 2 ? host_ctrl.t : host_ctrl.u;
+  if (shift) *shift = host_ctrl.c;
+  return SP2_OK;
+}
+
+}  // extern "C"

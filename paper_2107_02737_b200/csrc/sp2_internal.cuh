@@ -1,0 +1,213 @@
+// sp2_internal.cuh -- device-side control block, slots and the layer controller shared by the
+// kernels of libsp2_b200.  Product code: shares nothing with oracle/.
+//
+// Iterate representation:  X_n = c_n*I + Y_n,  Y_n = (Yh + Ym) * 2^-t_n
+// with Yh, Ym FP16 planes (Eq. 20-21: X = X^(0) + X^(1)), c_n an fp64 device
+// scalar that follows the same scalar map as the layer (c <- c^2 or 2c - c^2).  The first-order
+// iterate is Z_n = (Zh + Zm) * 2^-u_n.
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+#include "sp2.h"
+
+#define SP2_LAYER_CAP 128          // size of the per-layer history arrays (max_layers <= 126)
+#define SP2_FP16_TARGET_LOG2 15    // planes are scaled so that (bound on max|.|) * 2^t <= 2^15 < 65504
+
+struct Sp2Slot {      // one partial per producer (block / epilogue warp); reduced in index order
+  double tr;          // sum of stored diagonal values (scaled units)
+  double fro;         // sum of squares of stored values, upper triangle counted twice (scaled units^2)
+  double tracc;       // sum of the raw diagonal accumulators of a Y^2 unit (input scaled units^2), else 0
+  float mx;           // max |stored value| (scaled units)
+  float pad;
+};
+
+struct Sp2BoundSlot { // per block of the bounds kernel
+  double lo, hi;      // min_i(H_ii - r_i), max_i(H_ii + r_i)
+  double tr;          // sum_i H_ii
+  double mx;          // max |H_ij|
+  double sum;         // sum |H_ij| (non-finite detector)
+};
+
+struct Sp2Coef {      // epilogue coefficients of the layer about to run (scaled units)
+  float a1y_hi, a1y_lo, a2y;   // Y' = (a1y_hi + a1y_lo) * (Yh+Ym) + a2y * acc
+  float a1z_hi, a1z_lo, a2z;   // Z' likewise with the (YZ+ZY) accumulator
+};
+
+struct Sp2Ctrl {
+  // problem (written by k_init)
+  int N, n_occ, npad, with_response;
+  int max_layers, user_bounds, forced_layers, pad0;
+  unsigned long long forced_signs;
+  double tol, user_eps_min, user_eps_max;
+  // input layer (written by k_setup)
+  double eps_min, eps_max, delta, tr_h, maxabs_h, maxabs_h1;
+  // iterate state
+  double c;             // shift of the current iterate
+  int t, u;             // plane exponents of the current iterate (Y, Z)
+  int t_in;             // exponent of the Y planes the running layer READS (for the trace identity)
+  int pad2;
+  double sigma_last;    // +1 / -1: branch of the layer that is running / ran last
+  double fro_in;        // ||Y||_F^2 (TRUE units) of the iterate the running layer reads
+  int n;                // index of the layer about to run = number of layers applied so far
+  int done;             // 1: no more layers (converged, failed or capped)
+  int status;           // sp2_status_t
+  int stop_reason;
+  unsigned int ticket;  // last-block election of the layer kernel
+  int pad1;
+  double tr_y, fro_y, max_y, tr_z, fro_z, max_z;  // reduced partials of the current iterate, TRUE units
+  Sp2Coef coef;
+  unsigned long long sign_mask[2];
+  double tr_x[SP2_LAYER_CAP];
+  double e[SP2_LAYER_CAP];
+  // finalise
+  double tr_d, tr_dh, tr_d1;
+};
+
+// ----------------------------------------------------------------------------------------------
+// small device helpers
+__device__ __forceinline__ double sp2_exp2i(int k) { return scalbn(1.0, k); }
+
+// largest k with bound * 2^k <= 2^SP2_FP16_TARGET_LOG2, clamped so that every epilogue
+// coefficient 2^(t'-2t) stays an fp32 normal.
+__device__ __forceinline__ int sp2_pick_exponent(double bound) {
+  if (!(bound > 0.0) || !isfinite(bound)) return 40;
+  int ex;
+  frexp(bound, &ex);              // bound = m * 2^ex, m in [0.5, 1)  ->  bound <= 2^ex
+  int k = SP2_FP16_TARGET_LOG2 - ex;
+  return max(-30, min(40, k));
+}
+
+__device__ __forceinline__ void sp2_split_f32(double a, float& hi, float& lo) {
+  hi = (float)a;
+  lo = (float)(a - (double)hi);
+}
+
+// Stop test at the top of layer n ("until all eigenvalues ... sufficiently close to
+// 1 or 0"; "idempotency conditions ... estimated from traces of intermediate
+// matrices").  DESIGN.md reading R4.  Returns a stop_reason (0 = continue).
+__device__ inline int sp2_stop_rule(const Sp2Ctrl* c, int n, double tr_x) {
+  const double e_n = c->e[n];
+  const bool near_occ = fabs(tr_x - (double)c->n_occ) < 0.5;
+  if (c->forced_layers > 0) return n >= c->forced_layers ? 6 : 0;
+  if (c->tol > 0.0 && e_n >= 0.0 && e_n <= c->tol && near_occ) return 1;
+  if (n >= 3) {
+    const int s1 = (int)((c->sign_mask[(n - 1) >> 6] >> ((n - 1) & 63)) & 1ull);
+    const int s2 = (int)((c->sign_mask[(n - 2) >> 6] >> ((n - 2) & 63)) & 1ull);
+    const double e2 = c->e[n - 2];
+    if (s1 != s2 && e2 < 1.0 && (e_n <= 0.0 || e_n > 4.5 * e2 * e2)) return 2;
+  }
+  if (e_n <= 0.0 && near_occ) return 3;
+  if (n >= c->max_layers) return 4;
+  return 0;
+}
+
+// The controller: runs once per layer boundary in ONE thread, after the partial sums of the
+// current iterate (tr Y, ||Y||_F^2, max|Y|, same for Z; TRUE units) were stored in *c.
+// Decides stop / branch for layer n = c->n and writes the epilogue coefficients of that layer.
+//   tr X   = N c + tr Y
+//   tr X^2 = N c^2 + 2 c tr Y + ||Y||_F^2        (X symmetric => tr X^2 = ||X||_F^2)
+// so the branch of layer n is known before its GEMM runs (no host round trip, PAPER.md:186 does
+// this on the CPU).
+__device__ inline void sp2_controller(Sp2Ctrl* c) {
+  const int n = c->n;
+  const double N = (double)c->N;
+  const double cc = c->c;
+  if (!isfinite(c->fro_y) || !isfinite(c->tr_y) || !isfinite(c->max_y) ||
+      (c->with_response && (!isfinite(c->fro_z) || !isfinite(c->max_z)))) {
+    c->done = 1; c->status = SP2_ERR_NONFINITE; c->stop_reason = 0;
+    return;
+  }
+  const double tr_x = N * cc + c->tr_y;
+  const double tr_x2 = N * cc * cc + 2.0 * cc * c->tr_y + c->fro_y;
+  c->tr_x[n] = tr_x;
+  c->e[n] = tr_x - tr_x2;
+  const int stop = sp2_stop_rule(c, n, tr_x);
+  if (stop) {
+    c->done = 1; c->stop_reason = stop;
+    c->status = (stop == 4) ? SP2_WARN_NOT_CONVERGED : SP2_OK;
+    return;
+  }
+  const double nocc = (double)c->n_occ;
+  bool plus = fabs(tr_x2 - nocc) < fabs(2.0 * tr_x - tr_x2 - nocc);   // ties -> '-' (reading R3)
+  if (c->forced_layers > 0) plus = (c->forced_signs >> n) & 1ull;
+  if (plus) c->sign_mask[n >> 6] |= (1ull << (n & 63));
+  const double alpha = plus ? 2.0 * cc : 2.0 - 2.0 * cc;    // X^2     = c^2 I + 2c Y + Y^2
+  const double sigma = plus ? 1.0 : -1.0;                   // 2X - X^2 = (2c-c^2) I + (2-2c) Y - Y^2
+  const double c_next = plus ? cc * cc : 2.0 * cc - cc * cc;
+  // bounds on max|Y'|, max|Z'|: |(Y^2)_ij| <= ||Y||_2^2 and
+  // ||Y||_2 <= min(||Y||_F, s) with s = max(c, 1-c) because spec(X) is inside [0,1].
+  const double s = fmax(cc, 1.0 - cc) * 1.001 + 1e-6;
+  const double y2 = fmin(c->fro_y, s * s);
+  const double by = fabs(alpha) * c->max_y + y2;
+  const int t_next = sp2_pick_exponent(by);
+  const int t = c->t;
+  sp2_split_f32(alpha * sp2_exp2i(t_next - t), c->coef.a1y_hi, c->coef.a1y_lo);
+  c->coef.a2y = (float)(sigma * sp2_exp2i(t_next - 2 * t));
+  if (c->with_response) {
+    const double bz = fabs(alpha) * c->max_z + 2.0 * sqrt(y2) * sqrt(c->fro_z);
+    const int u_next = sp2_pick_exponent(bz);
+    const int u = c->u;
+    sp2_split_f32(alpha * sp2_exp2i(u_next - u), c->coef.a1z_hi, c->coef.a1z_lo);
+    c->coef.a2z = (float)(sigma * sp2_exp2i(u_next - t - u));
+    c->u = u_next;    // exponents describe the iterate the layer WRITES; the layer itself only
+  }                   // needs coef, so they can be advanced here
+  c->t_in = t;
+  c->sigma_last = sigma;
+  c->fro_in = c->fro_y;
+  c->t = t_next;
+  c->c = c_next;
+  c->n = n + 1;
+}
+
+// Trace identity: tcgen05 accumulates in FP32 with
+// truncation, which biases every diagonal accumulator (a sum of squares) low by ~1 ulp per MMA.
+// The bias is coherent over the diagonal, i.e. close to a multiple of I, and the exact value of
+// its trace is known: tr(Y^2) = ||Y||_F^2, which the PREVIOUS epilogue summed with round-to-nearest
+// arithmetic.  The difference is folded into the scalar shift c, so tr X stays exact.
+__device__ inline void sp2_trace_identity(Sp2Ctrl* c, double tracc_scaled) {
+  const double tr_acc = tracc_scaled * sp2_exp2i(-2 * c->t_in);
+  const double bias = c->fro_in - tr_acc;          // = -tr(E) >= 0 for a truncating accumulator
+  if (isfinite(bias)) c->c += c->sigma_last * bias / (double)c->N;
+}
+
+// Reduce `count` slots in index order with one 256-thread block; result valid in thread 0.
+// Deterministic: fixed per-thread strided order, then a fixed shared-memory tree.
+__device__ inline void sp2_reduce_slots(const Sp2Slot* slots, int count, double* red /* smem 4*256 */,
+                                        double& tr, double& fro, double& mx, double& tracc) {
+  const int tid = threadIdx.x;
+  const int nt = blockDim.x;      // must be 256
+  double a = 0.0, b = 0.0, m = 0.0, d = 0.0;
+  for (int i = tid; i < count; i += nt) {
+    a += slots[i].tr;
+    b += slots[i].fro;
+    d += slots[i].tracc;
+    const double v = (double)slots[i].mx;
+    m = (v > m || v != v) ? v : m;   // NaN-propagating max
+  }
+  red[tid] = a; red[256 + tid] = b; red[512 + tid] = m; red[768 + tid] = d;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (tid < w) {
+      red[tid] += red[tid + w];
+      red[256 + tid] += red[256 + tid + w];
+      red[768 + tid] += red[768 + tid + w];
+      const double o = red[512 + tid + w], q = red[512 + tid];
+      red[512 + tid] = (o > q || o != o) ? o : q;
+    }
+    __syncthreads();
+  }
+  tr = red[0]; fro = red[256]; mx = red[512]; tracc = red[768];
+  __syncthreads();
+}
+
+// One element of the fused epilogue: new value from the old stored pair and the
+// accumulator, split into the next hi/lo planes.  Returns the value as the NEXT layer will see it.
+__device__ __forceinline__ float sp2_epilogue_elem(float old, float acc, float a1hi, float a1lo, float a2,
+                                                   __half& hi, __half& lo) {
+  const float y = fmaf(a1hi, old, fmaf(a1lo, old, a2 * acc));
+  hi = __float2half_rn(y);
+  const float r = y - __half2float(hi);
+  lo = __float2half_rn(r);
+  return __half2float(hi) + __half2float(lo);
+}

@@ -1,0 +1,581 @@
+// sp2_layer.cu -- one DNN-SP2 layer as a persistent, warp-specialised
+// sm_100a kernel: TMA -> shared-memory ring -> tcgen05.mma (FP16 x FP16 -> FP32 in TMEM) -> fused
+// epilogue (update, hi/lo split, mirrored store, trace partials) -> last CTA runs the controller.
+//
+// What a layer computes: X_{n+1} = X_n^2 or 2X_n - X_n^2.  With the shifted
+// iterate X = c I + Y this is Y' = alpha*Y + sigma*Y^2 and, for the first-order iterate,
+// Z' = alpha*Z + sigma*(YZ + ZY).  With the dual half-precision representation of PAPER.md:153-170
+// (Eq. 20-22)  Y = h + m, Z = p + q  the products are
+//     Y^2     ~ h h + h m + m h                                   (m m dropped, Eq. 22)
+//     YZ + ZY ~ (h p + h q + m p) + (p h + p m + q h)
+// All planes are symmetric, so B[k][j] = B[j][k] and both operands of every product are K-major
+// row panels of the same row-major plane; only tiles on or above the diagonal are computed and
+// every result is written to (i,j) and (j,i), which keeps the planes bit-symmetric.
+//
+// A work unit = one output tile of one product class, expressed as `passes` sweeps over k of
+//     acc += A0 B0^T + A0 B1^T + A1 B0^T
+// (Y^2: one pass with A=(h,m) rows i, B=(h,m) rows j;  YZ+ZY: pass 0 A=(h,m), B=(p,q); pass 1
+// A=(p,q), B=(h,m)).
+//
+// CG = 1: tile 128x128, one CTA, UMMA 128x128x16.  CG = 2: tile 256x256 on a CTA pair
+// (cta_group::2, UMMA 256x256x16); each CTA loads 128 rows of A and 128 rows of B per plane.
+#include <cuda.h>
+#include "sp2_internal.cuh"
+#include "sp2_layer.h"
+
+namespace {
+
+constexpr int kBK = 64;                       // k elements per stage (128 bytes: SWIZZLE_128B row)
+constexpr int kRows = 128;                    // rows per TMA box / per CTA operand tile
+constexpr int kStages = 3;
+constexpr int kPlaneTileBytes = kRows * kBK * 2;          // 16 KB
+constexpr int kStageBytes = 4 * kPlaneTileBytes;          // A0, A1, B0, B1 = 64 KB
+constexpr int kThreads = 256;
+constexpr long long kSpinLimit = 1ll << 26;   // mbarrier watchdog: trap instead of hanging the GPU
+
+// ---------------------------------------------------------------------------------- PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done = 0;
+  long long spins = 0;
+  while (true) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    if (done) break;
+    if (++spins > kSpinLimit) __trap();
+  }
+}
+// arrive on a barrier of CTA `rank` of the cluster (rank may be the own CTA)
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t rank) {
+  uint32_t remote;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(bar), "r"(rank));
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+template <int CG>
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0, int c1) {
+  if constexpr (CG == 1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1)
+        : "memory");
+  } else {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1)
+        : "memory");
+  }
+}
+
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+template <int CG>
+__device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t ncols) {
+  if constexpr (CG == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(ncols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  } else {
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(ncols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+  }
+}
+template <int CG>
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+  if constexpr (CG == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+  else asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+
+// D[tmem] (+)= A[smem] * B[smem]^T, FP16 inputs, FP32 accumulate
+template <int CG>
+__device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  if constexpr (CG == 1) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+  } else {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+  }
+}
+// all previously issued MMAs of this thread -> one arrival on `bar` (same offset in every CTA of the mask)
+template <int CG>
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  if constexpr (CG == 1) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+  } else {
+    const uint16_t mask = 3;
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(bar), "h"(mask)
+                 : "memory");
+  }
+}
+
+// 32 lanes x 32 columns of FP32 from TMEM (lane = accumulator row)
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+        "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+        "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+        "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+      : "r"(taddr)
+      : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// K-major, SWIZZLE_128B shared-memory matrix descriptor (sm_100 format): rows of 128 bytes,
+// 8-row groups 1024 bytes apart.
+__device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFFu) >> 4);       // start address >> 4            bits [0,14)
+  d |= (uint64_t)1 << 16;                         // leading byte offset (unused)  bits [16,30)
+  d |= (uint64_t)(1024 >> 4) << 32;               // stride byte offset = 1024 B   bits [32,46)
+  d |= (uint64_t)1 << 46;                         // descriptor version (sm_100)   bits [46,48)
+  d |= (uint64_t)2 << 61;                         // layout: SWIZZLE_128B          bits [61,64)
+  return d;
+}
+// kind::f16 instruction descriptor: D = F32, A = B = F16, both K-major, M x N
+__host__ __device__ constexpr uint32_t make_idesc(int M, int N) {
+  return (1u << 4) | (0u << 7) | (0u << 10) | (0u << 15) | (0u << 16) | ((uint32_t)(N >> 3) << 17) |
+         ((uint32_t)(M >> 4) << 24);
+}
+
+struct alignas(8) SmemBarriers {
+  uint64_t full[kStages];
+  uint64_t empty[kStages];
+  uint64_t tmem_full[2];
+  uint64_t tmem_empty[2];
+  uint32_t tmem_base;
+  uint32_t is_last;
+};
+
+__device__ __forceinline__ uint4 ld_global_v4(const void* p) {
+  uint4 r;
+  asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+
+__device__ __forceinline__ uint32_t u4_word(const uint4& v, int i) {
+  return i == 0 ? v.x : (i == 1 ? v.y : (i == 2 ? v.z : v.w));
+}
+
+// ----------------------------------------------------------------------------------------------
+// shared tail of both engines: last block reduces the slots (index order) and runs the controller
+__device__ inline void layer_tail(Sp2Ctrl* ctrl, const Sp2Slot* slots, int n_y, int n_z, int y_first,
+                                  unsigned int n_blocks, uint32_t* is_last_smem, double* red) {
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    const unsigned int old = atomicAdd(&ctrl->ticket, 1u);
+    *is_last_smem = (old == n_blocks - 1) ? 1u : 0u;
+  }
+  __syncthreads();
+  if (!*is_last_smem) return;
+  __threadfence();
+  double tr, fro, mx, tracc, trz = 0.0, froz = 0.0, mxz = 0.0, unused;
+  // slot array: [z slots (n_z)][y slots (n_y)] when y_first == n_z
+  sp2_reduce_slots(slots + y_first, n_y, red, tr, fro, mx, tracc);
+  if (n_z > 0) sp2_reduce_slots(slots, n_z, red, trz, froz, mxz, unused);
+  if (threadIdx.x == 0) {
+    sp2_trace_identity(ctrl, tracc);
+    const double sy = sp2_exp2i(-ctrl->t), sz = sp2_exp2i(-ctrl->u);
+    ctrl->tr_y = tr * sy; ctrl->fro_y = fro * sy * sy; ctrl->max_y = mx * sy;
+    ctrl->tr_z = trz * sz; ctrl->fro_z = froz * sz * sz; ctrl->max_z = mxz * sz;
+    ctrl->ticket = 0;
+    sp2_controller(ctrl);
+  }
+}
+
+// ----------------------------------------------------------------------------------------------
+template <int CG>
+__global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant__ Sp2LayerArgs a) {
+  constexpr int TILE = 128 * CG;          // output tile edge
+  constexpr int UM = 128 * CG, UN = 128 * CG;
+  constexpr int ACC_COLS = UN;            // FP32 accumulator columns per buffer
+  constexpr uint32_t TMEM_COLS = 2 * ACC_COLS;
+  constexpr uint32_t IDESC = make_idesc(UM, UN);
+
+  if (a.ctrl->done) return;               // uniform over the grid: written before this launch
+
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  SmemBarriers* bars = reinterpret_cast<SmemBarriers*>(smem + kStages * kStageBytes);
+  __shared__ double red[4 * 256];
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;
+  const int cluster_id = blockIdx.x / CG;
+  const int n_clusters = gridDim.x / CG;
+  const bool leader = (rank == 0);
+
+  const int n_tiles = a.n_tiles;
+  const int n_units = a.with_response ? 2 * n_tiles : n_tiles;
+  const int KB = a.npad / kBK;
+
+  if (warp == 0 && lane == 0) {
+    for (int i = 0; i < 4; ++i) asm volatile("prefetch.tensormap [%0];" ::"l"(&a.tm[i]) : "memory");
+  }
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < kStages; ++s) { mbar_init(smem_u32(&bars->full[s]), 1); mbar_init(smem_u32(&bars->empty[s]), 1); }
+    for (int s = 0; s < 2; ++s) { mbar_init(smem_u32(&bars->tmem_full[s]), 1); mbar_init(smem_u32(&bars->tmem_empty[s]), 4 * CG); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 2) tmem_alloc<CG>(smem_u32(&bars->tmem_base), TMEM_COLS);
+  tc_fence_before();
+  if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(&bars->tmem_base);
+
+  if (warp == 0) {
+    // ===================================== TMA producer (one lane, every CTA) ==================
+    if (elect_one()) {
+      int stage = 0; uint32_t phase = 0;
+      uint32_t full_bar[kStages];
+      for (int s = 0; s < kStages; ++s) {
+        full_bar[s] = smem_u32(&bars->full[s]);
+        if constexpr (CG == 2) asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(full_bar[s]) : "r"(full_bar[s]), "r"(0));
+      }
+      for (int u = cluster_id; u < n_units; u += n_clusters) {
+        const bool wunit = a.with_response && u < n_tiles;
+        const int2 tij = a.tiles[wunit ? u : (a.with_response ? u - n_tiles : u)];
+        const int row_a = tij.x * TILE + (int)rank * kRows;
+        const int row_b = tij.y * TILE + (int)rank * kRows;
+        const int passes = wunit ? 2 : 1;
+        for (int p = 0; p < passes; ++p) {
+          // Y^2: A = (Yh, Ym), B = (Yh, Ym).  W pass 0: A = (Yh, Ym), B = (Zh, Zm).  W pass 1: A = (Zh, Zm), B = (Yh, Ym).
+          const int ma = (wunit && p == 1) ? 2 : 0;
+          const int mb = (wunit && p == 0) ? 2 : 0;
+          for (int kb = 0; kb < KB; ++kb) {
+            mbar_wait(smem_u32(&bars->empty[stage]), phase ^ 1u);
+            const uint32_t dst = smem_u32(smem + stage * kStageBytes);
+            if (CG == 1 || leader) mbar_expect_tx(smem_u32(&bars->full[stage]), (uint32_t)(CG * kStageBytes));
+            tma_load_2d<CG>(dst + 0 * kPlaneTileBytes, &a.tm[ma + 0], full_bar[stage], kb * kBK, row_a);
+            tma_load_2d<CG>(dst + 1 * kPlaneTileBytes, &a.tm[ma + 1], full_bar[stage], kb * kBK, row_a);
+            tma_load_2d<CG>(dst + 2 * kPlaneTileBytes, &a.tm[mb + 0], full_bar[stage], kb * kBK, row_b);
+            tma_load_2d<CG>(dst + 3 * kPlaneTileBytes, &a.tm[mb + 1], full_bar[stage], kb * kBK, row_b);
+            if (++stage == kStages) { stage = 0; phase ^= 1u; }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================================== MMA issuer (one lane of the leader CTA) ==============
+    if (leader && elect_one()) {
+      int stage = 0; uint32_t phase = 0;
+      int as = 0; uint32_t aphase = 0;
+      for (int u = cluster_id; u < n_units; u += n_clusters) {
+        const bool wunit = a.with_response && u < n_tiles;
+        const int iters = (wunit ? 2 : 1) * KB;
+        mbar_wait(smem_u32(&bars->tmem_empty[as]), aphase ^ 1u);
+        tc_fence_after();
+        const uint32_t acc = tmem_base + (uint32_t)(as * ACC_COLS);
+        for (int it = 0; it < iters; ++it) {
+          mbar_wait(smem_u32(&bars->full[stage]), phase);
+          tc_fence_after();
+          const uint32_t sa = smem_u32(smem + stage * kStageBytes);
+          const uint64_t dA0 = make_smem_desc(sa + 0 * kPlaneTileBytes);
+          const uint64_t dA1 = make_smem_desc(sa + 1 * kPlaneTileBytes);
+          const uint64_t dB0 = make_smem_desc(sa + 2 * kPlaneTileBytes);
+          const uint64_t dB1 = make_smem_desc(sa + 3 * kPlaneTileBytes);
+#pragma unroll
+          for (int k = 0; k < kBK / 16; ++k) {
+            const uint64_t ko = (uint64_t)(k * 2);     // 16 elements * 2 B = 32 B -> >>4 = 2
+            umma_f16<CG>(acc, dA0 + ko, dB0 + ko, IDESC, (it | k) ? 1u : 0u);
+            umma_f16<CG>(acc, dA0 + ko, dB1 + ko, IDESC, 1u);
+            umma_f16<CG>(acc, dA1 + ko, dB0 + ko, IDESC, 1u);
+          }
+          umma_commit<CG>(smem_u32(&bars->empty[stage]));     // smem slot free when these MMAs retire
+          if (++stage == kStages) { stage = 0; phase ^= 1u; }
+        }
+        umma_commit<CG>(smem_u32(&bars->tmem_full[as]));       // accumulator complete
+        if (++as == 2) { as = 0; aphase ^= 1u; }
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================================== epilogue warps (4 per CTA) ===========================
+    const int q = warp & 3;                       // TMEM lane quarter this warp may read
+    const Sp2Coef cf = a.ctrl->coef;
+    int as = 0; uint32_t aphase = 0;
+    for (int u = cluster_id; u < n_units; u += n_clusters) {
+      const bool wunit = a.with_response && u < n_tiles;
+      const int2 tij = a.tiles[wunit ? u : (a.with_response ? u - n_tiles : u)];
+      const int pl = wunit ? 2 : 0;
+      const float a1hi = wunit ? cf.a1z_hi : cf.a1y_hi, a1lo = wunit ? cf.a1z_lo : cf.a1y_lo;
+      const float a2 = wunit ? cf.a2z : cf.a2y;
+      const __half* __restrict__ in_h = a.in[pl];
+      const __half* __restrict__ in_m = a.in[pl + 1];
+      __half* __restrict__ out_h = a.out[pl];
+      __half* __restrict__ out_m = a.out[pl + 1];
+      const int gi = tij.x * TILE + (int)rank * kRows + q * 32 + lane;   // global row of this thread
+      const int j0 = tij.y * TILE;
+      const size_t npad = (size_t)a.npad;
+
+      mbar_wait(smem_u32(&bars->tmem_full[as]), aphase);
+      tc_fence_after();
+      double tr = 0.0, fro = 0.0, tracc = 0.0;
+      float mx = 0.f;
+#pragma unroll 1
+      for (int ch = 0; ch < ACC_COLS / 32; ++ch) {
+        uint32_t v[32];
+        __syncwarp();
+        tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * ACC_COLS + ch * 32), v);
+        if (ch == ACC_COLS / 32 - 1) {            // accumulator fully read: hand the buffer back
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) {
+            if constexpr (CG == 2) mbar_arrive_cluster(smem_u32(&bars->tmem_empty[as]), 0);
+            else mbar_arrive(smem_u32(&bars->tmem_empty[as]));
+          }
+        }
+        const int gj0 = j0 + ch * 32;
+        // gi = 32-aligned base + lane and gj0 is 32-aligned, so both tests are warp-uniform
+        if (gj0 + 31 < gi) continue;              // chunk entirely below the diagonal: mirrored by its transpose
+        const bool full = gj0 > gi;               // chunk entirely above the diagonal
+        uint4 oh[4], om[4];
+        const uint4* ph = reinterpret_cast<const uint4*>(in_h + (size_t)gi * npad + gj0);
+        const uint4* pm = reinterpret_cast<const uint4*>(in_m + (size_t)gi * npad + gj0);
+#pragma unroll
+        for (int w = 0; w < 4; ++w) { oh[w] = ld_global_v4(ph + w); om[w] = ld_global_v4(pm + w); }
+        uint32_t nh[16], nm[16];                  // packed pairs of new hi / lo halves
+        float fsum = 0.f;
+#pragma unroll
+        for (int pr = 0; pr < 16; ++pr) {
+          const uint32_t wh = u4_word(oh[pr >> 2], pr & 3), wm = u4_word(om[pr >> 2], pr & 3);
+          __half h0, m0, h1, m1;
+          const float old0 = __half2float(__ushort_as_half((unsigned short)(wh & 0xffffu))) +
+                             __half2float(__ushort_as_half((unsigned short)(wm & 0xffffu)));
+          const float old1 = __half2float(__ushort_as_half((unsigned short)(wh >> 16))) +
+                             __half2float(__ushort_as_half((unsigned short)(wm >> 16)));
+          const float s0 = sp2_epilogue_elem(old0, __uint_as_float(v[2 * pr]), a1hi, a1lo, a2, h0, m0);
+          const float s1 = sp2_epilogue_elem(old1, __uint_as_float(v[2 * pr + 1]), a1hi, a1lo, a2, h1, m1);
+          nh[pr] = (uint32_t)__half_as_ushort(h0) | ((uint32_t)__half_as_ushort(h1) << 16);
+          nm[pr] = (uint32_t)__half_as_ushort(m0) | ((uint32_t)__half_as_ushort(m1) << 16);
+          const int gja = gj0 + 2 * pr, gjb = gja + 1;
+          const float wa = (gja > gi) ? 2.f : (gja == gi ? 1.f : 0.f);
+          const float wb = (gjb > gi) ? 2.f : (gjb == gi ? 1.f : 0.f);
+          fsum = fmaf(wa * s0, s0, fsum);
+          fsum = fmaf(wb * s1, s1, fsum);
+          if (gja == gi) { tr += (double)s0; tracc += (double)__uint_as_float(v[2 * pr]); }
+          if (gjb == gi) { tr += (double)s1; tracc += (double)__uint_as_float(v[2 * pr + 1]); }
+          if (gja >= gi) mx = (fabsf(s0) > mx || s0 != s0) ? fabsf(s0) : mx;
+          if (gjb >= gi) mx = (fabsf(s1) > mx || s1 != s1) ? fabsf(s1) : mx;
+        }
+        fro += (double)fsum;
+        unsigned short* oh16 = reinterpret_cast<unsigned short*>(out_h);
+        unsigned short* om16 = reinterpret_cast<unsigned short*>(out_m);
+        if (full) {
+          uint4* qh = reinterpret_cast<uint4*>(out_h + (size_t)gi * npad + gj0);
+          uint4* qm = reinterpret_cast<uint4*>(out_m + (size_t)gi * npad + gj0);
+#pragma unroll
+          for (int w = 0; w < 4; ++w) {
+            qh[w] = make_uint4(nh[4 * w], nh[4 * w + 1], nh[4 * w + 2], nh[4 * w + 3]);
+            qm[w] = make_uint4(nm[4 * w], nm[4 * w + 1], nm[4 * w + 2], nm[4 * w + 3]);
+          }
+#pragma unroll
+          for (int pr = 0; pr < 16; ++pr) {       // mirrored image: lanes = consecutive rows -> 64 B per store
+            oh16[(size_t)(gj0 + 2 * pr) * npad + gi] = (unsigned short)(nh[pr] & 0xffffu);
+            om16[(size_t)(gj0 + 2 * pr) * npad + gi] = (unsigned short)(nm[pr] & 0xffffu);
+            oh16[(size_t)(gj0 + 2 * pr + 1) * npad + gi] = (unsigned short)(nh[pr] >> 16);
+            om16[(size_t)(gj0 + 2 * pr + 1) * npad + gi] = (unsigned short)(nm[pr] >> 16);
+          }
+        } else {                                  // the chunk that holds the diagonal: element-wise, gj >= gi only
+#pragma unroll
+          for (int pr = 0; pr < 16; ++pr) {
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+              const int gj = gj0 + 2 * pr + e;
+              const unsigned short hv = (unsigned short)(e ? (nh[pr] >> 16) : (nh[pr] & 0xffffu));
+              const unsigned short mv = (unsigned short)(e ? (nm[pr] >> 16) : (nm[pr] & 0xffffu));
+              if (gj >= gi) { oh16[(size_t)gi * npad + gj] = hv; om16[(size_t)gi * npad + gj] = mv; }
+              if (gj > gi) { oh16[(size_t)gj * npad + gi] = hv; om16[(size_t)gj * npad + gi] = mv; }
+            }
+          }
+        }
+      }
+      // warp partial -> slot (fixed shuffle tree: deterministic)
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        tr += __shfl_xor_sync(0xffffffffu, tr, o);
+        fro += __shfl_xor_sync(0xffffffffu, fro, o);
+        tracc += __shfl_xor_sync(0xffffffffu, tracc, o);
+        const float qv = __shfl_xor_sync(0xffffffffu, mx, o);
+        mx = (qv > mx || qv != qv) ? qv : mx;
+      }
+      if (lane == 0) {
+        Sp2Slot s; s.tr = tr; s.fro = fro; s.tracc = wunit ? 0.0 : tracc; s.mx = mx; s.pad = 0.f;
+        a.slots[((size_t)u * CG + rank) * 4 + q] = s;
+      }
+      if (++as == 2) { as = 0; aphase ^= 1u; }
+    }
+  }
+
+  // ===================================== teardown ==============================================
+  tc_fence_before();
+  if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
+  if (warp == 2) tmem_dealloc<CG>(tmem_base, TMEM_COLS);
+
+  const int per_unit = CG * 4;
+  const int n_z = a.with_response ? n_tiles * per_unit : 0;
+  layer_tail(a.ctrl, a.slots, n_tiles * per_unit, n_z, n_z, gridDim.x, &bars->is_last, red);
+}
+
+// ----------------------------------------------------------------------------------------------
+// SIMT debug engine (tests only): same planes, same unit semantics, same epilogue element function,
+// plain FP32 FMA mainloop.  16x16 output elements per block, blockIdx.y = product class.
+__global__ void __launch_bounds__(256) k_layer_simt(Sp2LayerArgs a) {
+  if (a.ctrl->done) return;
+  __shared__ double red[4 * 256];
+  __shared__ uint32_t is_last;
+  __shared__ double rs[3][8];
+  __shared__ float rm[8];
+  const int nb = a.npad / 16;
+  const int n_blk_tri = nb * (nb + 1) / 2;
+  const int cls = blockIdx.y;                  // 0: Y^2, 1: YZ + ZY
+  int bi = 0, rem = blockIdx.x;
+  while (rem >= nb - bi) { rem -= nb - bi; ++bi; }
+  const int bj = bi + rem;
+  const int r = threadIdx.x >> 4, cidx = threadIdx.x & 15;
+  const int gi = bi * 16 + r, gj = bj * 16 + cidx;
+  const size_t npad = (size_t)a.npad;
+  const __half* Yh = a.in[0]; const __half* Ym = a.in[1];
+  const __half* Zh = a.in[2]; const __half* Zm = a.in[3];
+  float acc = 0.f;
+  if (cls == 0) {
+    for (int k = 0; k < a.npad; ++k) {
+      const float hi_ = __half2float(Yh[gi * npad + k]), mi = __half2float(Ym[gi * npad + k]);
+      const float hj = __half2float(Yh[gj * npad + k]), mj = __half2float(Ym[gj * npad + k]);
+      acc = fmaf(hi_, hj, acc); acc = fmaf(hi_, mj, acc); acc = fmaf(mi, hj, acc);
+    }
+  } else {
+    for (int k = 0; k < a.npad; ++k) {
+      const float hi_ = __half2float(Yh[gi * npad + k]), mi = __half2float(Ym[gi * npad + k]);
+      const float hj = __half2float(Yh[gj * npad + k]), mj = __half2float(Ym[gj * npad + k]);
+      const float pi_ = __half2float(Zh[gi * npad + k]), qi = __half2float(Zm[gi * npad + k]);
+      const float pj = __half2float(Zh[gj * npad + k]), qj = __half2float(Zm[gj * npad + k]);
+      acc = fmaf(hi_, pj, acc); acc = fmaf(hi_, qj, acc); acc = fmaf(mi, pj, acc);
+      acc = fmaf(pi_, hj, acc); acc = fmaf(pi_, mj, acc); acc = fmaf(qi, hj, acc);
+    }
+  }
+  const Sp2Coef cf = a.ctrl->coef;
+  const int pl = cls ? 2 : 0;
+  const float a1hi = cls ? cf.a1z_hi : cf.a1y_hi, a1lo = cls ? cf.a1z_lo : cf.a1y_lo, a2 = cls ? cf.a2z : cf.a2y;
+  double tr = 0.0, fro = 0.0, tracc = 0.0;
+  float mx = 0.f;
+  if (gj >= gi) {
+    const float old = __half2float(a.in[pl][gi * npad + gj]) + __half2float(a.in[pl + 1][gi * npad + gj]);
+    __half nh, nm;
+    const float s = sp2_epilogue_elem(old, acc, a1hi, a1lo, a2, nh, nm);
+    a.out[pl][gi * npad + gj] = nh; a.out[pl + 1][gi * npad + gj] = nm;
+    if (gj > gi) { a.out[pl][gj * npad + gi] = nh; a.out[pl + 1][gj * npad + gi] = nm; }
+    fro = (gj > gi ? 2.0 : 1.0) * (double)s * (double)s;
+    if (gj == gi) { tr = (double)s; if (cls == 0) tracc = (double)acc; }
+    mx = (s != s) ? s : fabsf(s);
+  }
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    tr += __shfl_xor_sync(0xffffffffu, tr, o);
+    fro += __shfl_xor_sync(0xffffffffu, fro, o);
+    tracc += __shfl_xor_sync(0xffffffffu, tracc, o);
+    const float qv = __shfl_xor_sync(0xffffffffu, mx, o);
+    mx = (qv > mx || qv != qv) ? qv : mx;
+  }
+  if (lane == 0) { rs[0][warp] = tr; rs[1][warp] = fro; rs[2][warp] = tracc; rm[warp] = mx; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    Sp2Slot s; s.tr = 0; s.fro = 0; s.tracc = 0; s.mx = 0.f; s.pad = 0.f;
+    for (int w = 0; w < 8; ++w) { s.tr += rs[0][w]; s.fro += rs[1][w]; s.tracc += rs[2][w]; s.mx = (rm[w] > s.mx || rm[w] != rm[w]) ? rm[w] : s.mx; }
+    // layout [z slots][y slots]
+    const int n_z = a.with_response ? n_blk_tri : 0;
+    a.slots[(cls ? 0 : n_z) + blockIdx.x] = s;
+  }
+  const int n_z = a.with_response ? n_blk_tri : 0;
+  layer_tail(a.ctrl, a.slots, n_blk_tri, n_z, n_z, gridDim.x * gridDim.y, &is_last, red);
+}
+
+}  // namespace
+
+// ----------------------------------------------------------------------------------------------
+size_t sp2_layer_smem_bytes() { return (size_t)kStages * kStageBytes + sizeof(SmemBarriers) + 1024; }
+
+int sp2_layer_slots(int npad, int cta_group, int with_response, int engine) {
+  if (engine == SP2_ENGINE_SIMT_DEBUG) {
+    const int nb = npad / 16;
+    return nb * (nb + 1) / 2 * (with_response ? 2 : 1);
+  }
+  const int nt = npad / (128 * cta_group);
+  return nt * (nt + 1) / 2 * cta_group * 4 * (with_response ? 2 : 1);
+}
+
+cudaError_t sp2_layer_configure() {
+  cudaError_t e = cudaFuncSetAttribute(k_layer_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp2_layer_smem_bytes());
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_layer_tc<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp2_layer_smem_bytes());
+  return e;
+}
+
+cudaError_t sp2_launch_layer(const Sp2LayerArgs& args, int engine, int cta_group, int num_sms, cudaStream_t s) {
+  if (engine == SP2_ENGINE_SIMT_DEBUG) {
+    const int nb = args.npad / 16;
+    dim3 grid(nb * (nb + 1) / 2, args.with_response ? 2 : 1);
+    k_layer_simt<<<grid, 256, 0, s>>>(args);
+    return cudaGetLastError();
+  }
+  const int n_units = args.n_tiles * (args.with_response ? 2 : 1);
+  cudaLaunchConfig_t cfg = {};
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = sp2_layer_smem_bytes();
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  if (cta_group == 2) {
+    int clusters = num_sms / 2;
+    if (clusters > n_units) clusters = n_units;
+    cfg.gridDim = dim3(2 * clusters);
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_layer_tc<2>, args);
+  }
+  int ctas = num_sms;
+  if (ctas > n_units) ctas = n_units;
+  cfg.gridDim = dim3(ctas);
+  cfg.attrs = nullptr; cfg.numAttrs = 0;
+  return cudaLaunchKernelEx(&cfg, k_layer_tc<1>, args);
+}

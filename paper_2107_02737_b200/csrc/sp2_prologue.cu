@@ -1,0 +1,436 @@
+// sp2_prologue.cu -- input layer of DNN-SP2 and the finalise pass (a6).
+// All three are HBM-bound streaming kernels: coalesced row reads, warp-shuffle reductions, fp64
+// accumulation, per-block slots reduced in fixed order (no float atomics -> deterministic).
+//
+//   a1  k_bounds     Gershgorin discs r_i = sum_{j!=i} |H_ij|, eps_min/max, tr H, max|H|
+//   --  k_setup      reduce a1, Delta, c_0 = tr(X_0)/N, first plane exponents
+//   a2  k_rescale    Y_0 = X_0 - c_0 I with X_0 = (eps_max I - H)/Delta, Z_0 = -H1/Delta, hi/lo FP16 split
+//                    (PAPER.md:145 input layer; Eq. 20-21 dual representation)
+//   --  k_ctrl0      reduce a2 partials, run the controller for layer 0
+//   a6  k_finalise   D = c_L I + Y_L, D1 = Z_L in the caller's dtype, tr D, tr(DH), tr D1
+#include "sp2_internal.cuh"
+
+namespace {
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// 16-byte vector loads: float4 / double2
+__device__ __forceinline__ void abs_acc(const float4& x, double& s, double& m) {
+  const double a = fabs((double)x.x), b = fabs((double)x.y), c = fabs((double)x.z), d = fabs((double)x.w);
+  s += (a + b) + (c + d);
+  m = fmax(m, fmax(fmax(a, b), fmax(c, d)));
+}
+__device__ __forceinline__ void abs_acc(const double2& x, double& s, double& m) {
+  const double a = fabs(x.x), b = fabs(x.y);
+  s += a + b;
+  m = fmax(m, fmax(a, b));
+}
+template <typename T> struct Vec16;
+template <> struct Vec16<float> { using type = float4; static constexpr int n = 4; };
+template <> struct Vec16<double> { using type = double2; static constexpr int n = 2; };
+
+// ------------------------------------------------------------------------------------------
+// a1: one warp per row, 8 rows per 256-thread block.  mode 0: full Gershgorin; mode 1: only
+// max|.| and the non-finite detector (used for H1).
+template <typename T>
+__global__ void __launch_bounds__(256) k_bounds(const T* __restrict__ H, long ld, int N, int mode,
+                                                Sp2BoundSlot* __restrict__ slots) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int row = blockIdx.x * 8 + warp;
+  double lo = INFINITY, hi = -INFINITY, tr = 0.0, mx = 0.0, sum = 0.0;
+  if (row < N) {
+    const T* r = H + (size_t)row * ld;
+    double s = 0.0, m = 0.0;
+    const bool vec_ok = ((reinterpret_cast<uintptr_t>(r) & 15) == 0);
+    int j0 = 0;
+    if (vec_ok) {
+      using V = typename Vec16<T>::type;
+      constexpr int VN = Vec16<T>::n;
+      const V* rv = reinterpret_cast<const V*>(r);
+      const int nv = N / VN;
+      for (int v = lane; v < nv; v += 32) abs_acc(__ldg(rv + v), s, m);
+      j0 = nv * VN;
+    }
+    for (int j = j0 + lane; j < N; j += 32) {
+      const double a = fabs((double)__ldg(r + j));
+      s += a;
+      m = fmax(m, a);
+    }
+    s = warp_sum(s);
+    m = warp_max(m);
+    const double d = (double)__ldg(r + row);
+    const double rad = s - fabs(d);          // sum over j != i
+    lo = d - rad; hi = d + rad; tr = d; mx = m; sum = s;
+  }
+  __shared__ double sh[5][8];
+  if (lane == 0) { sh[0][warp] = lo; sh[1][warp] = hi; sh[2][warp] = tr; sh[3][warp] = mx; sh[4][warp] = sum; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    Sp2BoundSlot o;
+    o.lo = sh[0][0]; o.hi = sh[1][0]; o.tr = sh[2][0]; o.mx = sh[3][0]; o.sum = sh[4][0];
+    for (int w = 1; w < 8; ++w) {
+      o.lo = fmin(o.lo, sh[0][w]); o.hi = fmax(o.hi, sh[1][w]);
+      o.tr += sh[2][w]; o.mx = fmax(o.mx, sh[3][w]); o.sum += sh[4][w];
+    }
+    (void)mode;
+    slots[blockIdx.x] = o;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// Reduce the bound slots, fix the input layer and the first plane exponents.  One block.
+__global__ void __launch_bounds__(256) k_setup(Sp2Ctrl* c, const Sp2BoundSlot* sh_slots, int n_h,
+                                               const Sp2BoundSlot* s1_slots, int n_h1) {
+  __shared__ double red[5][256];
+  const int tid = threadIdx.x;
+  double lo = INFINITY, hi = -INFINITY, tr = 0.0, mx = 0.0, sum = 0.0, mx1 = 0.0, sum1 = 0.0;
+  for (int i = tid; i < n_h; i += 256) {
+    lo = fmin(lo, sh_slots[i].lo); hi = fmax(hi, sh_slots[i].hi);
+    tr += sh_slots[i].tr; mx = fmax(mx, sh_slots[i].mx); sum += sh_slots[i].sum;
+  }
+  for (int i = tid; i < n_h1; i += 256) { mx1 = fmax(mx1, s1_slots[i].mx); sum1 += s1_slots[i].sum; }
+  red[0][tid] = lo; red[1][tid] = hi; red[2][tid] = tr; red[3][tid] = fmax(mx, 0.0); red[4][tid] = sum + sum1;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (tid < w) {
+      red[0][tid] = fmin(red[0][tid], red[0][tid + w]);
+      red[1][tid] = fmax(red[1][tid], red[1][tid + w]);
+      red[2][tid] += red[2][tid + w];
+      red[3][tid] = fmax(red[3][tid], red[3][tid + w]);
+      red[4][tid] += red[4][tid + w];
+    }
+    __syncthreads();
+  }
+  __shared__ double red1[256];
+  red1[tid] = mx1;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (tid < w) red1[tid] = fmax(red1[tid], red1[tid + w]);
+    __syncthreads();
+  }
+  if (tid != 0) return;
+  c->tr_h = red[2][0];
+  c->maxabs_h = red[3][0];
+  c->maxabs_h1 = red1[0];
+  double eps_min = red[0][0], eps_max = red[1][0];
+  if (c->user_bounds) { eps_min = c->user_eps_min; eps_max = c->user_eps_max; }
+  c->eps_min = eps_min; c->eps_max = eps_max;
+  const double delta = eps_max - eps_min;
+  c->delta = delta;
+  if (!isfinite(red[4][0]) || !isfinite(eps_min) || !isfinite(eps_max)) {
+    c->done = 1; c->status = SP2_ERR_NONFINITE; return;
+  }
+  if (!(delta > 0.0)) { c->done = 1; c->status = SP2_ERR_DEGENERATE; return; }
+  // X_0 = (eps_max I - H)/Delta;  c_0 = tr(X_0)/N;  Y_0 = X_0 - c_0 I
+  const double N = (double)c->N;
+  c->c = (eps_max - c->tr_h / N) / delta;
+  // |Y0_ij| <= (max|H| + |tr H|/N) / Delta
+  c->t = sp2_pick_exponent((c->maxabs_h + fabs(c->tr_h) / N) / delta);
+  c->u = sp2_pick_exponent(c->maxabs_h1 / delta);
+}
+
+// ------------------------------------------------------------------------------------------
+// a2: 32x32 tile pairs (bi <= bj).  Each block reads H tile (bi,bj) and (bj,bi), forms the
+// symmetrised value, and writes both mirror images of the hi/lo planes with coalesced rows, so
+// the planes are bit-symmetric by construction.  which = 0: Y from H, 1: Z from H1.
+// Pads (rows/cols >= N up to npad) are written as zero.
+template <typename T>
+__global__ void __launch_bounds__(256) k_rescale(const T* __restrict__ H, long ld, const Sp2Ctrl* __restrict__ c,
+                                                 int which, __half* __restrict__ Ph, __half* __restrict__ Pm,
+                                                 int npad, Sp2Slot* __restrict__ slots) {
+  if (c->done) return;
+  __shared__ double t1[32][33];
+  __shared__ double t2[32][33];
+  const int nb = npad >> 5;
+  // decode blockIdx.x -> (bi, bj), bi <= bj, row-major over the upper triangle:
+  // row bi starts at bi*nb - bi*(bi-1)/2
+  const long idx = blockIdx.x;
+  int bi = (int)floor(((2.0 * nb + 1.0) - sqrt((2.0 * nb + 1.0) * (2.0 * nb + 1.0) - 8.0 * (double)idx)) * 0.5);
+  bi = max(0, min(nb - 1, bi));
+  while (bi > 0 && (long)bi * nb - (long)bi * (bi - 1) / 2 > idx) --bi;
+  while ((long)(bi + 1) * nb - (long)(bi + 1) * bi / 2 <= idx) ++bi;
+  const int bj = bi + (int)(idx - ((long)bi * nb - (long)bi * (bi - 1) / 2));
+  const int N = c->N;
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;   // 32 x 8
+  for (int r = ty; r < 32; r += 8) {
+    const int gi = bi * 32 + r, gj = bj * 32 + tx;
+    t1[r][tx] = (gi < N && gj < N) ? (double)__ldg(H + (size_t)gi * ld + gj) : 0.0;
+    const int hi_ = bj * 32 + r, hj = bi * 32 + tx;
+    t2[r][tx] = (hi_ < N && hj < N) ? (double)__ldg(H + (size_t)hi_ * ld + hj) : 0.0;
+  }
+  __syncthreads();
+  const double inv_delta = 1.0 / c->delta;
+  const double shift = which == 0 ? c->tr_h / (double)N : 0.0;   // Y0_ii = (tr H/N - H_ii)/Delta
+  const double scale = sp2_exp2i(which == 0 ? c->t : c->u);
+  double tr = 0.0, fro = 0.0;
+  float mx = 0.f;
+  for (int r = ty; r < 32; r += 8) {
+    // upper image: element (gi, gj) = (bi*32 + r, bj*32 + tx)
+    {
+      const int gi = bi * 32 + r, gj = bj * 32 + tx;
+      double v = 0.0;
+      if (gi < N && gj < N) {
+        const double hsym = 0.5 * (t1[r][tx] + t2[tx][r]);
+        v = ((gi == gj ? shift : 0.0) - hsym) * inv_delta * scale;
+      }
+      const __half h = __float2half_rn((float)v);
+      const __half m = __float2half_rn((float)(v - (double)__half2float(h)));
+      Ph[(size_t)gi * npad + gj] = h;
+      Pm[(size_t)gi * npad + gj] = m;
+      const float s = __half2float(h) + __half2float(m);
+      const double w = (gj > gi) ? 2.0 : (gj == gi ? 1.0 : 0.0);
+      fro += w * (double)s * (double)s;
+      if (gi == gj) tr += (double)s;
+      if (gj >= gi) mx = fmaxf(mx, fabsf(s));
+      if (s != s) mx = s;
+    }
+    // lower image: element (gi, gj) = (bj*32 + r, bi*32 + tx), only for off-diagonal tile pairs
+    if (bi != bj) {
+      const int gi = bj * 32 + r, gj = bi * 32 + tx;
+      double v = 0.0;
+      if (gi < N && gj < N) {
+        const double hsym = 0.5 * (t1[tx][r] + t2[r][tx]);
+        v = (0.0 - hsym) * inv_delta * scale;
+      }
+      const __half h = __float2half_rn((float)v);
+      const __half m = __float2half_rn((float)(v - (double)__half2float(h)));
+      Ph[(size_t)gi * npad + gj] = h;
+      Pm[(size_t)gi * npad + gj] = m;
+    }
+  }
+  // block reduce -> slot
+  __shared__ double rs[2][8];
+  __shared__ float rm[8];
+  tr = warp_sum(tr); fro = warp_sum(fro);
+  float mxx = mx;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const float q = __shfl_xor_sync(0xffffffffu, mxx, o);
+    mxx = (q > mxx || q != q) ? q : mxx;
+  }
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (lane == 0) { rs[0][warp] = tr; rs[1][warp] = fro; rm[warp] = mxx; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    Sp2Slot o; o.tr = 0.0; o.fro = 0.0; o.tracc = 0.0; o.mx = 0.f; o.pad = 0.f;
+    for (int w = 0; w < 8; ++w) {
+      o.tr += rs[0][w]; o.fro += rs[1][w];
+      o.mx = (rm[w] > o.mx || rm[w] != rm[w]) ? rm[w] : o.mx;
+    }
+    slots[blockIdx.x] = o;
+  }
+}
+
+// Reduce the a2 partials into TRUE units and run the controller for layer 0.  One block.
+__global__ void __launch_bounds__(256) k_ctrl0(Sp2Ctrl* c, const Sp2Slot* ys, const Sp2Slot* zs, int count) {
+  if (c->done) return;
+  __shared__ double red[4 * 256];
+  double tr, fro, mx, unused;
+  sp2_reduce_slots(ys, count, red, tr, fro, mx, unused);
+  double trz = 0.0, froz = 0.0, mxz = 0.0;
+  if (c->with_response) sp2_reduce_slots(zs, count, red, trz, froz, mxz, unused);
+  if (threadIdx.x != 0) return;
+  const double sy = sp2_exp2i(-c->t), sz = sp2_exp2i(-c->u);
+  c->tr_y = tr * sy; c->fro_y = fro * sy * sy; c->max_y = mx * sy;
+  c->tr_z = trz * sz; c->fro_z = froz * sz * sz; c->max_z = mxz * sz;
+  sp2_controller(c);
+}
+
+// ------------------------------------------------------------------------------------------
+// a6: D = c I + (Yh+Ym) 2^-t, D1 = (Zh+Zm) 2^-u;  tr D, tr(DH), tr D1.  One warp per row.
+// The final iterate lives in buffer (layers & 1); both candidates are passed.
+template <typename TI, typename TO>
+__global__ void __launch_bounds__(256) k_finalise(const Sp2Ctrl* __restrict__ c,
+                                                  const __half* __restrict__ Yh0, const __half* __restrict__ Ym0,
+                                                  const __half* __restrict__ Yh1, const __half* __restrict__ Ym1,
+                                                  const __half* __restrict__ Zh0, const __half* __restrict__ Zm0,
+                                                  const __half* __restrict__ Zh1, const __half* __restrict__ Zm1,
+                                                  int npad, const TI* __restrict__ H, long ldh,
+                                                  TO* __restrict__ D, TO* __restrict__ D1, long ldo,
+                                                  double* __restrict__ slots /* 3 per block */) {
+  const int st = c->status;
+  if (st != SP2_OK && st != SP2_WARN_NOT_CONVERGED) return;
+  const int N = c->N;
+  const int par = c->n & 1;
+  const __half* Yh = par ? Yh1 : Yh0;
+  const __half* Ym = par ? Ym1 : Ym0;
+  const __half* Zh = par ? Zh1 : Zh0;
+  const __half* Zm = par ? Zm1 : Zm0;
+  const bool resp = c->with_response && D1 != nullptr;
+  const double sy = sp2_exp2i(-c->t), sz = sp2_exp2i(-c->u), shift = c->c;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int row = blockIdx.x * 8 + warp;
+  double trd = 0.0, trdh = 0.0, trd1 = 0.0;
+  if (row < N) {
+    const __half2* yh = reinterpret_cast<const __half2*>(Yh + (size_t)row * npad);
+    const __half2* ym = reinterpret_cast<const __half2*>(Ym + (size_t)row * npad);
+    const __half2* zh = reinterpret_cast<const __half2*>(Zh + (size_t)row * npad);
+    const __half2* zm = reinterpret_cast<const __half2*>(Zm + (size_t)row * npad);
+    const TI* h = H + (size_t)row * ldh;
+    TO* d = D + (size_t)row * ldo;
+    TO* d1 = resp ? D1 + (size_t)row * ldo : nullptr;
+    for (int j2 = lane; 2 * j2 < N; j2 += 32) {
+      const float2 a = __half22float2(yh[j2]);
+      const float2 b = __half22float2(ym[j2]);
+      float2 p = make_float2(0.f, 0.f), q = p;
+      if (resp) { p = __half22float2(zh[j2]); q = __half22float2(zm[j2]); }
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int j = 2 * j2 + e;
+        if (j >= N) break;
+        const double y = (double)((e ? a.y : a.x) + (e ? b.y : b.x)) * sy;
+        const double x = y + (j == row ? shift : 0.0);
+        d[j] = (TO)x;
+        trdh += x * (double)__ldg(h + j);
+        if (j == row) trd += x;
+        if (resp) {
+          const double z = (double)((e ? p.y : p.x) + (e ? q.y : q.x)) * sz;
+          d1[j] = (TO)z;
+          if (j == row) trd1 += z;
+        }
+      }
+    }
+  }
+  trd = warp_sum(trd); trdh = warp_sum(trdh); trd1 = warp_sum(trd1);
+  __shared__ double sh[3][8];
+  if (lane == 0) { sh[0][warp] = trd; sh[1][warp] = trdh; sh[2][warp] = trd1; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = 0, b = 0, e = 0;
+    for (int w = 0; w < 8; ++w) { a += sh[0][w]; b += sh[1][w]; e += sh[2][w]; }
+    slots[3 * blockIdx.x + 0] = a; slots[3 * blockIdx.x + 1] = b; slots[3 * blockIdx.x + 2] = e;
+  }
+}
+
+__global__ void __launch_bounds__(256) k_finalise_reduce(Sp2Ctrl* c, const double* slots, int count,
+                                                         sp2_result_t* ring_entry) {
+  __shared__ double red[3][256];
+  const int tid = threadIdx.x;
+  double a = 0, b = 0, e = 0;
+  const int st = c->status;
+  const bool ok = (st == SP2_OK || st == SP2_WARN_NOT_CONVERGED);
+  if (ok)
+    for (int i = tid; i < count; i += 256) { a += slots[3 * i]; b += slots[3 * i + 1]; e += slots[3 * i + 2]; }
+  red[0][tid] = a; red[1][tid] = b; red[2][tid] = e;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (tid < w) { red[0][tid] += red[0][tid + w]; red[1][tid] += red[1][tid + w]; red[2][tid] += red[2][tid + w]; }
+    __syncthreads();
+  }
+  if (tid != 0) return;
+  c->tr_d = red[0][0]; c->tr_dh = red[1][0]; c->tr_d1 = red[2][0];
+  sp2_result_t r;
+  r.status = c->status; r.layers = c->n; r.sign_mask[0] = c->sign_mask[0]; r.sign_mask[1] = c->sign_mask[1];
+  r.stop_reason = c->stop_reason; r.reserved = 0;
+  r.tr_d = c->tr_d; r.tr_dh = c->tr_dh; r.tr_d1 = c->tr_d1;
+  r.idem_est = ok ? c->e[c->n] : 0.0;
+  r.eps_min = c->eps_min; r.eps_max = c->eps_max; r.gpu_ms = 0.f; r.kernel_launches = 0;
+  *ring_entry = r;
+}
+
+// Trivial occupations (N_occ = 0 -> D = 0, N_occ = N -> D = I; D1 = 0), answered from the definition.
+template <typename TO>
+__global__ void __launch_bounds__(256) k_trivial(Sp2Ctrl* c, TO* __restrict__ D, TO* __restrict__ D1, long ldo,
+                                                 sp2_result_t* ring_entry) {
+  const int N = c->N;
+  const double diag = (c->n_occ == 0) ? 0.0 : 1.0;
+  for (size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x; idx < (size_t)N * N;
+       idx += (size_t)gridDim.x * blockDim.x) {
+    const int i = (int)(idx / N), j = (int)(idx % N);
+    D[(size_t)i * ldo + j] = (TO)(i == j ? diag : 0.0);
+    if (D1) D1[(size_t)i * ldo + j] = (TO)0.0;
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    const int st = c->status;   // k_setup may have flagged NONFINITE; DEGENERATE is fine here
+    sp2_result_t r;
+    r.status = (st == SP2_ERR_NONFINITE) ? st : SP2_OK;
+    r.layers = 0; r.sign_mask[0] = r.sign_mask[1] = 0; r.stop_reason = 5; r.reserved = 0;
+    r.tr_d = diag * N; r.tr_dh = diag * c->tr_h; r.tr_d1 = 0.0; r.idem_est = 0.0;
+    r.eps_min = c->eps_min; r.eps_max = c->eps_max; r.gpu_ms = 0.f; r.kernel_launches = 0;
+    *ring_entry = r;
+  }
+}
+
+__global__ void k_init(Sp2Ctrl* c, int N, int n_occ, int npad, int with_response, int max_layers,
+                       int user_bounds, double eps_min, double eps_max, double tol,
+                       int forced_layers, unsigned long long forced_signs) {
+  // one thread: reset the whole control block
+  Sp2Ctrl z;
+  memset(&z, 0, sizeof(z));
+  z.N = N; z.n_occ = n_occ; z.npad = npad; z.with_response = with_response;
+  z.max_layers = max_layers; z.user_bounds = user_bounds; z.user_eps_min = eps_min; z.user_eps_max = eps_max;
+  z.tol = tol; z.forced_layers = forced_layers; z.forced_signs = forced_signs;
+  *c = z;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// host-side launchers (called from sp2_api.cu)
+#define SP2_DISPATCH_IN(dt, CALL_F32, CALL_F64) \
+  do { if ((dt) == SP2_F32) { CALL_F32; } else { CALL_F64; } } while (0)
+
+void sp2_launch_init(Sp2Ctrl* c, int N, int n_occ, int npad, int with_response, int max_layers,
+                     int user_bounds, double eps_min, double eps_max, double tol, int forced_layers,
+                     unsigned long long forced_signs, cudaStream_t s) {
+  k_init<<<1, 1, 0, s>>>(c, N, n_occ, npad, with_response, max_layers, user_bounds, eps_min, eps_max, tol,
+                         forced_layers, forced_signs);
+}
+
+int sp2_bounds_blocks(int N) { return (N + 7) / 8; }
+
+void sp2_launch_bounds(const void* H, sp2_dtype_t dt, long ld, int N, int mode, Sp2BoundSlot* slots, cudaStream_t s) {
+  const int grid = sp2_bounds_blocks(N);
+  SP2_DISPATCH_IN(dt, (k_bounds<float><<<grid, 256, 0, s>>>((const float*)H, ld, N, mode, slots)),
+                  (k_bounds<double><<<grid, 256, 0, s>>>((const double*)H, ld, N, mode, slots)));
+}
+
+void sp2_launch_setup(Sp2Ctrl* c, const Sp2BoundSlot* sh, int n_h, const Sp2BoundSlot* s1, int n_h1, cudaStream_t s) {
+  k_setup<<<1, 256, 0, s>>>(c, sh, n_h, s1, n_h1);
+}
+
+int sp2_rescale_blocks(int npad) { const int nb = npad / 32; return nb * (nb + 1) / 2; }
+
+void sp2_launch_rescale(const void* H, sp2_dtype_t dt, long ld, const Sp2Ctrl* c, int which, __half* Ph, __half* Pm,
+                        int npad, Sp2Slot* slots, cudaStream_t s) {
+  const int grid = sp2_rescale_blocks(npad);
+  SP2_DISPATCH_IN(dt, (k_rescale<float><<<grid, 256, 0, s>>>((const float*)H, ld, c, which, Ph, Pm, npad, slots)),
+                  (k_rescale<double><<<grid, 256, 0, s>>>((const double*)H, ld, c, which, Ph, Pm, npad, slots)));
+}
+
+void sp2_launch_ctrl0(Sp2Ctrl* c, const Sp2Slot* ys, const Sp2Slot* zs, int count, cudaStream_t s) {
+  k_ctrl0<<<1, 256, 0, s>>>(c, ys, zs, count);
+}
+
+int sp2_finalise_blocks(int N) { return (N + 7) / 8; }
+
+void sp2_launch_finalise(Sp2Ctrl* c, __half* const planes[8], int npad, const void* H, sp2_dtype_t in_dt, long ldh,
+                         void* D, void* D1, sp2_dtype_t out_dt, long ldo, int N, double* slots,
+                         sp2_result_t* ring_entry, cudaStream_t s) {
+  const int grid = sp2_finalise_blocks(N);
+#define SP2_FIN(TI, TO)                                                                                     \
+  k_finalise<TI, TO><<<grid, 256, 0, s>>>(c, planes[0], planes[1], planes[2], planes[3], planes[4], planes[5], \
+                                          planes[6], planes[7], npad, (const TI*)H, ldh, (TO*)D, (TO*)D1, ldo, slots)
+  if (in_dt == SP2_F32 && out_dt == SP2_F32) SP2_FIN(float, float);
+  else if (in_dt == SP2_F32 && out_dt == SP2_F64) SP2_FIN(float, double);
+  else if (in_dt == SP2_F64 && out_dt == SP2_F32) SP2_FIN(double, float);
+  else SP2_FIN(double, double);
+#undef SP2_FIN
+  k_finalise_reduce<<<1, 256, 0, s>>>(c, slots, grid, ring_entry);
+}
+
+void sp2_launch_trivial(Sp2Ctrl* c, void* D, void* D1, sp2_dtype_t out_dt, long ldo, int N,
+                        sp2_result_t* ring_entry, cudaStream_t s) {
+  const int grid = (int)(((size_t)N * N + 255) / 256 > 4096 ? 4096 : ((size_t)N * N + 255) / 256);
+  if (out_dt == SP2_F32) k_trivial<float><<<grid, 256, 0, s>>>(c, (float*)D, (float*)D1, ldo, ring_entry);
+  else k_trivial<double><<<grid, 256, 0, s>>>(c, (double*)D, (double*)D1, ldo, ring_entry);
+}
