@@ -19,7 +19,7 @@
 // launchers defined in sp2_prologue.cu
 void sp2_launch_init(Sp2Ctrl* c, int N, int n_occ, int npad, int with_response, int max_layers, int user_bounds,
                      double eps_min, double eps_max, double tol, int forced_layers, unsigned long long forced_signs,
-                     cudaStream_t s);
+                     int no_recentre, cudaStream_t s);
 int sp2_bounds_blocks(int N);
 void sp2_launch_bounds(const void* H, sp2_dtype_t dt, long ld, int N, int mode, Sp2BoundSlot* slots, cudaStream_t s);
 void sp2_launch_setup(Sp2Ctrl* c, const Sp2BoundSlot* sh, int n_h, const Sp2BoundSlot* s1, int n_h1, cudaStream_t s);
@@ -107,7 +107,7 @@ struct sp2_handle_s {
   sp2_options_t opt;
   PFN_cuTensorMapEncodeTiled_v12000 encode;
   // per-(N, cta_group) cache
-  int cur_npad, cur_cg, cur_resp;
+  int cur_n, cur_npad, cur_cg, cur_resp, cur_seg;
   Sp2LayerArgs args[2];          // parity 0: buffer 0 -> 1, parity 1: buffer 1 -> 0
   std::vector<int2> tiles_host;
   cudaEvent_t ev0, ev1;
@@ -176,7 +176,9 @@ int pick_cta_group(sp2_handle_t h, int npad) {
 sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   const int npad = pad_n(N);
   const int cg = pick_cta_group(h, npad);
-  if (h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp) return SP2_OK;
+  int seg = h->opt.seg_kb;
+  if (seg != 1 && seg != 2 && seg != 4) seg = 4;
+  if (h->cur_n == N && h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp && h->cur_seg == seg) return SP2_OK;
   const int nt = npad / (128 * cg);
   build_tiles(nt, h->tiles_host);
   SP2_CUDA(h, cudaMemcpyAsync(h->tiles(), h->tiles_host.data(), h->tiles_host.size() * sizeof(int2),
@@ -194,9 +196,9 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
       if (st != SP2_OK) return st;
     }
     a.ctrl = h->ctrl(); a.slots = h->slots(); a.tiles = h->tiles();
-    a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = resp; a.pad = 0;
+    a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = resp; a.seg_kb = seg;
   }
-  h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp;
+  h->cur_n = N; h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp; h->cur_seg = seg;
   return SP2_OK;
 }
 
@@ -228,7 +230,7 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const void* H1, sp2_dt
   if (forced) max_layers = forced;
   int launches = 0;
   Sp2Ctrl* c = h->ctrl();
-  sp2_launch_init(c, N, N_occ, npad, resp, max_layers, o.user_bounds, o.eps_min, o.eps_max, tol, forced, o.forced_signs, s);
+  sp2_launch_init(c, N, N_occ, npad, resp, max_layers, o.user_bounds, o.eps_min, o.eps_max, tol, forced, o.forced_signs, o.no_recentre, s);
   ++launches;
   sp2_launch_bounds(H, in_dt, ldh, N, 0, h->bslots(0), s); ++launches;
   if (resp) { sp2_launch_bounds(H1, in_dt, ldh, N, 1, h->bslots(1), s); ++launches; }
@@ -330,7 +332,7 @@ sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_work
   h->n_max = n_max; h->flags = flags; h->device = dev; h->num_sms = prop.multiProcessorCount;
   h->ws = static_cast<uint8_t*>(d_workspace); h->ws_bytes = bytes; h->L = L;
   default_options(&h->opt);
-  h->cur_npad = -1; h->cur_cg = -1; h->cur_resp = -1;
+  h->cur_n = -1; h->cur_npad = -1; h->cur_cg = -1; h->cur_resp = -1; h->cur_seg = -1;
   h->last_cuda_error = 0; h->launches = 0; h->seq_active = 0;
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
@@ -360,6 +362,7 @@ sp2_status_t sp2_set_options(sp2_handle_t h, const sp2_options_t* opt) {
   if (!opt) { default_options(&h->opt); return SP2_OK; }
   if (opt->engine != SP2_ENGINE_TCGEN05 && opt->engine != SP2_ENGINE_SIMT_DEBUG) return SP2_ERR_INVALID_ARG;
   if (opt->cta_group < 0 || opt->cta_group > 2) return SP2_ERR_INVALID_ARG;
+  if (opt->seg_kb != 0 && opt->seg_kb != 1 && opt->seg_kb != 2 && opt->seg_kb != 4) return SP2_ERR_INVALID_ARG;
   if (opt->user_bounds && !(opt->eps_max > opt->eps_min)) return SP2_ERR_INVALID_ARG;
   h->opt = *opt;
   return SP2_OK;

@@ -32,12 +32,13 @@ struct Sp2BoundSlot { // per block of the bounds kernel
 struct Sp2Coef {      // epilogue coefficients of the layer about to run (scaled units)
   float a1y_hi, a1y_lo, a2y;   // Y' = (a1y_hi + a1y_lo) * (Yh+Ym) + a2y * acc
   float a1z_hi, a1z_lo, a2z;   // Z' likewise with the (YZ+ZY) accumulator
+  float dsh_hi, dsh_lo;        // added to the diagonal of Y' (re-centring of the shift c), scaled units
 };
 
 struct Sp2Ctrl {
   // problem (written by k_init)
   int N, n_occ, npad, with_response;
-  int max_layers, user_bounds, forced_layers, pad0;
+  int max_layers, user_bounds, forced_layers, no_recentre;
   unsigned long long forced_signs;
   double tol, user_eps_min, user_eps_max;
   // input layer (written by k_setup)
@@ -134,16 +135,23 @@ __device__ inline void sp2_controller(Sp2Ctrl* c) {
   if (plus) c->sign_mask[n >> 6] |= (1ull << (n & 63));
   const double alpha = plus ? 2.0 * cc : 2.0 - 2.0 * cc;    // X^2     = c^2 I + 2c Y + Y^2
   const double sigma = plus ? 1.0 : -1.0;                   // 2X - X^2 = (2c-c^2) I + (2-2c) Y - Y^2
-  const double c_next = plus ? cc * cc : 2.0 * cc - cc * cc;
+  const double c_map = plus ? cc * cc : 2.0 * cc - cc * cc;
+  // Re-centre: X' = c_map I + (alpha Y + sigma Y^2) is stored as c_next I + Y' with c_next = tr(X')/N,
+  // which is known exactly before the layer runs.  tr Y' ~ 0 keeps the diagonal of Y' small and its
+  // spectrum as symmetric as the occupation allows.
+  const double tr_next = plus ? tr_x2 : 2.0 * tr_x - tr_x2;
+  const double c_next = (c->forced_layers > 0 && c->no_recentre) ? c_map : tr_next / N;
+  const double dshift = c_map - c_next;
   // bounds on max|Y'|, max|Z'|: |(Y^2)_ij| <= ||Y||_2^2 and
   // ||Y||_2 <= min(||Y||_F, s) with s = max(c, 1-c) because spec(X) is inside [0,1].
   const double s = fmax(cc, 1.0 - cc) * 1.001 + 1e-6;
   const double y2 = fmin(c->fro_y, s * s);
-  const double by = fabs(alpha) * c->max_y + y2;
+  const double by = fabs(alpha) * c->max_y + y2 + fabs(dshift);
   const int t_next = sp2_pick_exponent(by);
   const int t = c->t;
   sp2_split_f32(alpha * sp2_exp2i(t_next - t), c->coef.a1y_hi, c->coef.a1y_lo);
   c->coef.a2y = (float)(sigma * sp2_exp2i(t_next - 2 * t));
+  sp2_split_f32(dshift * sp2_exp2i(t_next), c->coef.dsh_hi, c->coef.dsh_lo);
   if (c->with_response) {
     const double bz = fabs(alpha) * c->max_z + 2.0 * sqrt(y2) * sqrt(c->fro_z);
     const int u_next = sp2_pick_exponent(bz);
@@ -176,16 +184,18 @@ __device__ inline void sp2_trace_identity(Sp2Ctrl* c, double tracc_scaled) {
 __device__ inline void sp2_reduce_slots(const Sp2Slot* slots, int count, double* red /* smem 4*256 */,
                                         double& tr, double& fro, double& mx, double& tracc) {
   const int tid = threadIdx.x;
-  const int nt = blockDim.x;      // must be 256
+  const int nt = 256;             // blockDim.x >= 256; extra threads only join the barriers
   double a = 0.0, b = 0.0, m = 0.0, d = 0.0;
-  for (int i = tid; i < count; i += nt) {
-    a += slots[i].tr;
-    b += slots[i].fro;
-    d += slots[i].tracc;
-    const double v = (double)slots[i].mx;
-    m = (v > m || v != v) ? v : m;   // NaN-propagating max
+  if (tid < nt) {
+    for (int i = tid; i < count; i += nt) {
+      a += slots[i].tr;
+      b += slots[i].fro;
+      d += slots[i].tracc;
+      const double v = (double)slots[i].mx;
+      m = (v > m || v != v) ? v : m;   // NaN-propagating max
+    }
+    red[tid] = a; red[256 + tid] = b; red[512 + tid] = m; red[768 + tid] = d;
   }
-  red[tid] = a; red[256 + tid] = b; red[512 + tid] = m; red[768 + tid] = d;
   __syncthreads();
   for (int w = 128; w > 0; w >>= 1) {
     if (tid < w) {
@@ -204,8 +214,8 @@ __device__ inline void sp2_reduce_slots(const Sp2Slot* slots, int count, double*
 // One element of the fused epilogue: new value from the old stored pair and the
 // accumulator, split into the next hi/lo planes.  Returns the value as the NEXT layer will see it.
 __device__ __forceinline__ float sp2_epilogue_elem(float old, float acc, float a1hi, float a1lo, float a2,
-                                                   __half& hi, __half& lo) {
-  const float y = fmaf(a1hi, old, fmaf(a1lo, old, a2 * acc));
+                                                   float dsh_hi, float dsh_lo, __half& hi, __half& lo) {
+  const float y = fmaf(a1hi, old, fmaf(a1lo, old, fmaf(a2, acc, dsh_lo))) + dsh_hi;
   hi = __float2half_rn(y);
   const float r = y - __half2float(hi);
   lo = __float2half_rn(r);

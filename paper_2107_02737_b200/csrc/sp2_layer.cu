@@ -30,7 +30,10 @@ constexpr int kRows = 128;                    // rows per TMA box / per CTA oper
 constexpr int kStages = 3;
 constexpr int kPlaneTileBytes = kRows * kBK * 2;          // 16 KB
 constexpr int kStageBytes = 4 * kPlaneTileBytes;          // A0, A1, B0, B1 = 64 KB
-constexpr int kThreads = 256;
+constexpr int kThreads = 384;                 // 4 producer-side warps + 8 consumer warps
+constexpr int kConsumerWarps = 8;
+constexpr int kRegsProducer = 40;             // setmaxnreg budgets: 128*40 + 256*232 <= 65536
+constexpr int kRegsConsumer = 232;
 constexpr long long kSpinLimit = 1ll << 26;   // mbarrier watchdog: trap instead of hanging the GPU
 
 // ---------------------------------------------------------------------------------- PTX helpers
@@ -224,11 +227,94 @@ __device__ inline void layer_tail(Sp2Ctrl* ctrl, const Sp2Slot* slots, int n_y, 
 }
 
 // ----------------------------------------------------------------------------------------------
+// Epilogue of one 32-column chunk held in registers (acc[0..31] = FP32 sums of row gi, columns
+// gj0..gj0+31): update, split, mirrored store, partial sums.
+struct EpiPartials { double tr, fro, tracc; float mx; };
+
+__device__ __forceinline__ void epilogue_chunk(const float* acc, int gi, int gj0, size_t npad,
+                                               const __half* __restrict__ in_h, const __half* __restrict__ in_m,
+                                               __half* __restrict__ out_h, __half* __restrict__ out_m,
+                                               float a1hi, float a1lo, float a2, float dsh_hi, float dsh_lo,
+                                               EpiPartials& P) {
+  // gi = 32-aligned base + lane and gj0 is 32-aligned, so both tests are warp-uniform
+  if (gj0 + 31 < gi) return;                // chunk entirely below the diagonal: mirrored by its transpose
+  const bool full = gj0 > gi;               // chunk entirely above the diagonal
+  const uint4* ph = reinterpret_cast<const uint4*>(in_h + (size_t)gi * npad + gj0);
+  const uint4* pm = reinterpret_cast<const uint4*>(in_m + (size_t)gi * npad + gj0);
+  unsigned short* oh16 = reinterpret_cast<unsigned short*>(out_h);
+  unsigned short* om16 = reinterpret_cast<unsigned short*>(out_m);
+  float fsum = 0.f;
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {             // 8 columns at a time keeps the live register set small
+    const uint4 oh = ld_global_v4(ph + w), om = ld_global_v4(pm + w);
+    uint32_t nh[4], nm[4];                  // packed pairs of new hi / lo halves
+#pragma unroll
+    for (int pr = 0; pr < 4; ++pr) {
+      const uint32_t wh = u4_word(oh, pr), wm = u4_word(om, pr);
+      __half h0, m0, h1, m1;
+      const float old0 = __half2float(__ushort_as_half((unsigned short)(wh & 0xffffu))) +
+                         __half2float(__ushort_as_half((unsigned short)(wm & 0xffffu)));
+      const float old1 = __half2float(__ushort_as_half((unsigned short)(wh >> 16))) +
+                         __half2float(__ushort_as_half((unsigned short)(wm >> 16)));
+      const int ci = 8 * w + 2 * pr;
+      const int gja = gj0 + ci, gjb = gja + 1;
+      const float s0 = sp2_epilogue_elem(old0, acc[ci], a1hi, a1lo, a2, gja == gi ? dsh_hi : 0.f,
+                                         gja == gi ? dsh_lo : 0.f, h0, m0);
+      const float s1 = sp2_epilogue_elem(old1, acc[ci + 1], a1hi, a1lo, a2, gjb == gi ? dsh_hi : 0.f,
+                                         gjb == gi ? dsh_lo : 0.f, h1, m1);
+      nh[pr] = (uint32_t)__half_as_ushort(h0) | ((uint32_t)__half_as_ushort(h1) << 16);
+      nm[pr] = (uint32_t)__half_as_ushort(m0) | ((uint32_t)__half_as_ushort(m1) << 16);
+      const float wa = (gja > gi) ? 2.f : (gja == gi ? 1.f : 0.f);
+      const float wb = (gjb > gi) ? 2.f : (gjb == gi ? 1.f : 0.f);
+      fsum = fmaf(wa * s0, s0, fsum);
+      fsum = fmaf(wb * s1, s1, fsum);
+      if (gja == gi) { P.tr += (double)s0; P.tracc += (double)acc[ci]; }
+      if (gjb == gi) { P.tr += (double)s1; P.tracc += (double)acc[ci + 1]; }
+      if (gja >= gi) P.mx = (fabsf(s0) > P.mx || s0 != s0) ? fabsf(s0) : P.mx;
+      if (gjb >= gi) P.mx = (fabsf(s1) > P.mx || s1 != s1) ? fabsf(s1) : P.mx;
+    }
+    if (full) {
+      *reinterpret_cast<uint4*>(out_h + (size_t)gi * npad + gj0 + 8 * w) = make_uint4(nh[0], nh[1], nh[2], nh[3]);
+      *reinterpret_cast<uint4*>(out_m + (size_t)gi * npad + gj0 + 8 * w) = make_uint4(nm[0], nm[1], nm[2], nm[3]);
+#pragma unroll
+      for (int pr = 0; pr < 4; ++pr) {      // mirrored image: lanes = consecutive rows -> 64 B per store
+        const size_t r0 = (size_t)(gj0 + 8 * w + 2 * pr) * npad + gi;
+        oh16[r0] = (unsigned short)(nh[pr] & 0xffffu);
+        om16[r0] = (unsigned short)(nm[pr] & 0xffffu);
+        oh16[r0 + npad] = (unsigned short)(nh[pr] >> 16);
+        om16[r0 + npad] = (unsigned short)(nm[pr] >> 16);
+      }
+    } else {                                // the chunk that holds the diagonal: element-wise, gj >= gi only
+#pragma unroll
+      for (int pr = 0; pr < 4; ++pr) {
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int gj = gj0 + 8 * w + 2 * pr + e;
+          const unsigned short hv = (unsigned short)(e ? (nh[pr] >> 16) : (nh[pr] & 0xffffu));
+          const unsigned short mv = (unsigned short)(e ? (nm[pr] >> 16) : (nm[pr] & 0xffffu));
+          if (gj >= gi) { oh16[(size_t)gi * npad + gj] = hv; om16[(size_t)gi * npad + gj] = mv; }
+          if (gj > gi) { oh16[(size_t)gj * npad + gi] = hv; om16[(size_t)gj * npad + gi] = mv; }
+        }
+      }
+    }
+  }
+  P.fro += (double)fsum;
+}
+
+// ----------------------------------------------------------------------------------------------
+// Warp roles (384 threads): warp 0 TMA producer, warp 1 MMA issuer, warp 2 TMEM allocator, warp 3
+// idle; warps 4..11 consumers.  The k range of a unit is cut into segments of seg_kb k-blocks; each
+// segment is accumulated by the tensor core into a fresh TMEM buffer (2 buffers, ping-pong) and
+// the consumers add the finished segment into FP32 register sums with round-to-nearest adds.
+// This bounds the length of the truncating in-TMEM accumulation (DESIGN.md "Tensor-core
+// truncation bias") and costs no tensor time: the drain overlaps the next segment's MMAs.
 template <int CG>
 __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant__ Sp2LayerArgs a) {
   constexpr int TILE = 128 * CG;          // output tile edge
   constexpr int UM = 128 * CG, UN = 128 * CG;
-  constexpr int ACC_COLS = UN;            // FP32 accumulator columns per buffer
+  constexpr int ACC_COLS = UN;            // FP32 accumulator columns per TMEM buffer
+  constexpr int WCOLS = ACC_COLS / 2;     // columns per consumer warp (two warps per TMEM lane quarter)
+  constexpr int NCH = WCOLS / 32;         // 32-column chunks per consumer warp
   constexpr uint32_t TMEM_COLS = 2 * ACC_COLS;
   constexpr uint32_t IDESC = make_idesc(UM, UN);
 
@@ -248,13 +334,14 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   const int n_tiles = a.n_tiles;
   const int n_units = a.with_response ? 2 * n_tiles : n_tiles;
   const int KB = a.npad / kBK;
+  const int seg_kb = a.seg_kb;            // k-blocks per TMEM accumulation segment (divides KB)
 
   if (warp == 0 && lane == 0) {
     for (int i = 0; i < 4; ++i) asm volatile("prefetch.tensormap [%0];" ::"l"(&a.tm[i]) : "memory");
   }
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < kStages; ++s) { mbar_init(smem_u32(&bars->full[s]), 1); mbar_init(smem_u32(&bars->empty[s]), 1); }
-    for (int s = 0; s < 2; ++s) { mbar_init(smem_u32(&bars->tmem_full[s]), 1); mbar_init(smem_u32(&bars->tmem_empty[s]), 4 * CG); }
+    for (int s = 0; s < 2; ++s) { mbar_init(smem_u32(&bars->tmem_full[s]), 1); mbar_init(smem_u32(&bars->tmem_empty[s]), kConsumerWarps * CG); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 2) tmem_alloc<CG>(smem_u32(&bars->tmem_base), TMEM_COLS);
@@ -263,186 +350,145 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   tc_fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(&bars->tmem_base);
 
-  if (warp == 0) {
-    // ===================================== TMA producer (one lane, every CTA) ==================
-    if (elect_one()) {
-      int stage = 0; uint32_t phase = 0;
-      uint32_t full_bar[kStages];
-      for (int s = 0; s < kStages; ++s) {
-        full_bar[s] = smem_u32(&bars->full[s]);
-        if constexpr (CG == 2) asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(full_bar[s]) : "r"(full_bar[s]), "r"(0));
-      }
-      for (int u = cluster_id; u < n_units; u += n_clusters) {
-        const bool wunit = a.with_response && u < n_tiles;
-        const int2 tij = a.tiles[wunit ? u : (a.with_response ? u - n_tiles : u)];
-        const int row_a = tij.x * TILE + (int)rank * kRows;
-        const int row_b = tij.y * TILE + (int)rank * kRows;
-        const int passes = wunit ? 2 : 1;
-        for (int p = 0; p < passes; ++p) {
-          // Y^2: A = (Yh, Ym), B = (Yh, Ym).  W pass 0: A = (Yh, Ym), B = (Zh, Zm).  W pass 1: A = (Zh, Zm), B = (Yh, Ym).
-          const int ma = (wunit && p == 1) ? 2 : 0;
-          const int mb = (wunit && p == 0) ? 2 : 0;
-          for (int kb = 0; kb < KB; ++kb) {
-            mbar_wait(smem_u32(&bars->empty[stage]), phase ^ 1u);
-            const uint32_t dst = smem_u32(smem + stage * kStageBytes);
-            if (CG == 1 || leader) mbar_expect_tx(smem_u32(&bars->full[stage]), (uint32_t)(CG * kStageBytes));
-            tma_load_2d<CG>(dst + 0 * kPlaneTileBytes, &a.tm[ma + 0], full_bar[stage], kb * kBK, row_a);
-            tma_load_2d<CG>(dst + 1 * kPlaneTileBytes, &a.tm[ma + 1], full_bar[stage], kb * kBK, row_a);
-            tma_load_2d<CG>(dst + 2 * kPlaneTileBytes, &a.tm[mb + 0], full_bar[stage], kb * kBK, row_b);
-            tma_load_2d<CG>(dst + 3 * kPlaneTileBytes, &a.tm[mb + 1], full_bar[stage], kb * kBK, row_b);
-            if (++stage == kStages) { stage = 0; phase ^= 1u; }
+  if (warp < 4) {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsProducer));
+    if (warp == 0) {
+      // =================================== TMA producer (one lane, every CTA) ==================
+      if (elect_one()) {
+        int stage = 0; uint32_t phase = 0;
+        uint32_t full_bar[kStages];
+        for (int s = 0; s < kStages; ++s) {
+          full_bar[s] = smem_u32(&bars->full[s]);
+          if constexpr (CG == 2) asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(full_bar[s]) : "r"(full_bar[s]), "r"(0));
+        }
+        for (int u = cluster_id; u < n_units; u += n_clusters) {
+          const bool wunit = a.with_response && u < n_tiles;
+          const int2 tij = a.tiles[wunit ? u : (a.with_response ? u - n_tiles : u)];
+          const int row_a = tij.x * TILE + (int)rank * kRows;
+          const int row_b = tij.y * TILE + (int)rank * kRows;
+          const int passes = wunit ? 2 : 1;
+          for (int p = 0; p < passes; ++p) {
+            // Y^2: A = (Yh, Ym), B = (Yh, Ym).  W pass 0: A = (Yh, Ym), B = (Zh, Zm).  W pass 1: A = (Zh, Zm), B = (Yh, Ym).
+            const int ma = (wunit && p == 1) ? 2 : 0;
+            const int mb = (wunit && p == 0) ? 2 : 0;
+            for (int kb = 0; kb < KB; ++kb) {
+              mbar_wait(smem_u32(&bars->empty[stage]), phase ^ 1u);
+              const uint32_t dst = smem_u32(smem + stage * kStageBytes);
+              if (CG == 1 || leader) mbar_expect_tx(smem_u32(&bars->full[stage]), (uint32_t)(CG * kStageBytes));
+              tma_load_2d<CG>(dst + 0 * kPlaneTileBytes, &a.tm[ma + 0], full_bar[stage], kb * kBK, row_a);
+              tma_load_2d<CG>(dst + 1 * kPlaneTileBytes, &a.tm[ma + 1], full_bar[stage], kb * kBK, row_a);
+              tma_load_2d<CG>(dst + 2 * kPlaneTileBytes, &a.tm[mb + 0], full_bar[stage], kb * kBK, row_b);
+              tma_load_2d<CG>(dst + 3 * kPlaneTileBytes, &a.tm[mb + 1], full_bar[stage], kb * kBK, row_b);
+              if (++stage == kStages) { stage = 0; phase ^= 1u; }
+            }
           }
         }
       }
-    }
-  } else if (warp == 1) {
-    // ===================================== MMA issuer (one lane of the leader CTA) ==============
-    if (leader && elect_one()) {
-      int stage = 0; uint32_t phase = 0;
-      int as = 0; uint32_t aphase = 0;
-      for (int u = cluster_id; u < n_units; u += n_clusters) {
-        const bool wunit = a.with_response && u < n_tiles;
-        const int iters = (wunit ? 2 : 1) * KB;
-        mbar_wait(smem_u32(&bars->tmem_empty[as]), aphase ^ 1u);
-        tc_fence_after();
-        const uint32_t acc = tmem_base + (uint32_t)(as * ACC_COLS);
-        for (int it = 0; it < iters; ++it) {
-          mbar_wait(smem_u32(&bars->full[stage]), phase);
-          tc_fence_after();
-          const uint32_t sa = smem_u32(smem + stage * kStageBytes);
-          const uint64_t dA0 = make_smem_desc(sa + 0 * kPlaneTileBytes);
-          const uint64_t dA1 = make_smem_desc(sa + 1 * kPlaneTileBytes);
-          const uint64_t dB0 = make_smem_desc(sa + 2 * kPlaneTileBytes);
-          const uint64_t dB1 = make_smem_desc(sa + 3 * kPlaneTileBytes);
+    } else if (warp == 1) {
+      // =================================== MMA issuer (one lane of the leader CTA) ==============
+      if (leader && elect_one()) {
+        int stage = 0; uint32_t phase = 0;
+        int as = 0; uint32_t aphase = 0;
+        for (int u = cluster_id; u < n_units; u += n_clusters) {
+          const bool wunit = a.with_response && u < n_tiles;
+          const int n_seg = (wunit ? 2 : 1) * KB / seg_kb;
+          for (int sg = 0; sg < n_seg; ++sg) {
+            mbar_wait(smem_u32(&bars->tmem_empty[as]), aphase ^ 1u);
+            tc_fence_after();
+            const uint32_t acc = tmem_base + (uint32_t)(as * ACC_COLS);
+            for (int it = 0; it < seg_kb; ++it) {
+              mbar_wait(smem_u32(&bars->full[stage]), phase);
+              tc_fence_after();
+              const uint32_t sa = smem_u32(smem + stage * kStageBytes);
+              const uint64_t dA0 = make_smem_desc(sa + 0 * kPlaneTileBytes);
+              const uint64_t dA1 = make_smem_desc(sa + 1 * kPlaneTileBytes);
+              const uint64_t dB0 = make_smem_desc(sa + 2 * kPlaneTileBytes);
+              const uint64_t dB1 = make_smem_desc(sa + 3 * kPlaneTileBytes);
 #pragma unroll
-          for (int k = 0; k < kBK / 16; ++k) {
-            const uint64_t ko = (uint64_t)(k * 2);     // 16 elements * 2 B = 32 B -> >>4 = 2
-            umma_f16<CG>(acc, dA0 + ko, dB0 + ko, IDESC, (it | k) ? 1u : 0u);
-            umma_f16<CG>(acc, dA0 + ko, dB1 + ko, IDESC, 1u);
-            umma_f16<CG>(acc, dA1 + ko, dB0 + ko, IDESC, 1u);
+              for (int k = 0; k < kBK / 16; ++k) {
+                const uint64_t ko = (uint64_t)(k * 2);     // 16 elements * 2 B = 32 B -> >>4 = 2
+                // small cross terms first, the dominant hi*hi product last
+                umma_f16<CG>(acc, dA0 + ko, dB1 + ko, IDESC, (it | k) ? 1u : 0u);
+                umma_f16<CG>(acc, dA1 + ko, dB0 + ko, IDESC, 1u);
+                umma_f16<CG>(acc, dA0 + ko, dB0 + ko, IDESC, 1u);
+              }
+              umma_commit<CG>(smem_u32(&bars->empty[stage]));   // smem slot free when these MMAs retire
+              if (++stage == kStages) { stage = 0; phase ^= 1u; }
+            }
+            umma_commit<CG>(smem_u32(&bars->tmem_full[as]));     // segment accumulator complete
+            if (++as == 2) { as = 0; aphase ^= 1u; }
           }
-          umma_commit<CG>(smem_u32(&bars->empty[stage]));     // smem slot free when these MMAs retire
-          if (++stage == kStages) { stage = 0; phase ^= 1u; }
         }
-        umma_commit<CG>(smem_u32(&bars->tmem_full[as]));       // accumulator complete
-        if (++as == 2) { as = 0; aphase ^= 1u; }
       }
     }
-  } else if (warp >= 4) {
-    // ===================================== epilogue warps (4 per CTA) ===========================
+  } else {
+    // ===================================== consumer warps (8 per CTA) ===========================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsConsumer));
+    const int cw = warp - 4;
     const int q = warp & 3;                       // TMEM lane quarter this warp may read
+    const int hh = cw >> 2;                       // which half of the accumulator columns
     const Sp2Coef cf = a.ctrl->coef;
     int as = 0; uint32_t aphase = 0;
     for (int u = cluster_id; u < n_units; u += n_clusters) {
       const bool wunit = a.with_response && u < n_tiles;
       const int2 tij = a.tiles[wunit ? u : (a.with_response ? u - n_tiles : u)];
+      const int n_seg = (wunit ? 2 : 1) * KB / seg_kb;
+      float sums[WCOLS];
+      for (int sg = 0; sg < n_seg; ++sg) {
+        mbar_wait(smem_u32(&bars->tmem_full[as]), aphase);
+        tc_fence_after();
+        const uint32_t tcol = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * ACC_COLS + hh * WCOLS);
+        if (sg == 0) {
+#pragma unroll
+          for (int ch = 0; ch < NCH; ++ch) {
+            uint32_t v[32];
+            tmem_ld32(tcol + ch * 32, v);
+#pragma unroll
+            for (int i = 0; i < 32; ++i) sums[ch * 32 + i] = __uint_as_float(v[i]);
+          }
+        } else {
+#pragma unroll
+          for (int ch = 0; ch < NCH; ++ch) {
+            uint32_t v[32];
+            tmem_ld32(tcol + ch * 32, v);
+#pragma unroll
+            for (int i = 0; i < 32; ++i) sums[ch * 32 + i] += __uint_as_float(v[i]);
+          }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+          if constexpr (CG == 2) mbar_arrive_cluster(smem_u32(&bars->tmem_empty[as]), 0);
+          else mbar_arrive(smem_u32(&bars->tmem_empty[as]));
+        }
+        if (++as == 2) { as = 0; aphase ^= 1u; }
+      }
+      // ---- fused epilogue from the register sums
       const int pl = wunit ? 2 : 0;
       const float a1hi = wunit ? cf.a1z_hi : cf.a1y_hi, a1lo = wunit ? cf.a1z_lo : cf.a1y_lo;
       const float a2 = wunit ? cf.a2z : cf.a2y;
-      const __half* __restrict__ in_h = a.in[pl];
-      const __half* __restrict__ in_m = a.in[pl + 1];
-      __half* __restrict__ out_h = a.out[pl];
-      __half* __restrict__ out_m = a.out[pl + 1];
       const int gi = tij.x * TILE + (int)rank * kRows + q * 32 + lane;   // global row of this thread
-      const int j0 = tij.y * TILE;
-      const size_t npad = (size_t)a.npad;
-
-      mbar_wait(smem_u32(&bars->tmem_full[as]), aphase);
-      tc_fence_after();
-      double tr = 0.0, fro = 0.0, tracc = 0.0;
-      float mx = 0.f;
-#pragma unroll 1
-      for (int ch = 0; ch < ACC_COLS / 32; ++ch) {
-        uint32_t v[32];
-        __syncwarp();
-        tmem_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * ACC_COLS + ch * 32), v);
-        if (ch == ACC_COLS / 32 - 1) {            // accumulator fully read: hand the buffer back
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) {
-            if constexpr (CG == 2) mbar_arrive_cluster(smem_u32(&bars->tmem_empty[as]), 0);
-            else mbar_arrive(smem_u32(&bars->tmem_empty[as]));
-          }
-        }
-        const int gj0 = j0 + ch * 32;
-        // gi = 32-aligned base + lane and gj0 is 32-aligned, so both tests are warp-uniform
-        if (gj0 + 31 < gi) continue;              // chunk entirely below the diagonal: mirrored by its transpose
-        const bool full = gj0 > gi;               // chunk entirely above the diagonal
-        uint4 oh[4], om[4];
-        const uint4* ph = reinterpret_cast<const uint4*>(in_h + (size_t)gi * npad + gj0);
-        const uint4* pm = reinterpret_cast<const uint4*>(in_m + (size_t)gi * npad + gj0);
+      const bool shift_row = !wunit && gi < a.n;        // zero padding stays zero
+      const float dsh_hi = shift_row ? cf.dsh_hi : 0.f, dsh_lo = shift_row ? cf.dsh_lo : 0.f;
+      const int j0 = tij.y * TILE + hh * WCOLS;
+      EpiPartials P; P.tr = 0.0; P.fro = 0.0; P.tracc = 0.0; P.mx = 0.f;
 #pragma unroll
-        for (int w = 0; w < 4; ++w) { oh[w] = ld_global_v4(ph + w); om[w] = ld_global_v4(pm + w); }
-        uint32_t nh[16], nm[16];                  // packed pairs of new hi / lo halves
-        float fsum = 0.f;
-#pragma unroll
-        for (int pr = 0; pr < 16; ++pr) {
-          const uint32_t wh = u4_word(oh[pr >> 2], pr & 3), wm = u4_word(om[pr >> 2], pr & 3);
-          __half h0, m0, h1, m1;
-          const float old0 = __half2float(__ushort_as_half((unsigned short)(wh & 0xffffu))) +
-                             __half2float(__ushort_as_half((unsigned short)(wm & 0xffffu)));
-          const float old1 = __half2float(__ushort_as_half((unsigned short)(wh >> 16))) +
-                             __half2float(__ushort_as_half((unsigned short)(wm >> 16)));
-          const float s0 = sp2_epilogue_elem(old0, __uint_as_float(v[2 * pr]), a1hi, a1lo, a2, h0, m0);
-          const float s1 = sp2_epilogue_elem(old1, __uint_as_float(v[2 * pr + 1]), a1hi, a1lo, a2, h1, m1);
-          nh[pr] = (uint32_t)__half_as_ushort(h0) | ((uint32_t)__half_as_ushort(h1) << 16);
-          nm[pr] = (uint32_t)__half_as_ushort(m0) | ((uint32_t)__half_as_ushort(m1) << 16);
-          const int gja = gj0 + 2 * pr, gjb = gja + 1;
-          const float wa = (gja > gi) ? 2.f : (gja == gi ? 1.f : 0.f);
-          const float wb = (gjb > gi) ? 2.f : (gjb == gi ? 1.f : 0.f);
-          fsum = fmaf(wa * s0, s0, fsum);
-          fsum = fmaf(wb * s1, s1, fsum);
-          if (gja == gi) { tr += (double)s0; tracc += (double)__uint_as_float(v[2 * pr]); }
-          if (gjb == gi) { tr += (double)s1; tracc += (double)__uint_as_float(v[2 * pr + 1]); }
-          if (gja >= gi) mx = (fabsf(s0) > mx || s0 != s0) ? fabsf(s0) : mx;
-          if (gjb >= gi) mx = (fabsf(s1) > mx || s1 != s1) ? fabsf(s1) : mx;
-        }
-        fro += (double)fsum;
-        unsigned short* oh16 = reinterpret_cast<unsigned short*>(out_h);
-        unsigned short* om16 = reinterpret_cast<unsigned short*>(out_m);
-        if (full) {
-          uint4* qh = reinterpret_cast<uint4*>(out_h + (size_t)gi * npad + gj0);
-          uint4* qm = reinterpret_cast<uint4*>(out_m + (size_t)gi * npad + gj0);
-#pragma unroll
-          for (int w = 0; w < 4; ++w) {
-            qh[w] = make_uint4(nh[4 * w], nh[4 * w + 1], nh[4 * w + 2], nh[4 * w + 3]);
-            qm[w] = make_uint4(nm[4 * w], nm[4 * w + 1], nm[4 * w + 2], nm[4 * w + 3]);
-          }
-#pragma unroll
-          for (int pr = 0; pr < 16; ++pr) {       // mirrored image: lanes = consecutive rows -> 64 B per store
-            oh16[(size_t)(gj0 + 2 * pr) * npad + gi] = (unsigned short)(nh[pr] & 0xffffu);
-            om16[(size_t)(gj0 + 2 * pr) * npad + gi] = (unsigned short)(nm[pr] & 0xffffu);
-            oh16[(size_t)(gj0 + 2 * pr + 1) * npad + gi] = (unsigned short)(nh[pr] >> 16);
-            om16[(size_t)(gj0 + 2 * pr + 1) * npad + gi] = (unsigned short)(nm[pr] >> 16);
-          }
-        } else {                                  // the chunk that holds the diagonal: element-wise, gj >= gi only
-#pragma unroll
-          for (int pr = 0; pr < 16; ++pr) {
-#pragma unroll
-            for (int e = 0; e < 2; ++e) {
-              const int gj = gj0 + 2 * pr + e;
-              const unsigned short hv = (unsigned short)(e ? (nh[pr] >> 16) : (nh[pr] & 0xffffu));
-              const unsigned short mv = (unsigned short)(e ? (nm[pr] >> 16) : (nm[pr] & 0xffffu));
-              if (gj >= gi) { oh16[(size_t)gi * npad + gj] = hv; om16[(size_t)gi * npad + gj] = mv; }
-              if (gj > gi) { oh16[(size_t)gj * npad + gi] = hv; om16[(size_t)gj * npad + gi] = mv; }
-            }
-          }
-        }
-      }
+      for (int ch = 0; ch < NCH; ++ch)
+        epilogue_chunk(&sums[ch * 32], gi, j0 + ch * 32, (size_t)a.npad, a.in[pl], a.in[pl + 1], a.out[pl], a.out[pl + 1],
+                       a1hi, a1lo, a2, dsh_hi, dsh_lo, P);
       // warp partial -> slot (fixed shuffle tree: deterministic)
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {
-        tr += __shfl_xor_sync(0xffffffffu, tr, o);
-        fro += __shfl_xor_sync(0xffffffffu, fro, o);
-        tracc += __shfl_xor_sync(0xffffffffu, tracc, o);
-        const float qv = __shfl_xor_sync(0xffffffffu, mx, o);
-        mx = (qv > mx || qv != qv) ? qv : mx;
+        P.tr += __shfl_xor_sync(0xffffffffu, P.tr, o);
+        P.fro += __shfl_xor_sync(0xffffffffu, P.fro, o);
+        P.tracc += __shfl_xor_sync(0xffffffffu, P.tracc, o);
+        const float qv = __shfl_xor_sync(0xffffffffu, P.mx, o);
+        P.mx = (qv > P.mx || qv != qv) ? qv : P.mx;
       }
       if (lane == 0) {
-        Sp2Slot s; s.tr = tr; s.fro = fro; s.tracc = wunit ? 0.0 : tracc; s.mx = mx; s.pad = 0.f;
-        a.slots[((size_t)u * CG + rank) * 4 + q] = s;
+        Sp2Slot s; s.tr = P.tr; s.fro = P.fro; s.tracc = wunit ? 0.0 : P.tracc; s.mx = P.mx; s.pad = 0.f;
+        a.slots[((size_t)u * CG + rank) * kConsumerWarps + cw] = s;
       }
-      if (++as == 2) { as = 0; aphase ^= 1u; }
     }
   }
 
@@ -451,7 +497,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
   if (warp == 2) tmem_dealloc<CG>(tmem_base, TMEM_COLS);
 
-  const int per_unit = CG * 4;
+  const int per_unit = CG * kConsumerWarps;
   const int n_z = a.with_response ? n_tiles * per_unit : 0;
   layer_tail(a.ctrl, a.slots, n_tiles * per_unit, n_z, n_z, gridDim.x, &bars->is_last, red);
 }
@@ -501,7 +547,8 @@ __global__ void __launch_bounds__(256) k_layer_simt(Sp2LayerArgs a) {
   if (gj >= gi) {
     const float old = __half2float(a.in[pl][gi * npad + gj]) + __half2float(a.in[pl + 1][gi * npad + gj]);
     __half nh, nm;
-    const float s = sp2_epilogue_elem(old, acc, a1hi, a1lo, a2, nh, nm);
+    const bool dg = (gj == gi) && cls == 0 && gi < a.n;
+    const float s = sp2_epilogue_elem(old, acc, a1hi, a1lo, a2, dg ? cf.dsh_hi : 0.f, dg ? cf.dsh_lo : 0.f, nh, nm);
     a.out[pl][gi * npad + gj] = nh; a.out[pl + 1][gi * npad + gj] = nm;
     if (gj > gi) { a.out[pl][gj * npad + gi] = nh; a.out[pl + 1][gj * npad + gi] = nm; }
     fro = (gj > gi ? 2.0 : 1.0) * (double)s * (double)s;
@@ -541,7 +588,7 @@ int sp2_layer_slots(int npad, int cta_group, int with_response, int engine) {
     return nb * (nb + 1) / 2 * (with_response ? 2 : 1);
   }
   const int nt = npad / (128 * cta_group);
-  return nt * (nt + 1) / 2 * cta_group * 4 * (with_response ? 2 : 1);
+  return nt * (nt + 1) / 2 * cta_group * kConsumerWarps * (with_response ? 2 : 1);
 }
 
 cudaError_t sp2_layer_configure() {

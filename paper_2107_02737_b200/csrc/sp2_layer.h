@@ -14,10 +14,11 @@ struct alignas(64) Sp2LayerArgs {
   Sp2Ctrl* ctrl;
   Sp2Slot* slots;        // [z-class slots][y-class slots]
   const int2* tiles;     // (ti, tj), ti <= tj, upper-triangular tile list in L2-friendly order
+  int n;                 // true dimension (rows/cols >= n are zero padding and stay zero)
   int npad;              // padded dimension (multiple of the tile edge)
   int n_tiles;           // number of upper-triangular tiles
   int with_response;
-  int pad;
+  int seg_kb;            // k-blocks (of 64) per in-TMEM accumulation segment; divides npad/64
 };
 
 size_t sp2_layer_smem_bytes();

@@ -362,13 +362,13 @@ __global__ void __launch_bounds__(256) k_trivial(Sp2Ctrl* c, TO* __restrict__ D,
 
 __global__ void k_init(Sp2Ctrl* c, int N, int n_occ, int npad, int with_response, int max_layers,
                        int user_bounds, double eps_min, double eps_max, double tol,
-                       int forced_layers, unsigned long long forced_signs) {
+                       int forced_layers, unsigned long long forced_signs, int no_recentre) {
   // one thread: reset the whole control block
   Sp2Ctrl z;
   memset(&z, 0, sizeof(z));
   z.N = N; z.n_occ = n_occ; z.npad = npad; z.with_response = with_response;
   z.max_layers = max_layers; z.user_bounds = user_bounds; z.user_eps_min = eps_min; z.user_eps_max = eps_max;
-  z.tol = tol; z.forced_layers = forced_layers; z.forced_signs = forced_signs;
+  z.tol = tol; z.forced_layers = forced_layers; z.forced_signs = forced_signs; z.no_recentre = no_recentre;
   *c = z;
 }
 
@@ -381,9 +381,9 @@ __global__ void k_init(Sp2Ctrl* c, int N, int n_occ, int npad, int with_response
 
 void sp2_launch_init(Sp2Ctrl* c, int N, int n_occ, int npad, int with_response, int max_layers,
                      int user_bounds, double eps_min, double eps_max, double tol, int forced_layers,
-                     unsigned long long forced_signs, cudaStream_t s) {
+                     unsigned long long forced_signs, int no_recentre, cudaStream_t s) {
   k_init<<<1, 1, 0, s>>>(c, N, n_occ, npad, with_response, max_layers, user_bounds, eps_min, eps_max, tol,
-                         forced_layers, forced_signs);
+                         forced_layers, forced_signs, no_recentre);
 }
 
 int sp2_bounds_blocks(int N) { return (N + 7) / 8; }
