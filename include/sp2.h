@@ -94,7 +94,9 @@ typedef struct {
   double idem_est;                   /* last idempotency estimate e_L = tr X_L - tr X_L^2 */
   double eps_min, eps_max;           /* spectral bounds used by the input layer */
   float gpu_ms;                      /* device time of the call (CUDA events on `stream`), blocking calls only */
+  float layers_ms;                   /* device time of the layer-kernel launches alone (a3-a5), blocking calls only */
   int kernel_launches;               /* kernels of this library launched by the call */
+  int reserved2;
 } sp2_result_t;
 
 /* Bytes of device workspace needed for problems up to n_max (flags: SP2_WITH_*). 0 if n_max <= 0. */

@@ -17,6 +17,7 @@ from .sp2_oracle import (  # noqa: F401
     density_eigh,
     density_from_eigenpairs,
     response_closed_form,
+    response_closed_form_sampled,
     response_finite_difference,
     sp2_spectrum_simulator,
 )

@@ -48,6 +48,7 @@ __all__ = [
     "density_eigh",
     "density_from_eigenpairs",
     "response_closed_form",
+    "response_closed_form_sampled",
     "response_finite_difference",
     "sp2_spectrum_simulator",
 ]
@@ -260,6 +261,27 @@ def response_closed_form(Q, lam, n_occ, H1):
     M[np.ix_(occ, un)] = blk
     M[np.ix_(un, occ)] = blk.T
     return Q @ M @ Q.T
+
+
+def response_closed_form_sampled(Q, lam, n_occ, H1, rows, cols):
+    """Entries D1[rows[k], cols[k]] of ``response_closed_form`` without forming the N x N result
+    (sampled parity checks at full size).  Same formula: with C_o / C_u the occupied / unoccupied
+    eigenvector blocks and B = (C_o^T H1 C_u) / (lam_o - lam_u),
+        D1 = C_o B C_u^T + C_u B^T C_o^T,
+    so  D1_ij = sum_{o,u} B_ou (C_o[i,o] C_u[j,u] + C_u[i,u] C_o[j,o]).
+    """
+    Q = np.asarray(Q, dtype=np.float64)
+    lam = np.asarray(lam, dtype=np.float64)
+    H1 = np.asarray(H1, dtype=np.float64)
+    order = np.argsort(lam, kind="stable")
+    occ, un = order[:n_occ], order[n_occ:]
+    Co, Cu = Q[:, occ], Q[:, un]
+    B = (Co.T @ H1 @ Cu) / (lam[occ][:, None] - lam[un][None, :])
+    rows = np.asarray(rows)
+    cols = np.asarray(cols)
+    left = Co[rows, :] @ B                   # (k, n_un)
+    right = Co[cols, :] @ B
+    return np.einsum("ku,ku->k", left, Cu[cols, :]) + np.einsum("ku,ku->k", right, Cu[rows, :])
 
 
 def response_finite_difference(H, H1, n_occ, eps=1e-5):

@@ -110,7 +110,8 @@ struct sp2_handle_s {
   int cur_n, cur_npad, cur_cg, cur_resp, cur_seg;
   Sp2LayerArgs args[2];          // parity 0: buffer 0 -> 1, parity 1: buffer 1 -> 0
   std::vector<int2> tiles_host;
-  cudaEvent_t ev0, ev1;
+  cudaEvent_t ev0, ev1, evl0, evl1;
+  int time_layers;               // record evl0/evl1 around the layer launches of the next solve
   sp2_result_t* h_result;        // pinned
   int last_cuda_error;
   unsigned long long launches;
@@ -241,11 +242,13 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const void* H1, sp2_dt
     if (resp) { sp2_launch_rescale(H1, in_dt, ldh, c, 1, h->plane(2, 0), h->plane(3, 0), npad, h->slots2(), s); ++launches; }
     sp2_launch_rescale(H, in_dt, ldh, c, 0, h->plane(0, 0), h->plane(1, 0), npad, h->slots(), s); ++launches;
     sp2_launch_ctrl0(c, h->slots(), h->slots2(), sp2_rescale_blocks(npad), s); ++launches;
+    if (h->time_layers) SP2_CUDA(h, cudaEventRecord(h->evl0, s));
     for (int n = 0; n < max_layers; ++n) {
       cudaError_t e = sp2_launch_layer(h->args[n & 1], o.engine, h->cur_cg, h->num_sms, s);
       if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
       ++launches;
     }
+    if (h->time_layers) SP2_CUDA(h, cudaEventRecord(h->evl1, s));
     __half* planes[8] = {h->plane(0, 0), h->plane(1, 0), h->plane(0, 1), h->plane(1, 1),
                          h->plane(resp ? 2 : 0, 0), h->plane(resp ? 3 : 1, 0), h->plane(resp ? 2 : 0, 1), h->plane(resp ? 3 : 1, 1)};
     sp2_launch_finalise(c, planes, npad, H, in_dt, ldh, D, resp ? D1 : nullptr, out_dt, ldd, N, h->fslots(),
@@ -286,7 +289,10 @@ sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const void* H1, sp2_d
     }
   }
   int launches = 0;
+  const bool layers_timed = !(N_occ == 0 || N_occ == N);
+  h->time_layers = 1;
   st = enqueue_solve(h, dH, dH1, in_dt, dld_in, N, N_occ, tol, dD, dD1, out_dt, dld_out, 0, s, &launches);
+  h->time_layers = 0;
   if (st != SP2_OK) return st;
   if (host_buffers) {
     SP2_CUDA(h, cudaMemcpy2DAsync(D, (size_t)ldd * out_sz, dD, (size_t)N * out_sz, (size_t)N * out_sz, N,
@@ -302,6 +308,8 @@ sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const void* H1, sp2_d
   SP2_CUDA(h, cudaEventElapsedTime(&ms, h->ev0, h->ev1));
   sp2_result_t r = *h->h_result;
   r.gpu_ms = ms;
+  r.layers_ms = 0.f;
+  if (layers_timed) SP2_CUDA(h, cudaEventElapsedTime(&r.layers_ms, h->evl0, h->evl1));
   r.kernel_launches = launches;
   if (out) *out = r;
   return (sp2_status_t)r.status;
@@ -340,7 +348,9 @@ sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_work
   if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) { delete h; return SP2_ERR_CUDA; }
   h->encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(fn);
   if (sp2_layer_configure() != cudaSuccess) { delete h; return SP2_ERR_CUDA; }
-  if (cudaEventCreate(&h->ev0) != cudaSuccess || cudaEventCreate(&h->ev1) != cudaSuccess) { delete h; return SP2_ERR_CUDA; }
+  if (cudaEventCreate(&h->ev0) != cudaSuccess || cudaEventCreate(&h->ev1) != cudaSuccess ||
+      cudaEventCreate(&h->evl0) != cudaSuccess || cudaEventCreate(&h->evl1) != cudaSuccess) { delete h; return SP2_ERR_CUDA; }
+  h->time_layers = 0;
   if (cudaMallocHost(reinterpret_cast<void**>(&h->h_result), sizeof(sp2_result_t) * kRingCap) != cudaSuccess) {
     delete h; return SP2_ERR_CUDA;
   }
@@ -352,6 +362,8 @@ sp2_status_t sp2_destroy(sp2_handle_t h) {
   if (!h) return SP2_ERR_INVALID_ARG;
   cudaEventDestroy(h->ev0);
   cudaEventDestroy(h->ev1);
+  cudaEventDestroy(h->evl0);
+  cudaEventDestroy(h->evl1);
   cudaFreeHost(h->h_result);
   delete h;
   return SP2_OK;

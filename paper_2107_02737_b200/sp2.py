@@ -58,7 +58,7 @@ class Sp2Result(C.Structure):
         ("stop_reason", C.c_int), ("reserved", C.c_int),
         ("tr_d", C.c_double), ("tr_dh", C.c_double), ("tr_d1", C.c_double),
         ("idem_est", C.c_double), ("eps_min", C.c_double), ("eps_max", C.c_double),
-        ("gpu_ms", C.c_float), ("kernel_launches", C.c_int),
+        ("gpu_ms", C.c_float), ("layers_ms", C.c_float), ("kernel_launches", C.c_int), ("reserved2", C.c_int),
     ]
 
     def as_dict(self):
@@ -66,7 +66,7 @@ class Sp2Result(C.Structure):
             "+" if (self.sign_mask[n >> 6] >> (n & 63)) & 1 else "-" for n in range(self.layers))
         return dict(status=self.status, layers=self.layers, signs=signs, stop_reason=self.stop_reason,
                     tr_d=self.tr_d, tr_dh=self.tr_dh, tr_d1=self.tr_d1, idem_est=self.idem_est,
-                    eps_min=self.eps_min, eps_max=self.eps_max, gpu_ms=self.gpu_ms,
+                    eps_min=self.eps_min, eps_max=self.eps_max, gpu_ms=self.gpu_ms, layers_ms=self.layers_ms,
                     kernel_launches=self.kernel_launches)
 
 

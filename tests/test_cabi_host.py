@@ -1,0 +1,93 @@
+"""CPU-only checks of the boundary: the C-ABI library loads, exports every symbol that
+include/sp2.h declares, and its host-side logic (sizes, status strings, argument checks that
+need no device) behaves.  No compute call is made here."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "sp2.h")
+
+
+@pytest.fixture(scope="module")
+def sp2():
+    from paper_2107_02737_b200 import build
+
+    build.build()                       # nvcc cross-compiles without a GPU
+    from paper_2107_02737_b200 import sp2 as mod
+
+    return mod
+
+
+def _declared_symbols():
+    text = open(HEADER).read()
+    return sorted(set(re.findall(r"SP2_API\s+[\w\s\*]+?\b(sp2_\w+)\s*\(", text)))
+
+
+def test_header_declares_the_calls_north_star_names():
+    names = _declared_symbols()
+    for must in ("sp2_density", "sp2_response", "sp2_sequence_begin", "sp2_sequence_step", "sp2_sequence_end",
+                 "sp2_workspace_bytes", "sp2_create", "sp2_destroy"):
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol(sp2):
+    names = _declared_symbols()
+    assert len(names) >= 17
+    for n in names:
+        assert hasattr(sp2.lib, n), f"{n} declared in include/sp2.h but not exported"
+    assert sorted(sp2.EXPORTS) == names          # the Python binding covers the whole header
+
+
+def test_struct_layouts_match_the_header(sp2):
+    # sizes implied by the C declarations (natural alignment, LP64)
+    assert ctypes.sizeof(sp2.Sp2Options) == 56
+    assert ctypes.sizeof(sp2.Sp2Result) == 96
+    assert sp2.Sp2Result.tr_d.offset == 32 and sp2.Sp2Result.gpu_ms.offset == 80
+
+
+def test_workspace_bytes_and_status_strings(sp2):
+    assert sp2.workspace_bytes(0) == 0 and sp2.workspace_bytes(-5) == 0
+    b1 = sp2.workspace_bytes(1024)
+    b2 = sp2.workspace_bytes(1024, sp2.SP2_WITH_RESPONSE)
+    b3 = sp2.workspace_bytes(1024, sp2.SP2_WITH_RESPONSE | sp2.SP2_WITH_HOST_STAGING)
+    plane = 1024 * 1024 * 2
+    assert b1 >= 4 * plane and b2 - b1 >= 4 * plane - 4096
+    assert b3 - b2 >= 4 * 1024 * 1024 * 8
+    # padding to the 256-wide tile: N = 6000 needs 6144^2 planes
+    assert sp2.workspace_bytes(6000) >= 4 * 6144 * 6144 * 2
+    # memory claim of DESIGN.md: N = 16384 density-only fits in ~2.2 GB of workspace
+    assert sp2.workspace_bytes(16384) < 2.3 * 2 ** 30
+    assert sp2.status_string(sp2.SP2_OK) == "ok"
+    assert "degenerate" in sp2.status_string(sp2.SP2_ERR_DEGENERATE)
+    assert "unknown" in sp2.status_string(99)
+
+
+def test_calls_fail_loudly_without_a_handle_or_device(sp2):
+    lib = sp2.lib
+    h = ctypes.c_void_p()
+    assert lib.sp2_create(ctypes.byref(h), 128, 0, None, 0) == sp2.SP2_ERR_WORKSPACE
+    assert lib.sp2_create(None, 128, 0, None, 0) == sp2.SP2_ERR_INVALID_ARG
+    assert lib.sp2_destroy(None) == sp2.SP2_ERR_INVALID_ARG
+    assert lib.sp2_set_options(None, None) == sp2.SP2_ERR_INVALID_ARG
+    assert lib.sp2_launch_count(None) == 0
+    import torch
+
+    if not torch.cuda.is_available():
+        with pytest.raises(RuntimeError):          # the product path has no CPU fallback
+            sp2.Sp2Handle(128)
+
+
+def test_product_path_does_not_touch_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2107_02737_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith(".py"):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2107_02737_b200" not in src and "from paper_2107_02737_b200" not in src

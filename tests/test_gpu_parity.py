@@ -1,0 +1,311 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the float64 CPU oracle.
+
+Tolerances are BASELINE.json's north_star:
+    max|dD_ij| <= 1e-4,  |tr D - N_occ| <= 1e-3,  |d tr(DH)|/|tr(DH)| <= 1e-5,
+    max|dD1_ij| <= 1e-3 * max|D1|.
+Layer count and sign string may differ from the oracle near ties / at the rounding floor
+(reading R4); parity is on D, D1, tr D, tr(DH).
+"""
+import numpy as np
+import pytest
+
+from paper_2107_02737_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL_D, TOL_TR, TOL_E, TOL_D1 = 1e-4, 1e-3, 1e-5, 1e-3
+
+
+@pytest.fixture(scope="module")
+def torch_mod():
+    import torch
+
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def sp2(torch_mod):
+    from paper_2107_02737_b200 import sp2 as mod   # raises if libsp2_b200.so is missing: no fallback
+
+    return mod
+
+
+def _solve(sp2, torch, p, response=None, **opts):
+    cfg = p["cfg"]
+    response = cfg.response if response is None else response
+    h = sp2.Sp2Handle(p["n"], response=response)
+    if opts:
+        h.set_options(**opts)
+    H = torch.from_numpy(p["H"]).cuda()
+    if response:
+        H1 = torch.from_numpy(p["H1"]).cuda()
+        D, D1, r = h.response(H, H1, p["n_occ"])
+        out = (D.cpu().numpy().astype(np.float64), D1.cpu().numpy().astype(np.float64), r)
+    else:
+        D, r = h.density(H, p["n_occ"])
+        out = (D.cpu().numpy().astype(np.float64), None, r)
+    h.close()
+    return out
+
+
+def _check_against_oracle(p, D, D1, r, oracle):
+    n_occ = p["n_occ"]
+    H64 = p["H"].astype(np.float64)
+    ref = oracle.sp2_density(H64, n_occ, H1=None if D1 is None else p["H1"].astype(np.float64))
+    assert r["status"] == 0
+    assert np.abs(D - ref["D"]).max() <= TOL_D
+    assert abs(r["tr_d"] - n_occ) <= TOL_TR
+    assert abs(r["tr_dh"] - ref["tr_dh"]) <= TOL_E * abs(ref["tr_dh"])
+    assert np.array_equal(D, D.T)                              # bit-symmetric by construction
+    assert abs(r["layers"] - ref["layers"]) <= 6
+    k = min(r["layers"], ref["layers"]) - 6                    # early branches are not noise-driven
+    assert r["signs"][:k] == ref["signs"][:k]
+    assert r["eps_min"] == pytest.approx(ref["eps_min"], rel=1e-12)
+    assert r["eps_max"] == pytest.approx(ref["eps_max"], rel=1e-12)
+    if D1 is not None:
+        assert np.abs(D1 - ref["D1"]).max() <= TOL_D1 * np.abs(ref["D1"]).max()
+        assert np.array_equal(D1, D1.T)
+        assert abs(r["tr_d1"]) <= 1e-3 * np.abs(ref["D1"]).max() * len(D1) ** 0.5
+    return ref
+
+
+# ------------------------------------------------------------------------------- configs 1, 2
+def test_config1_tiny_n128(sp2, torch_mod):
+    import oracle
+
+    p = inputs.make_problem(inputs.CONFIGS[1])
+    D, D1, r = _solve(sp2, torch_mod, p)
+    _check_against_oracle(p, D, D1, r, oracle)
+    D_eig, _ = oracle.density_eigh(p["H"], p["n_occ"])          # the definition, not only the loop
+    assert np.abs(D - D_eig).max() <= TOL_D
+
+
+def test_config2_n1024_response(sp2, torch_mod):
+    import oracle
+
+    p = inputs.make_problem(inputs.CONFIGS[2])
+    D, D1, r = _solve(sp2, torch_mod, p)
+    _check_against_oracle(p, D, D1, r, oracle)
+    D1_pt = oracle.response_closed_form(p["Q"], p["lam"], p["n_occ"], p["H1"])
+    assert np.abs(D1 - D1_pt).max() <= TOL_D1 * np.abs(D1_pt).max()
+
+
+@pytest.mark.parametrize("cta_group", [1, 2])
+@pytest.mark.parametrize("n, base, response", [(300, 2, True), (77, 1, False), (520, 3, False), (641, 4, True)])
+def test_ragged_sizes_both_tile_shapes(sp2, torch_mod, n, base, response, cta_group):
+    """Sizes that are not tile multiples (zero padding must stay inert), several tiles, f32 and f64
+    inputs, 1/2 and 2/3 filling, both CTA-group code paths."""
+    import oracle
+
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[base], n), want_h1=response)
+    D, D1, r = _solve(sp2, torch_mod, p, response=response, cta_group=cta_group)
+    _check_against_oracle(p, D, D1, r, oracle)
+
+
+def test_segment_lengths_and_simt_scaffold_agree(sp2, torch_mod):
+    import oracle
+
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[4], 768))
+    ref = None
+    for opts in (dict(seg_kb=4), dict(seg_kb=2), dict(seg_kb=1), dict(engine=sp2.SP2_ENGINE_SIMT_DEBUG)):
+        D, D1, r = _solve(sp2, torch_mod, p, **opts)
+        ref = ref or _check_against_oracle(p, D, D1, r, oracle)
+        assert np.abs(D - ref["D"]).max() <= TOL_D
+        assert np.abs(D1 - ref["D1"]).max() <= TOL_D1 * np.abs(ref["D1"]).max()
+
+
+def test_runs_are_bitwise_reproducible(sp2, torch_mod):
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[2], 900))
+    a = _solve(sp2, torch_mod, p)
+    b = _solve(sp2, torch_mod, p)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    assert a[2]["signs"] == b[2]["signs"] and a[2]["tr_dh"] == b[2]["tr_dh"]
+
+
+# ------------------------------------------------------------------------------- one layer
+@pytest.mark.parametrize("sign", ["+", "-"])
+def test_single_layer_against_float64_product(sp2, torch_mod, sign):
+    """One forced layer: X_1 = X_0^2 or 2 X_0 - X_0^2 in float64 from the oracle's input layer
+    versus the planes the kernel wrote (c I + (hi + lo) 2^-t).  Error budget: FP16 hi/lo split
+    2^-22 of max|Y| per element twice (input split, output split) plus FP32 accumulation."""
+    import oracle
+
+    torch = torch_mod
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[2], 384), want_h1=True)
+    h = sp2.Sp2Handle(p["n"], response=True)
+    h.set_options(forced_signs=sign)
+    H = torch.from_numpy(p["H"]).cuda()
+    H1 = torch.from_numpy(p["H1"]).cuda()
+    h.response(H, H1, p["n_occ"])
+    n = p["n"]
+    planes = [h.debug_plane(k) for k in range(4)]
+    shift = planes[0][2]
+    Y = (planes[0][0].double() + planes[1][0].double()).cpu().numpy()[:n, :n] * 2.0 ** (-planes[0][1])
+    Z = (planes[2][0].double() + planes[3][0].double()).cpu().numpy()[:n, :n] * 2.0 ** (-planes[2][1])
+    pad = (planes[0][0].double().abs() + planes[1][0].double().abs()).cpu().numpy()
+    assert pad[n:, :].max() == 0.0 and pad[:, n:].max() == 0.0          # padding stays exactly zero
+    h.close()
+    lo, hi = oracle.gershgorin_bounds(p["H"])
+    X0 = oracle.rescale_to_unit_interval(p["H"], lo, hi)
+    Z0 = -p["H1"] / (hi - lo)
+    W = X0 @ Z0 + Z0 @ X0
+    X1 = X0 @ X0 if sign == "+" else 2 * X0 - X0 @ X0
+    Z1 = W if sign == "+" else 2 * Z0 - W
+    X1_gpu = shift * np.eye(n) + Y
+    assert np.abs(X1_gpu - X1).max() <= 8 * 2.0 ** -22 * np.abs(X1 - np.diag(np.diag(X1))).max() + 2e-9
+    assert np.abs(Z - Z1).max() <= 8 * 2.0 ** -22 * np.abs(Z1).max()
+    assert np.array_equal(Y, Y.T) and np.array_equal(Z, Z.T)
+
+
+# ------------------------------------------------------------------------------- closed forms
+def test_tiny_closed_forms(sp2, torch_mod):
+    """tests/golden/closed_forms.txt cases A (diagonal 4x4) and B (2x2, converged on entry, with response)."""
+    torch = torch_mod
+    h = sp2.Sp2Handle(8, response=True)
+    HA = torch.diag(torch.tensor([-2.0, -1.0, 1.0, 2.0], dtype=torch.float64)).cuda()
+    D, r = h.density(HA, 2)
+    assert r["status"] == 0 and (r["eps_min"], r["eps_max"]) == (-2.0, 2.0)
+    np.testing.assert_allclose(D.cpu().numpy(), np.diag([1.0, 1.0, 0.0, 0.0]), atol=1e-6)
+    assert r["tr_dh"] == pytest.approx(-3.0, abs=1e-5)
+    assert r["signs"].startswith("-++")                          # tie at n = 0 goes to '-'
+    HB = torch.tensor([[0.0, 1.0], [1.0, 0.0]], dtype=torch.float64).cuda()
+    H1 = torch.tensor([[1.0, 0.0], [0.0, -1.0]], dtype=torch.float64).cuda()
+    D, D1, r = h.response(HB, H1, 1)
+    np.testing.assert_allclose(D.cpu().numpy(), [[0.5, -0.5], [-0.5, 0.5]], atol=1e-6)
+    np.testing.assert_allclose(D1.cpu().numpy(), [[-0.5, 0.0], [0.0, 0.5]], atol=1e-6)
+    assert r["tr_dh"] == pytest.approx(-1.0, abs=1e-6) and r["layers"] <= 2
+    h.close()
+
+
+# ------------------------------------------------------------------------------- edge cases
+def test_edge_cases_and_error_statuses(sp2, torch_mod):
+    torch = torch_mod
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[1], 96))
+    n = p["n"]
+    H = torch.from_numpy(p["H"]).cuda()
+    h = sp2.Sp2Handle(128, response=True)
+    # trivial occupations answered from the definition
+    D, r = h.density(H, 0)
+    assert r["status"] == 0 and r["layers"] == 0 and float(D.abs().max()) == 0.0
+    D, r = h.density(H, n)
+    assert torch.equal(D, torch.eye(n, dtype=D.dtype, device=D.device))
+    assert r["tr_dh"] == pytest.approx(float(torch.trace(H)), rel=1e-12)
+    # H = c I: no spectral width
+    with pytest.raises(sp2.Sp2Error) as ei:
+        h.density(3.0 * torch.eye(n, dtype=torch.float64, device="cuda"), n // 2)
+    assert ei.value.status == sp2.SP2_ERR_DEGENERATE
+    # NaN / Inf in the input
+    Hn = H.clone()
+    Hn[5, 7] = float("nan")
+    with pytest.raises(sp2.Sp2Error) as ei:
+        h.density(Hn, n // 2)
+    assert ei.value.status == sp2.SP2_ERR_NONFINITE
+    Hn[5, 7] = float("inf")
+    with pytest.raises(sp2.Sp2Error) as ei:
+        h.density(Hn, n // 2)
+    assert ei.value.status == sp2.SP2_ERR_NONFINITE
+    # layer cap: status NOT_CONVERGED, D still written
+    h.set_options(max_layers=5)
+    D, r = h.density(H, p["n_occ"])
+    assert r["status"] == sp2.SP2_WARN_NOT_CONVERGED and r["layers"] == 5 and r["stop_reason"] == 4
+    assert bool(torch.isfinite(D).all())
+    h.set_options()
+    # invalid arguments
+    for bad in (lambda: h.density(H, n + 1), lambda: h.density(H, -1),
+                lambda: h.density(torch.zeros(200, 200, dtype=torch.float64, device="cuda"), 3)):
+        with pytest.raises(sp2.Sp2Error) as ei:
+            bad()
+        assert ei.value.status == sp2.SP2_ERR_INVALID_ARG
+    # response needs a response handle
+    h2 = sp2.Sp2Handle(128)
+    with pytest.raises(sp2.Sp2Error):
+        h2.response(H, H, 3)
+    h2.close()
+    # the handle still works after every error above
+    D, r = h.density(H, p["n_occ"])
+    assert r["status"] == 0 and abs(r["tr_d"] - p["n_occ"]) < TOL_TR
+    h.close()
+
+
+def test_pitch_dtypes_user_bounds_and_tol(sp2, torch_mod):
+    import oracle
+
+    torch = torch_mod
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[3], 200))    # f32 input
+    n, n_occ = p["n"], p["n_occ"]
+    ref = oracle.sp2_density(p["H"].astype(np.float64), n_occ)
+    h = sp2.Sp2Handle(256)
+    big = torch.zeros(n, n + 24, dtype=torch.float32, device="cuda")       # ld > N on input
+    big[:, :n] = torch.from_numpy(p["H"]).cuda()
+    outbig = torch.full((n, n + 8), 7.0, dtype=torch.float64, device="cuda")  # ld > N, other dtype on output
+    D, r = h.density(big[:, :n], n_occ, out=outbig[:, :n])
+    assert np.abs(D.cpu().numpy() - ref["D"]).max() <= TOL_D
+    assert float(outbig[:, n:].min()) == 7.0                              # nothing written past N
+    # exact spectral bounds from the generator: same projector, fewer layers
+    lam = p["lam"]
+    h.set_options(user_bounds=(lam.min() - 1e-3, lam.max() + 1e-3))
+    D2, r2 = h.density(big[:, :n], n_occ, out_dtype=torch.float32)
+    assert r2["layers"] < r["layers"] and np.abs(D2.double().cpu().numpy() - ref["D"]).max() <= TOL_D
+    h.set_options()
+    # tol stop rule fires earlier than the parameter-free one
+    D3, r3 = h.density(big[:, :n], n_occ, tol=1e-2)
+    assert r3["stop_reason"] == 1 and r3["layers"] <= r["layers"] and 0 <= r3["idem_est"] <= 1e-2
+    tr_x, e = h.debug_history()
+    assert len(e) == r3["layers"] + 1 and e[-1] == pytest.approx(r3["idem_est"])
+    h.close()
+
+
+def test_host_buffer_calls(sp2, torch_mod):
+    import oracle
+
+    torch = torch_mod
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[2], 260))
+    n, n_occ = p["n"], p["n_occ"]
+    ref = oracle.sp2_density(p["H"], n_occ, H1=p["H1"])
+    h = sp2.Sp2Handle(n, response=True, host_staging=True)
+    D = np.empty((n, n))
+    Dr, r = h.density_host(p["H"], n_occ, D)                       # pageable numpy buffers
+    assert np.abs(D - ref["D"]).max() <= TOL_D
+    Hp = torch.from_numpy(p["H"]).pin_memory()
+    H1p = torch.from_numpy(p["H1"]).pin_memory()
+    Dp = torch.empty(n, n, dtype=torch.float64).pin_memory()
+    D1p = torch.empty(n, n, dtype=torch.float64).pin_memory()
+    h.response_host(Hp, H1p, n_occ, Dp, D1p)                       # pinned torch buffers
+    assert np.abs(Dp.numpy() - ref["D"]).max() <= TOL_D
+    assert np.abs(D1p.numpy() - ref["D1"]).max() <= TOL_D1 * np.abs(ref["D1"]).max()
+    assert h.launch_count > 0
+    h.close()
+    h3 = sp2.Sp2Handle(n)
+    with pytest.raises(sp2.Sp2Error) as ei:                        # no staging in this workspace
+        h3.density_host(p["H"], n_occ, D)
+    assert ei.value.status == sp2.SP2_ERR_WORKSPACE
+    h3.close()
+
+
+def test_sequence_call_small(sp2, torch_mod):
+    """config-5 shape at N = 512: H_t = H_0 + t*1e-3*P, every step against the oracle."""
+    import oracle
+
+    torch = torch_mod
+    cfg = inputs.scaled_config(inputs.CONFIGS[5], 512)
+    p = inputs.make_problem(cfg, want_p=True)
+    n, n_occ = p["n"], p["n_occ"]
+    H0 = torch.from_numpy(p["H"]).cuda()
+    P = torch.from_numpy(p["P"]).cuda()
+    steps = [0, 1, 7, 49]
+    Hs = [H0 + float(t) * 1e-3 * P for t in steps]
+    Ds = [torch.empty(n, n, dtype=torch.float32, device="cuda") for _ in steps]
+    h = sp2.Sp2Handle(n)
+    h.sequence_begin(n, n_occ, n_steps_hint=len(steps))
+    for Ht, Dt in zip(Hs, Ds):
+        h.sequence_step(Ht, Dt)                                   # no synchronisation between steps
+    res = h.sequence_end()
+    assert len(res) == len(steps)
+    for Ht, Dt, r in zip(Hs, Ds, res):
+        ref = oracle.sp2_density(Ht.cpu().numpy().astype(np.float64), n_occ)
+        assert r["status"] == 0
+        assert np.abs(Dt.cpu().numpy().astype(np.float64) - ref["D"]).max() <= TOL_D
+        assert abs(r["tr_d"] - n_occ) <= TOL_TR
+        assert abs(r["tr_dh"] - ref["tr_dh"]) <= TOL_E * abs(ref["tr_dh"])
+    h.close()

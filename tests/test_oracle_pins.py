@@ -276,3 +276,16 @@ def test_response_is_linear_and_sign_sensitive(cfg2):
     r2 = oracle.sp2_density(p["H"], 20, H1=-3.0 * p["H1"])
     np.testing.assert_allclose(r2["D1"], -3.0 * r["D1"], atol=1e-12)
     assert np.abs(p["H"] @ p["H1"] - p["H1"] @ p["H"]).max() > 1e-3
+
+
+def test_sampled_response_entries_match_the_full_closed_form():
+    cfg = inputs.Sp2Config("t", 2, 60, 22, (-1.5, -0.25), (0.25, 1.5), "f64", True)
+    p = inputs.make_problem(cfg)
+    full = oracle.response_closed_form(p["Q"], p["lam"], 22, p["H1"])
+    rows = np.array([0, 3, 59, 17, 40, 40])
+    cols = np.array([0, 51, 59, 3, 7, 40])
+    got = oracle.response_closed_form_sampled(p["Q"], p["lam"], 22, p["H1"], rows, cols)
+    np.testing.assert_allclose(got, full[rows, cols], rtol=0, atol=1e-13 * np.abs(full).max())
+    # and against the finite difference of the definition (independent of both closed forms)
+    fd = oracle.response_finite_difference(p["H"], p["H1"], 22, eps=1e-5)
+    np.testing.assert_allclose(got, fd[rows, cols], rtol=0, atol=1e-6 * np.abs(full).max())
