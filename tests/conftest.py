@@ -28,3 +28,18 @@ def pytest_collection_modifyitems(config, items):
     for it in items:
         if "gpu" in it.keywords:
             it.add_marker(skip)
+
+
+@pytest.fixture(scope="session")
+def torch_cuda():
+    import torch
+
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="session")
+def sp2(torch_cuda):
+    from paper_2107_02737_b200 import sp2 as mod   # raises if libsp2_b200.so is missing: no fallback
+
+    return mod

@@ -1,0 +1,126 @@
+"""GPU parity at BASELINE.json's full sizes (configs 3, 4, 5), in the launch configuration bench.py
+times.  The float64 SP2 loop of the oracle would take minutes to hours here, so D is compared with
+the oracle's DEFINITION evaluated from the generator's eigenpairs (oracle.density_from_eigenpairs,
+Eq. 17: exact projector, sampled element by element) and D1 with the sampled closed form of
+first-order perturbation theory; plus properties that hold at any size (trace, band energy,
+bit-symmetry) and float64 idempotency / commutator / response identities evaluated with torch on the
+GPU as a labelled CROSS-CHECK (torch is the harness here, never the library).
+"""
+import numpy as np
+import pytest
+
+from paper_2107_02737_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL_D, TOL_TR, TOL_E, TOL_D1 = 1e-4, 1e-3, 1e-5, 1e-3
+
+
+def _samples(n, k=4000, seed=7):
+    rng = np.random.default_rng(seed)
+    rows = np.concatenate([rng.integers(0, n, k), np.arange(0, n, max(1, n // 512)), [0, n - 1, n - 1]])
+    cols = np.concatenate([rng.integers(0, n, k), np.arange(0, n, max(1, n // 512)), [n - 1, 0, n - 1]])
+    return rows, cols
+
+
+def _gather(torch, M, rows, cols):
+    return M[torch.from_numpy(rows).cuda(), torch.from_numpy(cols).cuda()].double().cpu().numpy()
+
+
+def _crosscheck_projector(torch, D, H, n_occ):
+    """float64 invariants on the GPU (cross-check, not the oracle): idempotency and [H, D] = 0."""
+    D64, H64 = D.double(), H.double()
+    idem = float(torch.linalg.norm(D64 @ D64 - D64)) / n_occ ** 0.5
+    comm = float(torch.linalg.norm(H64 @ D64 - D64 @ H64)) / float(torch.linalg.norm(H64))
+    return idem, comm
+
+
+def test_config3_waterbox_n6000_f32(torch_cuda, sp2):
+    import oracle
+
+    torch = torch_cuda
+    p = inputs.make_problem(inputs.CONFIGS[3], device="cuda")
+    n, n_occ = p["n"], p["n_occ"]
+    assert (n, n_occ, p["H"].dtype) == (6000, 4000, np.float32)
+    H = torch.from_numpy(p["H"]).cuda()
+    h = sp2.Sp2Handle(n)
+    D, r = h.density(H, n_occ)
+    h.close()
+    rows, cols = _samples(n)
+    De = oracle.density_from_eigenpairs(p["Q"], p["lam"], n_occ, rows, cols)
+    assert r["status"] == 0 and 25 <= r["layers"] <= 50
+    assert np.abs(_gather(torch, D, rows, cols) - De).max() <= TOL_D
+    assert abs(r["tr_d"] - n_occ) <= TOL_TR
+    E = inputs.band_energy_closed_form(p["lam"], n_occ)
+    assert abs(r["tr_dh"] - E) <= TOL_E * abs(E)
+    assert bool(torch.equal(D, D.T))
+    idem, comm = _crosscheck_projector(torch, D, H, n_occ)
+    assert idem < 1e-4 and comm < 1e-5
+
+
+def test_config4_smallgap_n8192_response(torch_cuda, sp2):
+    import oracle
+
+    torch = torch_cuda
+    p = inputs.make_problem(inputs.CONFIGS[4], device="cuda")
+    n, n_occ = p["n"], p["n_occ"]
+    assert (n, n_occ) == (8192, 4096)
+    H = torch.from_numpy(p["H"]).cuda()
+    H1 = torch.from_numpy(p["H1"]).cuda()
+    h = sp2.Sp2Handle(n, response=True)
+    D, D1, r = h.response(H, H1, n_occ)
+    h.close()
+    rows, cols = _samples(n)
+    De = oracle.density_from_eigenpairs(p["Q"], p["lam"], n_occ, rows, cols)
+    D1e = oracle.response_closed_form_sampled(p["Q"], p["lam"], n_occ, p["H1"], rows, cols)
+    scale1 = np.abs(D1e).max()
+    assert r["status"] == 0 and 35 <= r["layers"] <= 52                     # BASELINE.json: ~35-45 layers
+    assert np.abs(_gather(torch, D, rows, cols) - De).max() <= TOL_D
+    assert np.abs(_gather(torch, D1, rows, cols) - D1e).max() <= TOL_D1 * scale1
+    assert abs(r["tr_d"] - n_occ) <= TOL_TR
+    E = inputs.band_energy_closed_form(p["lam"], n_occ)
+    assert abs(r["tr_dh"] - E) <= TOL_E * abs(E)
+    assert bool(torch.equal(D, D.T)) and bool(torch.equal(D1, D1.T))
+    assert abs(r["tr_d1"]) <= 1e-3 * scale1 * n ** 0.5
+    idem, comm = _crosscheck_projector(torch, D, H, n_occ)
+    assert idem < 1e-4 and comm < 1e-5
+    # derivative of D^2 = D (cross-check in float64 on the GPU): D D1 + D1 D = D1
+    resid = float((D @ D1 + D1 @ D - D1).abs().max())
+    assert resid <= TOL_D1 * scale1
+
+
+def test_config5_md_sequence_n16384(torch_cuda, sp2):
+    """H_t = H_0 + t*1e-3*P formed on the device by the harness; steps t = 0, 25, 49 of the 50-step
+    sweep go through sp2_sequence_* without a host synchronisation in between."""
+    import oracle
+
+    torch = torch_cuda
+    p = inputs.make_problem(inputs.CONFIGS[5], device="cuda", want_p=True)
+    n, n_occ = p["n"], p["n_occ"]
+    assert (n, n_occ, p["H"].dtype) == (16384, 8192, np.float32)
+    H0 = torch.from_numpy(p["H"]).cuda()
+    P = torch.from_numpy(p["P"]).cuda()
+    steps = [0, 25, 49]
+    h = sp2.Sp2Handle(n)
+    Ht = [H0 + float(t) * 1e-3 * P for t in steps]
+    Dt = [torch.empty_like(H0) for _ in steps]
+    h.sequence_begin(n, n_occ, n_steps_hint=len(steps))
+    for a, b in zip(Ht, Dt):
+        h.sequence_step(a, b)
+    res = h.sequence_end()
+    h.close()
+    assert [r["status"] for r in res] == [0, 0, 0]
+    rows, cols = _samples(n, k=2000)
+    De = oracle.density_from_eigenpairs(p["Q"], p["lam"], n_occ, rows, cols)
+    assert np.abs(_gather(torch, Dt[0], rows, cols) - De).max() <= TOL_D          # t = 0: exact projector
+    E0 = inputs.band_energy_closed_form(p["lam"], n_occ)
+    assert abs(res[0]["tr_dh"] - E0) <= TOL_E * abs(E0)
+    for a, b, r in zip(Ht, Dt, res):
+        assert 30 <= r["layers"] <= 50
+        assert abs(r["tr_d"] - n_occ) <= TOL_TR
+        assert bool(torch.equal(b, b.T))
+        idem, comm = _crosscheck_projector(torch, b, a, n_occ)                     # t > 0: invariants (cross-check)
+        assert idem < 1e-4 and comm < 1e-5
+    # first-order consistency of the band energy along the sweep: dE/dt = 1e-3 * tr(D P)
+    dE_pred = 25e-3 * float((Dt[0].double() * P.double()).sum())
+    assert abs((res[1]["tr_dh"] - res[0]["tr_dh"]) - dE_pred) <= 0.05 * abs(dE_pred) + 1e-3
