@@ -158,6 +158,13 @@ SP2_API int sp2_debug_history(sp2_handle_t handle, double* tr_x, double* e, int 
  * ping-pong buffer; exponent and shift are still those of X_L).  c is returned in *shift. */
 SP2_API sp2_status_t sp2_debug_plane(sp2_handle_t handle, int which, size_t* offset, long* pitch, int* exponent, double* shift);
 
+/* Host-only: the static work lists of the layer kernel for n_tiles upper-triangular tiles,
+ * segs_per_pass k-segments per product pass and n_clusters CTA(-pair)s.  Each item is 8 ints
+ * {unit, seg0, seg1, kind (0 whole, 1 contributor, 2 owner), slot, nparts, flag_id, 0}; item_begin has
+ * n_clusters + 1 entries.  Returns the number of items (-1 on bad arguments). */
+SP2_API int sp2_debug_schedule(int n_tiles, int with_response, int segs_per_pass, int n_clusters, int* items8,
+                               int capacity, int* item_begin);
+
 #ifdef __cplusplus
 }
 #endif

@@ -10,6 +10,7 @@
 #include <cuda_runtime.h>
 #include <new>
 #include <string.h>
+#include <utility>
 #include <vector>
 
 #include "sp2.h"
@@ -39,6 +40,7 @@ namespace {
 constexpr int kRingCap = 4096;
 constexpr int kPadTo = 256;          // npad is a multiple of the largest tile edge
 constexpr int kSimtMaxN = 4096;
+constexpr int kMaxClusters = 256;   // >= SM count of any sm_100 part
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline int pad_n(int n) { return (int)align_up((size_t)n, kPadTo); }
@@ -51,6 +53,7 @@ struct Layout {
   size_t off_bslots, bslots_count;
   size_t off_fslots;
   size_t off_tiles, tiles_count;
+  size_t off_items, items_cap, off_item_begin, off_scratch, scratch_bytes, off_flags;
   size_t off_ctrl, off_ring;
   size_t off_staging, staging_each;
   size_t total;
@@ -80,6 +83,14 @@ Layout make_layout(int n_max, int flags) {
   const size_t nt1 = npad / 128;
   L.tiles_count = nt1 * (nt1 + 1) / 2;
   L.off_tiles = off; off += align_up(L.tiles_count * sizeof(int2), 1024);
+  L.items_cap = 2 * L.tiles_count + 1024;
+  L.off_items = off; off += align_up(L.items_cap * sizeof(Sp2Item), 1024);
+  L.off_item_begin = off; off += align_up((kMaxClusters + 1) * sizeof(int), 1024);
+  L.scratch_bytes = 2 * (size_t)kMaxClusters * sp2_layer_scratch_slot_bytes(1);
+  if (2 * (size_t)(kMaxClusters / 2) * sp2_layer_scratch_slot_bytes(2) > L.scratch_bytes)
+    L.scratch_bytes = 2 * (size_t)(kMaxClusters / 2) * sp2_layer_scratch_slot_bytes(2);
+  L.off_scratch = off; off += align_up(L.scratch_bytes, 1024);
+  L.off_flags = off; off += align_up(2 * kMaxClusters * sizeof(unsigned int), 1024);
   L.off_ctrl = off; off += align_up(sizeof(Sp2Ctrl), 1024);
   L.off_ring = off; off += align_up((size_t)kRingCap * sizeof(sp2_result_t), 1024);
   if (flags & SP2_WITH_HOST_STAGING) {
@@ -110,6 +121,9 @@ struct sp2_handle_s {
   int cur_n, cur_npad, cur_cg, cur_resp, cur_seg;
   Sp2LayerArgs args[2];          // parity 0: buffer 0 -> 1, parity 1: buffer 1 -> 0
   std::vector<int2> tiles_host;
+  std::vector<Sp2Item> items_host;
+  std::vector<int> item_begin_host;
+  int n_flags, n_clusters;
   cudaEvent_t ev0, ev1, evl0, evl1;
   int time_layers;               // record evl0/evl1 around the layer launches of the next solve
   sp2_result_t* h_result;        // pinned
@@ -129,6 +143,10 @@ struct sp2_handle_s {
   Sp2BoundSlot* bslots(int i) const { return reinterpret_cast<Sp2BoundSlot*>(ws + L.off_bslots) + (size_t)i * L.bslots_count; }
   double* fslots() const { return reinterpret_cast<double*>(ws + L.off_fslots); }
   int2* tiles() const { return reinterpret_cast<int2*>(ws + L.off_tiles); }
+  Sp2Item* items() const { return reinterpret_cast<Sp2Item*>(ws + L.off_items); }
+  int* item_begin() const { return reinterpret_cast<int*>(ws + L.off_item_begin); }
+  float* scratch() const { return reinterpret_cast<float*>(ws + L.off_scratch); }
+  unsigned int* split_flags() const { return reinterpret_cast<unsigned int*>(ws + L.off_flags); }
   Sp2Ctrl* ctrl() const { return reinterpret_cast<Sp2Ctrl*>(ws + L.off_ctrl); }
   sp2_result_t* ring() const { return reinterpret_cast<sp2_result_t*>(ws + L.off_ring); }
   void* staging(int i) const { return ws + L.off_staging + (size_t)i * L.staging_each; }
@@ -153,6 +171,79 @@ void build_tiles(int nt, std::vector<int2>& out) {
       for (int ti = gi * G; ti < (gi + 1) * G && ti < nt; ++ti)
         for (int tj = gj * G; tj < (gj + 1) * G && tj < nt; ++tj)
           if (tj >= ti) out.push_back(make_int2(ti, tj));
+}
+
+// Static work lists.  Units (first the 2-pass YZ+ZY units, then the Y^2
+// units, each list in the L2-friendly tile order) are dealt whole to the least-loaded CTA(-pair) --
+// equal costs make that a round-robin whose concurrent units are neighbours -- as long as they fit
+// under T = ceil(total segments / clusters).  The units that do not fit (the last, partial wave) are cut
+// along k into parts that fill every cluster up to T; the cluster holding the last part owns the
+// epilogue.  Loads differ by at most one segment.
+void build_schedule(int n_tiles, int resp, int segs_y, int nC, std::vector<Sp2Item>& items,
+                    std::vector<int>& begin, int* n_flags, int* n_slots) {
+  const int n_units = n_tiles * (resp ? 2 : 1);
+  auto cost = [&](int u) { return (resp && u < n_tiles) ? 2 * segs_y : segs_y; };
+  long long total = 0;
+  for (int u = 0; u < n_units; ++u) total += cost(u);
+  const int T = (int)((total + nC - 1) / nC);
+  std::vector<int> load(nC, 0);
+  std::vector<std::vector<Sp2Item>> full(nC), contrib(nC), owner(nC);
+  std::vector<int> leftover;
+  for (int u = 0; u < n_units; ++u) {
+    int best = 0;
+    for (int c = 1; c < nC; ++c) if (load[c] < load[best]) best = c;
+    if (load[best] + cost(u) <= T) {
+      Sp2Item it = {u, 0, cost(u), 0, 0, 0, 0, 0};
+      full[best].push_back(it);
+      load[best] += cost(u);
+    } else {
+      leftover.push_back(u);
+    }
+  }
+  int flags = 0, slots = 0;
+  for (int u : leftover) {
+    int pos = 0;
+    const int cu = cost(u);
+    std::vector<std::pair<int, Sp2Item>> parts;     // (cluster, item)
+    while (pos < cu) {
+      int best = 0;
+      for (int c = 1; c < nC; ++c) if (T - load[c] > T - load[best]) best = c;
+      int take = T - load[best];
+      if (take <= 0) take = cu - pos;               // cannot happen (T * nC >= total); stay safe
+      if (take > cu - pos) take = cu - pos;
+      Sp2Item it = {u, pos, pos + take, 1, 0, 0, flags, 0};
+      parts.push_back(std::make_pair(best, it));
+      load[best] += take;
+      pos += take;
+    }
+    const int np = (int)parts.size() - 1;            // contributors
+    if (np == 0) {
+      parts[0].second.kind = 0;
+      full[parts[0].first].push_back(parts[0].second);
+      continue;
+    }
+    for (int k = 0; k < np; ++k) {
+      parts[k].second.slot = slots + k;
+      contrib[parts[k].first].push_back(parts[k].second);
+    }
+    Sp2Item& own = parts[np].second;
+    own.kind = 2; own.slot = slots; own.nparts = np;
+    owner[parts[np].first].push_back(own);
+    slots += np;
+    ++flags;
+  }
+  items.clear();
+  begin.assign(nC + 1, 0);
+  for (int c = 0; c < nC; ++c) {
+    begin[c] = (int)items.size();
+    // contributors never wait, owners only wait for contributors: whole units, then contributors, then owners
+    items.insert(items.end(), full[c].begin(), full[c].end());
+    items.insert(items.end(), contrib[c].begin(), contrib[c].end());
+    items.insert(items.end(), owner[c].begin(), owner[c].end());
+  }
+  begin[nC] = (int)items.size();
+  *n_flags = flags;
+  *n_slots = slots;
 }
 
 sp2_status_t encode_plane_map(sp2_handle_t h, CUtensorMap* map, const __half* base, int npad) {
@@ -184,7 +275,23 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   build_tiles(nt, h->tiles_host);
   SP2_CUDA(h, cudaMemcpyAsync(h->tiles(), h->tiles_host.data(), h->tiles_host.size() * sizeof(int2),
                               cudaMemcpyHostToDevice, s));
-  SP2_CUDA(h, cudaStreamSynchronize(s));     // tiles_host may be rebuilt by the next prepare
+  int n_units = (int)h->tiles_host.size() * (resp ? 2 : 1);
+  int nC = h->num_sms / cg;
+  if (nC > kMaxClusters / cg) nC = kMaxClusters / cg;
+  if (nC > n_units) nC = n_units;
+  int n_slots = 0;
+  build_schedule((int)h->tiles_host.size(), resp, (npad / 64) / seg, nC, h->items_host, h->item_begin_host,
+                 &h->n_flags, &n_slots);
+  h->n_clusters = nC;
+  if (h->items_host.size() > h->L.items_cap || (size_t)n_slots * sp2_layer_scratch_slot_bytes(cg) > h->L.scratch_bytes ||
+      h->n_flags > 2 * kMaxClusters)
+    return SP2_ERR_WORKSPACE;
+  SP2_CUDA(h, cudaMemcpyAsync(h->items(), h->items_host.data(), h->items_host.size() * sizeof(Sp2Item),
+                              cudaMemcpyHostToDevice, s));
+  SP2_CUDA(h, cudaMemcpyAsync(h->item_begin(), h->item_begin_host.data(), h->item_begin_host.size() * sizeof(int),
+                              cudaMemcpyHostToDevice, s));
+  SP2_CUDA(h, cudaMemsetAsync(h->split_flags(), 0, 2 * kMaxClusters * sizeof(unsigned int), s));
+  SP2_CUDA(h, cudaStreamSynchronize(s));     // host vectors may be rebuilt by the next prepare
   for (int par = 0; par < 2; ++par) {
     Sp2LayerArgs& a = h->args[par];
     memset(&a, 0, sizeof(a));
@@ -197,6 +304,8 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
       if (st != SP2_OK) return st;
     }
     a.ctrl = h->ctrl(); a.slots = h->slots(); a.tiles = h->tiles();
+    a.items = h->items(); a.item_begin = h->item_begin(); a.scratch = h->scratch(); a.flags = h->split_flags();
+    a.n_flags = h->n_flags; a.n_clusters = h->n_clusters;
     a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = resp; a.seg_kb = seg;
   }
   h->cur_n = N; h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp; h->cur_seg = seg;
@@ -244,7 +353,7 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const void* H1, sp2_dt
     sp2_launch_ctrl0(c, h->slots(), h->slots2(), sp2_rescale_blocks(npad), s); ++launches;
     if (h->time_layers) SP2_CUDA(h, cudaEventRecord(h->evl0, s));
     for (int n = 0; n < max_layers; ++n) {
-      cudaError_t e = sp2_launch_layer(h->args[n & 1], o.engine, h->cur_cg, h->num_sms, s);
+      cudaError_t e = sp2_launch_layer(h->args[n & 1], o.engine, h->cur_cg, s);
       if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
       ++launches;
     }
@@ -467,6 +576,18 @@ const char* sp2_status_string(sp2_status_t s) {
 
 int sp2_last_cuda_error(sp2_handle_t h) { return h ? h->last_cuda_error : 0; }
 unsigned long long sp2_launch_count(sp2_handle_t h) { return h ? h->launches : 0ull; }
+
+int sp2_debug_schedule(int n_tiles, int with_response, int segs_per_pass, int n_clusters, int* items8, int capacity,
+                       int* item_begin) {
+  if (n_tiles <= 0 || segs_per_pass <= 0 || n_clusters <= 0) return -1;
+  std::vector<Sp2Item> items;
+  std::vector<int> begin;
+  int n_flags = 0, n_slots = 0;
+  build_schedule(n_tiles, with_response, segs_per_pass, n_clusters, items, begin, &n_flags, &n_slots);
+  for (size_t i = 0; i < items.size() && (int)i < capacity; ++i) memcpy(items8 + 8 * i, &items[i], sizeof(Sp2Item));
+  if (item_begin) for (int c = 0; c <= n_clusters; ++c) item_begin[c] = begin[c];
+  return (int)items.size();
+}
 
 int sp2_debug_history(sp2_handle_t h, double* tr_x, double* e, int capacity) {
   if (!h) return -1;

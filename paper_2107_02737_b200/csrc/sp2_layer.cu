@@ -202,7 +202,8 @@ __device__ __forceinline__ uint32_t u4_word(const uint4& v, int i) {
 // ----------------------------------------------------------------------------------------------
 // shared tail of both engines: last block reduces the slots (index order) and runs the controller
 __device__ inline void layer_tail(Sp2Ctrl* ctrl, const Sp2Slot* slots, int n_y, int n_z, int y_first,
-                                  unsigned int n_blocks, uint32_t* is_last_smem, double* red) {
+                                  unsigned int n_blocks, uint32_t* is_last_smem, double* red,
+                                  unsigned int* flags = nullptr, int n_flags = 0) {
   __syncthreads();
   if (threadIdx.x == 0) {
     __threadfence();
@@ -212,6 +213,7 @@ __device__ inline void layer_tail(Sp2Ctrl* ctrl, const Sp2Slot* slots, int n_y, 
   __syncthreads();
   if (!*is_last_smem) return;
   __threadfence();
+  for (int i = threadIdx.x; i < n_flags; i += blockDim.x) flags[i] = 0u;   // every split unit was consumed
   double tr, fro, mx, tracc, trz = 0.0, froz = 0.0, mxz = 0.0, unused;
   // slot array: [z slots (n_z)][y slots (n_y)] when y_first == n_z
   sp2_reduce_slots(slots + y_first, n_y, red, tr, fro, mx, tracc);
@@ -328,13 +330,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;
   const int cluster_id = blockIdx.x / CG;
-  const int n_clusters = gridDim.x / CG;
   const bool leader = (rank == 0);
 
   const int n_tiles = a.n_tiles;
-  const int n_units = a.with_response ? 2 * n_tiles : n_tiles;
   const int KB = a.npad / kBK;
   const int seg_kb = a.seg_kb;            // k-blocks per TMEM accumulation segment (divides KB)
+  const int item_lo = a.item_begin[cluster_id], item_hi = a.item_begin[cluster_id + 1];
 
   if (warp == 0 && lane == 0) {
     for (int i = 0; i < 4; ++i) asm volatile("prefetch.tensormap [%0];" ::"l"(&a.tm[i]) : "memory");
@@ -361,17 +362,20 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
           full_bar[s] = smem_u32(&bars->full[s]);
           if constexpr (CG == 2) asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(full_bar[s]) : "r"(full_bar[s]), "r"(0));
         }
-        for (int u = cluster_id; u < n_units; u += n_clusters) {
+        for (int iti = item_lo; iti < item_hi; ++iti) {
+          const Sp2Item I = a.items[iti];
+          const int u = I.unit;
           const bool wunit = a.with_response && u < n_tiles;
           const int2 tij = a.tiles[wunit ? u : (a.with_response ? u - n_tiles : u)];
           const int row_a = tij.x * TILE + (int)rank * kRows;
           const int row_b = tij.y * TILE + (int)rank * kRows;
-          const int passes = wunit ? 2 : 1;
-          for (int p = 0; p < passes; ++p) {
-            // Y^2: A = (Yh, Ym), B = (Yh, Ym).  W pass 0: A = (Yh, Ym), B = (Zh, Zm).  W pass 1: A = (Zh, Zm), B = (Yh, Ym).
-            const int ma = (wunit && p == 1) ? 2 : 0;
-            const int mb = (wunit && p == 0) ? 2 : 0;
-            for (int kb = 0; kb < KB; ++kb) {
+          {
+            for (int g = I.seg0 * seg_kb; g < I.seg1 * seg_kb; ++g) {
+              // Y^2: A = (Yh, Ym), B = (Yh, Ym).  W pass 0: A = (Yh, Ym), B = (Zh, Zm).  W pass 1: A = (Zh, Zm), B = (Yh, Ym).
+              const int p = (g >= KB) ? 1 : 0;
+              const int kb = g - p * KB;
+              const int ma = (wunit && p == 1) ? 2 : 0;
+              const int mb = (wunit && p == 0) ? 2 : 0;
               mbar_wait(smem_u32(&bars->empty[stage]), phase ^ 1u);
               const uint32_t dst = smem_u32(smem + stage * kStageBytes);
               if (CG == 1 || leader) mbar_expect_tx(smem_u32(&bars->full[stage]), (uint32_t)(CG * kStageBytes));
@@ -389,10 +393,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
       if (leader && elect_one()) {
         int stage = 0; uint32_t phase = 0;
         int as = 0; uint32_t aphase = 0;
-        for (int u = cluster_id; u < n_units; u += n_clusters) {
-          const bool wunit = a.with_response && u < n_tiles;
-          const int n_seg = (wunit ? 2 : 1) * KB / seg_kb;
-          for (int sg = 0; sg < n_seg; ++sg) {
+        for (int iti = item_lo; iti < item_hi; ++iti) {
+          const Sp2Item I = a.items[iti];
+          for (int sg = I.seg0; sg < I.seg1; ++sg) {
             mbar_wait(smem_u32(&bars->tmem_empty[as]), aphase ^ 1u);
             tc_fence_after();
             const uint32_t acc = tmem_base + (uint32_t)(as * ACC_COLS);
@@ -429,16 +432,17 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
     const int hh = cw >> 2;                       // which half of the accumulator columns
     const Sp2Coef cf = a.ctrl->coef;
     int as = 0; uint32_t aphase = 0;
-    for (int u = cluster_id; u < n_units; u += n_clusters) {
+    for (int iti = item_lo; iti < item_hi; ++iti) {
+      const Sp2Item I = a.items[iti];
+      const int u = I.unit;
       const bool wunit = a.with_response && u < n_tiles;
       const int2 tij = a.tiles[wunit ? u : (a.with_response ? u - n_tiles : u)];
-      const int n_seg = (wunit ? 2 : 1) * KB / seg_kb;
       float sums[WCOLS];
-      for (int sg = 0; sg < n_seg; ++sg) {
+      for (int sg = I.seg0; sg < I.seg1; ++sg) {
         mbar_wait(smem_u32(&bars->tmem_full[as]), aphase);
         tc_fence_after();
         const uint32_t tcol = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * ACC_COLS + hh * WCOLS);
-        if (sg == 0) {
+        if (sg == I.seg0) {
 #pragma unroll
           for (int ch = 0; ch < NCH; ++ch) {
             uint32_t v[32];
@@ -462,6 +466,31 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
           else mbar_arrive(smem_u32(&bars->tmem_empty[as]));
         }
         if (++as == 2) { as = 0; aphase ^= 1u; }
+      }
+      // ---- split-k units of the last wave: hand the partial sums over / collect them
+      constexpr size_t kWarpFloats = (size_t)WCOLS * 32;
+      if (I.kind == 1) {
+        float* dst = a.scratch + (((size_t)I.slot * CG + rank) * kConsumerWarps + cw) * kWarpFloats + lane;
+#pragma unroll
+        for (int c = 0; c < WCOLS; ++c) dst[c * 32] = sums[c];       // lanes contiguous: 128 B per store
+        __syncwarp();
+        if (lane == 0) { __threadfence(); atomicAdd(a.flags + I.flag_id, 1u); }
+        continue;
+      }
+      if (I.kind == 2) {
+        if (lane == 0) {
+          const unsigned int target = (unsigned int)(I.nparts * kConsumerWarps * CG);
+          long long spins = 0;
+          while (*reinterpret_cast<volatile unsigned int*>(a.flags + I.flag_id) < target)
+            if (++spins > kSpinLimit) __trap();
+          __threadfence();
+        }
+        __syncwarp();
+        for (int pp = 0; pp < I.nparts; ++pp) {
+          const float* src = a.scratch + (((size_t)(I.slot + pp) * CG + rank) * kConsumerWarps + cw) * kWarpFloats + lane;
+#pragma unroll
+          for (int c = 0; c < WCOLS; ++c) sums[c] += __ldcg(src + c * 32);
+        }
       }
       // ---- fused epilogue from the register sums
       const int pl = wunit ? 2 : 0;
@@ -499,7 +528,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
 
   const int per_unit = CG * kConsumerWarps;
   const int n_z = a.with_response ? n_tiles * per_unit : 0;
-  layer_tail(a.ctrl, a.slots, n_tiles * per_unit, n_z, n_z, gridDim.x, &bars->is_last, red);
+  layer_tail(a.ctrl, a.slots, n_tiles * per_unit, n_z, n_z, gridDim.x, &bars->is_last, red, a.flags, a.n_flags);
 }
 
 // ----------------------------------------------------------------------------------------------
@@ -598,31 +627,30 @@ cudaError_t sp2_layer_configure() {
   return e;
 }
 
-cudaError_t sp2_launch_layer(const Sp2LayerArgs& args, int engine, int cta_group, int num_sms, cudaStream_t s) {
+size_t sp2_layer_scratch_slot_bytes(int cta_group) {
+  return (size_t)cta_group * kConsumerWarps * (128 * cta_group / 2) * 32 * sizeof(float);
+}
+
+cudaError_t sp2_launch_layer(const Sp2LayerArgs& args, int engine, int cta_group, cudaStream_t s) {
   if (engine == SP2_ENGINE_SIMT_DEBUG) {
     const int nb = args.npad / 16;
     dim3 grid(nb * (nb + 1) / 2, args.with_response ? 2 : 1);
     k_layer_simt<<<grid, 256, 0, s>>>(args);
     return cudaGetLastError();
   }
-  const int n_units = args.n_tiles * (args.with_response ? 2 : 1);
   cudaLaunchConfig_t cfg = {};
   cfg.blockDim = dim3(kThreads);
   cfg.dynamicSmemBytes = sp2_layer_smem_bytes();
   cfg.stream = s;
   cudaLaunchAttribute attr[1];
   if (cta_group == 2) {
-    int clusters = num_sms / 2;
-    if (clusters > n_units) clusters = n_units;
-    cfg.gridDim = dim3(2 * clusters);
+    cfg.gridDim = dim3(2 * args.n_clusters);
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, k_layer_tc<2>, args);
   }
-  int ctas = num_sms;
-  if (ctas > n_units) ctas = n_units;
-  cfg.gridDim = dim3(ctas);
+  cfg.gridDim = dim3(args.n_clusters);
   cfg.attrs = nullptr; cfg.numAttrs = 0;
   return cudaLaunchKernelEx(&cfg, k_layer_tc<1>, args);
 }

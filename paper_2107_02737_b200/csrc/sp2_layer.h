@@ -5,6 +5,16 @@
 #include <cuda_runtime.h>
 #include "sp2_internal.cuh"
 
+// One entry of a CTA(-pair)'s static work list: segments [seg0, seg1) of the k sweep(s) of `unit`.
+// kind 0: the whole unit (accumulate, epilogue).  Units of the last, partial wave are cut along k so
+// that every CTA(-pair) gets the same number of segments: kind 1 = contributor (accumulate, store the
+// FP32 partial sums to scratch slot `slot`, bump flags[flag_id]); kind 2 = owner (accumulate, wait for
+// `nparts` contributors, add their partials from slots slot..slot+nparts-1 in that order, epilogue).
+struct Sp2Item {
+  int unit, seg0, seg1, kind;
+  int slot, nparts, flag_id, pad;
+};
+
 // Arguments of one layer launch.  tm[] are TMA descriptors of the INPUT planes (Yh, Ym, Zh, Zm):
 // 2-D FP16 tensors npad x npad, box 64 (k) x 128 (rows), SWIZZLE_128B.
 struct alignas(64) Sp2LayerArgs {
@@ -14,6 +24,12 @@ struct alignas(64) Sp2LayerArgs {
   Sp2Ctrl* ctrl;
   Sp2Slot* slots;        // [z-class slots][y-class slots]
   const int2* tiles;     // (ti, tj), ti <= tj, upper-triangular tile list in L2-friendly order
+  const Sp2Item* items;  // work lists of all CTA(-pair)s, concatenated
+  const int* item_begin; // [n_clusters + 1] offsets into items
+  float* scratch;        // split-k partial sums
+  unsigned int* flags;   // one arrival counter per split unit (zero between launches)
+  int n_flags;
+  int n_clusters;        // CTA(-pair)s the work lists were built for (= grid size / cta_group)
   int n;                 // true dimension (rows/cols >= n are zero padding and stay zero)
   int npad;              // padded dimension (multiple of the tile edge)
   int n_tiles;           // number of upper-triangular tiles
@@ -24,4 +40,5 @@ struct alignas(64) Sp2LayerArgs {
 size_t sp2_layer_smem_bytes();
 int sp2_layer_slots(int npad, int cta_group, int with_response, int engine);
 cudaError_t sp2_layer_configure();
-cudaError_t sp2_launch_layer(const Sp2LayerArgs& args, int engine, int cta_group, int num_sms, cudaStream_t s);
+cudaError_t sp2_launch_layer(const Sp2LayerArgs& args, int engine, int cta_group, cudaStream_t s);
+size_t sp2_layer_scratch_slot_bytes(int cta_group);

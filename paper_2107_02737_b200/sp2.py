@@ -37,7 +37,7 @@ EXPORTS = [
     "sp2_density", "sp2_response", "sp2_density_host", "sp2_response_host",
     "sp2_sequence_begin", "sp2_sequence_step", "sp2_sequence_end",
     "sp2_status_string", "sp2_last_cuda_error", "sp2_launch_count",
-    "sp2_debug_history", "sp2_debug_plane",
+    "sp2_debug_history", "sp2_debug_plane", "sp2_debug_schedule",
 ]
 
 
@@ -116,10 +116,25 @@ def _load():
     lib.sp2_debug_history.argtypes = [vp, C.POINTER(d), C.POINTER(d), i]
     lib.sp2_debug_plane.restype = i
     lib.sp2_debug_plane.argtypes = [vp, i, C.POINTER(sz), C.POINTER(l), C.POINTER(i), C.POINTER(d)]
+    lib.sp2_debug_schedule.restype = i
+    lib.sp2_debug_schedule.argtypes = [i, i, i, i, C.POINTER(i), i, C.POINTER(i)]
     return lib
 
 
 lib = _load()
+
+
+def debug_schedule(n_tiles: int, with_response: bool, segs_per_pass: int, n_clusters: int):
+    """Host-only: work lists of the layer kernel -> list (per cluster) of dicts."""
+    cap = 2 * n_tiles * 2 + 4 * n_clusters + 16
+    buf = (C.c_int * (8 * cap))()
+    begin = (C.c_int * (n_clusters + 1))()
+    cnt = lib.sp2_debug_schedule(n_tiles, int(with_response), segs_per_pass, n_clusters, buf, cap, begin)
+    if cnt < 0 or cnt > cap:
+        raise ValueError("bad schedule arguments")
+    keys = ("unit", "seg0", "seg1", "kind", "slot", "nparts", "flag_id")
+    items = [dict(zip(keys, buf[8 * k:8 * k + 7])) for k in range(cnt)]
+    return [items[begin[c]:begin[c + 1]] for c in range(n_clusters)]
 
 
 def status_string(status: int) -> str:

@@ -35,7 +35,7 @@ def test_header_declares_the_calls_north_star_names():
 
 def test_library_exports_every_declared_symbol(sp2):
     names = _declared_symbols()
-    assert len(names) >= 17
+    assert len(names) >= 18
     for n in names:
         assert hasattr(sp2.lib, n), f"{n} declared in include/sp2.h but not exported"
     assert sorted(sp2.EXPORTS) == names          # the Python binding covers the whole header
@@ -91,3 +91,44 @@ def test_product_path_does_not_touch_the_oracle():
         if f.endswith(".py"):
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2107_02737_b200" not in src and "from paper_2107_02737_b200" not in src
+
+
+@pytest.mark.parametrize("n_tiles, resp, segs, ncl", [(528, False, 32, 74), (528, True, 32, 74), (36, True, 4, 148),
+                                                      (10, False, 4, 74), (3, True, 1, 3), (300, False, 24, 74),
+                                                      (2080, False, 64, 74), (1, False, 1, 1)])
+def test_work_schedule_covers_every_segment_once_and_is_balanced(sp2, n_tiles, resp, segs, ncl):
+    lists = sp2.debug_schedule(n_tiles, resp, segs, ncl)
+    n_units = n_tiles * (2 if resp else 1)
+    cost = lambda u: 2 * segs if (resp and u < n_tiles) else segs
+    cover = {u: [0] * cost(u) for u in range(n_units)}
+    loads, owners, contribs = [], {}, {}
+    for items in lists:
+        load, seen_owner = 0, False
+        for it in items:
+            assert 0 <= it["seg0"] < it["seg1"] <= cost(it["unit"])
+            for sgm in range(it["seg0"], it["seg1"]):
+                cover[it["unit"]][sgm] += 1
+            load += it["seg1"] - it["seg0"]
+            if it["kind"] == 2:
+                seen_owner = True
+                owners[it["unit"]] = it
+            else:
+                assert not seen_owner              # owners (which wait) come last: no wait cycles
+            if it["kind"] == 1:
+                contribs.setdefault(it["unit"], []).append(it)
+            if it["kind"] == 0:
+                assert (it["seg0"], it["seg1"]) == (0, cost(it["unit"]))
+        loads.append(load)
+    assert all(v == 1 for u in cover for v in cover[u])           # every segment exactly once
+    total = sum(cost(u) for u in range(n_units))
+    assert max(loads) == -(-total // ncl)                         # optimal makespan, in segments
+    assert sum(loads) == total and max(loads) - min(loads) < ncl
+    assert set(owners) == set(contribs)
+    slots = []
+    for u, own in owners.items():
+        cs = contribs[u]
+        assert own["nparts"] == len(cs) and all(c["flag_id"] == own["flag_id"] for c in cs)
+        assert sorted(c["slot"] for c in cs) == list(range(own["slot"], own["slot"] + own["nparts"]))
+        slots += [c["slot"] for c in cs]
+    assert len(set(slots)) == len(slots) and len(slots) <= 2 * ncl
+    assert len({o["flag_id"] for o in owners.values()}) == len(owners)
