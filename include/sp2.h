@@ -77,9 +77,14 @@ typedef struct {
   int forced_layers;      /* debug: > 0 runs exactly this many layers, no stop test */
   unsigned long long forced_signs; /* debug: with forced_layers, bit n = 1 -> layer n is X^2, else 2X - X^2 */
   int cta_group;    /* 0 = auto; 1 = 128x128 tiles, one CTA; 2 = 256x256 tiles on a CTA pair (cta_group::2) */
-  int seg_kb;       /* 0 = default (4); 1, 2 or 4: k-blocks of 64 accumulated inside the tensor core before the
-                       FP32 round-to-nearest add in registers (shorter = less truncation bias) */
+  int seg_kb;       /* 0 = default (4); 1, 2, 4, 8, 16 or 32 (must divide npad/64): k-blocks of 64 accumulated inside
+                       the tensor core before the FP32 round-to-nearest add in registers (shorter = less
+                       truncation bias, more drains) */
+  int seg_first;    /* 0 = default (1 = off): segments merged into each of the first two TMEM hand-offs of a work
+                       unit (longer run-ahead during the previous epilogue; measured no gain, more truncation bias) */
   int no_recentre;  /* debug, with forced_layers only: keep c on the scalar map instead of c = tr(X)/N */
+  int debug_flags;  /* performance experiments only (results are WRONG): 1 = skip the epilogue's global loads/stores,
+                       2 = issue only the hi*hi product */
 } sp2_options_t;
 
 typedef struct {

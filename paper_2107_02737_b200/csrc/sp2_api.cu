@@ -118,7 +118,7 @@ struct sp2_handle_s {
   sp2_options_t opt;
   PFN_cuTensorMapEncodeTiled_v12000 encode;
   // per-(N, cta_group) cache
-  int cur_n, cur_npad, cur_cg, cur_resp, cur_seg;
+  int cur_n, cur_npad, cur_cg, cur_resp, cur_seg, cur_dbg, cur_first;
   Sp2LayerArgs args[2];          // parity 0: buffer 0 -> 1, parity 1: buffer 1 -> 0
   std::vector<int2> tiles_host;
   std::vector<Sp2Item> items_host;
@@ -249,10 +249,12 @@ void build_schedule(int n_tiles, int resp, int segs_y, int nC, std::vector<Sp2It
 sp2_status_t encode_plane_map(sp2_handle_t h, CUtensorMap* map, const __half* base, int npad) {
   cuuint64_t gdim[2] = {(cuuint64_t)npad, (cuuint64_t)npad};
   cuuint64_t gstride[1] = {(cuuint64_t)npad * 2};
-  cuuint32_t box[2] = {64, 128};
+  const int bk = sp2_layer_box_k();
+  cuuint32_t box[2] = {(cuuint32_t)bk, 128};
   cuuint32_t estr[2] = {1, 1};
   CUresult r = h->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<__half*>(base), gdim, gstride, box, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, bk == 64 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
+                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) { h->last_cuda_error = 100000 + (int)r; return SP2_ERR_CUDA; }
   return SP2_OK;
@@ -269,8 +271,10 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   const int npad = pad_n(N);
   const int cg = pick_cta_group(h, npad);
   int seg = h->opt.seg_kb;
-  if (seg != 1 && seg != 2 && seg != 4) seg = 4;
-  if (h->cur_n == N && h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp && h->cur_seg == seg) return SP2_OK;
+  if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = 4;
+  while ((npad / 64) % seg) seg >>= 1;
+  if (h->cur_n == N && h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp && h->cur_seg == seg &&
+      h->cur_dbg == h->opt.debug_flags && h->cur_first == h->opt.seg_first) return SP2_OK;
   const int nt = npad / (128 * cg);
   build_tiles(nt, h->tiles_host);
   SP2_CUDA(h, cudaMemcpyAsync(h->tiles(), h->tiles_host.data(), h->tiles_host.size() * sizeof(int2),
@@ -279,6 +283,7 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   int nC = h->num_sms / cg;
   if (nC > kMaxClusters / cg) nC = kMaxClusters / cg;
   if (nC > n_units) nC = n_units;
+  if (h->opt.debug_flags >> 8) { int lim = h->opt.debug_flags >> 8; if (nC > lim) nC = lim; }   // experiments: fewer CTA(-pair)s
   int n_slots = 0;
   build_schedule((int)h->tiles_host.size(), resp, (npad / 64) / seg, nC, h->items_host, h->item_begin_host,
                  &h->n_flags, &n_slots);
@@ -305,10 +310,11 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
     }
     a.ctrl = h->ctrl(); a.slots = h->slots(); a.tiles = h->tiles();
     a.items = h->items(); a.item_begin = h->item_begin(); a.scratch = h->scratch(); a.flags = h->split_flags();
-    a.n_flags = h->n_flags; a.n_clusters = h->n_clusters;
+    a.n_flags = h->n_flags; a.n_clusters = h->n_clusters; a.debug_flags = h->opt.debug_flags;
+    a.seg_first = (h->opt.seg_first >= 1 && h->opt.seg_first <= 16) ? h->opt.seg_first : 1;
     a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = resp; a.seg_kb = seg;
   }
-  h->cur_n = N; h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp; h->cur_seg = seg;
+  h->cur_n = N; h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp; h->cur_seg = seg; h->cur_dbg = h->opt.debug_flags; h->cur_first = h->opt.seg_first;
   return SP2_OK;
 }
 
@@ -483,7 +489,8 @@ sp2_status_t sp2_set_options(sp2_handle_t h, const sp2_options_t* opt) {
   if (!opt) { default_options(&h->opt); return SP2_OK; }
   if (opt->engine != SP2_ENGINE_TCGEN05 && opt->engine != SP2_ENGINE_SIMT_DEBUG) return SP2_ERR_INVALID_ARG;
   if (opt->cta_group < 0 || opt->cta_group > 2) return SP2_ERR_INVALID_ARG;
-  if (opt->seg_kb != 0 && opt->seg_kb != 1 && opt->seg_kb != 2 && opt->seg_kb != 4) return SP2_ERR_INVALID_ARG;
+  if (opt->seg_kb != 0 && opt->seg_kb != 1 && opt->seg_kb != 2 && opt->seg_kb != 4 && opt->seg_kb != 8 &&
+      opt->seg_kb != 16 && opt->seg_kb != 32) return SP2_ERR_INVALID_ARG;
   if (opt->user_bounds && !(opt->eps_max > opt->eps_min)) return SP2_ERR_INVALID_ARG;
   h->opt = *opt;
   return SP2_OK;

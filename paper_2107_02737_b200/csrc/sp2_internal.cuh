@@ -140,7 +140,16 @@ __device__ inline void sp2_controller(Sp2Ctrl* c) {
   // which is known exactly before the layer runs.  tr Y' ~ 0 keeps the diagonal of Y' small and its
   // spectrum as symmetric as the occupation allows.
   const double tr_next = plus ? tr_x2 : 2.0 * tr_x - tr_x2;
-  const double c_next = (c->forced_layers > 0 && c->no_recentre) ? c_map : tr_next / N;
+  // Centre: the MIDPOINT of the two eigenvalue clusters (the occupied fraction f = N_occ/N near b, the
+  // rest near a), so that y^2 is the same for both and the tensor-core truncation bias, which is
+  // proportional to Y^2, stays a multiple of I that the trace identity removes.  For two clusters
+  // mean = a + f (b - a) and variance = f (1 - f) (b - a)^2, hence midpoint = mean + sigma (1/2 - f)/sqrt(f (1 - f));
+  // sigma is taken from the current iterate (any c is valid; it only matters near convergence, where
+  // sigma has settled).  f = 1/2 gives c = tr X/N.
+  const double f_occ = nocc / N;
+  const double var_x = fmax(tr_x2 / N - (tr_x / N) * (tr_x / N), 0.0);
+  const double c_mid = tr_next / N + sqrt(var_x) * (0.5 - f_occ) / sqrt(f_occ * (1.0 - f_occ));
+  const double c_next = (c->forced_layers > 0 && c->no_recentre) ? c_map : fmin(fmax(c_mid, 0.0), 1.0);
   const double dshift = c_map - c_next;
   // bounds on max|Y'|, max|Z'|: |(Y^2)_ij| <= ||Y||_2^2 and
   // ||Y||_2 <= min(||Y||_F, s) with s = max(c, 1-c) because spec(X) is inside [0,1].

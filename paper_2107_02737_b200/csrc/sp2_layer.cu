@@ -25,13 +25,21 @@
 
 namespace {
 
-constexpr int kBK = 64;                       // k elements per stage (128 bytes: SWIZZLE_128B row)
+// Shared-memory ring: the feed is latency-bound (one stage = 4 TMA boxes takes ~2700 cycles to land,
+// measured), so what matters is the number of BYTES in flight.  Stages of 32 k-elements (32 KB) x 7
+// keep up to 192 KB in flight; 64 x 3 only 128 KB.
+constexpr int kBK = 32;                       // k elements per stage (64-byte rows: SWIZZLE_64B)
 constexpr int kRows = 128;                    // rows per TMA box / per CTA operand tile
-constexpr int kStages = 3;
-constexpr int kPlaneTileBytes = kRows * kBK * 2;          // 16 KB
-constexpr int kStageBytes = 4 * kPlaneTileBytes;          // A0, A1, B0, B1 = 64 KB
+constexpr int kStages = 7;
+constexpr int kPlaneTileBytes = kRows * kBK * 2;          // 8 KB
+constexpr int kStageBytes = 4 * kPlaneTileBytes;          // A0, A1, B0, B1 = 32 KB
+constexpr int kSwizzleBytes = kBK * 2;                    // swizzle span = one row of the box
+static_assert(kBK == 32 || kBK == 64, "box rows are 64 or 128 bytes");
 constexpr int kThreads = 384;                 // 4 producer-side warps + 8 consumer warps
-constexpr int kConsumerWarps = 8;
+constexpr int kConsumerWarps = 8;              // warps 0..7
+// The issue arbiter favours high warp ids: the latency-critical single-thread roles sit above the consumers,
+// otherwise the 8 epilogue warps starve the MMA issuer (measured: -10 % at N = 8192).
+constexpr int kWarpTma = 8, kWarpMma = 9, kWarpAlloc = 10;
 constexpr int kRegsProducer = 40;             // setmaxnreg budgets: 128*40 + 256*232 <= 65536
 constexpr int kRegsConsumer = 232;
 constexpr long long kSpinLimit = 1ll << 26;   // mbarrier watchdog: trap instead of hanging the GPU
@@ -163,15 +171,15 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
   asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
-// K-major, SWIZZLE_128B shared-memory matrix descriptor (sm_100 format): rows of 128 bytes,
+// K-major swizzled shared-memory matrix descriptor (sm_100 format): rows of kSwizzleBytes bytes,
 // 8-row groups 1024 bytes apart.
 __device__ __forceinline__ uint64_t make_smem_desc(uint32_t saddr) {
   uint64_t d = 0;
   d |= (uint64_t)((saddr & 0x3FFFFu) >> 4);       // start address >> 4            bits [0,14)
   d |= (uint64_t)1 << 16;                         // leading byte offset (unused)  bits [16,30)
-  d |= (uint64_t)(1024 >> 4) << 32;               // stride byte offset = 1024 B   bits [32,46)
+  d |= (uint64_t)((8 * kSwizzleBytes) >> 4) << 32; // stride byte offset: 8-row group  bits [32,46)
   d |= (uint64_t)1 << 46;                         // descriptor version (sm_100)   bits [46,48)
-  d |= (uint64_t)2 << 61;                         // layout: SWIZZLE_128B          bits [61,64)
+  d |= (uint64_t)(kSwizzleBytes == 128 ? 2 : 4) << 61;  // layout: SWIZZLE_128B = 2, SWIZZLE_64B = 4   bits [61,64)
   return d;
 }
 // kind::f16 instruction descriptor: D = F32, A = B = F16, both K-major, M x N
@@ -193,6 +201,15 @@ __device__ __forceinline__ uint4 ld_global_v4(const void* p) {
   uint4 r;
   asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
   return r;
+}
+
+// streaming (evict-first) stores: the new planes are not re-read in this launch and must not push the
+// operand panels out of L2
+__device__ __forceinline__ void st_cs_v4(void* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.global.cs.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ void st_cs_u16(void* p, uint32_t v) {
+  asm volatile("st.global.cs.u16 [%0], %1;" ::"l"(p), "h"((unsigned short)v) : "memory");
 }
 
 __device__ __forceinline__ uint32_t u4_word(const uint4& v, int i) {
@@ -233,60 +250,92 @@ __device__ inline void layer_tail(Sp2Ctrl* ctrl, const Sp2Slot* slots, int n_y, 
 // gj0..gj0+31): update, split, mirrored store, partial sums.
 struct EpiPartials { double tr, fro, tracc; float mx; };
 
-__device__ __forceinline__ void epilogue_chunk(const float* acc, int gi, int gj0, size_t npad,
-                                               const __half* __restrict__ in_h, const __half* __restrict__ in_m,
-                                               __half* __restrict__ out_h, __half* __restrict__ out_m,
-                                               float a1hi, float a1lo, float a2, float dsh_hi, float dsh_lo,
-                                               EpiPartials& P) {
-  // gi = 32-aligned base + lane and gj0 is 32-aligned, so both tests are warp-uniform
-  if (gj0 + 31 < gi) return;                // chunk entirely below the diagonal: mirrored by its transpose
-  const bool full = gj0 > gi;               // chunk entirely above the diagonal
+// Old-tile prefetch buffer of the epilogue: the hi and lo words of one 32-column chunk of this
+// thread's row (4 + 4 uint4 = 32 registers), refilled one chunk ahead while the current chunk is
+// processed, so the epilogue is never stalled on a global-load round trip.
+struct EpiOld { uint4 h[4], m[4]; };
+
+__device__ __forceinline__ void epilogue_prefetch(EpiOld& o, int gi, int gj0, size_t npad,
+                                                  const __half* __restrict__ in_h, const __half* __restrict__ in_m) {
   const uint4* ph = reinterpret_cast<const uint4*>(in_h + (size_t)gi * npad + gj0);
   const uint4* pm = reinterpret_cast<const uint4*>(in_m + (size_t)gi * npad + gj0);
-  unsigned short* oh16 = reinterpret_cast<unsigned short*>(out_h);
-  unsigned short* om16 = reinterpret_cast<unsigned short*>(out_m);
-  float fsum = 0.f;
 #pragma unroll
-  for (int w = 0; w < 4; ++w) {             // 8 columns at a time keeps the live register set small
-    const uint4 oh = ld_global_v4(ph + w), om = ld_global_v4(pm + w);
-    uint32_t nh[4], nm[4];                  // packed pairs of new hi / lo halves
+  for (int w = 0; w < 4; ++w) { o.h[w] = ld_global_v4(ph + w); o.m[w] = ld_global_v4(pm + w); }
+}
+
+__device__ __forceinline__ float2 h2_to_f2(uint32_t w) {
+  return __half22float2(*reinterpret_cast<const __half2*>(&w));
+}
+__device__ __forceinline__ uint32_t f2_to_h2(float a, float b) {
+  const __half2 h = __floats2half2_rn(a, b);
+  return *reinterpret_cast<const uint32_t*>(&h);
+}
+
+// One 32-column chunk.  FULL = the chunk lies entirely above the diagonal (the common case: no
+// diagonal element, every element counts twice in ||.||_F^2 and is stored twice); the statistics
+// then use the FP32 value before the split (it differs from the stored hi+lo by an unbiased 2^-22
+// relative rounding; a non-finite value still reaches the controller through the Frobenius sum).
+// !FULL = the chunk that holds the diagonal: exact stored values, gj >= gi only, diagonal shift.
+template <bool FULL>
+__device__ __forceinline__ void epilogue_chunk(const float* acc, EpiOld& old, const uint4* next_h, const uint4* next_m,
+                                               int gi, int gj0,
+                                               size_t npad, __half* __restrict__ out_h, __half* __restrict__ out_m,
+                                               float a1hi, float a1lo, float a2, float dsh_hi, float dsh_lo,
+                                               EpiPartials& P) {
+  unsigned short* th = reinterpret_cast<unsigned short*>(out_h) + (size_t)gj0 * npad + gi;   // mirrored image
+  unsigned short* tm = reinterpret_cast<unsigned short*>(out_m) + (size_t)gj0 * npad + gi;
+  float fsum = 0.f, mx = P.mx;
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {               // 8 columns at a time keeps the live register set small
+    uint32_t nh[4], nm[4];                    // packed pairs of new hi / lo halves
+    const uint4 oh = old.h[w], om = old.m[w];
+    if (next_h) { old.h[w] = ld_global_v4(next_h + w); old.m[w] = ld_global_v4(next_m + w); }   // one chunk ahead
 #pragma unroll
     for (int pr = 0; pr < 4; ++pr) {
-      const uint32_t wh = u4_word(oh, pr), wm = u4_word(om, pr);
-      __half h0, m0, h1, m1;
-      const float old0 = __half2float(__ushort_as_half((unsigned short)(wh & 0xffffu))) +
-                         __half2float(__ushort_as_half((unsigned short)(wm & 0xffffu)));
-      const float old1 = __half2float(__ushort_as_half((unsigned short)(wh >> 16))) +
-                         __half2float(__ushort_as_half((unsigned short)(wm >> 16)));
+      const float2 fh = h2_to_f2(u4_word(oh, pr)), fm = h2_to_f2(u4_word(om, pr));
+      const float old0 = fh.x + fm.x, old1 = fh.y + fm.y;
       const int ci = 8 * w + 2 * pr;
-      const int gja = gj0 + ci, gjb = gja + 1;
-      const float s0 = sp2_epilogue_elem(old0, acc[ci], a1hi, a1lo, a2, gja == gi ? dsh_hi : 0.f,
-                                         gja == gi ? dsh_lo : 0.f, h0, m0);
-      const float s1 = sp2_epilogue_elem(old1, acc[ci + 1], a1hi, a1lo, a2, gjb == gi ? dsh_hi : 0.f,
-                                         gjb == gi ? dsh_lo : 0.f, h1, m1);
-      nh[pr] = (uint32_t)__half_as_ushort(h0) | ((uint32_t)__half_as_ushort(h1) << 16);
-      nm[pr] = (uint32_t)__half_as_ushort(m0) | ((uint32_t)__half_as_ushort(m1) << 16);
-      const float wa = (gja > gi) ? 2.f : (gja == gi ? 1.f : 0.f);
-      const float wb = (gjb > gi) ? 2.f : (gjb == gi ? 1.f : 0.f);
-      fsum = fmaf(wa * s0, s0, fsum);
-      fsum = fmaf(wb * s1, s1, fsum);
-      if (gja == gi) { P.tr += (double)s0; P.tracc += (double)acc[ci]; }
-      if (gjb == gi) { P.tr += (double)s1; P.tracc += (double)acc[ci + 1]; }
-      if (gja >= gi) P.mx = (fabsf(s0) > P.mx || s0 != s0) ? fabsf(s0) : P.mx;
-      if (gjb >= gi) P.mx = (fabsf(s1) > P.mx || s1 != s1) ? fabsf(s1) : P.mx;
-    }
-    if (full) {
-      *reinterpret_cast<uint4*>(out_h + (size_t)gi * npad + gj0 + 8 * w) = make_uint4(nh[0], nh[1], nh[2], nh[3]);
-      *reinterpret_cast<uint4*>(out_m + (size_t)gi * npad + gj0 + 8 * w) = make_uint4(nm[0], nm[1], nm[2], nm[3]);
-#pragma unroll
-      for (int pr = 0; pr < 4; ++pr) {      // mirrored image: lanes = consecutive rows -> 64 B per store
-        const size_t r0 = (size_t)(gj0 + 8 * w + 2 * pr) * npad + gi;
-        oh16[r0] = (unsigned short)(nh[pr] & 0xffffu);
-        om16[r0] = (unsigned short)(nm[pr] & 0xffffu);
-        oh16[r0 + npad] = (unsigned short)(nh[pr] >> 16);
-        om16[r0 + npad] = (unsigned short)(nm[pr] >> 16);
+      float y0 = fmaf(a1hi, old0, fmaf(a1lo, old0, a2 * acc[ci]));
+      float y1 = fmaf(a1hi, old1, fmaf(a1lo, old1, a2 * acc[ci + 1]));
+      if (!FULL) {
+        if (gj0 + ci == gi) y0 = (y0 + dsh_lo) + dsh_hi;
+        if (gj0 + ci + 1 == gi) y1 = (y1 + dsh_lo) + dsh_hi;
       }
-    } else {                                // the chunk that holds the diagonal: element-wise, gj >= gi only
+      nh[pr] = f2_to_h2(y0, y1);
+      const float2 hb = h2_to_f2(nh[pr]);
+      nm[pr] = f2_to_h2(y0 - hb.x, y1 - hb.y);
+      if (FULL) {
+        fsum = fmaf(y0, y0, fsum);
+        fsum = fmaf(y1, y1, fsum);
+        mx = fmaxf(mx, fmaxf(fabsf(y0), fabsf(y1)));
+      } else {
+        const float2 mb = h2_to_f2(nm[pr]);
+        const float s0 = hb.x + mb.x, s1 = hb.y + mb.y;
+        const int gja = gj0 + ci, gjb = gja + 1;
+        const float wa = (gja > gi) ? 2.f : (gja == gi ? 1.f : 0.f);
+        const float wb = (gjb > gi) ? 2.f : (gjb == gi ? 1.f : 0.f);
+        fsum = fmaf(wa * s0, s0, fsum);
+        fsum = fmaf(wb * s1, s1, fsum);
+        if (gja == gi) { P.tr += (double)s0; P.tracc += (double)acc[ci]; }
+        if (gjb == gi) { P.tr += (double)s1; P.tracc += (double)acc[ci + 1]; }
+        if (gja >= gi) mx = fmaxf(mx, fabsf(s0));
+        if (gjb >= gi) mx = fmaxf(mx, fabsf(s1));
+      }
+    }
+    if (FULL) {
+      st_cs_v4(out_h + (size_t)gi * npad + gj0 + 8 * w, nh[0], nh[1], nh[2], nh[3]);
+      st_cs_v4(out_m + (size_t)gi * npad + gj0 + 8 * w, nm[0], nm[1], nm[2], nm[3]);
+#pragma unroll
+      for (int pr = 0; pr < 4; ++pr) {        // lanes = consecutive rows -> 64 contiguous bytes per warp store
+        st_cs_u16(th, nh[pr] & 0xffffu);
+        st_cs_u16(tm, nm[pr] & 0xffffu);
+        st_cs_u16(th + npad, nh[pr] >> 16);
+        st_cs_u16(tm + npad, nm[pr] >> 16);
+        th += 2 * npad; tm += 2 * npad;
+      }
+    } else {
+      unsigned short* oh16 = reinterpret_cast<unsigned short*>(out_h);
+      unsigned short* om16 = reinterpret_cast<unsigned short*>(out_m);
 #pragma unroll
       for (int pr = 0; pr < 4; ++pr) {
 #pragma unroll
@@ -300,12 +349,38 @@ __device__ __forceinline__ void epilogue_chunk(const float* acc, int gi, int gj0
       }
     }
   }
-  P.fro += (double)fsum;
+  P.mx = mx;
+  P.fro += (double)(FULL ? 2.f * fsum : fsum);
+}
+
+// Fused epilogue of this thread's row over NCH chunks of 32 columns held in registers
+// (acc[0 .. 32 NCH) = FP32 sums of row gi, columns j0 ..): update, split, mirrored store, partial sums.
+// `old` holds chunk 0 on entry and is refilled one chunk ahead.
+template <int NCH>
+__device__ __forceinline__ void epilogue_row(const float* acc, EpiOld& old, int gi, int j0, size_t npad,
+                                             const __half* __restrict__ in_h, const __half* __restrict__ in_m,
+                                             __half* __restrict__ out_h, __half* __restrict__ out_m,
+                                             float a1hi, float a1lo, float a2, float dsh_hi, float dsh_lo,
+                                             EpiPartials& P) {
+#pragma unroll
+  for (int ch = 0; ch < NCH; ++ch) {
+    const int gj0 = j0 + ch * 32;
+    const uint4* nxh = (ch + 1 < NCH) ? reinterpret_cast<const uint4*>(in_h + (size_t)gi * npad + gj0 + 32) : nullptr;
+    const uint4* nxm = (ch + 1 < NCH) ? reinterpret_cast<const uint4*>(in_m + (size_t)gi * npad + gj0 + 32) : nullptr;
+    // gi = 32-aligned base + lane and gj0 is 32-aligned, so both tests are warp-uniform
+    if (gj0 > gi) {                           // entirely above the diagonal
+      epilogue_chunk<true>(&acc[ch * 32], old, nxh, nxm, gi, gj0, npad, out_h, out_m, a1hi, a1lo, a2, dsh_hi, dsh_lo, P);
+    } else if (gj0 + 31 >= gi) {              // holds the diagonal
+      epilogue_chunk<false>(&acc[ch * 32], old, nxh, nxm, gi, gj0, npad, out_h, out_m, a1hi, a1lo, a2, dsh_hi, dsh_lo, P);
+    } else if (nxh) {                         // entirely below: mirrored by its transpose; keep the prefetch rolling
+      epilogue_prefetch(old, gi, gj0 + 32, npad, in_h, in_m);
+    }
+  }
 }
 
 // ----------------------------------------------------------------------------------------------
-// Warp roles (384 threads): warp 0 TMA producer, warp 1 MMA issuer, warp 2 TMEM allocator, warp 3
-// idle; warps 4..11 consumers.  The k range of a unit is cut into segments of seg_kb k-blocks; each
+// Warp roles (384 threads): warps 0..7 consumers; warp 8 TMA producer, warp 9 MMA issuer, warp 10 TMEM
+// allocator, warp 11 idle.  The k range of a unit is cut into segments of seg_kb k-blocks; each
 // segment is accumulated by the tensor core into a fresh TMEM buffer (2 buffers, ping-pong) and
 // the consumers add the finished segment into FP32 register sums with round-to-nearest adds.
 // This bounds the length of the truncating in-TMEM accumulation (DESIGN.md "Tensor-core
@@ -325,7 +400,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
   SmemBarriers* bars = reinterpret_cast<SmemBarriers*>(smem + kStages * kStageBytes);
-  __shared__ double red[4 * 256];
+  double* red = reinterpret_cast<double*>(smem);   // the ring is idle when the tail reduction runs
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = (CG == 2) ? cluster_ctarank() : 0u;
@@ -333,27 +408,27 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   const bool leader = (rank == 0);
 
   const int n_tiles = a.n_tiles;
-  const int KB = a.npad / kBK;
-  const int seg_kb = a.seg_kb;            // k-blocks per TMEM accumulation segment (divides KB)
+  const int KB = a.npad / kBK;            // ring stages per k sweep
+  const int seg_kb = a.seg_kb * (64 / kBK);   // ring stages per TMEM accumulation segment (divides KB)
   const int item_lo = a.item_begin[cluster_id], item_hi = a.item_begin[cluster_id + 1];
 
-  if (warp == 0 && lane == 0) {
+  if (warp == kWarpTma && lane == 0) {
     for (int i = 0; i < 4; ++i) asm volatile("prefetch.tensormap [%0];" ::"l"(&a.tm[i]) : "memory");
   }
-  if (warp == 1 && lane == 0) {
+  if (warp == kWarpMma && lane == 0) {
     for (int s = 0; s < kStages; ++s) { mbar_init(smem_u32(&bars->full[s]), 1); mbar_init(smem_u32(&bars->empty[s]), 1); }
     for (int s = 0; s < 2; ++s) { mbar_init(smem_u32(&bars->tmem_full[s]), 1); mbar_init(smem_u32(&bars->tmem_empty[s]), kConsumerWarps * CG); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 2) tmem_alloc<CG>(smem_u32(&bars->tmem_base), TMEM_COLS);
+  if (warp == kWarpAlloc) tmem_alloc<CG>(smem_u32(&bars->tmem_base), TMEM_COLS);
   tc_fence_before();
   if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(&bars->tmem_base);
 
-  if (warp < 4) {
+  if (warp >= kConsumerWarps) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsProducer));
-    if (warp == 0) {
+    if (warp == kWarpTma) {
       // =================================== TMA producer (one lane, every CTA) ==================
       if (elect_one()) {
         int stage = 0; uint32_t phase = 0;
@@ -388,18 +463,22 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
           }
         }
       }
-    } else if (warp == 1) {
+    } else if (warp == kWarpMma) {
       // =================================== MMA issuer (one lane of the leader CTA) ==============
       if (leader && elect_one()) {
         int stage = 0; uint32_t phase = 0;
         int as = 0; uint32_t aphase = 0;
         for (int iti = item_lo; iti < item_hi; ++iti) {
           const Sp2Item I = a.items[iti];
-          for (int sg = I.seg0; sg < I.seg1; ++sg) {
+          for (int sg = I.seg0, ho = 0; sg < I.seg1; ++ho) {
+            // the first two hand-offs of an item are longer, so that the tensor core has work while the
+            // consumers are still in the previous unit's epilogue
+            const int len = (ho < 2) ? min(a.seg_first, I.seg1 - sg) : 1;
+            sg += len;
             mbar_wait(smem_u32(&bars->tmem_empty[as]), aphase ^ 1u);
             tc_fence_after();
             const uint32_t acc = tmem_base + (uint32_t)(as * ACC_COLS);
-            for (int it = 0; it < seg_kb; ++it) {
+            for (int it = 0; it < len * seg_kb; ++it) {
               mbar_wait(smem_u32(&bars->full[stage]), phase);
               tc_fence_after();
               const uint32_t sa = smem_u32(smem + stage * kStageBytes);
@@ -411,9 +490,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
               for (int k = 0; k < kBK / 16; ++k) {
                 const uint64_t ko = (uint64_t)(k * 2);     // 16 elements * 2 B = 32 B -> >>4 = 2
                 // small cross terms first, the dominant hi*hi product last
-                umma_f16<CG>(acc, dA0 + ko, dB1 + ko, IDESC, (it | k) ? 1u : 0u);
-                umma_f16<CG>(acc, dA1 + ko, dB0 + ko, IDESC, 1u);
-                umma_f16<CG>(acc, dA0 + ko, dB0 + ko, IDESC, 1u);
+                if (!(a.debug_flags & 2)) {
+                  umma_f16<CG>(acc, dA0 + ko, dB1 + ko, IDESC, (it | k) ? 1u : 0u);
+                  umma_f16<CG>(acc, dA1 + ko, dB0 + ko, IDESC, 1u);
+                  umma_f16<CG>(acc, dA0 + ko, dB0 + ko, IDESC, 1u);
+                } else {
+                  umma_f16<CG>(acc, dA0 + ko, dB0 + ko, IDESC, (it | k) ? 1u : 0u);
+                }
               }
               umma_commit<CG>(smem_u32(&bars->empty[stage]));   // smem slot free when these MMAs retire
               if (++stage == kStages) { stage = 0; phase ^= 1u; }
@@ -427,7 +510,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   } else {
     // ===================================== consumer warps (8 per CTA) ===========================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsConsumer));
-    const int cw = warp - 4;
+    const int cw = warp;
     const int q = warp & 3;                       // TMEM lane quarter this warp may read
     const int hh = cw >> 2;                       // which half of the accumulator columns
     const Sp2Coef cf = a.ctrl->coef;
@@ -438,11 +521,19 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
       const bool wunit = a.with_response && u < n_tiles;
       const int2 tij = a.tiles[wunit ? u : (a.with_response ? u - n_tiles : u)];
       float sums[WCOLS];
-      for (int sg = I.seg0; sg < I.seg1; ++sg) {
+      const int pl = wunit ? 2 : 0;
+      const int gi = tij.x * TILE + (int)rank * kRows + q * 32 + lane;   // global row of this thread
+      const int j0 = tij.y * TILE + hh * WCOLS;
+      EpiOld old;
+      for (int sg = I.seg0, ho = 0; sg < I.seg1; ++ho) {
+        const int len = (ho < 2) ? min(a.seg_first, I.seg1 - sg) : 1;     // same hand-off lengths as the MMA issuer
+        sg += len;
+        // the old tile's first chunk is fetched under the last hand-off's MMAs
+        if (sg == I.seg1 && I.kind != 1) epilogue_prefetch(old, gi, j0, (size_t)a.npad, a.in[pl], a.in[pl + 1]);
         mbar_wait(smem_u32(&bars->tmem_full[as]), aphase);
         tc_fence_after();
         const uint32_t tcol = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * ACC_COLS + hh * WCOLS);
-        if (sg == I.seg0) {
+        if (ho == 0) {
 #pragma unroll
           for (int ch = 0; ch < NCH; ++ch) {
             uint32_t v[32];
@@ -453,6 +544,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
         } else {
 #pragma unroll
           for (int ch = 0; ch < NCH; ++ch) {
+            if ((a.debug_flags & 4) && ch > 0) break;      // experiment: drain a quarter of the accumulator
             uint32_t v[32];
             tmem_ld32(tcol + ch * 32, v);
 #pragma unroll
@@ -493,18 +585,19 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
         }
       }
       // ---- fused epilogue from the register sums
-      const int pl = wunit ? 2 : 0;
       const float a1hi = wunit ? cf.a1z_hi : cf.a1y_hi, a1lo = wunit ? cf.a1z_lo : cf.a1y_lo;
       const float a2 = wunit ? cf.a2z : cf.a2y;
-      const int gi = tij.x * TILE + (int)rank * kRows + q * 32 + lane;   // global row of this thread
       const bool shift_row = !wunit && gi < a.n;        // zero padding stays zero
       const float dsh_hi = shift_row ? cf.dsh_hi : 0.f, dsh_lo = shift_row ? cf.dsh_lo : 0.f;
-      const int j0 = tij.y * TILE + hh * WCOLS;
       EpiPartials P; P.tr = 0.0; P.fro = 0.0; P.tracc = 0.0; P.mx = 0.f;
+      if (a.debug_flags & 1) {
+        float t = 0.f;
 #pragma unroll
-      for (int ch = 0; ch < NCH; ++ch)
-        epilogue_chunk(&sums[ch * 32], gi, j0 + ch * 32, (size_t)a.npad, a.in[pl], a.in[pl + 1], a.out[pl], a.out[pl + 1],
-                       a1hi, a1lo, a2, dsh_hi, dsh_lo, P);
+        for (int c = 0; c < WCOLS; ++c) t += sums[c];
+        P.fro = (double)t;
+      } else
+        epilogue_row<NCH>(sums, old, gi, j0, (size_t)a.npad, a.in[pl], a.in[pl + 1], a.out[pl], a.out[pl + 1],
+                          a1hi, a1lo, a2, dsh_hi, dsh_lo, P);
       // warp partial -> slot (fixed shuffle tree: deterministic)
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {
@@ -524,7 +617,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   // ===================================== teardown ==============================================
   tc_fence_before();
   if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
-  if (warp == 2) tmem_dealloc<CG>(tmem_base, TMEM_COLS);
+  if (warp == kWarpAlloc) tmem_dealloc<CG>(tmem_base, TMEM_COLS);
 
   const int per_unit = CG * kConsumerWarps;
   const int n_z = a.with_response ? n_tiles * per_unit : 0;
@@ -609,6 +702,8 @@ __global__ void __launch_bounds__(256) k_layer_simt(Sp2LayerArgs a) {
 }  // namespace
 
 // ----------------------------------------------------------------------------------------------
+int sp2_layer_box_k() { return kBK; }
+
 size_t sp2_layer_smem_bytes() { return (size_t)kStages * kStageBytes + sizeof(SmemBarriers) + 1024; }
 
 int sp2_layer_slots(int npad, int cta_group, int with_response, int engine) {

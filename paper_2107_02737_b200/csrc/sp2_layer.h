@@ -16,7 +16,7 @@ struct Sp2Item {
 };
 
 // Arguments of one layer launch.  tm[] are TMA descriptors of the INPUT planes (Yh, Ym, Zh, Zm):
-// 2-D FP16 tensors npad x npad, box 64 (k) x 128 (rows), SWIZZLE_128B.
+// 2-D FP16 tensors npad x npad, box sp2_layer_box_k() (k) x 128 (rows), swizzle = box row bytes.
 struct alignas(64) Sp2LayerArgs {
   CUtensorMap tm[4];
   const __half* in[4];   // the same input planes as raw pointers (epilogue reads the old tile)
@@ -29,6 +29,8 @@ struct alignas(64) Sp2LayerArgs {
   float* scratch;        // split-k partial sums
   unsigned int* flags;   // one arrival counter per split unit (zero between launches)
   int n_flags;
+  int seg_first;         // segments merged into each of the first two TMEM hand-offs of an item
+  int debug_flags;       // sp2_options_t.debug_flags
   int n_clusters;        // CTA(-pair)s the work lists were built for (= grid size / cta_group)
   int n;                 // true dimension (rows/cols >= n are zero padding and stay zero)
   int npad;              // padded dimension (multiple of the tile edge)
@@ -38,6 +40,7 @@ struct alignas(64) Sp2LayerArgs {
 };
 
 size_t sp2_layer_smem_bytes();
+int sp2_layer_box_k();   // k extent of the TMA box (32: SWIZZLE_64B, 64: SWIZZLE_128B)
 int sp2_layer_slots(int npad, int cta_group, int with_response, int engine);
 cudaError_t sp2_layer_configure();
 cudaError_t sp2_launch_layer(const Sp2LayerArgs& args, int engine, int cta_group, cudaStream_t s);
