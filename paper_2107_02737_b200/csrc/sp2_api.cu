@@ -128,6 +128,7 @@ struct sp2_handle_s {
   int time_layers;               // record evl0/evl1 around the layer launches of the next solve
   sp2_result_t* h_result;        // pinned
   int last_cuda_error;
+  int layers_hint;               // layers + slack of the last converged solve of the current shape (0 = unknown)
   unsigned long long launches;
   // sequence state
   int seq_active, seq_N, seq_nocc, seq_steps;
@@ -282,7 +283,7 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   int n_units = (int)h->tiles_host.size() * (resp ? 2 : 1);
   int nC = h->num_sms / cg;
   if (nC > kMaxClusters / cg) nC = kMaxClusters / cg;
-  if (nC > n_units) nC = n_units;
+  (void)n_units;   // fewer units than CTA(-pair)s: the schedule splits them along k, every SM gets work
   if (h->opt.debug_flags >> 8) { int lim = h->opt.debug_flags >> 8; if (nC > lim) nC = lim; }   // experiments: fewer CTA(-pair)s
   int n_slots = 0;
   build_schedule((int)h->tiles_host.size(), resp, (npad / 64) / seg, nC, h->items_host, h->item_begin_host,
@@ -314,6 +315,7 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
     a.seg_first = (h->opt.seg_first >= 1 && h->opt.seg_first <= 16) ? h->opt.seg_first : 1;
     a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = resp; a.seg_kb = seg;
   }
+  h->layers_hint = 0;
   h->cur_n = N; h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp; h->cur_seg = seg; h->cur_dbg = h->opt.debug_flags; h->cur_first = h->opt.seg_first;
   return SP2_OK;
 }
@@ -332,18 +334,44 @@ sp2_status_t check_args(sp2_handle_t h, const void* H, const void* H1, int want_
   return SP2_OK;
 }
 
-// enqueue one whole solve on `s`; the result struct lands in ring[ring_idx]
+// enqueue layer launches [first, first + count) on `s`
+sp2_status_t enqueue_layers(sp2_handle_t h, int first, int count, cudaStream_t s, int* launches) {
+  for (int n = first; n < first + count; ++n) {
+    cudaError_t e = sp2_launch_layer(h->args[n & 1], h->opt.engine, h->cur_cg, s);
+    if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
+    ++*launches;
+  }
+  return SP2_OK;
+}
+
+sp2_status_t enqueue_finalise(sp2_handle_t h, const void* H, sp2_dtype_t in_dt, long ldh, int N, int resp, void* D, void* D1,
+                              sp2_dtype_t out_dt, long ldd, int ring_idx, cudaStream_t s, int* launches) {
+  __half* planes[8] = {h->plane(0, 0), h->plane(1, 0), h->plane(0, 1), h->plane(1, 1),
+                       h->plane(resp ? 2 : 0, 0), h->plane(resp ? 3 : 1, 0), h->plane(resp ? 2 : 0, 1), h->plane(resp ? 3 : 1, 1)};
+  sp2_launch_finalise(h->ctrl(), planes, h->cur_npad, H, in_dt, ldh, D, resp ? D1 : nullptr, out_dt, ldd, N, h->fslots(),
+                      h->ring() + ring_idx, s);
+  *launches += 2;
+  return SP2_OK;
+}
+
+int effective_max_layers(const sp2_options_t& o) {
+  if (o.forced_layers > 0) return o.forced_layers > 64 ? 64 : o.forced_layers;
+  return o.max_layers <= 0 ? 100 : (o.max_layers > 126 ? 126 : o.max_layers);
+}
+
+// enqueue one whole solve on `s`; the result struct lands in ring[ring_idx].  Only `n_layers` of the
+// max_layers layer launches are enqueued (the caller tops up if the solve turns out unfinished:
+// k_finalise_reduce then reports SP2_INTERNAL_INCOMPLETE).
 sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const void* H1, sp2_dtype_t in_dt, long ldh, int N, int N_occ,
                            double tol, void* D, void* D1, sp2_dtype_t out_dt, long ldd, int ring_idx, cudaStream_t s,
-                           int* launches_out) {
+                           int n_layers, int* launches_out) {
   const int resp = (H1 != nullptr) ? 1 : 0;
   sp2_status_t st = prepare(h, N, resp, s);
   if (st != SP2_OK) return st;
   const int npad = h->cur_npad;
   const sp2_options_t& o = h->opt;
-  int max_layers = o.max_layers <= 0 ? 100 : (o.max_layers > 126 ? 126 : o.max_layers);
-  int forced = o.forced_layers > 0 ? (o.forced_layers > 64 ? 64 : o.forced_layers) : 0;
-  if (forced) max_layers = forced;
+  const int max_layers = effective_max_layers(o);
+  const int forced = o.forced_layers > 0 ? max_layers : 0;
   int launches = 0;
   Sp2Ctrl* c = h->ctrl();
   sp2_launch_init(c, N, N_occ, npad, resp, max_layers, o.user_bounds, o.eps_min, o.eps_max, tol, forced, o.forced_signs, o.no_recentre, s);
@@ -358,17 +386,10 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const void* H1, sp2_dt
     sp2_launch_rescale(H, in_dt, ldh, c, 0, h->plane(0, 0), h->plane(1, 0), npad, h->slots(), s); ++launches;
     sp2_launch_ctrl0(c, h->slots(), h->slots2(), sp2_rescale_blocks(npad), s); ++launches;
     if (h->time_layers) SP2_CUDA(h, cudaEventRecord(h->evl0, s));
-    for (int n = 0; n < max_layers; ++n) {
-      cudaError_t e = sp2_launch_layer(h->args[n & 1], o.engine, h->cur_cg, s);
-      if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
-      ++launches;
-    }
+    st = enqueue_layers(h, 0, n_layers, s, &launches);
+    if (st != SP2_OK) return st;
     if (h->time_layers) SP2_CUDA(h, cudaEventRecord(h->evl1, s));
-    __half* planes[8] = {h->plane(0, 0), h->plane(1, 0), h->plane(0, 1), h->plane(1, 1),
-                         h->plane(resp ? 2 : 0, 0), h->plane(resp ? 3 : 1, 0), h->plane(resp ? 2 : 0, 1), h->plane(resp ? 3 : 1, 1)};
-    sp2_launch_finalise(c, planes, npad, H, in_dt, ldh, D, resp ? D1 : nullptr, out_dt, ldd, N, h->fslots(),
-                        h->ring() + ring_idx, s);
-    launches += 2;
+    enqueue_finalise(h, H, in_dt, ldh, N, resp, D, D1, out_dt, ldd, ring_idx, s, &launches);
   }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
@@ -405,26 +426,48 @@ sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const void* H1, sp2_d
   }
   int launches = 0;
   const bool layers_timed = !(N_occ == 0 || N_occ == N);
+  // The layer count is only known on the device.  Launch as many layers as the previous solve of this
+  // shape needed (+ slack) instead of max_layers early-exit launches; if the solve turns out unfinished,
+  // top up once with the rest (the answer is the same: the device controller decides when to stop).
+  const int max_layers = effective_max_layers(h->opt);
+  int n_first = max_layers;
+  if (h->opt.forced_layers <= 0 && h->layers_hint > 0 && h->layers_hint < max_layers) n_first = h->layers_hint;
   h->time_layers = 1;
-  st = enqueue_solve(h, dH, dH1, in_dt, dld_in, N, N_occ, tol, dD, dD1, out_dt, dld_out, 0, s, &launches);
+  st = enqueue_solve(h, dH, dH1, in_dt, dld_in, N, N_occ, tol, dD, dD1, out_dt, dld_out, 0, s, n_first, &launches);
   h->time_layers = 0;
   if (st != SP2_OK) return st;
-  if (host_buffers) {
-    SP2_CUDA(h, cudaMemcpy2DAsync(D, (size_t)ldd * out_sz, dD, (size_t)N * out_sz, (size_t)N * out_sz, N,
-                                  cudaMemcpyDeviceToHost, s));
-    if (want_resp)
-      SP2_CUDA(h, cudaMemcpy2DAsync(D1, (size_t)ldd * out_sz, dD1, (size_t)N * out_sz, (size_t)N * out_sz, N,
+  float layers_ms = 0.f;
+  for (int pass = 0; pass < 2; ++pass) {
+    if (host_buffers) {
+      SP2_CUDA(h, cudaMemcpy2DAsync(D, (size_t)ldd * out_sz, dD, (size_t)N * out_sz, (size_t)N * out_sz, N,
                                     cudaMemcpyDeviceToHost, s));
+      if (want_resp)
+        SP2_CUDA(h, cudaMemcpy2DAsync(D1, (size_t)ldd * out_sz, dD1, (size_t)N * out_sz, (size_t)N * out_sz, N,
+                                      cudaMemcpyDeviceToHost, s));
+    }
+    SP2_CUDA(h, cudaMemcpyAsync(h->h_result, h->ring(), sizeof(sp2_result_t), cudaMemcpyDeviceToHost, s));
+    SP2_CUDA(h, cudaEventRecord(h->ev1, s));
+    SP2_CUDA(h, cudaStreamSynchronize(s));
+    if (layers_timed) {
+      float t = 0.f;
+      SP2_CUDA(h, cudaEventElapsedTime(&t, h->evl0, h->evl1));
+      layers_ms += t;
+    }
+    if (h->h_result->status != SP2_INTERNAL_INCOMPLETE || pass == 1) break;
+    SP2_CUDA(h, cudaEventRecord(h->evl0, s));                   // top-up: the remaining layer launches
+    st = enqueue_layers(h, n_first, max_layers - n_first, s, &launches);
+    if (st != SP2_OK) return st;
+    SP2_CUDA(h, cudaEventRecord(h->evl1, s));
+    enqueue_finalise(h, dH, in_dt, dld_in, N, want_resp, dD, dD1, out_dt, dld_out, 0, s, &launches);
+    h->launches += (unsigned long long)(max_layers - n_first + 2);
   }
-  SP2_CUDA(h, cudaMemcpyAsync(h->h_result, h->ring(), sizeof(sp2_result_t), cudaMemcpyDeviceToHost, s));
-  SP2_CUDA(h, cudaEventRecord(h->ev1, s));
-  SP2_CUDA(h, cudaStreamSynchronize(s));
   float ms = 0.f;
   SP2_CUDA(h, cudaEventElapsedTime(&ms, h->ev0, h->ev1));
   sp2_result_t r = *h->h_result;
+  if (r.status == SP2_INTERNAL_INCOMPLETE) r.status = SP2_ERR_CUDA;   // cannot happen: the top-up ran max_layers
+  if (r.status == SP2_OK && layers_timed) h->layers_hint = r.layers + 6;
   r.gpu_ms = ms;
-  r.layers_ms = 0.f;
-  if (layers_timed) SP2_CUDA(h, cudaEventElapsedTime(&r.layers_ms, h->evl0, h->evl1));
+  r.layers_ms = layers_ms;
   r.kernel_launches = launches;
   if (out) *out = r;
   return (sp2_status_t)r.status;
@@ -456,7 +499,7 @@ sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_work
   h->ws = static_cast<uint8_t*>(d_workspace); h->ws_bytes = bytes; h->L = L;
   default_options(&h->opt);
   h->cur_n = -1; h->cur_npad = -1; h->cur_cg = -1; h->cur_resp = -1; h->cur_seg = -1;
-  h->last_cuda_error = 0; h->launches = 0; h->seq_active = 0;
+  h->last_cuda_error = 0; h->launches = 0; h->seq_active = 0; h->layers_hint = 0;
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
@@ -486,13 +529,14 @@ sp2_status_t sp2_destroy(sp2_handle_t h) {
 
 sp2_status_t sp2_set_options(sp2_handle_t h, const sp2_options_t* opt) {
   if (!h) return SP2_ERR_INVALID_ARG;
-  if (!opt) { default_options(&h->opt); return SP2_OK; }
+  if (!opt) { default_options(&h->opt); h->layers_hint = 0; return SP2_OK; }
   if (opt->engine != SP2_ENGINE_TCGEN05 && opt->engine != SP2_ENGINE_SIMT_DEBUG) return SP2_ERR_INVALID_ARG;
   if (opt->cta_group < 0 || opt->cta_group > 2) return SP2_ERR_INVALID_ARG;
   if (opt->seg_kb != 0 && opt->seg_kb != 1 && opt->seg_kb != 2 && opt->seg_kb != 4 && opt->seg_kb != 8 &&
       opt->seg_kb != 16 && opt->seg_kb != 32) return SP2_ERR_INVALID_ARG;
   if (opt->user_bounds && !(opt->eps_max > opt->eps_min)) return SP2_ERR_INVALID_ARG;
   h->opt = *opt;
+  h->layers_hint = 0;
   return SP2_OK;
 }
 
@@ -545,7 +589,7 @@ sp2_status_t sp2_sequence_step(sp2_handle_t h, const void* dH_t, sp2_dtype_t in_
   sp2_status_t st = check_args(h, dH_t, nullptr, 0, in_dtype, ldh, h->seq_N, h->seq_nocc, dD_t, nullptr, out_dtype, ldd);
   if (st != SP2_OK) return st;
   st = enqueue_solve(h, dH_t, nullptr, in_dtype, ldh, h->seq_N, h->seq_nocc, h->seq_tol, dD_t, nullptr, out_dtype, ldd,
-                     h->seq_steps, h->seq_stream, nullptr);
+                     h->seq_steps, h->seq_stream, effective_max_layers(h->opt), nullptr);
   if (st == SP2_OK) ++h->seq_steps;
   return st;
 }

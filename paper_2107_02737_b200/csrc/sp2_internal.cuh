@@ -11,6 +11,7 @@
 #include <stdint.h>
 #include "sp2.h"
 
+#define SP2_INTERNAL_INCOMPLETE 100  // ring status: the enqueued layer launches ran out before the controller stopped
 #define SP2_LAYER_CAP 128          // size of the per-layer history arrays (max_layers <= 126)
 #define SP2_FP16_TARGET_LOG2 15    // planes are scaled so that (bound on max|.|) * 2^t <= 2^15 < 65504
 

@@ -258,7 +258,7 @@ __global__ void __launch_bounds__(256) k_finalise(const Sp2Ctrl* __restrict__ c,
                                                   TO* __restrict__ D, TO* __restrict__ D1, long ldo,
                                                   double* __restrict__ slots /* 3 per block */) {
   const int st = c->status;
-  if (st != SP2_OK && st != SP2_WARN_NOT_CONVERGED) return;
+  if (!c->done || (st != SP2_OK && st != SP2_WARN_NOT_CONVERGED)) return;
   const int N = c->N;
   const int par = c->n & 1;
   const __half* Yh = par ? Yh1 : Yh0;
@@ -316,7 +316,7 @@ __global__ void __launch_bounds__(256) k_finalise_reduce(Sp2Ctrl* c, const doubl
   __shared__ double red[3][256];
   const int tid = threadIdx.x;
   double a = 0, b = 0, e = 0;
-  const int st = c->status;
+  const int st = c->done ? c->status : SP2_INTERNAL_INCOMPLETE;
   const bool ok = (st == SP2_OK || st == SP2_WARN_NOT_CONVERGED);
   if (ok)
     for (int i = tid; i < count; i += 256) { a += slots[3 * i]; b += slots[3 * i + 1]; e += slots[3 * i + 2]; }
@@ -329,7 +329,7 @@ __global__ void __launch_bounds__(256) k_finalise_reduce(Sp2Ctrl* c, const doubl
   if (tid != 0) return;
   c->tr_d = red[0][0]; c->tr_dh = red[1][0]; c->tr_d1 = red[2][0];
   sp2_result_t r;
-  r.status = c->status; r.layers = c->n; r.sign_mask[0] = c->sign_mask[0]; r.sign_mask[1] = c->sign_mask[1];
+  r.status = st; r.layers = c->n; r.sign_mask[0] = c->sign_mask[0]; r.sign_mask[1] = c->sign_mask[1];
   r.stop_reason = c->stop_reason; r.reserved = 0;
   r.tr_d = c->tr_d; r.tr_dh = c->tr_dh; r.tr_d1 = c->tr_d1;
   r.idem_est = ok ? c->e[c->n] : 0.0;

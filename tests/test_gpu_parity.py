@@ -309,3 +309,25 @@ def test_sequence_call_small(sp2, torch_mod):
         assert abs(r["tr_d"] - n_occ) <= TOL_TR
         assert abs(r["tr_dh"] - ref["tr_dh"]) <= TOL_E * abs(ref["tr_dh"])
     h.close()
+
+
+def test_layer_count_hint_and_top_up(sp2, torch_mod):
+    """The host enqueues only as many layer launches as the previous solve of the same shape needed
+    (+ slack); a harder problem of the same shape must still converge through the one-off top-up."""
+    import oracle
+
+    torch = torch_mod
+    easy = inputs.make_problem(inputs.Sp2Config("easy", 1, 256, 128, (-2.0, -1.0), (1.0, 2.0), "f64", False))
+    hard = inputs.make_problem(inputs.Sp2Config("hard", 4, 256, 128, (-1.0, -0.004), (0.004, 1.0), "f64", False))
+    h = sp2.Sp2Handle(256)
+    He, Hh = torch.from_numpy(easy["H"]).cuda(), torch.from_numpy(hard["H"]).cuda()
+    D1, r1 = h.density(He, 128)                       # no hint yet: max_layers launches
+    D2, r2 = h.density(He, 128)                       # hint = layers + 6
+    assert torch.equal(D1, D2) and r1["layers"] == r2["layers"]
+    assert r2["kernel_launches"] == r1["kernel_launches"] - (100 - (r1["layers"] + 6))
+    D3, r3 = h.density(Hh, 128)                       # needs more layers than the hint: top-up
+    assert r3["status"] == 0 and r3["layers"] > r1["layers"] + 6
+    ref = oracle.sp2_density(hard["H"], 128)
+    assert np.abs(D3.cpu().numpy() - ref["D"]).max() <= TOL_D
+    assert abs(r3["tr_d"] - 128) <= TOL_TR
+    h.close()
