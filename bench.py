@@ -395,17 +395,71 @@ def run_ours(args):
     return 0
 
 
+def run_sequence(args):
+    """--workload sequence: BASELINE.json config 5 (N = 16384, N_occ = 8192, gap 0.2, f32): K consecutive MD-step
+    Hamiltonians H_t = H_0 + t 1e-3 P (formed on the device by this harness, outside the library) through
+    sp2_sequence_begin / step / end -- no host synchronisation between steps.  Extra workload, not the headline."""
+    import torch
+
+    from paper_2107_02737_b200 import inputs, sp2
+
+    rank, world, local = dist_env()
+    torch.cuda.set_device(local)
+    cfg = inputs.CONFIGS[5]
+    p = inputs.make_problem(cfg, seed=cfg.seed + rank, device="cuda", want_p=True)
+    n, n_occ = p["n"], p["n_occ"]
+    H0 = torch.from_numpy(p["H"]).cuda()
+    P = torch.from_numpy(p["P"]).cuda()
+    Ht = torch.empty_like(H0)
+    D = torch.empty_like(H0)
+    h = sp2.Sp2Handle(n)
+    for _ in range(max(args.warmup, 3)):
+        h.density(H0, n_occ, out=D)
+    stream = torch.cuda.current_stream()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local)
+    launches0 = h.launch_count
+    torch.cuda.synchronize()
+    sampler.start()
+    ev0.record(stream)
+    h.sequence_begin(n, n_occ, n_steps_hint=args.steps)
+    for t in range(args.steps):
+        torch.add(H0, P, alpha=1e-3 * t, out=Ht)        # harness, not library; stream-ordered before the step
+        h.sequence_step(Ht, D)
+    res = h.sequence_end()
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1)
+    layers = [r["layers"] for r in res]
+    flops = sum(logical_flops_per_layer(n, False) * L for L in layers)
+    line = {"metric": METRIC, "value": flops / (ms * 1e-3) / 1e12, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f16 hi/lo operand planes, f32 accumulate (f64 scalars)", "data": "synthetic",
+            "config": {"workload": f"config 5: N={n}, N_occ={n_occ}, gap 0.2, f32, {args.steps} consecutive H_t through "
+                                   "sp2_sequence_* (max_layers launches per step, one sync at the end)",
+                       "layers_per_step": layers, "issued_tflops": 1.5 * flops / (ms * 1e-3) / 1e12,
+                       "statuses": sorted({r["status"] for r in res}),
+                       "max_abs_trD_minus_nocc": max(abs(r["tr_d"] - n_occ) for r in res)},
+            "clocks": clocks, "gpu_launches": int(h.launch_count - launches0)}
+    print(json.dumps(line), flush=True)
+    h.close()
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--workload", choices=["response", "density"], default="response")
+    ap.add_argument("--workload", choices=["response", "density", "sequence"], default="response")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args(argv)
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload == "sequence":
+        return run_sequence(args)
     return run_ours(args)
 
 

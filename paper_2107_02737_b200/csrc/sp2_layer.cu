@@ -544,7 +544,6 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
         } else {
 #pragma unroll
           for (int ch = 0; ch < NCH; ++ch) {
-            if ((a.debug_flags & 4) && ch > 0) break;      // experiment: drain a quarter of the accumulator
             uint32_t v[32];
             tmem_ld32(tcol + ch * 32, v);
 #pragma unroll
