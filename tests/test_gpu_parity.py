@@ -331,3 +331,21 @@ def test_layer_count_hint_and_top_up(sp2, torch_mod):
     assert np.abs(D3.cpu().numpy() - ref["D"]).max() <= TOL_D
     assert abs(r3["tr_d"] - 128) <= TOL_TR
     h.close()
+
+
+def test_structured_sparse_chain(sp2, torch_mod):
+    """Tight-binding chain (mostly zeros, tight bounds, few layers): a magnitude structure very unlike the
+    dense random configs -- exercises the global plane exponents on a matrix whose entries span zeros."""
+    import oracle
+
+    torch = torch_mod
+    n = 1024
+    H, lam = inputs.ssh_chain(n, 1.0, 0.6, onsite=0.3)
+    ref = oracle.sp2_density(H, n // 2)
+    h = sp2.Sp2Handle(n)
+    D, r = h.density(torch.from_numpy(H).cuda(), n // 2)
+    h.close()
+    assert r["status"] == 0 and abs(r["layers"] - ref["layers"]) <= 4 and r["layers"] <= 20
+    assert np.abs(D.cpu().numpy() - ref["D"]).max() <= TOL_D
+    assert abs(r["tr_d"] - n // 2) <= TOL_TR
+    assert abs(r["tr_dh"] - lam[: n // 2].sum()) <= TOL_E * abs(lam[: n // 2].sum())

@@ -289,3 +289,20 @@ def test_sampled_response_entries_match_the_full_closed_form():
     # and against the finite difference of the definition (independent of both closed forms)
     fd = oracle.response_finite_difference(p["H"], p["H1"], 22, eps=1e-5)
     np.testing.assert_allclose(got, fd[rows, cols], rtol=0, atol=1e-6 * np.abs(full).max())
+
+
+def test_structured_chain_tight_bounds_paper_like_layer_count():
+    """Sparse tight-binding chain with TIGHT Gershgorin bounds: closed-form spectrum, and the layer
+    count drops to the paper's range ("between 14 and 16 deep layers") instead of the
+    35-45 of the dense random-Q configs."""
+    n = 512
+    H, lam = inputs.ssh_chain(n, 1.0, 0.6)
+    w = np.linalg.eigvalsh(H)
+    np.testing.assert_allclose(w, lam, atol=1e-12)                  # generator's closed form
+    lo, hi = oracle.gershgorin_bounds(H)
+    assert (lo, hi) == (-1.6, 1.6) and abs(w[0] - lo) < 1e-12       # tight
+    r = oracle.sp2_density(H, n // 2)
+    D_eig, _ = oracle.density_eigh(H, n // 2)
+    assert np.abs(r["D"] - D_eig).max() < 1e-12
+    assert 10 <= r["layers"] <= 18
+    assert r["tr_dh"] == pytest.approx(lam[: n // 2].sum(), rel=1e-12)
