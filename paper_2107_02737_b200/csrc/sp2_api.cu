@@ -261,16 +261,18 @@ sp2_status_t encode_plane_map(sp2_handle_t h, CUtensorMap* map, const __half* ba
   return SP2_OK;
 }
 
-int pick_cta_group(sp2_handle_t h, int npad) {
+// Tile shape: CTA pairs on 256x256 tiles (cta_group::2) halve the operand traffic per flop and win at large N;
+// single CTAs on 128x128 tiles have 4x more units to balance and less launch / cluster overhead and win below
+// (measured cross-over on B200: ~5600 density-only, ~4600 with response).
+int pick_cta_group(sp2_handle_t h, int npad, int resp) {
   if (h->opt.cta_group == 1 || h->opt.cta_group == 2) return h->opt.cta_group;
-  const int nt2 = npad / 256;
-  return (nt2 * (nt2 + 1) / 2 >= h->num_sms / 2) ? 2 : 1;
+  return npad >= (resp ? 4608 : 5632) ? 2 : 1;
 }
 
 // (re)build the per-problem launch state: tile list, TMA descriptors, ping-pong argument blocks
 sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   const int npad = pad_n(N);
-  const int cg = pick_cta_group(h, npad);
+  const int cg = pick_cta_group(h, npad, resp);
   int seg = h->opt.seg_kb;
   if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = 4;
   while ((npad / 64) % seg) seg >>= 1;

@@ -395,7 +395,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   constexpr uint32_t TMEM_COLS = 2 * ACC_COLS;
   constexpr uint32_t IDESC = make_idesc(UM, UN);
 
-  if (a.ctrl->done) return;               // uniform over the grid: written before this launch
+  // Programmatic dependent launch: let the next layer's CTAs be scheduled as soon as SMs free up; everything
+  // up to griddepcontrol.wait below (barrier init, TMEM allocation, work-list offsets) then overlaps the tail
+  // of the previous layer.  Nothing the previous launch wrote is read before the wait.
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
@@ -426,7 +429,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   tc_fence_after();
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(&bars->tmem_base);
 
-  if (warp >= kConsumerWarps) {
+  asm volatile("griddepcontrol.wait;" ::: "memory");    // previous layer complete, its writes visible
+  const bool active = *reinterpret_cast<volatile const int*>(&a.ctrl->done) == 0;   // uniform over the grid
+
+  if (!active) {
+    // converged (or failed) before this launch: nothing to do but release the TMEM columns
+  } else if (warp >= kConsumerWarps) {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsProducer));
     if (warp == kWarpTma) {
       // =================================== TMA producer (one lane, every CTA) ==================
@@ -617,6 +625,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   tc_fence_before();
   if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
   if (warp == kWarpAlloc) tmem_dealloc<CG>(tmem_base, TMEM_COLS);
+  if (!active) return;
 
   const int per_unit = CG * kConsumerWarps;
   const int n_z = a.with_response ? n_tiles * per_unit : 0;
@@ -736,15 +745,17 @@ cudaError_t sp2_launch_layer(const Sp2LayerArgs& args, int engine, int cta_group
   cfg.blockDim = dim3(kThreads);
   cfg.dynamicSmemBytes = sp2_layer_smem_bytes();
   cfg.stream = s;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;    // PDL: see the top of k_layer_tc
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
   if (cta_group == 2) {
     cfg.gridDim = dim3(2 * args.n_clusters);
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr; cfg.numAttrs = 1;
+    attr[1].id = cudaLaunchAttributeClusterDimension;
+    attr[1].val.clusterDim.x = 2; attr[1].val.clusterDim.y = 1; attr[1].val.clusterDim.z = 1;
+    cfg.numAttrs = 2;
     return cudaLaunchKernelEx(&cfg, k_layer_tc<2>, args);
   }
   cfg.gridDim = dim3(args.n_clusters);
-  cfg.attrs = nullptr; cfg.numAttrs = 0;
   return cudaLaunchKernelEx(&cfg, k_layer_tc<1>, args);
 }
