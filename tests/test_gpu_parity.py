@@ -349,3 +349,46 @@ def test_structured_sparse_chain(sp2, torch_mod):
     assert np.abs(D.cpu().numpy() - ref["D"]).max() <= TOL_D
     assert abs(r["tr_d"] - n // 2) <= TOL_TR
     assert abs(r["tr_dh"] - lam[: n // 2].sum()) <= TOL_E * abs(lam[: n // 2].sum())
+
+
+@pytest.mark.parametrize("n_occ", [1, 299])
+def test_extreme_occupations(sp2, torch_mod, n_occ):
+    """One occupied / one empty state: the midpoint centring of the shift goes to its limits."""
+    import oracle
+
+    torch = torch_mod
+    n = 300
+    rng = np.random.default_rng(5)
+    G = rng.standard_normal((n, n))
+    Q, _ = np.linalg.qr(G)
+    lam = np.concatenate([rng.uniform(-1.0, -0.6, n_occ), rng.uniform(0.6, 1.0, n - n_occ)])
+    H = (Q * lam) @ Q.T
+    H = 0.5 * (H + H.T)
+    ref = oracle.sp2_density(H, n_occ)
+    h = sp2.Sp2Handle(n)
+    D, r = h.density(torch.from_numpy(H).cuda(), n_occ)
+    h.close()
+    assert r["status"] == 0
+    assert np.abs(D.cpu().numpy() - ref["D"]).max() <= TOL_D
+    assert abs(r["tr_d"] - n_occ) <= TOL_TR
+    assert abs(r["tr_dh"] - ref["tr_dh"]) <= TOL_E * abs(ref["tr_dh"])
+
+
+@pytest.mark.parametrize("scale, shift", [(1e6, 0.0), (1e-6, 0.0), (1.0, 1e3)])
+def test_scale_and_shift_invariance(sp2, torch_mod, scale, shift):
+    """D(aH + bI) = D(H) for a > 0: the input layer removes scale and offset, and the
+    plane exponents must follow magnitudes far from 1."""
+    torch = torch_mod
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[2], 320), want_h1=True)
+    n, n_occ = p["n"], p["n_occ"]
+    h = sp2.Sp2Handle(n, response=True)
+    H = torch.from_numpy(p["H"]).cuda()
+    H1 = torch.from_numpy(p["H1"]).cuda()
+    D0, D10, r0 = h.response(H, H1, n_occ)
+    Hs = scale * H + shift * torch.eye(n, dtype=H.dtype, device=H.device)
+    D, D1, r = h.response(Hs, scale * H1, n_occ)
+    h.close()
+    assert r["status"] == 0 and abs(r["layers"] - r0["layers"]) <= 2
+    assert float((D - D0).abs().max()) <= 2e-6
+    assert float((D1 - D10).abs().max()) <= 1e-4 * float(D10.abs().max())    # D1 is invariant when H1 scales with H
+    assert abs(r["tr_dh"] - (scale * r0["tr_dh"] + shift * n_occ)) <= 1e-5 * abs(scale * r0["tr_dh"] + shift * n_occ)
