@@ -82,9 +82,9 @@ typedef struct {
                        truncation bias, more drains) */
   int seg_first;    /* 0 = default (1 = off): segments merged into each of the first two TMEM hand-offs of a work
                        unit (longer run-ahead during the previous epilogue; measured no gain, more truncation bias) */
-  int no_recentre;  /* debug, with forced_layers only: keep c on the scalar map instead of c = tr(X)/N */
+  int no_recentre;  /* debug, with forced_layers only: keep c on the scalar map instead of the cluster midpoint */
   int debug_flags;  /* performance experiments only (results are WRONG): 1 = skip the epilogue's global loads/stores,
-                       2 = issue only the hi*hi product */
+                       2 = issue only the hi*hi product; bits 8-15 = cap on the number of CTA(-pair)s */
 } sp2_options_t;
 
 typedef struct {

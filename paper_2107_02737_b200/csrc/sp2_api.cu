@@ -274,7 +274,9 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   const int npad = pad_n(N);
   const int cg = pick_cta_group(h, npad, resp);
   int seg = h->opt.seg_kb;
-  if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = 4;
+  // default: 4 k-blocks per in-TMEM segment; the residual truncation bias in tr D grows ~ N * segment length
+  // (2.4e-4 at N = 16384 against the 1e-3 bar), so very large problems take shorter segments
+  if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = npad > 16384 ? 2 : 4;
   while ((npad / 64) % seg) seg >>= 1;
   if (h->cur_n == N && h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp && h->cur_seg == seg &&
       h->cur_dbg == h->opt.debug_flags && h->cur_first == h->opt.seg_first) return SP2_OK;

@@ -392,3 +392,26 @@ def test_scale_and_shift_invariance(sp2, torch_mod, scale, shift):
     assert float((D - D0).abs().max()) <= 2e-6
     assert float((D1 - D10).abs().max()) <= 1e-4 * float(D10.abs().max())    # D1 is invariant when H1 scales with H
     assert abs(r["tr_dh"] - (scale * r0["tr_dh"] + shift * n_occ)) <= 1e-5 * abs(scale * r0["tr_dh"] + shift * n_occ)
+
+
+def test_runs_on_the_callers_stream(sp2, torch_mod):
+    """All work is enqueued on the stream the caller names (here torch's current non-default stream):
+    H is produced on that stream immediately before the call, with no synchronisation in between."""
+    import oracle
+
+    torch = torch_mod
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[1], 200))
+    n, n_occ = p["n"], p["n_occ"]
+    ref = oracle.sp2_density(2.0 * p["H"], n_occ)
+    h = sp2.Sp2Handle(n)
+    s = torch.cuda.Stream()
+    Hhalf = torch.from_numpy(p["H"]).cuda()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        big = torch.randn(4096, 4096, device="cuda")
+        for _ in range(20):
+            big = big @ big * 1e-4                    # keep the stream busy so that H is late
+        H = Hhalf + Hhalf                             # produced on stream s, after the busy work
+        D, r = h.density(H, n_occ)
+    assert r["status"] == 0 and np.abs(D.cpu().numpy() - ref["D"]).max() <= TOL_D
+    h.close()
