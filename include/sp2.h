@@ -64,6 +64,7 @@ typedef enum { SP2_F32 = 0, SP2_F64 = 1 } sp2_dtype_t;
 /* flags of sp2_workspace_bytes / sp2_create */
 #define SP2_WITH_RESPONSE 1     /* room for the first-order iterate Z (sp2_response) */
 #define SP2_WITH_HOST_STAGING 2 /* room for device copies of H, H1, D, D1 (the *_host calls), f64-sized */
+#define SP2_WITH_REFINEMENT 4   /* room for two float64 N x N iterates (sp2_options_t.refine_layers > 0) */
 
 /* layer engines (sp2_options_t.engine) */
 #define SP2_ENGINE_TCGEN05 0 /* product path: TMA + tcgen05.mma + TMEM */
@@ -77,6 +78,8 @@ typedef struct {
   int forced_layers;      /* debug: > 0 runs exactly this many layers, no stop test */
   unsigned long long forced_signs; /* debug: with forced_layers, bit n = 1 -> layer n is X^2, else 2X - X^2 */
   int cta_group;    /* 0 = auto; 1 = 128x128 tiles, one CTA; 2 = 256x256 tiles on a CTA pair (cta_group::2) */
+  int refine_layers; /* 0 = off (default); 1..4: float64 SP2 layers applied to the converged iterate before D is written
+                        (the paper uses 2); D1 is not refined.  Needs SP2_WITH_REFINEMENT */
   int seg_kb;       /* 0 = default (4); 1, 2, 4, 8, 16 or 32 (must divide npad/64): k-blocks of 64 accumulated inside
                        the tensor core before the FP32 round-to-nearest add in registers (shorter = less
                        truncation bias, more drains) */
@@ -92,7 +95,7 @@ typedef struct {
   int layers;                        /* number of layers applied (paper: 14-16 for water) */
   unsigned long long sign_mask[2];   /* bit n = 1 if layer n was X^2 ('+'), 0 if 2X - X^2 ('-') */
   int stop_reason;                   /* 1 tol, 2 floor (parameter-free), 3 idempotent on entry, 4 max_layers, 5 trivial N_occ, 6 forced */
-  int reserved;
+  int reserved;                      /* number of float64 refinement layers applied */
   double tr_d;                       /* tr D (should be N_occ) */
   double tr_dh;                      /* sum_ij D_ij H_ij */
   double tr_d1;                      /* tr D1 (should be 0); 0 when no response */

@@ -14,6 +14,7 @@ from .sp2_oracle import (  # noqa: F401
     rescale_to_unit_interval,
     sp2_stop,
     sp2_density,
+    sp2_refine_layers,
     density_eigh,
     density_from_eigenpairs,
     response_closed_form,

@@ -45,6 +45,7 @@ __all__ = [
     "rescale_to_unit_interval",
     "sp2_stop",
     "sp2_density",
+    "sp2_refine_layers",
     "density_eigh",
     "density_from_eigenpairs",
     "response_closed_form",
@@ -205,6 +206,23 @@ def sp2_density(H, n_occ, H1=None, tol=0.0, max_layers=100, bounds=None):
                 eps_min=eps_min, eps_max=eps_max, tr_d=float(np.trace(X)),
                 tr_dh=float(np.sum(X * H)),
                 tr_d1=None if Z is None else float(np.trace(Z)))
+
+
+def sp2_refine_layers(X, n_occ, layers=2):
+    """Refinement step of PAPER.md:170: "two extra layers in Eq. (19), with a higher-order double-precision
+    (64 bit) representation of X in the activation function ... where the eigenvalues are purified to be closer
+    to exactly 1 and 0".  ``X`` is an (approximately idempotent) iterate; ``layers`` more SP2 layers
+    X <- X^2 or 2X - X^2 are applied in float64 with the same trace rule as ``sp2_density`` (reading R3).
+    Returns (X_refined, signs)."""
+    X = np.array(X, dtype=np.float64)
+    signs = []
+    for _ in range(layers):
+        X2 = X @ X
+        t, t2 = float(np.trace(X)), float(np.trace(X2))
+        plus = abs(t2 - n_occ) < abs(2.0 * t - t2 - n_occ)
+        X = X2 if plus else 2.0 * X - X2
+        signs.append("+" if plus else "-")
+    return X, "".join(signs)
 
 
 def density_eigh(H, n_occ):

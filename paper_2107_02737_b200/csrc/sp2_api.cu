@@ -34,6 +34,11 @@ void sp2_launch_finalise(Sp2Ctrl* c, __half* const planes[8], int npad, const vo
                          sp2_result_t* ring_entry, cudaStream_t s);
 void sp2_launch_trivial(Sp2Ctrl* c, void* D, void* D1, sp2_dtype_t out_dt, long ldo, int N, sp2_result_t* ring_entry,
                         cudaStream_t s);
+// sp2_refine.cu
+cudaError_t sp2_refine_configure();
+int sp2_launch_refine(Sp2Ctrl* c, __half* const planes[4], int npad, int N, int n_layers, double* Xa, double* Xb,
+                      double* slots, unsigned int* ticket, const void* H, sp2_dtype_t in_dt, long ldh, void* D,
+                      sp2_dtype_t out_dt, long ldo, sp2_result_t* ring_entry, cudaStream_t s);
 
 namespace {
 
@@ -56,6 +61,7 @@ struct Layout {
   size_t off_items, items_cap, off_item_begin, off_scratch, scratch_bytes, off_flags;
   size_t off_ctrl, off_ring;
   size_t off_staging, staging_each;
+  size_t off_refine, refine_each, off_refine_slots;
   size_t total;
 };
 
@@ -96,6 +102,11 @@ Layout make_layout(int n_max, int flags) {
   if (flags & SP2_WITH_HOST_STAGING) {
     L.staging_each = align_up((size_t)n_max * (size_t)n_max * 8, 1024);
     L.off_staging = off; off += L.staging_each * (resp ? 4 : 2);
+  }
+  if (flags & SP2_WITH_REFINEMENT) {
+    L.refine_each = align_up(npad * npad * sizeof(double), 1024);
+    L.off_refine = off; off += 2 * L.refine_each;
+    L.off_refine_slots = off; off += align_up((2 * npad + 64) * sizeof(double), 1024);
   }
   L.total = off;
   return L;
@@ -151,6 +162,9 @@ struct sp2_handle_s {
   Sp2Ctrl* ctrl() const { return reinterpret_cast<Sp2Ctrl*>(ws + L.off_ctrl); }
   sp2_result_t* ring() const { return reinterpret_cast<sp2_result_t*>(ws + L.off_ring); }
   void* staging(int i) const { return ws + L.off_staging + (size_t)i * L.staging_each; }
+  double* refine_x(int i) const { return reinterpret_cast<double*>(ws + L.off_refine + (size_t)i * L.refine_each); }
+  double* refine_slots() const { return reinterpret_cast<double*>(ws + L.off_refine_slots); }
+  unsigned int* refine_ticket() const { return reinterpret_cast<unsigned int*>(refine_slots() + 2 * (size_t)pad_n(n_max) + 32); }
 };
 
 namespace {
@@ -335,6 +349,7 @@ sp2_status_t check_args(sp2_handle_t h, const void* H, const void* H1, int want_
   if (ldh < N || ldd < N) return SP2_ERR_INVALID_ARG;
   if ((in_dt != SP2_F32 && in_dt != SP2_F64) || (out_dt != SP2_F32 && out_dt != SP2_F64)) return SP2_ERR_INVALID_ARG;
   if (h->opt.engine == SP2_ENGINE_SIMT_DEBUG && pad_n(N) > kSimtMaxN) return SP2_ERR_INVALID_ARG;
+  if (h->opt.refine_layers > 0 && !(h->flags & SP2_WITH_REFINEMENT)) return SP2_ERR_WORKSPACE;
   return SP2_OK;
 }
 
@@ -355,6 +370,13 @@ sp2_status_t enqueue_finalise(sp2_handle_t h, const void* H, sp2_dtype_t in_dt, 
   sp2_launch_finalise(h->ctrl(), planes, h->cur_npad, H, in_dt, ldh, D, resp ? D1 : nullptr, out_dt, ldd, N, h->fslots(),
                       h->ring() + ring_idx, s);
   *launches += 2;
+  const int nref = h->opt.refine_layers;
+  if (nref > 0) {   // float64 refinement layers on the converged iterate; overwrites D, tr D, tr(DH)
+    __half* yp[4] = {h->plane(0, 0), h->plane(1, 0), h->plane(0, 1), h->plane(1, 1)};
+    const int k = sp2_launch_refine(h->ctrl(), yp, h->cur_npad, N, nref, h->refine_x(0), h->refine_x(1), h->refine_slots(),
+                                    h->refine_ticket(), H, in_dt, ldh, D, out_dt, ldd, h->ring() + ring_idx, s);
+    *launches += k;
+  }
   return SP2_OK;
 }
 
@@ -509,13 +531,14 @@ sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_work
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
   if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) { delete h; return SP2_ERR_CUDA; }
   h->encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(fn);
-  if (sp2_layer_configure() != cudaSuccess) { delete h; return SP2_ERR_CUDA; }
+  if (sp2_layer_configure() != cudaSuccess || sp2_refine_configure() != cudaSuccess) { delete h; return SP2_ERR_CUDA; }
   if (cudaEventCreate(&h->ev0) != cudaSuccess || cudaEventCreate(&h->ev1) != cudaSuccess ||
       cudaEventCreate(&h->evl0) != cudaSuccess || cudaEventCreate(&h->evl1) != cudaSuccess) { delete h; return SP2_ERR_CUDA; }
   h->time_layers = 0;
   if (cudaMallocHost(reinterpret_cast<void**>(&h->h_result), sizeof(sp2_result_t) * kRingCap) != cudaSuccess) {
     delete h; return SP2_ERR_CUDA;
   }
+  if (flags & SP2_WITH_REFINEMENT) cudaMemset(h->refine_slots(), 0, (2 * (size_t)pad_n(n_max) + 64) * sizeof(double));
   *handle = h;
   return SP2_OK;
 }
@@ -536,6 +559,7 @@ sp2_status_t sp2_set_options(sp2_handle_t h, const sp2_options_t* opt) {
   if (!opt) { default_options(&h->opt); h->layers_hint = 0; return SP2_OK; }
   if (opt->engine != SP2_ENGINE_TCGEN05 && opt->engine != SP2_ENGINE_SIMT_DEBUG) return SP2_ERR_INVALID_ARG;
   if (opt->cta_group < 0 || opt->cta_group > 2) return SP2_ERR_INVALID_ARG;
+  if (opt->refine_layers < 0 || opt->refine_layers > 4) return SP2_ERR_INVALID_ARG;
   if (opt->seg_kb != 0 && opt->seg_kb != 1 && opt->seg_kb != 2 && opt->seg_kb != 4 && opt->seg_kb != 8 &&
       opt->seg_kb != 16 && opt->seg_kb != 32) return SP2_ERR_INVALID_ARG;
   if (opt->user_bounds && !(opt->eps_max > opt->eps_min)) return SP2_ERR_INVALID_ARG;

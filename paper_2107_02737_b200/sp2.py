@@ -29,7 +29,7 @@ SP2_ERR_DEGENERATE = 6
 SP2_WARN_NOT_CONVERGED = 7
 
 SP2_F32, SP2_F64 = 0, 1
-SP2_WITH_RESPONSE, SP2_WITH_HOST_STAGING = 1, 2
+SP2_WITH_RESPONSE, SP2_WITH_HOST_STAGING, SP2_WITH_REFINEMENT = 1, 2, 4
 SP2_ENGINE_TCGEN05, SP2_ENGINE_SIMT_DEBUG = 0, 1
 
 EXPORTS = [
@@ -47,7 +47,7 @@ class Sp2Options(C.Structure):
         ("eps_min", C.c_double), ("eps_max", C.c_double),
         ("engine", C.c_int), ("forced_layers", C.c_int),
         ("forced_signs", C.c_ulonglong), ("cta_group", C.c_int),
-        ("seg_kb", C.c_int), ("seg_first", C.c_int), ("no_recentre", C.c_int), ("debug_flags", C.c_int),
+        ("refine_layers", C.c_int), ("seg_kb", C.c_int), ("seg_first", C.c_int), ("no_recentre", C.c_int), ("debug_flags", C.c_int),
     ]
 
 
@@ -65,7 +65,7 @@ class Sp2Result(C.Structure):
         signs = "".join(
             "+" if (self.sign_mask[n >> 6] >> (n & 63)) & 1 else "-" for n in range(self.layers))
         return dict(status=self.status, layers=self.layers, signs=signs, stop_reason=self.stop_reason,
-                    tr_d=self.tr_d, tr_dh=self.tr_dh, tr_d1=self.tr_d1, idem_est=self.idem_est,
+                    refine_layers=self.reserved, tr_d=self.tr_d, tr_dh=self.tr_dh, tr_d1=self.tr_d1, idem_est=self.idem_est,
                     eps_min=self.eps_min, eps_max=self.eps_max, gpu_ms=self.gpu_ms, layers_ms=self.layers_ms,
                     kernel_launches=self.kernel_launches)
 
@@ -166,13 +166,15 @@ def _np_dtype_code(a):
 class Sp2Handle:
     """sp2_create / sp2_destroy over a torch-owned workspace on the current CUDA device."""
 
-    def __init__(self, n_max: int, response: bool = False, host_staging: bool = False, device=None):
+    def __init__(self, n_max: int, response: bool = False, host_staging: bool = False, device=None,
+                 refinement: bool = False):
         import torch
 
         if not torch.cuda.is_available():
             raise RuntimeError("sp2-b200 needs a CUDA device (sm_100); there is no CPU fallback")
         self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
-        self.flags = (SP2_WITH_RESPONSE if response else 0) | (SP2_WITH_HOST_STAGING if host_staging else 0)
+        self.flags = ((SP2_WITH_RESPONSE if response else 0) | (SP2_WITH_HOST_STAGING if host_staging else 0)
+                      | (SP2_WITH_REFINEMENT if refinement else 0))
         self.n_max = int(n_max)
         nbytes = workspace_bytes(self.n_max, self.flags)
         with torch.cuda.device(self.device):

@@ -306,3 +306,26 @@ def test_structured_chain_tight_bounds_paper_like_layer_count():
     assert np.abs(r["D"] - D_eig).max() < 1e-12
     assert 10 <= r["layers"] <= 18
     assert r["tr_dh"] == pytest.approx(lam[: n // 2].sum(), rel=1e-12)
+
+
+def test_refinement_layers_purify_eigenvalues_and_keep_eigenvectors(cfg1):
+    """PAPER.md:170 refinement: two more layers act on the eigenvalues only.  Start from the exact projector with
+    its eigenvalues perturbed by +-1e-4: the scalar maps x^2 / 2x - x^2 predict every refined eigenvalue, the
+    eigenvectors do not move, the exact projector is a fixed point, and two layers square the error twice."""
+    Q, lam, n_occ, n = cfg1["Q"], cfg1["lam"], cfg1["n_occ"], cfg1["n"]
+    rng = np.random.default_rng(11)
+    occ = (np.argsort(np.argsort(lam)) < n_occ).astype(float)
+    x0 = occ + 1e-4 * rng.uniform(-1, 1, n)
+    X0 = (Q * x0) @ Q.T
+    X0 = 0.5 * (X0 + X0.T)
+    Xr, signs = oracle.sp2_refine_layers(X0, n_occ, layers=2)
+    x = x0.copy()
+    for sg in signs:                                   # the same branches on the scalar spectrum
+        x = x * x if sg == "+" else 2 * x - x * x
+    np.testing.assert_allclose(np.sort(np.linalg.eigvalsh(Xr)), np.sort(x), atol=1e-13)
+    assert signs in ("+-", "-+")                       # near idempotency the branches alternate
+    assert np.abs(x - occ).max() < 5e-8 and np.abs(x - occ).max() > 1e-10       # ~ (2 * 1e-4)^2
+    P = (Q * occ) @ Q.T
+    assert np.abs(Xr - P).max() < 1e-7 and np.linalg.norm(Xr @ P - P @ Xr) < 1e-12   # same eigenvectors
+    Pr, _ = oracle.sp2_refine_layers(P, n_occ, layers=2)
+    assert np.abs(Pr - P).max() < 1e-13                # the projector is a fixed point
