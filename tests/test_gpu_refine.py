@@ -56,3 +56,26 @@ def test_refinement_needs_its_workspace_and_f32_output(torch_cuda, sp2):
     assert r["status"] == 0 and r["refine_layers"] == 1 and D.dtype == torch.float32
     assert abs(r["tr_d"] - p["n_occ"]) < 1e-4              # a single layer purifies one side of the spectrum only
     h.close()
+
+
+def test_refinement_with_response_and_sequence(torch_cuda, sp2):
+    """D is refined, D1 is left as the FP16 stack produced it; the sequence call refines every step."""
+    torch = torch_cuda
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[2], 300), want_h1=True)
+    n, n_occ = p["n"], p["n_occ"]
+    H = torch.from_numpy(p["H"]).cuda()
+    H1 = torch.from_numpy(p["H1"]).cuda()
+    h = sp2.Sp2Handle(n, response=True, refinement=True)
+    D0, D10, r0 = h.response(H, H1, n_occ)
+    h.set_options(refine_layers=2)
+    D2, D12, r2 = h.response(H, H1, n_occ)
+    assert torch.equal(D10, D12) and r2["tr_d1"] == r0["tr_d1"]
+    assert abs(r2["tr_d"] - n_occ) < 1e-9 and float((D2 - D0).abs().max()) < 1e-5
+    Ds = [torch.empty_like(H) for _ in range(3)]
+    h.sequence_begin(n, n_occ, n_steps_hint=3)
+    for k, Dk in enumerate(Ds):
+        h.sequence_step(H + 1e-3 * k * H1, Dk)
+    res = h.sequence_end()
+    assert [r["refine_layers"] for r in res] == [2, 2, 2] and all(abs(r["tr_d"] - n_occ) < 1e-9 for r in res)
+    assert torch.equal(Ds[0], D2)
+    h.close()
