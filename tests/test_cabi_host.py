@@ -132,3 +132,30 @@ def test_work_schedule_covers_every_segment_once_and_is_balanced(sp2, n_tiles, r
         slots += [c["slot"] for c in cs]
     assert len(set(slots)) == len(slots) and len(slots) <= 2 * ncl
     assert len({o["flag_id"] for o in owners.values()}) == len(owners)
+
+
+def test_header_is_plain_c_and_links_from_c(sp2, tmp_path):
+    """include/sp2.h must be usable from C (no C++ / torch types): compile a C99 program against it, link the
+    shared library, and call the two entry points that need no device."""
+    import shutil
+    import subprocess
+
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("gcc not available")
+    src = tmp_path / "use_sp2.c"
+    src.write_text(
+        '#include <stdio.h>\n#include "sp2.h"\n'
+        "int main(void) {\n"
+        "  sp2_options_t o; sp2_result_t r; (void)o; (void)r;\n"
+        "  size_t b = sp2_workspace_bytes(1024, SP2_WITH_RESPONSE);\n"
+        '  printf("%zu %s %d\\n", b, sp2_status_string(SP2_ERR_DEGENERATE), (int)sizeof(sp2_result_t));\n'
+        "  return sp2_create(NULL, 8, 0, NULL, 0) == SP2_ERR_INVALID_ARG ? 0 : 1;\n"
+        "}\n")
+    exe = tmp_path / "use_sp2"
+    libdir = os.path.join(ROOT, "paper_2107_02737_b200")
+    subprocess.run([gcc, "-std=c99", "-Wall", "-Werror", "-pedantic", "-I", os.path.join(ROOT, "include"), str(src),
+                    "-o", str(exe), "-L", libdir, "-l:libsp2_b200.so", f"-Wl,-rpath,{libdir}"], check=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()
+    assert int(out[0]) == sp2.workspace_bytes(1024, sp2.SP2_WITH_RESPONSE)
+    assert "degenerate" in " ".join(out[1:-1]) and int(out[-1]) == 96
