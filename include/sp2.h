@@ -88,6 +88,10 @@ typedef struct {
                        truncation bias, more drains) */
   int seg_first;    /* 0 = default (1 = off): segments merged into each of the first two TMEM hand-offs of a work
                        unit (longer run-ahead during the previous epilogue; measured no gain, more truncation bias) */
+  int lo_bits;      /* 0 = default (11: full FP16 lo plane); 6..10: round the lo planes to that many significant bits.
+                       The B200 is power-capped during the layer stack and multiplier inputs with fewer toggling bits
+                       draw less power: lo_bits = 8 measured 0-5 % faster (within the box-to-box noise) at ~3x larger max|dD|,
+                       still > 10x inside the bars; kept as an experiment knob, not a recommendation */
   int no_recentre;  /* debug, with forced_layers only: keep c on the scalar map instead of the cluster midpoint */
   int debug_flags;  /* performance experiments only (results are WRONG): 1 = skip the epilogue's global loads/stores,
                        2 = issue only the hi*hi product; bits 8-15 = cap on the number of CTA(-pair)s */

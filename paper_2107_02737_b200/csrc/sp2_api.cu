@@ -129,7 +129,7 @@ struct sp2_handle_s {
   sp2_options_t opt;
   PFN_cuTensorMapEncodeTiled_v12000 encode;
   // per-(N, cta_group) cache
-  int cur_n, cur_npad, cur_cg, cur_resp, cur_seg, cur_dbg, cur_first;
+  int cur_n, cur_npad, cur_cg, cur_resp, cur_seg, cur_dbg, cur_first, cur_lo;
   Sp2LayerArgs args[2];          // parity 0: buffer 0 -> 1, parity 1: buffer 1 -> 0
   std::vector<int2> tiles_host;
   std::vector<Sp2Item> items_host;
@@ -293,7 +293,8 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = npad > 16384 ? 2 : 4;
   while ((npad / 64) % seg) seg >>= 1;
   if (h->cur_n == N && h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp && h->cur_seg == seg &&
-      h->cur_dbg == h->opt.debug_flags && h->cur_first == h->opt.seg_first) return SP2_OK;
+      h->cur_dbg == h->opt.debug_flags && h->cur_first == h->opt.seg_first &&
+      h->cur_lo == h->opt.lo_bits) return SP2_OK;
   const int nt = npad / (128 * cg);
   build_tiles(nt, h->tiles_host);
   SP2_CUDA(h, cudaMemcpyAsync(h->tiles(), h->tiles_host.data(), h->tiles_host.size() * sizeof(int2),
@@ -330,11 +331,12 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
     a.ctrl = h->ctrl(); a.slots = h->slots(); a.tiles = h->tiles();
     a.items = h->items(); a.item_begin = h->item_begin(); a.scratch = h->scratch(); a.flags = h->split_flags();
     a.n_flags = h->n_flags; a.n_clusters = h->n_clusters; a.debug_flags = h->opt.debug_flags;
+    a.lo_bits = (h->opt.lo_bits >= 6 && h->opt.lo_bits <= 10) ? h->opt.lo_bits : 11;
     a.seg_first = (h->opt.seg_first >= 1 && h->opt.seg_first <= 16) ? h->opt.seg_first : 1;
     a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = resp; a.seg_kb = seg;
   }
   h->layers_hint = 0;
-  h->cur_n = N; h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp; h->cur_seg = seg; h->cur_dbg = h->opt.debug_flags; h->cur_first = h->opt.seg_first;
+  h->cur_n = N; h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp; h->cur_seg = seg; h->cur_dbg = h->opt.debug_flags; h->cur_first = h->opt.seg_first; h->cur_lo = h->opt.lo_bits;
   return SP2_OK;
 }
 
@@ -560,6 +562,7 @@ sp2_status_t sp2_set_options(sp2_handle_t h, const sp2_options_t* opt) {
   if (opt->engine != SP2_ENGINE_TCGEN05 && opt->engine != SP2_ENGINE_SIMT_DEBUG) return SP2_ERR_INVALID_ARG;
   if (opt->cta_group < 0 || opt->cta_group > 2) return SP2_ERR_INVALID_ARG;
   if (opt->refine_layers < 0 || opt->refine_layers > 4) return SP2_ERR_INVALID_ARG;
+  if (opt->lo_bits != 0 && (opt->lo_bits < 6 || opt->lo_bits > 11)) return SP2_ERR_INVALID_ARG;
   if (opt->seg_kb != 0 && opt->seg_kb != 1 && opt->seg_kb != 2 && opt->seg_kb != 4 && opt->seg_kb != 8 &&
       opt->seg_kb != 16 && opt->seg_kb != 32) return SP2_ERR_INVALID_ARG;
   if (opt->user_bounds && !(opt->eps_max > opt->eps_min)) return SP2_ERR_INVALID_ARG;

@@ -281,7 +281,7 @@ __device__ __forceinline__ void epilogue_chunk(const float* acc, EpiOld& old, co
                                                int gi, int gj0,
                                                size_t npad, __half* __restrict__ out_h, __half* __restrict__ out_m,
                                                float a1hi, float a1lo, float a2, float dsh_hi, float dsh_lo,
-                                               EpiPartials& P) {
+                                               uint32_t lo_round, uint32_t lo_mask, EpiPartials& P) {
   unsigned short* th = reinterpret_cast<unsigned short*>(out_h) + (size_t)gj0 * npad + gi;   // mirrored image
   unsigned short* tm = reinterpret_cast<unsigned short*>(out_m) + (size_t)gj0 * npad + gi;
   float fsum = 0.f, mx = P.mx;
@@ -303,7 +303,7 @@ __device__ __forceinline__ void epilogue_chunk(const float* acc, EpiOld& old, co
       }
       nh[pr] = f2_to_h2(y0, y1);
       const float2 hb = h2_to_f2(nh[pr]);
-      nm[pr] = f2_to_h2(y0 - hb.x, y1 - hb.y);
+      nm[pr] = (f2_to_h2(y0 - hb.x, y1 - hb.y) + lo_round) & lo_mask;   // lo_mask = ~0: all 11 bits of the lo plane
       if (FULL) {
         fsum = fmaf(y0, y0, fsum);
         fsum = fmaf(y1, y1, fsum);
@@ -361,7 +361,7 @@ __device__ __forceinline__ void epilogue_row(const float* acc, EpiOld& old, int 
                                              const __half* __restrict__ in_h, const __half* __restrict__ in_m,
                                              __half* __restrict__ out_h, __half* __restrict__ out_m,
                                              float a1hi, float a1lo, float a2, float dsh_hi, float dsh_lo,
-                                             EpiPartials& P) {
+                                             uint32_t lo_round, uint32_t lo_mask, EpiPartials& P) {
 #pragma unroll
   for (int ch = 0; ch < NCH; ++ch) {
     const int gj0 = j0 + ch * 32;
@@ -369,9 +369,9 @@ __device__ __forceinline__ void epilogue_row(const float* acc, EpiOld& old, int 
     const uint4* nxm = (ch + 1 < NCH) ? reinterpret_cast<const uint4*>(in_m + (size_t)gi * npad + gj0 + 32) : nullptr;
     // gi = 32-aligned base + lane and gj0 is 32-aligned, so both tests are warp-uniform
     if (gj0 > gi) {                           // entirely above the diagonal
-      epilogue_chunk<true>(&acc[ch * 32], old, nxh, nxm, gi, gj0, npad, out_h, out_m, a1hi, a1lo, a2, dsh_hi, dsh_lo, P);
+      epilogue_chunk<true>(&acc[ch * 32], old, nxh, nxm, gi, gj0, npad, out_h, out_m, a1hi, a1lo, a2, dsh_hi, dsh_lo, lo_round, lo_mask, P);
     } else if (gj0 + 31 >= gi) {              // holds the diagonal
-      epilogue_chunk<false>(&acc[ch * 32], old, nxh, nxm, gi, gj0, npad, out_h, out_m, a1hi, a1lo, a2, dsh_hi, dsh_lo, P);
+      epilogue_chunk<false>(&acc[ch * 32], old, nxh, nxm, gi, gj0, npad, out_h, out_m, a1hi, a1lo, a2, dsh_hi, dsh_lo, lo_round, lo_mask, P);
     } else if (nxh) {                         // entirely below: mirrored by its transpose; keep the prefetch rolling
       epilogue_prefetch(old, gi, gj0 + 32, npad, in_h, in_m);
     }
@@ -522,6 +522,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
     const int q = warp & 3;                       // TMEM lane quarter this warp may read
     const int hh = cw >> 2;                       // which half of the accumulator columns
     const Sp2Coef cf = a.ctrl->coef;
+    // optional power saving: round the lo plane to lo_bits significant bits (fewer toggling multiplier inputs)
+    const int drop = 11 - a.lo_bits;
+    const uint32_t lo_mask = drop > 0 ? ~(((1u << drop) - 1u) * 0x00010001u) : 0xffffffffu;
+    const uint32_t lo_round = drop > 0 ? (1u << (drop - 1)) * 0x00010001u : 0u;
     int as = 0; uint32_t aphase = 0;
     for (int iti = item_lo; iti < item_hi; ++iti) {
       const Sp2Item I = a.items[iti];
@@ -604,7 +608,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
         P.fro = (double)t;
       } else
         epilogue_row<NCH>(sums, old, gi, j0, (size_t)a.npad, a.in[pl], a.in[pl + 1], a.out[pl], a.out[pl + 1],
-                          a1hi, a1lo, a2, dsh_hi, dsh_lo, P);
+                          a1hi, a1lo, a2, dsh_hi, dsh_lo, lo_round, lo_mask, P);
       // warp partial -> slot (fixed shuffle tree: deterministic)
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {

@@ -30,6 +30,7 @@ struct alignas(64) Sp2LayerArgs {
   unsigned int* flags;   // one arrival counter per split unit (zero between launches)
   int n_flags;
   int seg_first;         // segments merged into each of the first two TMEM hand-offs of an item
+  int lo_bits;           // significant bits kept in the lo planes (11 = all)
   int debug_flags;       // sp2_options_t.debug_flags
   int n_clusters;        // CTA(-pair)s the work lists were built for (= grid size / cta_group)
   int n;                 // true dimension (rows/cols >= n are zero padding and stay zero)
