@@ -451,13 +451,53 @@ def run_sequence(args):
     return 0
 
 
+def run_congruence(args):
+    """--workload congruence: sp2_congruence (H_orth = Z^T H Z) at N = 8192, float64 in and out.
+    Extra workload, not the headline; value = issued tensor Tflop/s of the two products
+    (2 products x 3 plane products x 2 N^3)."""
+    import torch
+
+    from paper_2107_02737_b200 import sp2
+
+    _, _, local = dist_env()
+    torch.cuda.set_device(local)
+    n = 8192
+    g = torch.Generator(device="cuda").manual_seed(20210714)
+    Z = torch.randn(n, n, dtype=torch.float64, device="cuda", generator=g) / n ** 0.5 + torch.eye(n, dtype=torch.float64, device="cuda")
+    X = torch.randn(n, n, dtype=torch.float64, device="cuda", generator=g)
+    X = 0.5 * (X + X.T)
+    C = torch.empty_like(X)
+    h = sp2.Sp2Handle(n, response=True)
+    for _ in range(max(args.warmup, 3)):
+        h.congruence(Z, X, out=C)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = h.launch_count
+    torch.cuda.synchronize()
+    ev0.record()
+    for _ in range(args.steps):
+        h.congruence(Z, X, out=C)
+    ev1.record()
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / args.steps
+    err = float((C - Z.T @ X @ Z).abs().max())          # cross-check with torch float64 (harness, not library)
+    line = {"metric": "issued Tflop/s of sp2_congruence (Z^T X Z, N=8192)", "value": 12.0 * n ** 3 / (ms * 1e-3) / 1e12,
+            "unit": "TFLOP/s (issued)", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16 hi/lo operand planes, f32 accumulate",
+            "data": "synthetic", "config": {"workload": "sp2_congruence: C = Z^T X Z, N=8192, f64 in/out, general Z, symmetric X",
+                                            "max_abs_err_vs_torch_f64": err, "max_abs_C": float(C.abs().max())},
+            "gpu_launches": int(h.launch_count - launches0)}
+    print(json.dumps(line), flush=True)
+    h.close()
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--workload", choices=["response", "density", "sequence"], default="response")
+    ap.add_argument("--workload", choices=["response", "density", "sequence", "congruence"], default="response")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--refine", type=int, default=0,
                     help="float64 refinement layers after the stack (PAPER.md:170; --workload density only); extra, not the headline")
@@ -466,6 +506,8 @@ def main(argv=None):
         return run_reference(args)
     if args.workload == "sequence":
         return run_sequence(args)
+    if args.workload == "congruence":
+        return run_congruence(args)
     return run_ours(args)
 
 

@@ -159,6 +159,15 @@ SP2_API sp2_status_t sp2_sequence_step(sp2_handle_t handle, const void* dH_t, sp
                                void* dD_t, sp2_dtype_t out_dtype, long ldd);
 SP2_API sp2_status_t sp2_sequence_end(sp2_handle_t handle, sp2_result_t* results, int* n_steps);
 
+/* Congruence transform of a symmetric matrix X with a (general) matrix Z, the step either side of the solver in a
+ * non-orthogonal basis (H_orth = Z^T H Z, D = Z D_orth Z^T with Z^T S Z = I):
+ *   transpose_first = 1:  C = Z^T X Z        transpose_first = 0:  C = Z X Z^T
+ * Device pointers, row-major, pitch ld (Z, X) / ldc (C); X symmetric.  Two products on the same tcgen05 mainloop as the
+ * layers (FP16 hi/lo planes, FP32 accumulation in k-segments, ~22-bit operands).  Needs SP2_WITH_RESPONSE (it borrows the
+ * second set of planes).  Blocking; C must not alias Z, X or the workspace. */
+SP2_API sp2_status_t sp2_congruence(sp2_handle_t handle, const void* dZ, const void* dX, sp2_dtype_t in_dtype, long ld, int N,
+                                    int transpose_first, void* dC, sp2_dtype_t out_dtype, long ldc, void* stream);
+
 /* Diagnostics. */
 SP2_API const char* sp2_status_string(sp2_status_t status);
 SP2_API int sp2_last_cuda_error(sp2_handle_t handle);            /* cudaError_t of the last failing CUDA call, 0 if none */

@@ -15,6 +15,7 @@ from .sp2_oracle import (  # noqa: F401
     sp2_stop,
     sp2_density,
     sp2_refine_layers,
+    congruence,
     density_eigh,
     density_from_eigenpairs,
     response_closed_form,

@@ -46,6 +46,7 @@ __all__ = [
     "sp2_stop",
     "sp2_density",
     "sp2_refine_layers",
+    "congruence",
     "density_eigh",
     "density_from_eigenpairs",
     "response_closed_form",
@@ -223,6 +224,15 @@ def sp2_refine_layers(X, n_occ, layers=2):
         X = X2 if plus else 2.0 * X - X2
         signs.append("+" if plus else "-")
     return X, "".join(signs)
+
+
+def congruence(Z, X, transpose_first=True):
+    """The transforms either side of the solver in a non-orthogonal basis: "H_orth = Z^T H Z, where
+    Z is the inverse factor of the overlap matrix, S, determined by the relation Z^T S Z = I", and back,
+    "D = Z D_orth Z^T".  transpose_first: Z^T X Z, else Z X Z^T."""
+    Z = np.asarray(Z, dtype=np.float64)
+    X = np.asarray(X, dtype=np.float64)
+    return Z.T @ X @ Z if transpose_first else Z @ X @ Z.T
 
 
 def density_eigh(H, n_occ):

@@ -34,6 +34,11 @@ void sp2_launch_finalise(Sp2Ctrl* c, __half* const planes[8], int npad, const vo
                          sp2_result_t* ring_entry, cudaStream_t s);
 void sp2_launch_trivial(Sp2Ctrl* c, void* D, void* D1, sp2_dtype_t out_dt, long ldo, int N, sp2_result_t* ring_entry,
                         cudaStream_t s);
+void sp2_launch_gsetup(Sp2Ctrl* c, const Sp2BoundSlot* sz, const Sp2BoundSlot* sa, int count, int N, sp2_result_t* ring_entry,
+                       cudaStream_t s);
+void sp2_launch_gswap(Sp2Ctrl* c, cudaStream_t s);
+void sp2_launch_split(const void* A, sp2_dtype_t dt, long ld, int N, int npad, int transpose, int which, const Sp2Ctrl* c,
+                      __half* Ph, __half* Pm, cudaStream_t s);
 // sp2_refine.cu
 cudaError_t sp2_refine_configure();
 int sp2_launch_refine(Sp2Ctrl* c, __half* const planes[4], int npad, int N, int n_layers, double* Xa, double* Xb,
@@ -87,7 +92,7 @@ Layout make_layout(int n_max, int flags) {
   L.off_bslots = off; off += align_up(2 * L.bslots_count * sizeof(Sp2BoundSlot), 1024);
   L.off_fslots = off; off += align_up(3 * (size_t)sp2_finalise_blocks(n_max) * sizeof(double), 1024);
   const size_t nt1 = npad / 128;
-  L.tiles_count = nt1 * (nt1 + 1) / 2;
+  L.tiles_count = nt1 * nt1;                 // the congruence products use every tile, the layers the upper triangle
   L.off_tiles = off; off += align_up(L.tiles_count * sizeof(int2), 1024);
   L.items_cap = 2 * L.tiles_count + 1024;
   L.off_items = off; off += align_up(L.items_cap * sizeof(Sp2Item), 1024);
@@ -640,6 +645,80 @@ sp2_status_t sp2_sequence_end(sp2_handle_t h, sp2_result_t* results, int* n_step
     if (h->h_result[i].status != SP2_OK && worst == SP2_OK) worst = (sp2_status_t)h->h_result[i].status;
   }
   return worst;
+}
+
+sp2_status_t sp2_congruence(sp2_handle_t h, const void* dZ, const void* dX, sp2_dtype_t in_dtype, long ld, int N,
+                            int transpose_first, void* dC, sp2_dtype_t out_dtype, long ldc, void* stream) {
+  if (!h || !dZ || !dX || !dC || N <= 0 || N > h->n_max || ld < N || ldc < N) return SP2_ERR_INVALID_ARG;
+  if ((in_dtype != SP2_F32 && in_dtype != SP2_F64) || (out_dtype != SP2_F32 && out_dtype != SP2_F64)) return SP2_ERR_INVALID_ARG;
+  if (!(h->flags & SP2_WITH_RESPONSE)) return SP2_ERR_WORKSPACE;      // needs the second set of planes
+  if (h->seq_active) return SP2_ERR_INVALID_ARG;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  const int npad = pad_n(N);
+  const int cg = pick_cta_group(h, npad, 0);
+  const int nt = npad / (128 * cg);
+  // launch state of the plain-product mode: every tile, grouped like the layer tiles
+  h->tiles_host.clear();
+  const int G = 8;
+  for (int gi = 0; gi < nt; gi += G)
+    for (int gj = 0; gj < nt; gj += G)
+      for (int ti = gi; ti < gi + G && ti < nt; ++ti)
+        for (int tj = gj; tj < gj + G && tj < nt; ++tj) h->tiles_host.push_back(make_int2(ti, tj));
+  int seg = 4;
+  while ((npad / 64) % seg) seg >>= 1;
+  int nC = h->num_sms / cg;
+  if (nC > kMaxClusters / cg) nC = kMaxClusters / cg;
+  int n_slots = 0;
+  build_schedule((int)h->tiles_host.size(), 0, (npad / 64) / seg, nC, h->items_host, h->item_begin_host, &h->n_flags, &n_slots);
+  h->n_clusters = nC;
+  h->cur_n = -1;                                   // the next solve rebuilds its own launch state
+  if (h->items_host.size() > h->L.items_cap || h->tiles_host.size() > h->L.tiles_count ||
+      (size_t)n_slots * sp2_layer_scratch_slot_bytes(cg) > h->L.scratch_bytes || h->n_flags > 2 * kMaxClusters)
+    return SP2_ERR_WORKSPACE;
+  SP2_CUDA(h, cudaMemcpyAsync(h->tiles(), h->tiles_host.data(), h->tiles_host.size() * sizeof(int2), cudaMemcpyHostToDevice, s));
+  SP2_CUDA(h, cudaMemcpyAsync(h->items(), h->items_host.data(), h->items_host.size() * sizeof(Sp2Item), cudaMemcpyHostToDevice, s));
+  SP2_CUDA(h, cudaMemcpyAsync(h->item_begin(), h->item_begin_host.data(), h->item_begin_host.size() * sizeof(int),
+                              cudaMemcpyHostToDevice, s));
+  SP2_CUDA(h, cudaMemsetAsync(h->split_flags(), 0, 2 * kMaxClusters * sizeof(unsigned int), s));
+  SP2_CUDA(h, cudaStreamSynchronize(s));
+  Sp2Ctrl* c = h->ctrl();
+  __half *Lh = h->plane(0, 0), *Lm = h->plane(1, 0), *Xh = h->plane(2, 0), *Xm = h->plane(3, 0), *Th = h->plane(2, 1),
+         *Tm = h->plane(3, 1);
+  // exponents, then planes: L = Z^T (C = Z^T X Z) or Z (C = Z X Z^T); X is symmetric
+  sp2_launch_init(c, N, 0, npad, 0, 1, 0, 0.0, 0.0, 0.0, 0, 0ull, 0, s);
+  sp2_launch_bounds(dZ, in_dtype, ld, N, 1, h->bslots(0), s);
+  sp2_launch_bounds(dX, in_dtype, ld, N, 1, h->bslots(1), s);
+  sp2_launch_gsetup(c, h->bslots(0), h->bslots(1), sp2_bounds_blocks(N), N, h->ring(), s);
+  sp2_launch_split(dZ, in_dtype, ld, N, npad, transpose_first ? 1 : 0, 0, c, Lh, Lm, s);
+  sp2_launch_split(dX, in_dtype, ld, N, npad, 0, 1, c, Xh, Xm, s);
+  int launches = 6;
+  Sp2LayerArgs a;
+  memset(&a, 0, sizeof(a));
+  a.ctrl = c; a.slots = h->slots(); a.tiles = h->tiles(); a.items = h->items(); a.item_begin = h->item_begin();
+  a.scratch = h->scratch(); a.flags = h->split_flags(); a.n_flags = h->n_flags; a.n_clusters = nC;
+  a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = 0; a.seg_kb = seg; a.seg_first = 1;
+  a.lo_bits = 11; a.gemm_mode = 1;
+  sp2_status_t st;
+  // T = L X^T (= L X): planes out
+  if ((st = encode_plane_map(h, &a.tm[0], Lh, npad)) != SP2_OK || (st = encode_plane_map(h, &a.tm[1], Lm, npad)) != SP2_OK ||
+      (st = encode_plane_map(h, &a.tm[2], Xh, npad)) != SP2_OK || (st = encode_plane_map(h, &a.tm[3], Xm, npad)) != SP2_OK)
+    return st;
+  a.out[0] = Th; a.out[1] = Tm; a.out_kind = 0;
+  cudaError_t e = sp2_launch_layer(a, SP2_ENGINE_TCGEN05, cg, s);
+  if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
+  sp2_launch_gswap(c, s);
+  // C = T L^T: the caller's matrix
+  if ((st = encode_plane_map(h, &a.tm[0], Th, npad)) != SP2_OK || (st = encode_plane_map(h, &a.tm[1], Tm, npad)) != SP2_OK ||
+      (st = encode_plane_map(h, &a.tm[2], Lh, npad)) != SP2_OK || (st = encode_plane_map(h, &a.tm[3], Lm, npad)) != SP2_OK)
+    return st;
+  a.out_kind = out_dtype == SP2_F64 ? 2 : 1; a.cout = dC; a.ldc = ldc;
+  e = sp2_launch_layer(a, SP2_ENGINE_TCGEN05, cg, s);
+  if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
+  launches += 3;
+  h->launches += (unsigned long long)launches;
+  SP2_CUDA(h, cudaMemcpyAsync(h->h_result, h->ring(), sizeof(sp2_result_t), cudaMemcpyDeviceToHost, s));
+  SP2_CUDA(h, cudaStreamSynchronize(s));
+  return (sp2_status_t)h->h_result->status;
 }
 
 const char* sp2_status_string(sp2_status_t s) {

@@ -64,6 +64,9 @@ struct Sp2Ctrl {
   double e[SP2_LAYER_CAP];
   // finalise
   double tr_d, tr_dh, tr_d1;
+  // plane exponents of the congruence products (sp2_congruence): operands A, B and the intermediate T
+  int g_ea, g_eb, g_et;      // exponents the running product reads: A operand, B operand, plane output
+  int g_el, g_ex, g_pad;     // exponents of the L (= Z or Z^T) planes and of the transformed matrix X
   // float64 refinement layers (sp2_refine.cu)
   double ref_tr, ref_fro;   // tr X and ||X||_F^2 of the current float64 iterate
   int ref_plus, ref_done;   // branch of the next refinement layer; layers applied

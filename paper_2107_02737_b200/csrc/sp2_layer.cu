@@ -378,6 +378,43 @@ __device__ __forceinline__ void epilogue_row(const float* acc, EpiOld& old, int 
   }
 }
 
+// Epilogue of the plain-product mode: this thread's row gi, columns j0 .. j0 + COLS of C = A B^T.
+//   out_kind 0: hi/lo FP16 planes at the exponent folded into `scale` (feeds the next product)
+//   out_kind 1 / 2: the caller's float / double matrix (rows and columns < n only)
+template <int COLS>
+__device__ __forceinline__ void gemm_epilogue(const float* acc, int gi, int j0, const Sp2LayerArgs& a, double scale) {
+  if (a.out_kind == 0) {
+    const float sc = (float)scale;
+    __half* ph = a.out[0] + (size_t)gi * a.npad + j0;
+    __half* pm = a.out[1] + (size_t)gi * a.npad + j0;
+#pragma unroll
+    for (int w = 0; w < COLS / 8; ++w) {
+      uint32_t nh[4], nm[4];
+#pragma unroll
+      for (int pr = 0; pr < 4; ++pr) {
+        const float y0 = acc[8 * w + 2 * pr] * sc, y1 = acc[8 * w + 2 * pr + 1] * sc;
+        nh[pr] = f2_to_h2(y0, y1);
+        const float2 hb = h2_to_f2(nh[pr]);
+        nm[pr] = f2_to_h2(y0 - hb.x, y1 - hb.y);
+      }
+      *reinterpret_cast<uint4*>(ph + 8 * w) = make_uint4(nh[0], nh[1], nh[2], nh[3]);
+      *reinterpret_cast<uint4*>(pm + 8 * w) = make_uint4(nm[0], nm[1], nm[2], nm[3]);
+    }
+    return;
+  }
+  if (gi >= a.n) return;
+  if (a.out_kind == 2) {
+    double* c = reinterpret_cast<double*>(a.cout) + (size_t)gi * a.ldc;
+#pragma unroll
+    for (int k = 0; k < COLS; ++k) if (j0 + k < a.n) c[j0 + k] = (double)acc[k] * scale;
+  } else {
+    float* c = reinterpret_cast<float*>(a.cout) + (size_t)gi * a.ldc;
+    const float sc = (float)scale;
+#pragma unroll
+    for (int k = 0; k < COLS; ++k) if (j0 + k < a.n) c[j0 + k] = acc[k] * sc;
+  }
+}
+
 // ----------------------------------------------------------------------------------------------
 // Warp roles (384 threads): warps 0..7 consumers; warp 8 TMA producer, warp 9 MMA issuer, warp 10 TMEM
 // allocator, warp 11 idle.  The k range of a unit is cut into segments of seg_kb k-blocks; each
@@ -385,7 +422,9 @@ __device__ __forceinline__ void epilogue_row(const float* acc, EpiOld& old, int 
 // the consumers add the finished segment into FP32 register sums with round-to-nearest adds.
 // This bounds the length of the truncating in-TMEM accumulation (DESIGN.md "Tensor-core
 // truncation bias") and costs no tensor time: the drain overlaps the next segment's MMAs.
-template <int CG>
+// MODE 0: one SP2 layer.  MODE 1: the same mainloop as a plain product C = A B^T of two hi/lo plane pairs (A = tm[0..1],
+// B = tm[2..3]; every tile, no mirror, no controller) for the congruence transforms of sp2_congruence.
+template <int CG, int MODE>
 __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant__ Sp2LayerArgs a) {
   constexpr int TILE = 128 * CG;          // output tile edge
   constexpr int UM = 128 * CG, UN = 128 * CG;
@@ -430,7 +469,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(&bars->tmem_base);
 
   asm volatile("griddepcontrol.wait;" ::: "memory");    // previous layer complete, its writes visible
-  const bool active = *reinterpret_cast<volatile const int*>(&a.ctrl->done) == 0;   // uniform over the grid
+  const bool active = MODE == 1 || *reinterpret_cast<volatile const int*>(&a.ctrl->done) == 0;   // uniform over the grid
 
   if (!active) {
     // converged (or failed) before this launch: nothing to do but release the TMEM columns
@@ -458,7 +497,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
               const int p = (g >= KB) ? 1 : 0;
               const int kb = g - p * KB;
               const int ma = (wunit && p == 1) ? 2 : 0;
-              const int mb = (wunit && p == 0) ? 2 : 0;
+              const int mb = (MODE == 1 || (wunit && p == 0)) ? 2 : 0;
               mbar_wait(smem_u32(&bars->empty[stage]), phase ^ 1u);
               const uint32_t dst = smem_u32(smem + stage * kStageBytes);
               if (CG == 1 || leader) mbar_expect_tx(smem_u32(&bars->full[stage]), (uint32_t)(CG * kStageBytes));
@@ -522,6 +561,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
     const int q = warp & 3;                       // TMEM lane quarter this warp may read
     const int hh = cw >> 2;                       // which half of the accumulator columns
     const Sp2Coef cf = a.ctrl->coef;
+    const double gemm_scale = MODE == 1 ? sp2_exp2i((a.out_kind == 0 ? a.ctrl->g_et : 0) - a.ctrl->g_ea - a.ctrl->g_eb) : 0.0;
     // optional power saving: round the lo plane to lo_bits significant bits (fewer toggling multiplier inputs)
     const int drop = 11 - a.lo_bits;
     const uint32_t lo_mask = drop > 0 ? ~(((1u << drop) - 1u) * 0x00010001u) : 0xffffffffu;
@@ -541,7 +581,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
         const int len = (ho < 2) ? min(a.seg_first, I.seg1 - sg) : 1;     // same hand-off lengths as the MMA issuer
         sg += len;
         // the old tile's first chunk is fetched under the last hand-off's MMAs
-        if (sg == I.seg1 && I.kind != 1) epilogue_prefetch(old, gi, j0, (size_t)a.npad, a.in[pl], a.in[pl + 1]);
+        if (MODE == 0 && sg == I.seg1 && I.kind != 1) epilogue_prefetch(old, gi, j0, (size_t)a.npad, a.in[pl], a.in[pl + 1]);
         mbar_wait(smem_u32(&bars->tmem_full[as]), aphase);
         tc_fence_after();
         const uint32_t tcol = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * ACC_COLS + hh * WCOLS);
@@ -595,6 +635,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
           for (int c = 0; c < WCOLS; ++c) sums[c] += __ldcg(src + c * 32);
         }
       }
+      if constexpr (MODE == 1) {                  // plain product: scale, (split,) store; no statistics
+        gemm_epilogue<WCOLS>(sums, gi, j0, a, gemm_scale);
+        continue;
+      }
       // ---- fused epilogue from the register sums
       const float a1hi = wunit ? cf.a1z_hi : cf.a1y_hi, a1lo = wunit ? cf.a1z_lo : cf.a1y_lo;
       const float a2 = wunit ? cf.a2z : cf.a2y;
@@ -630,6 +674,19 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
   if (warp == kWarpAlloc) tmem_dealloc<CG>(tmem_base, TMEM_COLS);
   if (!active) return;
+  if constexpr (MODE == 1) {                     // last CTA re-arms the split-k flags; no controller
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      __threadfence();
+      bars->is_last = (atomicAdd(&a.ctrl->ticket, 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (bars->is_last) {
+      for (int i = threadIdx.x; i < a.n_flags; i += blockDim.x) a.flags[i] = 0u;
+      if (threadIdx.x == 0) a.ctrl->ticket = 0u;
+    }
+    return;
+  }
 
   const int per_unit = CG * kConsumerWarps;
   const int n_z = a.with_response ? n_tiles * per_unit : 0;
@@ -728,9 +785,11 @@ int sp2_layer_slots(int npad, int cta_group, int with_response, int engine) {
 }
 
 cudaError_t sp2_layer_configure() {
-  cudaError_t e = cudaFuncSetAttribute(k_layer_tc<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp2_layer_smem_bytes());
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(k_layer_tc<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp2_layer_smem_bytes());
+  const int smem = (int)sp2_layer_smem_bytes();
+  cudaError_t e = cudaFuncSetAttribute(k_layer_tc<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_layer_tc<2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_layer_tc<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_layer_tc<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   return e;
 }
 
@@ -758,8 +817,8 @@ cudaError_t sp2_launch_layer(const Sp2LayerArgs& args, int engine, int cta_group
     attr[1].id = cudaLaunchAttributeClusterDimension;
     attr[1].val.clusterDim.x = 2; attr[1].val.clusterDim.y = 1; attr[1].val.clusterDim.z = 1;
     cfg.numAttrs = 2;
-    return cudaLaunchKernelEx(&cfg, k_layer_tc<2>, args);
+    return args.gemm_mode ? cudaLaunchKernelEx(&cfg, k_layer_tc<2, 1>, args) : cudaLaunchKernelEx(&cfg, k_layer_tc<2, 0>, args);
   }
   cfg.gridDim = dim3(args.n_clusters);
-  return cudaLaunchKernelEx(&cfg, k_layer_tc<1>, args);
+  return args.gemm_mode ? cudaLaunchKernelEx(&cfg, k_layer_tc<1, 1>, args) : cudaLaunchKernelEx(&cfg, k_layer_tc<1, 0>, args);
 }

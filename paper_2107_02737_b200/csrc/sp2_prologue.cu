@@ -337,6 +337,65 @@ __global__ void __launch_bounds__(256) k_finalise_reduce(Sp2Ctrl* c, const doubl
   *ring_entry = r;
 }
 
+// ------------------------------------------------------------------------------------------
+// Congruence transform support (sp2_congruence: H_orth = Z^T H Z, D = Z D_orth Z^T).
+// k_gsetup: plane exponents from max|.| of the two inputs; k_split: matrix (or its transpose) -> hi/lo planes;
+// k_gswap: operand exponents of the second product.
+__global__ void __launch_bounds__(256) k_gsetup(Sp2Ctrl* c, const Sp2BoundSlot* sz, const Sp2BoundSlot* sa, int count, int N,
+                                                sp2_result_t* ring_entry) {
+  __shared__ double red[3][256];
+  const int tid = threadIdx.x;
+  double mz = 0.0, ma = 0.0, sum = 0.0;
+  for (int i = tid; i < count; i += 256) { mz = fmax(mz, sz[i].mx); ma = fmax(ma, sa[i].mx); sum += sz[i].sum + sa[i].sum; }
+  red[0][tid] = mz; red[1][tid] = ma; red[2][tid] = sum;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (tid < w) {
+      red[0][tid] = fmax(red[0][tid], red[0][tid + w]);
+      red[1][tid] = fmax(red[1][tid], red[1][tid + w]);
+      red[2][tid] += red[2][tid + w];
+    }
+    __syncthreads();
+  }
+  if (tid != 0) return;
+  const double maxz = red[0][0], maxa = red[1][0];
+  c->g_el = sp2_pick_exponent(maxz);
+  c->g_ex = sp2_pick_exponent(maxa);
+  // |T_ij| = |sum_k L_ik A_jk| <= N max|L| max|A|: loose, but the lo plane keeps 2^-24 absolute resolution
+  c->g_et = sp2_pick_exponent((double)N * maxz * maxa);
+  c->g_ea = c->g_el; c->g_eb = c->g_ex;           // first product: A operand = L, B operand = X
+  sp2_result_t r;
+  memset(&r, 0, sizeof(r));
+  r.status = isfinite(red[2][0]) ? SP2_OK : SP2_ERR_NONFINITE;
+  *ring_entry = r;
+}
+
+__global__ void k_gswap(Sp2Ctrl* c) { c->g_ea = c->g_et; c->g_eb = c->g_el; }   // second product: T x L
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_split(const T* __restrict__ A, long ld, int N, int npad, int transpose, int which,
+                                               const Sp2Ctrl* __restrict__ c, __half* __restrict__ Ph, __half* __restrict__ Pm) {
+  __shared__ double t[32][33];
+  const int nb = npad >> 5;
+  const int bi = blockIdx.x / nb, bj = blockIdx.x % nb;       // output tile (rows bi, cols bj)
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  const double scale = sp2_exp2i(which == 0 ? c->g_el : c->g_ex);
+  // source tile: rows (transpose ? bj : bi), cols (transpose ? bi : bj), read with coalesced rows
+  for (int r = ty; r < 32; r += 8) {
+    const int si = (transpose ? bj : bi) * 32 + r, sj = (transpose ? bi : bj) * 32 + tx;
+    t[r][tx] = (si < N && sj < N) ? (double)__ldg(A + (size_t)si * ld + sj) : 0.0;
+  }
+  __syncthreads();
+  for (int r = ty; r < 32; r += 8) {
+    const double v = (transpose ? t[tx][r] : t[r][tx]) * scale;
+    const float vf = (float)v;
+    const __half hh = __float2half_rn(vf);
+    const __half mm = __float2half_rn((float)(v - (double)__half2float(hh)));
+    const size_t o = (size_t)(bi * 32 + r) * npad + bj * 32 + tx;
+    Ph[o] = hh; Pm[o] = mm;
+  }
+}
+
 // Trivial occupations (N_occ = 0 -> D = 0, N_occ = N -> D = I; D1 = 0), answered from the definition.
 template <typename TO>
 __global__ void __launch_bounds__(256) k_trivial(Sp2Ctrl* c, TO* __restrict__ D, TO* __restrict__ D1, long ldo,
@@ -433,4 +492,16 @@ void sp2_launch_trivial(Sp2Ctrl* c, void* D, void* D1, sp2_dtype_t out_dt, long 
   const int grid = (int)(((size_t)N * N + 255) / 256 > 4096 ? 4096 : ((size_t)N * N + 255) / 256);
   if (out_dt == SP2_F32) k_trivial<float><<<grid, 256, 0, s>>>(c, (float*)D, (float*)D1, ldo, ring_entry);
   else k_trivial<double><<<grid, 256, 0, s>>>(c, (double*)D, (double*)D1, ldo, ring_entry);
+}
+
+void sp2_launch_gsetup(Sp2Ctrl* c, const Sp2BoundSlot* sz, const Sp2BoundSlot* sa, int count, int N, sp2_result_t* ring_entry,
+                       cudaStream_t s) {
+  k_gsetup<<<1, 256, 0, s>>>(c, sz, sa, count, N, ring_entry);
+}
+void sp2_launch_gswap(Sp2Ctrl* c, cudaStream_t s) { k_gswap<<<1, 1, 0, s>>>(c); }
+void sp2_launch_split(const void* A, sp2_dtype_t dt, long ld, int N, int npad, int transpose, int which, const Sp2Ctrl* c,
+                      __half* Ph, __half* Pm, cudaStream_t s) {
+  const int nb = npad / 32;
+  SP2_DISPATCH_IN(dt, (k_split<float><<<nb * nb, 256, 0, s>>>((const float*)A, ld, N, npad, transpose, which, c, Ph, Pm)),
+                  (k_split<double><<<nb * nb, 256, 0, s>>>((const double*)A, ld, N, npad, transpose, which, c, Ph, Pm)));
 }

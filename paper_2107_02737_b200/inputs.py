@@ -155,3 +155,21 @@ def ssh_chain(n: int, t1: float = 1.0, t2: float = 0.6, onsite: float = 0.0, dty
     e = np.abs(t1 + t2 * np.exp(1j * k))
     lam = np.sort(np.concatenate([-e, e])) + onsite
     return np.ascontiguousarray(H.astype(dtype)), lam
+
+
+def overlap_problem(n: int, n_occ: int, seed: int = 7, gap: float = 0.4):
+    """A non-orthogonal stand-in: overlap S = I + 0.3 (B + B^T)/(2 sqrt n) (symmetric positive
+    definite, well conditioned), its Loewdin inverse factor Z = S^(-1/2), and H = Z^-T (Q diag(lam) Q^T) Z^-1 so that
+    the orthogonalised Hamiltonian Z^T H Z has the known, gapped spectrum lam.  Returns dict(H, S, Z, lam, Q)."""
+    rng = np.random.default_rng(seed)
+    B = rng.standard_normal((n, n))
+    S = np.eye(n) + 0.3 * (B + B.T) / (2.0 * math.sqrt(n))
+    w, V = np.linalg.eigh(S)
+    assert w.min() > 0.2
+    Z = (V / np.sqrt(w)) @ V.T                      # symmetric inverse square root
+    Zinv = (V * np.sqrt(w)) @ V.T
+    Q = _haar_q_numpy(rng.standard_normal((n, n)))
+    lam = np.concatenate([rng.uniform(-1.0, -gap / 2, n_occ), rng.uniform(gap / 2, 1.0, n - n_occ)])
+    Horth = (Q * lam) @ Q.T
+    H = Zinv @ (0.5 * (Horth + Horth.T)) @ Zinv
+    return dict(H=0.5 * (H + H.T), S=0.5 * (S + S.T), Z=0.5 * (Z + Z.T), lam=lam, Q=Q, n=n, n_occ=n_occ)

@@ -35,7 +35,7 @@ SP2_ENGINE_TCGEN05, SP2_ENGINE_SIMT_DEBUG = 0, 1
 EXPORTS = [
     "sp2_workspace_bytes", "sp2_create", "sp2_destroy", "sp2_set_options", "sp2_get_options",
     "sp2_density", "sp2_response", "sp2_density_host", "sp2_response_host",
-    "sp2_sequence_begin", "sp2_sequence_step", "sp2_sequence_end",
+    "sp2_sequence_begin", "sp2_sequence_step", "sp2_sequence_end", "sp2_congruence",
     "sp2_status_string", "sp2_last_cuda_error", "sp2_launch_count",
     "sp2_debug_history", "sp2_debug_plane", "sp2_debug_schedule",
 ]
@@ -106,6 +106,8 @@ def _load():
     lib.sp2_sequence_step.argtypes = [vp, vp, i, l, vp, i, l]
     lib.sp2_sequence_end.restype = i
     lib.sp2_sequence_end.argtypes = [vp, C.POINTER(Sp2Result), C.POINTER(i)]
+    lib.sp2_congruence.restype = i
+    lib.sp2_congruence.argtypes = [vp, vp, vp, i, l, i, i, vp, i, l, vp]
     lib.sp2_status_string.restype = C.c_char_p
     lib.sp2_status_string.argtypes = [i]
     lib.sp2_last_cuda_error.restype = i
@@ -315,6 +317,24 @@ class Sp2Handle:
                                    C.c_void_p(po), C.c_void_p(q1), do, lo, C.byref(r), self._stream())
         self._raise(st)
         return out, out1, r.as_dict()
+
+    def congruence(self, Z, X, transpose_first: bool = True, out=None, out_dtype=None):
+        """sp2_congruence: C = Z^T X Z (transpose_first) or Z X Z^T for symmetric X; CUDA tensors in, CUDA tensor out."""
+        import torch
+
+        n = X.shape[0]
+        self._check_dev(Z, n)
+        self._check_dev(X, n)
+        if Z.dtype != X.dtype or Z.stride(0) != X.stride(0):
+            raise ValueError("Z must have the dtype and pitch of X")
+        if out is None:
+            out = torch.empty((n, n), dtype=out_dtype or X.dtype, device=X.device)
+        self._check_dev(out, n)
+        st = lib.sp2_congruence(self._h, C.c_void_p(Z.data_ptr()), C.c_void_p(X.data_ptr()), _dtype_code(X), X.stride(0), n,
+                                1 if transpose_first else 0, C.c_void_p(out.data_ptr()), _dtype_code(out), out.stride(0),
+                                self._stream())
+        self._raise(st)
+        return out
 
     # ------------------------------------------------------------------ sequence calls
     def sequence_begin(self, n: int, n_occ: int, tol: float = 0.0, n_steps_hint: int = 64):

@@ -329,3 +329,28 @@ def test_refinement_layers_purify_eigenvalues_and_keep_eigenvectors(cfg1):
     assert np.abs(Xr - P).max() < 1e-7 and np.linalg.norm(Xr @ P - P @ Xr) < 1e-12   # same eigenvectors
     Pr, _ = oracle.sp2_refine_layers(P, n_occ, layers=2)
     assert np.abs(Pr - P).max() < 1e-13                # the projector is a fixed point
+
+
+def test_congruence_against_the_generalised_eigenproblem():
+    """with Z^T S Z = I, the orthogonalised problem has the spectrum of the generalised problem
+    H c = eps S c, and D = Z D_orth Z^T is the S-metric projector: D S D = D, tr(D S) = N_occ (scipy's generalised
+    eigensolver is the independent reference)."""
+    import scipy.linalg
+
+    q = inputs.overlap_problem(60, 25)
+    H, S, Z, n_occ = q["H"], q["S"], q["Z"], q["n_occ"]
+    np.testing.assert_allclose(oracle.congruence(Z, S), np.eye(60), atol=1e-12)         # Z^T S Z = I
+    Horth = oracle.congruence(Z, H)
+    eps, Cg = scipy.linalg.eigh(H, S)
+    np.testing.assert_allclose(np.linalg.eigvalsh(Horth), eps, atol=1e-11)
+    np.testing.assert_allclose(np.sort(eps), np.sort(q["lam"]), atol=1e-11)             # the generator's spectrum
+    Dorth, _ = oracle.density_eigh(Horth, n_occ)
+    D = oracle.congruence(Z, Dorth, transpose_first=False)
+    np.testing.assert_allclose(D, Cg[:, :n_occ] @ Cg[:, :n_occ].T, atol=1e-11)          # S-normalised eigenvectors
+    assert np.abs(D @ S @ D - D).max() < 1e-11 and abs(np.trace(D @ S) - n_occ) < 1e-11
+    # a non-symmetric Z tells Z^T X Z from Z X Z^T
+    rng = np.random.default_rng(2)
+    Zg = rng.standard_normal((5, 5)); X = rng.standard_normal((5, 5)); X = X + X.T
+    a = oracle.congruence(Zg, X, True); b = oracle.congruence(Zg, X, False)
+    assert a[1, 2] == pytest.approx(sum(Zg[k, 1] * X[k, l] * Zg[l, 2] for k in range(5) for l in range(5)))
+    assert b[1, 2] == pytest.approx(sum(Zg[1, k] * X[k, l] * Zg[2, l] for k in range(5) for l in range(5)))
