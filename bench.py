@@ -280,10 +280,12 @@ def run_ours(args):
     D = torch.empty_like(H)
     D1 = torch.empty_like(H) if response else None
     h = sp2.Sp2Handle(n, response=response, host_staging=True, refinement=args.refine > 0)
+    if args.lanczos > 0:
+        h.set_options(lanczos_steps=args.lanczos)
     if args.refine > 0:
         if response:
             raise SystemExit("--refine goes with --workload density")
-        h.set_options(refine_layers=args.refine)
+        h.set_options(refine_layers=args.refine, lanczos_steps=args.lanczos)
 
     def step():
         if response:
@@ -385,7 +387,7 @@ def run_ours(args):
             "dtype": "f16 hi/lo operand planes, f32 accumulate (f64 scalars)", "data": "synthetic",
             "config": {"workload": f"config {CONFIG_INDEX}: N={n}, N_occ={n_occ}, gap 0.05, f64 H"
                                    + (" and H1 -> D and D1 (sp2_response)" if response else " -> D (sp2_density)"),
-                       "replicas": world, "layers_per_step": layers, "refine_layers": args.refine,
+                       "replicas": world, "layers_per_step": layers, "refine_layers": args.refine, "lanczos_steps": args.lanczos,
                        "l2_policy": "inputs larger than L2 (H 537 MB, each FP16 plane 134 MB vs 126 MB L2)",
                        "flops_per_layer_logical": logical_flops_per_layer(n, response)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
@@ -499,6 +501,8 @@ def main(argv=None):
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--workload", choices=["response", "density", "sequence", "congruence"], default="response")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--lanczos", type=int, default=0,
+                    help="Lanczos steps for tighter spectral bounds (SURVEY 8(f) NEXT-3); extra, not the headline")
     ap.add_argument("--refine", type=int, default=0,
                     help="float64 refinement layers after the stack (PAPER.md:170; --workload density only); extra, not the headline")
     args = ap.parse_args(argv)

@@ -81,6 +81,9 @@ typedef struct {
   int forced_layers;      /* debug: > 0 runs exactly this many layers, no stop test */
   unsigned long long forced_signs; /* debug: with forced_layers, bit n = 1 -> layer n is X^2, else 2X - X^2 */
   int cta_group;    /* 0 = auto; 1 = 128x128 tiles, one CTA; 2 = 256x256 tiles on a CTA pair (cta_group::2) */
+  int lanczos_steps; /* 0 = off (default: Gershgorin bounds only); 1..32: that many Lanczos steps on H tighten the spectral
+                        bounds to [theta_min - beta_k, theta_max + beta_k] where that is inside the Gershgorin interval:
+                        fewer layers for dense matrices (the paper leaves accelerated variants aside) */
   int refine_layers; /* 0 = off (default); 1..4: float64 SP2 layers applied to the converged iterate before D is written
                         (the paper uses 2); D1 is not refined.  Needs SP2_WITH_REFINEMENT */
   int seg_kb;       /* 0 = default (4); 1, 2, 4, 8, 16 or 32 (must divide npad/64): k-blocks of 64 accumulated inside

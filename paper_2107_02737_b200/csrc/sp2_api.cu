@@ -39,6 +39,7 @@ void sp2_launch_gsetup(Sp2Ctrl* c, const Sp2BoundSlot* sz, const Sp2BoundSlot* s
 void sp2_launch_gswap(Sp2Ctrl* c, cudaStream_t s);
 void sp2_launch_split(const void* A, sp2_dtype_t dt, long ld, int N, int npad, int transpose, int which, const Sp2Ctrl* c,
                       __half* Ph, __half* Pm, cudaStream_t s);
+void sp2_launch_lanczos(Sp2Ctrl* c, const void* H, sp2_dtype_t dt, long ld, int N, int steps, double* vecs, cudaStream_t s);
 // sp2_refine.cu
 cudaError_t sp2_refine_configure();
 int sp2_launch_refine(Sp2Ctrl* c, __half* const planes[4], int npad, int N, int n_layers, double* Xa, double* Xb,
@@ -67,6 +68,7 @@ struct Layout {
   size_t off_ctrl, off_ring;
   size_t off_staging, staging_each;
   size_t off_refine, refine_each, off_refine_slots;
+  size_t off_lanczos;
   size_t total;
 };
 
@@ -108,6 +110,7 @@ Layout make_layout(int n_max, int flags) {
     L.staging_each = align_up((size_t)n_max * (size_t)n_max * 8, 1024);
     L.off_staging = off; off += L.staging_each * (resp ? 4 : 2);
   }
+  L.off_lanczos = off; off += align_up(3 * (size_t)n_max * sizeof(double), 1024);
   if (flags & SP2_WITH_REFINEMENT) {
     L.refine_each = align_up(npad * npad * sizeof(double), 1024);
     L.off_refine = off; off += 2 * L.refine_each;
@@ -167,6 +170,7 @@ struct sp2_handle_s {
   Sp2Ctrl* ctrl() const { return reinterpret_cast<Sp2Ctrl*>(ws + L.off_ctrl); }
   sp2_result_t* ring() const { return reinterpret_cast<sp2_result_t*>(ws + L.off_ring); }
   void* staging(int i) const { return ws + L.off_staging + (size_t)i * L.staging_each; }
+  double* lanczos_vecs() const { return reinterpret_cast<double*>(ws + L.off_lanczos); }
   double* refine_x(int i) const { return reinterpret_cast<double*>(ws + L.off_refine + (size_t)i * L.refine_each); }
   double* refine_slots() const { return reinterpret_cast<double*>(ws + L.off_refine_slots); }
   unsigned int* refine_ticket() const { return reinterpret_cast<unsigned int*>(refine_slots() + 2 * (size_t)pad_n(n_max) + 32); }
@@ -411,6 +415,11 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const void* H1, sp2_dt
   ++launches;
   sp2_launch_bounds(H, in_dt, ldh, N, 0, h->bslots(0), s); ++launches;
   if (resp) { sp2_launch_bounds(H1, in_dt, ldh, N, 1, h->bslots(1), s); ++launches; }
+  if (o.lanczos_steps > 0 && !o.user_bounds && N_occ > 0 && N_occ < N) {
+    const int k = o.lanczos_steps < N ? o.lanczos_steps : N - 1 > 0 ? N - 1 : 1;
+    sp2_launch_lanczos(c, H, in_dt, ldh, N, k, h->lanczos_vecs(), s);
+    launches += 2 + 2 * k;
+  }
   sp2_launch_setup(c, h->bslots(0), sp2_bounds_blocks(N), h->bslots(1), resp ? sp2_bounds_blocks(N) : 0, s); ++launches;
   if (N_occ == 0 || N_occ == N) {
     sp2_launch_trivial(c, D, D1, out_dt, ldd, N, h->ring() + ring_idx, s); ++launches;
@@ -567,6 +576,7 @@ sp2_status_t sp2_set_options(sp2_handle_t h, const sp2_options_t* opt) {
   if (opt->engine != SP2_ENGINE_TCGEN05 && opt->engine != SP2_ENGINE_SIMT_DEBUG) return SP2_ERR_INVALID_ARG;
   if (opt->cta_group < 0 || opt->cta_group > 2) return SP2_ERR_INVALID_ARG;
   if (opt->refine_layers < 0 || opt->refine_layers > 4) return SP2_ERR_INVALID_ARG;
+  if (opt->lanczos_steps < 0 || opt->lanczos_steps > 32) return SP2_ERR_INVALID_ARG;
   if (opt->lo_bits != 0 && (opt->lo_bits < 6 || opt->lo_bits > 11)) return SP2_ERR_INVALID_ARG;
   if (opt->seg_kb != 0 && opt->seg_kb != 1 && opt->seg_kb != 2 && opt->seg_kb != 4 && opt->seg_kb != 8 &&
       opt->seg_kb != 16 && opt->seg_kb != 32) return SP2_ERR_INVALID_ARG;

@@ -67,6 +67,10 @@ struct Sp2Ctrl {
   // plane exponents of the congruence products (sp2_congruence): operands A, B and the intermediate T
   int g_ea, g_eb, g_et;      // exponents the running product reads: A operand, B operand, plane output
   int g_el, g_ex, g_pad;     // exponents of the L (= Z or Z^T) planes and of the transformed matrix X
+  // Lanczos spectral bounds (optional, sp2_options_t.lanczos_steps)
+  int lanczos_steps, lanczos_pad;
+  double lz_alpha[32], lz_beta[33];   // tridiagonal T_k; lz_beta[j] couples j-1 and j, lz_beta[k] is the residual norm
+  double lz_min, lz_max;              // theta_min - beta_k, theta_max + beta_k
   // float64 refinement layers (sp2_refine.cu)
   double ref_tr, ref_fro;   // tr X and ||X||_F^2 of the current float64 iterate
   int ref_plus, ref_done;   // branch of the next refinement layer; layers applied

@@ -122,6 +122,11 @@ __global__ void __launch_bounds__(256) k_setup(Sp2Ctrl* c, const Sp2BoundSlot* s
   c->maxabs_h = red[3][0];
   c->maxabs_h1 = red1[0];
   double eps_min = red[0][0], eps_max = red[1][0];
+  if (c->lanczos_steps > 0 && isfinite(c->lz_min) && isfinite(c->lz_max) && c->lz_max > c->lz_min) {
+    // tighter bounds from k Lanczos steps, never wider than the Gershgorin discs
+    eps_min = fmax(eps_min, c->lz_min);
+    eps_max = fmin(eps_max, c->lz_max);
+  }
   if (c->user_bounds) { eps_min = c->user_eps_min; eps_max = c->user_eps_max; }
   c->eps_min = eps_min; c->eps_max = eps_max;
   const double delta = eps_max - eps_min;
@@ -338,6 +343,104 @@ __global__ void __launch_bounds__(256) k_finalise_reduce(Sp2Ctrl* c, const doubl
 }
 
 // ------------------------------------------------------------------------------------------
+// Optional tighter spectral bounds: k steps of the Lanczos process on H with a fixed start
+// vector; [theta_min - beta_k, theta_max + beta_k] (extreme Ritz values widened by the last residual norm, the
+// usual "safe" bound) replaces the Gershgorin interval where it is tighter.  HBM-bound: k reads of H.
+//   k_lz_init    v_0(i) = cos(0.7 i + 0.3), normalised
+//   k_lz_matvec  w = H v          (one warp per row, float64 accumulation)
+//   k_lz_step    alpha_j = w.v;  w -= alpha_j v + beta_j v_prev;  beta_{j+1} = |w|;  v_prev = v;  v = w / beta_{j+1}
+//   k_lz_finish  extreme eigenvalues of T_k by Sturm bisection
+__device__ inline double lz_block_sum(double v, double* sh /* 32 */) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+  __syncthreads();
+  double t = 0.0;
+  for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += sh[w];
+  return t;
+}
+
+__global__ void __launch_bounds__(1024) k_lz_init(Sp2Ctrl* c, int N, int steps, double* v, double* vprev) {
+  __shared__ double sh[32];
+  double s = 0.0;
+  for (int i = threadIdx.x; i < N; i += 1024) { const double x = cos(0.7 * (double)i + 0.3); v[i] = x; vprev[i] = 0.0; s += x * x; }
+  s = lz_block_sum(s, sh);
+  const double inv = 1.0 / sqrt(s);
+  for (int i = threadIdx.x; i < N; i += 1024) v[i] *= inv;
+  if (threadIdx.x == 0) { c->lanczos_steps = steps; c->lz_beta[0] = 0.0; c->lz_min = NAN; c->lz_max = NAN; }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) k_lz_matvec(const T* __restrict__ H, long ld, int N, const double* __restrict__ v,
+                                                   double* __restrict__ w) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int row = blockIdx.x * 8 + warp;
+  if (row >= N) return;
+  const T* r = H + (size_t)row * ld;
+  double s = 0.0;
+  for (int j = lane; j < N; j += 32) s += (double)__ldg(r + j) * v[j];
+  s = warp_sum(s);
+  if (lane == 0) w[row] = s;
+}
+
+__global__ void __launch_bounds__(1024) k_lz_step(Sp2Ctrl* c, int N, int j, double* v, double* vprev, double* w) {
+  __shared__ double sh[32];
+  const double beta = c->lz_beta[j];
+  double a = 0.0;
+  for (int i = threadIdx.x; i < N; i += 1024) a += w[i] * v[i];
+  a = lz_block_sum(a, sh);
+  double nn = 0.0;
+  for (int i = threadIdx.x; i < N; i += 1024) {
+    const double x = w[i] - a * v[i] - beta * vprev[i];
+    w[i] = x;
+    nn += x * x;
+  }
+  nn = lz_block_sum(nn, sh);
+  const double bnew = sqrt(nn);
+  const double inv = bnew > 0.0 ? 1.0 / bnew : 0.0;
+  for (int i = threadIdx.x; i < N; i += 1024) { vprev[i] = v[i]; v[i] = w[i] * inv; }
+  if (threadIdx.x == 0) { c->lz_alpha[j] = a; c->lz_beta[j + 1] = bnew; }
+}
+
+__global__ void k_lz_finish(Sp2Ctrl* c) {
+  const int k = c->lanczos_steps;
+  // eigenvalues of T_k lie in its own Gershgorin interval; count(x) = #eigenvalues < x by the Sturm recurrence
+  double lo = INFINITY, hi = -INFINITY;
+  for (int j = 0; j < k; ++j) {
+    const double r = (j > 0 ? fabs(c->lz_beta[j]) : 0.0) + (j + 1 < k ? fabs(c->lz_beta[j + 1]) : 0.0);
+    lo = fmin(lo, c->lz_alpha[j] - r);
+    hi = fmax(hi, c->lz_alpha[j] + r);
+  }
+  auto count_below = [&](double x) {
+    int cnt = 0;
+    double d = 1.0;
+    for (int j = 0; j < k; ++j) {
+      const double b2 = j > 0 ? c->lz_beta[j] * c->lz_beta[j] : 0.0;
+      d = (c->lz_alpha[j] - x) - (j > 0 ? b2 / d : 0.0);
+      if (d == 0.0) d = -1e-300;
+      if (d < 0.0) ++cnt;
+    }
+    return cnt;
+  };
+  double a = lo, b = hi;                 // smallest eigenvalue: count_below crosses from 0 to >= 1
+  for (int it = 0; it < 200 && b - a > 1e-14 * fmax(fabs(a), fabs(b)); ++it) {
+    const double m = 0.5 * (a + b);
+    if (count_below(m) >= 1) b = m; else a = m;
+  }
+  const double th_min = a;
+  a = lo; b = hi;                        // largest: count_below crosses from k-1 to k
+  for (int it = 0; it < 200 && b - a > 1e-14 * fmax(fabs(a), fabs(b)); ++it) {
+    const double m = 0.5 * (a + b);
+    if (count_below(m) >= k) b = m; else a = m;
+  }
+  const double th_max = b;
+  const double res = fabs(c->lz_beta[k]);
+  c->lz_min = th_min - res;
+  c->lz_max = th_max + res;
+}
+
+// ------------------------------------------------------------------------------------------
 // Congruence transform support (sp2_congruence: H_orth = Z^T H Z, D = Z D_orth Z^T).
 // k_gsetup: plane exponents from max|.| of the two inputs; k_split: matrix (or its transpose) -> hi/lo planes;
 // k_gswap: operand exponents of the second product.
@@ -504,4 +607,15 @@ void sp2_launch_split(const void* A, sp2_dtype_t dt, long ld, int N, int npad, i
   const int nb = npad / 32;
   SP2_DISPATCH_IN(dt, (k_split<float><<<nb * nb, 256, 0, s>>>((const float*)A, ld, N, npad, transpose, which, c, Ph, Pm)),
                   (k_split<double><<<nb * nb, 256, 0, s>>>((const double*)A, ld, N, npad, transpose, which, c, Ph, Pm)));
+}
+
+void sp2_launch_lanczos(Sp2Ctrl* c, const void* H, sp2_dtype_t dt, long ld, int N, int steps, double* vecs, cudaStream_t s) {
+  double* v = vecs; double* vprev = vecs + N; double* w = vecs + 2 * (size_t)N;
+  k_lz_init<<<1, 1024, 0, s>>>(c, N, steps, v, vprev);
+  for (int j = 0; j < steps; ++j) {
+    SP2_DISPATCH_IN(dt, (k_lz_matvec<float><<<(N + 7) / 8, 256, 0, s>>>((const float*)H, ld, N, v, w)),
+                    (k_lz_matvec<double><<<(N + 7) / 8, 256, 0, s>>>((const double*)H, ld, N, v, w)));
+    k_lz_step<<<1, 1024, 0, s>>>(c, N, j, v, vprev, w);
+  }
+  k_lz_finish<<<1, 1, 0, s>>>(c);
 }

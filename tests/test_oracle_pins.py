@@ -354,3 +354,25 @@ def test_congruence_against_the_generalised_eigenproblem():
     a = oracle.congruence(Zg, X, True); b = oracle.congruence(Zg, X, False)
     assert a[1, 2] == pytest.approx(sum(Zg[k, 1] * X[k, l] * Zg[l, 2] for k in range(5) for l in range(5)))
     assert b[1, 2] == pytest.approx(sum(Zg[1, k] * X[k, l] * Zg[2, l] for k in range(5) for l in range(5)))
+
+
+def test_lanczos_bounds_enclose_the_spectrum_and_are_tighter(cfg1):
+    """The Lanczos interval must contain every eigenvalue (LAPACK is the reference) on dense, sparse and diagonal
+    matrices, never be wider than Gershgorin, be far tighter for the dense random-Q configs, and give the SAME
+    projector in fewer layers."""
+    mats = [cfg1["H"], inputs.ssh_chain(200, 1.0, 0.6, onsite=0.3)[0], np.diag(np.linspace(-3.0, 5.0, 50)),
+            inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[3], 150))["H"].astype(np.float64)]
+    for H in mats:
+        w = np.linalg.eigvalsh(H)
+        g_lo, g_hi = oracle.gershgorin_bounds(H)
+        for k in (4, 12, 24):
+            lo, hi = oracle.lanczos_bounds(H, k)
+            assert lo <= w[0] + 1e-12 and hi >= w[-1] - 1e-12
+            assert lo >= g_lo - 1e-12 and hi <= g_hi + 1e-12
+    H, n_occ = cfg1["H"], cfg1["n_occ"]
+    lo, hi = oracle.lanczos_bounds(H, 12)
+    g_lo, g_hi = oracle.gershgorin_bounds(H)
+    assert (hi - lo) < 0.35 * (g_hi - g_lo)
+    r_g = oracle.sp2_density(H, n_occ)
+    r_l = oracle.sp2_density(H, n_occ, bounds=(lo, hi))
+    assert np.abs(r_g["D"] - r_l["D"]).max() < 1e-12 and r_l["layers"] <= r_g["layers"] - 3
