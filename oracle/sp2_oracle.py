@@ -22,9 +22,17 @@ PAPER.md:231 only names the Krylov kernel that consumes it):
 * first-order perturbation theory  -> ``response_closed_form``
 * central finite difference        -> ``response_finite_difference``
 
+and, for the rows SURVEY 8(f) marks "next":
+
+* float64 refinement layers          -> ``sp2_refine_layers``
+* congruence transforms of PAPER.md:137             -> ``congruence``
+* Lanczos spectral bounds (tighter than Gershgorin) -> ``lanczos_bounds``
+
 Pin status: every function here is pinned by ``tests/test_oracle_pins.py``
 (eigendecomposition, closed forms, invariants, textbook special cases,
-brute force on tiny inputs).  Nothing is "parity unpinned".
+brute force on tiny inputs, the generalised eigenproblem for the congruence,
+LAPACK spectra for the Lanczos enclosure, scalar eigenvalue maps for the
+refinement).  Nothing is "parity unpinned".
 
 Readings where the paper is silent (full list with reasons in DESIGN.md):
   R1  spectral bounds  = Gershgorin discs                     (PAPER.md:145 silent)
