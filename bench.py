@@ -419,6 +419,8 @@ def run_sequence(args):
     Ht = torch.empty_like(H0)
     D = torch.empty_like(H0)
     h = sp2.Sp2Handle(n)
+    if args.lanczos > 0:
+        h.set_options(lanczos_steps=args.lanczos)
     for _ in range(max(args.warmup, 3)):
         h.density(H0, n_occ, out=D)
     stream = torch.cuda.current_stream()
@@ -444,7 +446,7 @@ def run_sequence(args):
             "vs_baseline": None, "dtype": "f16 hi/lo operand planes, f32 accumulate (f64 scalars)", "data": "synthetic",
             "config": {"workload": f"config 5: N={n}, N_occ={n_occ}, gap 0.2, f32, {args.steps} consecutive H_t through "
                                    "sp2_sequence_* (max_layers launches per step, one sync at the end)",
-                       "layers_per_step": layers, "issued_tflops": 1.5 * flops / (ms * 1e-3) / 1e12,
+                       "lanczos_steps": args.lanczos, "layers_per_step": layers, "issued_tflops": 1.5 * flops / (ms * 1e-3) / 1e12,
                        "statuses": sorted({r["status"] for r in res}),
                        "max_abs_trD_minus_nocc": max(abs(r["tr_d"] - n_occ) for r in res)},
             "clocks": clocks, "gpu_launches": int(h.launch_count - launches0)}
