@@ -384,9 +384,10 @@ def run_ours(args):
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f16 hi/lo operand planes, f32 accumulate (f64 scalars)", "data": "synthetic",
+            "dtype": "f16", "data": "synthetic",
             "config": {"workload": f"config {CONFIG_INDEX}: N={n}, N_occ={n_occ}, gap 0.05, f64 H"
                                    + (" and H1 -> D and D1 (sp2_response)" if response else " -> D (sp2_density)"),
+                       "precision": "FP16 hi + lo operand planes (22 bits), FP32 accumulation in k-segments, f64 scalars, f64 in/out",
                        "replicas": world, "layers_per_step": layers, "refine_layers": args.refine, "lanczos_steps": args.lanczos,
                        "l2_policy": "inputs larger than L2 (H 537 MB, each FP16 plane 134 MB vs 126 MB L2)",
                        "flops_per_layer_logical": logical_flops_per_layer(n, response)},
@@ -443,7 +444,7 @@ def run_sequence(args):
     flops = sum(logical_flops_per_layer(n, False) * L for L in layers)
     line = {"metric": METRIC, "value": flops / (ms * 1e-3) / 1e12, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f16 hi/lo operand planes, f32 accumulate (f64 scalars)", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f16", "data": "synthetic",
             "config": {"workload": f"config 5: N={n}, N_occ={n_occ}, gap 0.2, f32, {args.steps} consecutive H_t through "
                                    "sp2_sequence_* (max_layers launches per step, one sync at the end)",
                        "lanczos_steps": args.lanczos, "layers_per_step": layers, "issued_tflops": 1.5 * flops / (ms * 1e-3) / 1e12,
@@ -486,7 +487,7 @@ def run_congruence(args):
     err = float((C - Z.T @ X @ Z).abs().max())          # cross-check with torch float64 (harness, not library)
     line = {"metric": "issued Tflop/s of sp2_congruence (Z^T X Z, N=8192)", "value": 12.0 * n ** 3 / (ms * 1e-3) / 1e12,
             "unit": "TFLOP/s (issued)", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16 hi/lo operand planes, f32 accumulate",
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16",
             "data": "synthetic", "config": {"workload": "sp2_congruence: C = Z^T X Z, N=8192, f64 in/out, general Z, symmetric X",
                                             "max_abs_err_vs_torch_f64": err, "max_abs_C": float(C.abs().max())},
             "gpu_launches": int(h.launch_count - launches0)}
