@@ -15,6 +15,7 @@ from .sp2_oracle import (  # noqa: F401
     rescale_to_unit_interval,
     sp2_stop,
     sp2_density,
+    sp2_response_batch,
     sp2_refine_layers,
     congruence,
     density_eigh,

@@ -27,12 +27,14 @@ and, for the rows SURVEY 8(f) marks "next":
 * float64 refinement layers          -> ``sp2_refine_layers``
 * congruence transforms of PAPER.md:137             -> ``congruence``
 * Lanczos spectral bounds (tighter than Gershgorin) -> ``lanczos_bounds``
+* several perturbations on one stack of layers      -> ``sp2_response_batch``
 
 Pin status: every function here is pinned by ``tests/test_oracle_pins.py``
 (eigendecomposition, closed forms, invariants, textbook special cases,
 brute force on tiny inputs, the generalised eigenproblem for the congruence,
 LAPACK spectra for the Lanczos enclosure, scalar eigenvalue maps for the
-refinement).  Nothing is "parity unpinned".
+refinement, perturbation theory and linearity for the batched response).
+Nothing is "parity unpinned".
 
 Readings where the paper is silent (full list with reasons in DESIGN.md):
   R1  spectral bounds  = Gershgorin discs                     (PAPER.md:145 silent)
@@ -54,6 +56,7 @@ __all__ = [
     "rescale_to_unit_interval",
     "sp2_stop",
     "sp2_density",
+    "sp2_response_batch",
     "sp2_refine_layers",
     "congruence",
     "density_eigh",
@@ -243,6 +246,56 @@ def sp2_density(H, n_occ, H1=None, tol=0.0, max_layers=100, bounds=None):
                 eps_min=eps_min, eps_max=eps_max, tr_d=float(np.trace(X)),
                 tr_dh=float(np.sum(X * H)),
                 tr_d1=None if Z is None else float(np.trace(Z)))
+
+
+def sp2_response_batch(H, n_occ, H1s, tol=0.0, max_layers=100, bounds=None):
+    """Several perturbations H1_b of the same H carried through ONE stack of layers (the
+    "preconditioned Krylov subspace approximation" of the kernel, asks for the response of the same
+    Hamiltonian to several perturbations per MD step).  Same loop as ``sp2_density``; reading R5 applied to every
+    Z_b = dX/d(lambda_b) with the zeroth-order signs:
+        Z_b0 = -H1_b/Delta;    '+':  Z_b <- X Z_b + Z_b X;    '-':  Z_b <- 2 Z_b - (X Z_b + Z_b X).
+    The first-order terms do not couple, so D1_b is the response ``sp2_density(H, n_occ, H1=H1_b)`` would return.
+
+    Returns a dict with D, D1 (list), layers, signs, stop, eps_min, eps_max, tr_d, tr_dh, tr_d1 (list).
+    """
+    H = _as_f64_symmetric(H, "H")
+    N = H.shape[0]
+    if not 0 <= n_occ <= N:
+        raise ValueError("n_occ out of range")
+    H1s = [_as_f64_symmetric(H1, "H1") for H1 in H1s]
+    for H1 in H1s:
+        if H1.shape != H.shape:
+            raise ValueError("H1 shape mismatch")
+    eps_min, eps_max = gershgorin_bounds(H) if bounds is None else map(float, bounds)
+    if n_occ == 0 or n_occ == N:
+        D = np.zeros((N, N)) if n_occ == 0 else np.eye(N)
+        return dict(D=D, D1=[np.zeros((N, N)) for _ in H1s], layers=0, signs="", stop="trivial", eps_min=eps_min,
+                    eps_max=eps_max, tr_d=float(n_occ), tr_dh=float(np.sum(D * H)), tr_d1=[0.0 for _ in H1s])
+    delta = eps_max - eps_min
+    X = rescale_to_unit_interval(H, eps_min, eps_max)            # PAPER.md:145
+    Zs = [-H1 / delta for H1 in H1s]                             # R5
+    e_hist, signs = [], []
+    n = 0
+    while True:
+        X2 = X @ X                                               # f(X) = X^2, PAPER.md:153
+        t = float(np.trace(X))
+        t2 = float(np.trace(X2))
+        e_hist.append(t - t2)                                    # PAPER.md:186
+        stop = sp2_stop(n, e_hist, signs, t, n_occ, tol, max_layers)
+        if stop is not None:
+            break
+        plus = abs(t2 - n_occ) < abs(2.0 * t - t2 - n_occ)       # R3, ties -> '-'
+        Ws = [X @ Z + Z @ X for Z in Zs]
+        if plus:                                                 # S_n = S_{n-1}^2
+            X = X2
+            Zs = Ws
+        else:                                                    # S_n = 2 S_{n-1} - S_{n-1}^2
+            X = 2.0 * X - X2
+            Zs = [2.0 * Z - W for Z, W in zip(Zs, Ws)]
+        signs.append("+" if plus else "-")
+        n += 1
+    return dict(D=X, D1=Zs, layers=n, signs="".join(signs), stop=stop, eps_min=eps_min, eps_max=eps_max,
+                tr_d=float(np.trace(X)), tr_dh=float(np.sum(X * H)), tr_d1=[float(np.trace(Z)) for Z in Zs])
 
 
 def sp2_refine_layers(X, n_occ, layers=2):

@@ -131,6 +131,19 @@ def make_problem(cfg: Sp2Config, seed: int | None = None, device: str = "cpu",
     return out
 
 
+def perturbations(n: int, nb: int, seed: int = 20210714, dtype=np.float64, decades: float = 1.0):
+    """nb symmetric perturbations for the batched response (stand-ins for the Krylov vectors of PAPER.md:231):
+    H1_b = 10^(-2 - decades * b) (G_b + G_b^T)/sqrt(2), G_b ~ N(0,1)^(n x n) -- magnitudes ``decades`` apart, so that a
+    shared plane exponent would lose the small ones."""
+    rng = np.random.default_rng(seed + 977)
+    out = []
+    for b in range(nb):
+        G = rng.standard_normal((n, n))
+        out.append(np.ascontiguousarray((10.0 ** (-2.0 - decades * b) * (G + G.T) / math.sqrt(2.0)).astype(dtype)))
+        del G
+    return out
+
+
 def band_energy_closed_form(lam, n_occ):
     """sum of the n_occ lowest generator eigenvalues (what tr(DH) must equal
     for an exact-arithmetic H; a property of the INPUT, not of the method)."""

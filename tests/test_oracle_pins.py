@@ -376,3 +376,27 @@ def test_lanczos_bounds_enclose_the_spectrum_and_are_tighter(cfg1):
     r_g = oracle.sp2_density(H, n_occ)
     r_l = oracle.sp2_density(H, n_occ, bounds=(lo, hi))
     assert np.abs(r_g["D"] - r_l["D"]).max() < 1e-12 and r_l["layers"] <= r_g["layers"] - 3
+
+
+def test_batched_response_vs_perturbation_theory_and_linearity():
+    """NEXT-4: every D1_b of the one-stack loop equals first-order perturbation theory for its own H1_b (an
+    index mix-up between the Z_b, a dropped factor or a shared update fails this), and the map H1 -> D1 is linear."""
+    cfg = inputs.Sp2Config("t", 2, 56, 21, (-1.5, -0.25), (0.25, 1.5), "f64", False)
+    p = inputs.make_problem(cfg)
+    H1s = inputs.perturbations(56, 3, seed=5)
+    r = oracle.sp2_response_batch(p["H"], 21, H1s)
+    D_eig, w = oracle.density_eigh(p["H"], 21)
+    assert np.abs(r["D"] - D_eig).max() < 1e-12
+    assert r["tr_dh"] == pytest.approx(w[:21].sum(), rel=1e-12)
+    for b, H1 in enumerate(H1s):
+        pt = oracle.response_closed_form(p["Q"], p["lam"], 21, H1)
+        assert np.abs(r["D1"][b] - pt).max() < 1e-11 * np.abs(pt).max()
+        assert abs(r["tr_d1"][b]) < 1e-10 * np.abs(pt).max() * 56
+    mix = 2.0 * H1s[0] - 30.0 * H1s[1] + 500.0 * H1s[2]
+    rm = oracle.sp2_response_batch(p["H"], 21, [mix])
+    want = 2.0 * r["D1"][0] - 30.0 * r["D1"][1] + 500.0 * r["D1"][2]
+    np.testing.assert_allclose(rm["D1"][0], want, rtol=0, atol=1e-11 * np.abs(want).max())
+    # trivial occupations and the empty batch
+    assert oracle.sp2_response_batch(p["H"], 0, H1s)["D1"][2].max() == 0.0
+    r0 = oracle.sp2_response_batch(p["H"], 21, [])
+    assert r0["D1"] == [] and r0["signs"] == r["signs"]
