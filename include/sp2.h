@@ -68,6 +68,8 @@ typedef enum { SP2_F32 = 0, SP2_F64 = 1 } sp2_dtype_t;
 #define SP2_WITH_RESPONSE 1     /* room for the first-order iterate Z (sp2_response) */
 #define SP2_WITH_HOST_STAGING 2 /* room for device copies of H, H1, D, D1 (the *_host calls), f64-sized */
 #define SP2_WITH_REFINEMENT 4   /* room for two float64 N x N iterates (sp2_options_t.refine_layers > 0) */
+#define SP2_MAX_BATCH 8         /* perturbations one sp2_response_batch call can carry */
+#define SP2_WITH_BATCH(nb) (((nb) & 15) << 8) /* room for nb first-order iterates (implies SP2_WITH_RESPONSE) */
 
 /* layer engines (sp2_options_t.engine) */
 #define SP2_ENGINE_TCGEN05 0 /* product path: TMA + tcgen05.mma + TMEM */
@@ -141,6 +143,17 @@ SP2_API sp2_status_t sp2_response(sp2_handle_t handle, const void* dH, const voi
                           int N, int N_occ, double tol,
                           void* dD, void* dD1, sp2_dtype_t out_dtype, long ldo,
                           sp2_result_t* out, void* stream);
+
+/* Batched response ("preconditioned Krylov subspace approximation" of the kernel
+ * needs the response of the same H to several perturbations per MD step): nb perturbations H1_b ride ONE stack
+ * of layers, Y^2 is formed once per layer and Y Z_b + Z_b Y once per perturbation, every Z_b with its own plane
+ * exponent.  dH1 / dD1 are HOST arrays of nb DEVICE pointers (same dtype and pitch as H / D); tr_d1 is a HOST
+ * array of nb doubles (may be NULL) that receives tr D1_b (out->tr_d1 = tr D1_0).  1 <= nb <= the nb given to
+ * SP2_WITH_BATCH at create (1 with plain SP2_WITH_RESPONSE).  Blocking.  No host-buffer twin. */
+SP2_API sp2_status_t sp2_response_batch(sp2_handle_t handle, const void* dH, const void* const* dH1, int nb,
+                                sp2_dtype_t in_dtype, long ld, int N, int N_occ, double tol,
+                                void* dD, void* const* dD1, sp2_dtype_t out_dtype, long ldo,
+                                double* tr_d1, sp2_result_t* out, void* stream);
 
 /* Host-buffer twins: hH/hH1/hD/hD1 are HOST pointers; H2D and D2H copies run on `stream` inside the
  * call.  Need SP2_WITH_HOST_STAGING (and SP2_WITH_RESPONSE for the response twin). */

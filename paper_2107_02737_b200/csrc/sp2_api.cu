@@ -29,9 +29,9 @@ void sp2_launch_rescale(const void* H, sp2_dtype_t dt, long ld, const Sp2Ctrl* c
                         int npad, Sp2Slot* slots, cudaStream_t s);
 void sp2_launch_ctrl0(Sp2Ctrl* c, const Sp2Slot* ys, const Sp2Slot* zs, int count, cudaStream_t s);
 int sp2_finalise_blocks(int N);
+void sp2_launch_finalise_reduce(Sp2Ctrl* c, int N, double* slots, sp2_result_t* ring_entry, cudaStream_t s);
 void sp2_launch_finalise(Sp2Ctrl* c, __half* const planes[8], int npad, const void* H, sp2_dtype_t in_dt, long ldh,
-                         void* D, void* D1, sp2_dtype_t out_dt, long ldo, int N, double* slots,
-                         sp2_result_t* ring_entry, cudaStream_t s);
+                         void* D, void* D1, sp2_dtype_t out_dt, long ldo, int N, int zb, double* slots, cudaStream_t s);
 void sp2_launch_trivial(Sp2Ctrl* c, void* D, void* D1, sp2_dtype_t out_dt, long ldo, int N, sp2_result_t* ring_entry,
                         cudaStream_t s);
 void sp2_launch_gsetup(Sp2Ctrl* c, const Sp2BoundSlot* sz, const Sp2BoundSlot* sa, int count, int N, sp2_result_t* ring_entry,
@@ -58,7 +58,8 @@ inline int pad_n(int n) { return (int)align_up((size_t)n, kPadTo); }
 
 struct Layout {
   size_t plane_bytes;     // one FP16 plane at n_max
-  size_t off_planes;      // 4 or 8 planes: [buf][Yh, Ym] then [buf][Zh, Zm]
+  int nb_max;             // perturbations the workspace has planes for (0: density only)
+  size_t off_planes;      // 4 + 4 nb_max planes: [buf][Yh, Ym] then, per perturbation, [buf][Zh, Zm]
   size_t off_slots, slots_count;
   size_t off_slots2;      // second slot array (Z partials of the prologue)
   size_t off_bslots, bslots_count;
@@ -76,10 +77,13 @@ Layout make_layout(int n_max, int flags) {
   Layout L;
   memset(&L, 0, sizeof(L));
   const size_t npad = (size_t)pad_n(n_max);
-  const bool resp = flags & SP2_WITH_RESPONSE;
+  int resp = (flags >> 8) & 15;                      // SP2_WITH_BATCH(nb)
+  if (resp > SP2_MAX_BATCH) resp = SP2_MAX_BATCH;
+  if (resp == 0 && (flags & SP2_WITH_RESPONSE)) resp = 1;
+  L.nb_max = resp;
   L.plane_bytes = align_up(npad * npad * 2, 1024);
   size_t off = 0;
-  L.off_planes = off; off += L.plane_bytes * (resp ? 8 : 4);
+  L.off_planes = off; off += L.plane_bytes * (4 + 4 * (size_t)resp);
   size_t s_tc = (size_t)sp2_layer_slots((int)npad, 1, resp, SP2_ENGINE_TCGEN05);
   size_t s_tc2 = (size_t)sp2_layer_slots((int)npad, 2, resp, SP2_ENGINE_TCGEN05);
   size_t s_simt = npad <= (size_t)kSimtMaxN ? (size_t)sp2_layer_slots((int)npad, 1, resp, SP2_ENGINE_SIMT_DEBUG) : 0;
@@ -89,14 +93,15 @@ Layout make_layout(int n_max, int flags) {
   if (s_simt > L.slots_count) L.slots_count = s_simt;
   if (s_resc > L.slots_count) L.slots_count = s_resc;
   L.off_slots = off; off += align_up(L.slots_count * sizeof(Sp2Slot), 1024);
-  L.off_slots2 = off; off += align_up(s_resc * sizeof(Sp2Slot), 1024);
+  const size_t nb1 = resp > 1 ? (size_t)resp : 1;
+  L.off_slots2 = off; off += align_up(nb1 * s_resc * sizeof(Sp2Slot), 1024);
   L.bslots_count = (size_t)sp2_bounds_blocks(n_max);
-  L.off_bslots = off; off += align_up(2 * L.bslots_count * sizeof(Sp2BoundSlot), 1024);
-  L.off_fslots = off; off += align_up(3 * (size_t)sp2_finalise_blocks(n_max) * sizeof(double), 1024);
+  L.off_bslots = off; off += align_up((1 + nb1) * L.bslots_count * sizeof(Sp2BoundSlot), 1024);
+  L.off_fslots = off; off += align_up(3 * nb1 * (size_t)sp2_finalise_blocks(n_max) * sizeof(double), 1024);
   const size_t nt1 = npad / 128;
   L.tiles_count = nt1 * nt1;                 // the congruence products use every tile, the layers the upper triangle
   L.off_tiles = off; off += align_up(L.tiles_count * sizeof(int2), 1024);
-  L.items_cap = 2 * L.tiles_count + 1024;
+  L.items_cap = (1 + nb1) * L.tiles_count + 1024;
   L.off_items = off; off += align_up(L.items_cap * sizeof(Sp2Item), 1024);
   L.off_item_begin = off; off += align_up((kMaxClusters + 1) * sizeof(int), 1024);
   L.scratch_bytes = 2 * (size_t)kMaxClusters * sp2_layer_scratch_slot_bytes(1);
@@ -131,6 +136,7 @@ void default_options(sp2_options_t* o) {
 
 struct sp2_handle_s {
   int n_max, flags, device, num_sms;
+  int nb_max;                    // perturbations the workspace can carry (0: density only)
   uint8_t* ws;
   size_t ws_bytes;
   Layout L;
@@ -154,12 +160,12 @@ struct sp2_handle_s {
   double seq_tol;
   cudaStream_t seq_stream;
 
-  __half* plane(int which /*0 Yh,1 Ym,2 Zh,3 Zm*/, int buf) const {
-    const int idx = (which < 2) ? (buf * 2 + which) : (4 + buf * 2 + (which - 2));
+  __half* plane(int which /*0 Yh, 1 Ym, 2 + 2b Zh of perturbation b, 3 + 2b Zm*/, int buf) const {
+    const int idx = (which < 2) ? (buf * 2 + which) : (4 + 4 * ((which - 2) >> 1) + buf * 2 + (which & 1));
     return reinterpret_cast<__half*>(ws + L.off_planes + (size_t)idx * L.plane_bytes);
   }
   Sp2Slot* slots() const { return reinterpret_cast<Sp2Slot*>(ws + L.off_slots); }
-  Sp2Slot* slots2() const { return reinterpret_cast<Sp2Slot*>(ws + L.off_slots2); }
+  Sp2Slot* slots2() const { return reinterpret_cast<Sp2Slot*>(ws + L.off_slots2); }   // nb arrays of sp2_rescale_blocks
   Sp2BoundSlot* bslots(int i) const { return reinterpret_cast<Sp2BoundSlot*>(ws + L.off_bslots) + (size_t)i * L.bslots_count; }
   double* fslots() const { return reinterpret_cast<double*>(ws + L.off_fslots); }
   int2* tiles() const { return reinterpret_cast<int2*>(ws + L.off_tiles); }
@@ -197,7 +203,7 @@ void build_tiles(int nt, std::vector<int2>& out) {
           if (tj >= ti) out.push_back(make_int2(ti, tj));
 }
 
-// Static work lists.  Units (first the 2-pass YZ+ZY units, then the Y^2
+// Static work lists.  Units (first the 2-pass YZ+ZY units of every perturbation, then the Y^2
 // units, each list in the L2-friendly tile order) are dealt whole to the least-loaded CTA(-pair) --
 // equal costs make that a round-robin whose concurrent units are neighbours -- as long as they fit
 // under T = ceil(total segments / clusters).  The units that do not fit (the last, partial wave) are cut
@@ -205,8 +211,8 @@ void build_tiles(int nt, std::vector<int2>& out) {
 // epilogue.  Loads differ by at most one segment.
 void build_schedule(int n_tiles, int resp, int segs_y, int nC, std::vector<Sp2Item>& items,
                     std::vector<int>& begin, int* n_flags, int* n_slots) {
-  const int n_units = n_tiles * (resp ? 2 : 1);
-  auto cost = [&](int u) { return (resp && u < n_tiles) ? 2 * segs_y : segs_y; };
+  const int n_units = n_tiles * (1 + resp);          // resp = number of perturbations; their units come first
+  auto cost = [&](int u) { return (u < resp * n_tiles) ? 2 * segs_y : segs_y; };
   long long total = 0;
   for (int u = 0; u < n_units; ++u) total += cost(u);
   const int T = (int)((total + nC - 1) / nC);
@@ -308,7 +314,7 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   build_tiles(nt, h->tiles_host);
   SP2_CUDA(h, cudaMemcpyAsync(h->tiles(), h->tiles_host.data(), h->tiles_host.size() * sizeof(int2),
                               cudaMemcpyHostToDevice, s));
-  int n_units = (int)h->tiles_host.size() * (resp ? 2 : 1);
+  int n_units = (int)h->tiles_host.size() * (1 + resp);
   int nC = h->num_sms / cg;
   if (nC > kMaxClusters / cg) nC = kMaxClusters / cg;
   (void)n_units;   // fewer units than CTA(-pair)s: the schedule splits them along k, every SM gets work
@@ -329,8 +335,8 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   for (int par = 0; par < 2; ++par) {
     Sp2LayerArgs& a = h->args[par];
     memset(&a, 0, sizeof(a));
-    for (int w = 0; w < 4; ++w) {
-      const bool have = (w < 2) || (h->flags & SP2_WITH_RESPONSE);
+    for (int w = 0; w < 2 + 2 * (resp > 1 ? resp : 1); ++w) {
+      const bool have = (w < 2) || (w < 2 + 2 * h->nb_max);
       const __half* in = have ? h->plane(w, par) : h->plane(w & 1, par);
       __half* out = have ? h->plane(w, par ^ 1) : h->plane(w & 1, par ^ 1);
       a.in[w] = in; a.out[w] = out;
@@ -349,12 +355,27 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   return SP2_OK;
 }
 
-sp2_status_t check_args(sp2_handle_t h, const void* H, const void* H1, int want_resp, sp2_dtype_t in_dt, long ldh, int N,
-                        int N_occ, void* D, void* D1, sp2_dtype_t out_dt, long ldd) {
+// the perturbations of one solve (device pointers, or host pointers for the *_host twins)
+struct Pert {
+  int nb;
+  const void* H1[SP2_MAX_BATCH];
+  void* D1[SP2_MAX_BATCH];
+};
+
+Pert make_pert(const void* H1, void* D1) {
+  Pert P;
+  memset(&P, 0, sizeof(P));
+  if (H1 || D1) { P.nb = 1; P.H1[0] = H1; P.D1[0] = D1; }
+  return P;
+}
+
+sp2_status_t check_args(sp2_handle_t h, const void* H, const Pert& P, sp2_dtype_t in_dt, long ldh, int N,
+                        int N_occ, void* D, sp2_dtype_t out_dt, long ldd) {
   if (!h) return SP2_ERR_INVALID_ARG;
   if (!H || !D) return SP2_ERR_INVALID_ARG;
-  if (want_resp && (!H1 || !D1)) return SP2_ERR_INVALID_ARG;
-  if (want_resp && !(h->flags & SP2_WITH_RESPONSE)) return SP2_ERR_INVALID_ARG;
+  if (P.nb < 0 || P.nb > SP2_MAX_BATCH) return SP2_ERR_INVALID_ARG;
+  for (int b = 0; b < P.nb; ++b) if (!P.H1[b] || !P.D1[b]) return SP2_ERR_INVALID_ARG;
+  if (P.nb > h->nb_max) return P.nb > 1 && h->nb_max > 0 ? SP2_ERR_WORKSPACE : SP2_ERR_INVALID_ARG;
   if (N <= 0 || N > h->n_max) return SP2_ERR_INVALID_ARG;
   if (N_occ < 0 || N_occ > N) return SP2_ERR_INVALID_ARG;
   if (ldh < N || ldd < N) return SP2_ERR_INVALID_ARG;
@@ -374,13 +395,18 @@ sp2_status_t enqueue_layers(sp2_handle_t h, int first, int count, cudaStream_t s
   return SP2_OK;
 }
 
-sp2_status_t enqueue_finalise(sp2_handle_t h, const void* H, sp2_dtype_t in_dt, long ldh, int N, int resp, void* D, void* D1,
+sp2_status_t enqueue_finalise(sp2_handle_t h, const void* H, sp2_dtype_t in_dt, long ldh, int N, const Pert& P, void* D,
                               sp2_dtype_t out_dt, long ldd, int ring_idx, cudaStream_t s, int* launches) {
-  __half* planes[8] = {h->plane(0, 0), h->plane(1, 0), h->plane(0, 1), h->plane(1, 1),
-                       h->plane(resp ? 2 : 0, 0), h->plane(resp ? 3 : 1, 0), h->plane(resp ? 2 : 0, 1), h->plane(resp ? 3 : 1, 1)};
-  sp2_launch_finalise(h->ctrl(), planes, h->cur_npad, H, in_dt, ldh, D, resp ? D1 : nullptr, out_dt, ldd, N, h->fslots(),
-                      h->ring() + ring_idx, s);
-  *launches += 2;
+  for (int b = 0; b < (P.nb > 0 ? P.nb : 1); ++b) {   // D (+ D1_0), then D1_b alone for the rest of a batch
+    const int zh = P.nb ? 2 + 2 * b : 0, zm = P.nb ? 3 + 2 * b : 1;
+    __half* planes[8] = {h->plane(0, 0), h->plane(1, 0), h->plane(0, 1), h->plane(1, 1),
+                         h->plane(zh, 0), h->plane(zm, 0), h->plane(zh, 1), h->plane(zm, 1)};
+    sp2_launch_finalise(h->ctrl(), planes, h->cur_npad, H, in_dt, ldh, b == 0 ? D : nullptr, P.nb ? P.D1[b] : nullptr, out_dt,
+                        ldd, N, b, h->fslots(), s);
+    ++*launches;
+  }
+  sp2_launch_finalise_reduce(h->ctrl(), N, h->fslots(), h->ring() + ring_idx, s);
+  ++*launches;
   const int nref = h->opt.refine_layers;
   if (nref > 0) {   // float64 refinement layers on the converged iterate; overwrites D, tr D, tr(DH)
     __half* yp[4] = {h->plane(0, 0), h->plane(1, 0), h->plane(0, 1), h->plane(1, 1)};
@@ -399,10 +425,10 @@ int effective_max_layers(const sp2_options_t& o) {
 // enqueue one whole solve on `s`; the result struct lands in ring[ring_idx].  Only `n_layers` of the
 // max_layers layer launches are enqueued (the caller tops up if the solve turns out unfinished:
 // k_finalise_reduce then reports SP2_INTERNAL_INCOMPLETE).
-sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const void* H1, sp2_dtype_t in_dt, long ldh, int N, int N_occ,
-                           double tol, void* D, void* D1, sp2_dtype_t out_dt, long ldd, int ring_idx, cudaStream_t s,
+sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dtype_t in_dt, long ldh, int N, int N_occ,
+                           double tol, void* D, sp2_dtype_t out_dt, long ldd, int ring_idx, cudaStream_t s,
                            int n_layers, int* launches_out) {
-  const int resp = (H1 != nullptr) ? 1 : 0;
+  const int resp = P.nb;
   sp2_status_t st = prepare(h, N, resp, s);
   if (st != SP2_OK) return st;
   const int npad = h->cur_npad;
@@ -414,7 +440,10 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const void* H1, sp2_dt
   sp2_launch_init(c, N, N_occ, npad, resp, max_layers, o.user_bounds, o.eps_min, o.eps_max, tol, forced, o.forced_signs, o.no_recentre, s);
   ++launches;
   sp2_launch_bounds(H, in_dt, ldh, N, 0, h->bslots(0), s); ++launches;
-  if (resp) { sp2_launch_bounds(H1, in_dt, ldh, N, 1, h->bslots(1), s); ++launches; }
+  for (int b = 0; b < resp; ++b) {    // one slot array of sp2_bounds_blocks(N) per perturbation, contiguous (k_setup)
+    sp2_launch_bounds(P.H1[b], in_dt, ldh, N, 1, h->bslots(1) + (size_t)b * sp2_bounds_blocks(N), s);
+    ++launches;
+  }
   if (o.lanczos_steps > 0 && !o.user_bounds && N_occ > 0 && N_occ < N) {
     const int k = o.lanczos_steps < N ? o.lanczos_steps : N - 1 > 0 ? N - 1 : 1;
     sp2_launch_lanczos(c, H, in_dt, ldh, N, k, h->lanczos_vecs(), s);
@@ -422,16 +451,23 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const void* H1, sp2_dt
   }
   sp2_launch_setup(c, h->bslots(0), sp2_bounds_blocks(N), h->bslots(1), resp ? sp2_bounds_blocks(N) : 0, s); ++launches;
   if (N_occ == 0 || N_occ == N) {
-    sp2_launch_trivial(c, D, D1, out_dt, ldd, N, h->ring() + ring_idx, s); ++launches;
+    sp2_launch_trivial(c, D, resp ? P.D1[0] : nullptr, out_dt, ldd, N, h->ring() + ring_idx, s); ++launches;
+    const size_t out_sz = out_dt == SP2_F32 ? 4 : 8;
+    for (int b = 1; b < resp; ++b)
+      SP2_CUDA(h, cudaMemset2DAsync(P.D1[b], (size_t)ldd * out_sz, 0, (size_t)N * out_sz, N, s));
   } else {
-    if (resp) { sp2_launch_rescale(H1, in_dt, ldh, c, 1, h->plane(2, 0), h->plane(3, 0), npad, h->slots2(), s); ++launches; }
+    for (int b = 0; b < resp; ++b) {
+      sp2_launch_rescale(P.H1[b], in_dt, ldh, c, 1 + b, h->plane(2 + 2 * b, 0), h->plane(3 + 2 * b, 0), npad,
+                         h->slots2() + (size_t)b * sp2_rescale_blocks(npad), s);
+      ++launches;
+    }
     sp2_launch_rescale(H, in_dt, ldh, c, 0, h->plane(0, 0), h->plane(1, 0), npad, h->slots(), s); ++launches;
     sp2_launch_ctrl0(c, h->slots(), h->slots2(), sp2_rescale_blocks(npad), s); ++launches;
     if (h->time_layers) SP2_CUDA(h, cudaEventRecord(h->evl0, s));
     st = enqueue_layers(h, 0, n_layers, s, &launches);
     if (st != SP2_OK) return st;
     if (h->time_layers) SP2_CUDA(h, cudaEventRecord(h->evl1, s));
-    enqueue_finalise(h, H, in_dt, ldh, N, resp, D, D1, out_dt, ldd, ring_idx, s, &launches);
+    enqueue_finalise(h, H, in_dt, ldh, N, P, D, out_dt, ldd, ring_idx, s, &launches);
   }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
@@ -440,14 +476,17 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const void* H1, sp2_dt
   return SP2_OK;
 }
 
-sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const void* H1, sp2_dtype_t in_dt, long ldh, int N, int N_occ,
-                            double tol, void* D, void* D1, sp2_dtype_t out_dt, long ldd, sp2_result_t* out, cudaStream_t s,
-                            bool host_buffers) {
-  const int want_resp = (H1 != nullptr || D1 != nullptr) ? 1 : 0;
-  sp2_status_t st = check_args(h, H, H1, want_resp, in_dt, ldh, N, N_occ, D, D1, out_dt, ldd);
+sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dtype_t in_dt, long ldh, int N, int N_occ,
+                            double tol, void* D, sp2_dtype_t out_dt, long ldd, sp2_result_t* out, cudaStream_t s,
+                            bool host_buffers, double* tr_d1 = nullptr) {
+  const int want_resp = P.nb;
+  sp2_status_t st = check_args(h, H, P, in_dt, ldh, N, N_occ, D, out_dt, ldd);
   if (st != SP2_OK) return st;
   if (h->seq_active) return SP2_ERR_INVALID_ARG;
-  const void* dH = H; const void* dH1 = H1; void* dD = D; void* dD1 = D1;
+  if (host_buffers && P.nb > 1) return SP2_ERR_INVALID_ARG;
+  const void* H1 = P.H1[0]; void* D1 = P.D1[0];
+  Pert dP = P;                        // device-side pointers of the perturbations
+  const void* dH = H; void* dD = D; void* dD1 = D1;
   long dld_in = ldh, dld_out = ldd;
   const size_t in_sz = in_dt == SP2_F32 ? 4 : 8, out_sz = out_dt == SP2_F32 ? 4 : 8;
   // make sure the launch state is ready before the timed region starts
@@ -461,7 +500,7 @@ sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const void* H1, sp2_d
     SP2_CUDA(h, cudaMemcpy2DAsync(h->staging(0), (size_t)N * in_sz, H, (size_t)ldh * in_sz, (size_t)N * in_sz, N,
                                   cudaMemcpyHostToDevice, s));
     if (want_resp) {
-      dH1 = h->staging(2); dD1 = h->staging(3);
+      dP.H1[0] = h->staging(2); dP.D1[0] = dD1 = h->staging(3);
       SP2_CUDA(h, cudaMemcpy2DAsync(h->staging(2), (size_t)N * in_sz, H1, (size_t)ldh * in_sz, (size_t)N * in_sz, N,
                                     cudaMemcpyHostToDevice, s));
     }
@@ -475,7 +514,7 @@ sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const void* H1, sp2_d
   int n_first = max_layers;
   if (h->opt.forced_layers <= 0 && h->layers_hint > 0 && h->layers_hint < max_layers) n_first = h->layers_hint;
   h->time_layers = 1;
-  st = enqueue_solve(h, dH, dH1, in_dt, dld_in, N, N_occ, tol, dD, dD1, out_dt, dld_out, 0, s, n_first, &launches);
+  st = enqueue_solve(h, dH, dP, in_dt, dld_in, N, N_occ, tol, dD, out_dt, dld_out, 0, s, n_first, &launches);
   h->time_layers = 0;
   if (st != SP2_OK) return st;
   float layers_ms = 0.f;
@@ -488,6 +527,8 @@ sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const void* H1, sp2_d
                                       cudaMemcpyDeviceToHost, s));
     }
     SP2_CUDA(h, cudaMemcpyAsync(h->h_result, h->ring(), sizeof(sp2_result_t), cudaMemcpyDeviceToHost, s));
+    if (tr_d1)    // the pinned result ring is idle outside a sequence: entry 1.. carries tr D1_b
+      SP2_CUDA(h, cudaMemcpyAsync(h->h_result + 1, h->ctrl()->tr_d1, sizeof(double) * SP2_MAX_BATCH, cudaMemcpyDeviceToHost, s));
     SP2_CUDA(h, cudaEventRecord(h->ev1, s));
     SP2_CUDA(h, cudaStreamSynchronize(s));
     if (layers_timed) {
@@ -500,8 +541,8 @@ sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const void* H1, sp2_d
     st = enqueue_layers(h, n_first, max_layers - n_first, s, &launches);
     if (st != SP2_OK) return st;
     SP2_CUDA(h, cudaEventRecord(h->evl1, s));
-    enqueue_finalise(h, dH, in_dt, dld_in, N, want_resp, dD, dD1, out_dt, dld_out, 0, s, &launches);
-    h->launches += (unsigned long long)(max_layers - n_first + 2);
+    enqueue_finalise(h, dH, in_dt, dld_in, N, dP, dD, out_dt, dld_out, 0, s, &launches);
+    h->launches += (unsigned long long)(max_layers - n_first + 1 + (want_resp > 1 ? want_resp : 1));
   }
   float ms = 0.f;
   SP2_CUDA(h, cudaEventElapsedTime(&ms, h->ev0, h->ev1));
@@ -512,6 +553,11 @@ sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const void* H1, sp2_d
   r.layers_ms = layers_ms;
   r.kernel_launches = launches;
   if (out) *out = r;
+  if (tr_d1) {
+    const bool trivial = (N_occ == 0 || N_occ == N);
+    const double* t = reinterpret_cast<const double*>(h->h_result + 1);
+    for (int b = 0; b < P.nb; ++b) tr_d1[b] = trivial ? 0.0 : t[b];
+  }
   return (sp2_status_t)r.status;
 }
 
@@ -537,7 +583,8 @@ sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_work
   if (prop.major != 10) return SP2_ERR_ARCH;
   sp2_handle_s* h = new (std::nothrow) sp2_handle_s();
   if (!h) return SP2_ERR_INVALID_ARG;
-  h->n_max = n_max; h->flags = flags; h->device = dev; h->num_sms = prop.multiProcessorCount;
+  if (L.nb_max > 0) flags |= SP2_WITH_RESPONSE;
+  h->n_max = n_max; h->flags = flags; h->device = dev; h->num_sms = prop.multiProcessorCount; h->nb_max = L.nb_max;
   h->ws = static_cast<uint8_t*>(d_workspace); h->ws_bytes = bytes; h->L = L;
   default_options(&h->opt);
   h->cur_n = -1; h->cur_npad = -1; h->cur_cg = -1; h->cur_resp = -1; h->cur_seg = -1;
@@ -594,20 +641,33 @@ sp2_status_t sp2_get_options(sp2_handle_t h, sp2_options_t* opt) {
 
 sp2_status_t sp2_density(sp2_handle_t h, const void* dH, sp2_dtype_t in_dtype, long ldh, int N, int N_occ, double tol,
                          void* dD, sp2_dtype_t out_dtype, long ldd, sp2_result_t* out, void* stream) {
-  return blocking_solve(h, dH, nullptr, in_dtype, ldh, N, N_occ, tol, dD, nullptr, out_dtype, ldd, out,
+  return blocking_solve(h, dH, make_pert(nullptr, nullptr), in_dtype, ldh, N, N_occ, tol, dD, out_dtype, ldd, out,
                         static_cast<cudaStream_t>(stream), false);
 }
 
 sp2_status_t sp2_response(sp2_handle_t h, const void* dH, const void* dH1, sp2_dtype_t in_dtype, long ld, int N, int N_occ,
                           double tol, void* dD, void* dD1, sp2_dtype_t out_dtype, long ldo, sp2_result_t* out, void* stream) {
   if (!dH1 || !dD1) return SP2_ERR_INVALID_ARG;
-  return blocking_solve(h, dH, dH1, in_dtype, ld, N, N_occ, tol, dD, dD1, out_dtype, ldo, out,
+  return blocking_solve(h, dH, make_pert(dH1, dD1), in_dtype, ld, N, N_occ, tol, dD, out_dtype, ldo, out,
                         static_cast<cudaStream_t>(stream), false);
+}
+
+sp2_status_t sp2_response_batch(sp2_handle_t h, const void* dH, const void* const* dH1, int nb, sp2_dtype_t in_dtype, long ld,
+                                int N, int N_occ, double tol, void* dD, void* const* dD1, sp2_dtype_t out_dtype, long ldo,
+                                double* tr_d1, sp2_result_t* out, void* stream) {
+  if (!dH1 || !dD1 || nb < 1 || nb > SP2_MAX_BATCH) return SP2_ERR_INVALID_ARG;
+  Pert P;
+  memset(&P, 0, sizeof(P));
+  P.nb = nb;
+  for (int b = 0; b < nb; ++b) { P.H1[b] = dH1[b]; P.D1[b] = dD1[b]; }
+  double tr_local[SP2_MAX_BATCH];
+  return blocking_solve(h, dH, P, in_dtype, ld, N, N_occ, tol, dD, out_dtype, ldo, out, static_cast<cudaStream_t>(stream),
+                        false, tr_d1 ? tr_d1 : tr_local);
 }
 
 sp2_status_t sp2_density_host(sp2_handle_t h, const void* hH, sp2_dtype_t in_dtype, long ldh, int N, int N_occ, double tol,
                               void* hD, sp2_dtype_t out_dtype, long ldd, sp2_result_t* out, void* stream) {
-  return blocking_solve(h, hH, nullptr, in_dtype, ldh, N, N_occ, tol, hD, nullptr, out_dtype, ldd, out,
+  return blocking_solve(h, hH, make_pert(nullptr, nullptr), in_dtype, ldh, N, N_occ, tol, hD, out_dtype, ldd, out,
                         static_cast<cudaStream_t>(stream), true);
 }
 
@@ -615,7 +675,7 @@ sp2_status_t sp2_response_host(sp2_handle_t h, const void* hH, const void* hH1, 
                                int N_occ, double tol, void* hD, void* hD1, sp2_dtype_t out_dtype, long ldo,
                                sp2_result_t* out, void* stream) {
   if (!hH1 || !hD1) return SP2_ERR_INVALID_ARG;
-  return blocking_solve(h, hH, hH1, in_dtype, ld, N, N_occ, tol, hD, hD1, out_dtype, ldo, out,
+  return blocking_solve(h, hH, make_pert(hH1, hD1), in_dtype, ld, N, N_occ, tol, hD, out_dtype, ldo, out,
                         static_cast<cudaStream_t>(stream), true);
 }
 
@@ -632,9 +692,10 @@ sp2_status_t sp2_sequence_step(sp2_handle_t h, const void* dH_t, sp2_dtype_t in_
                                sp2_dtype_t out_dtype, long ldd) {
   if (!h || !h->seq_active) return SP2_ERR_INVALID_ARG;
   if (h->seq_steps >= kRingCap) return SP2_ERR_INVALID_ARG;
-  sp2_status_t st = check_args(h, dH_t, nullptr, 0, in_dtype, ldh, h->seq_N, h->seq_nocc, dD_t, nullptr, out_dtype, ldd);
+  const Pert none = make_pert(nullptr, nullptr);
+  sp2_status_t st = check_args(h, dH_t, none, in_dtype, ldh, h->seq_N, h->seq_nocc, dD_t, out_dtype, ldd);
   if (st != SP2_OK) return st;
-  st = enqueue_solve(h, dH_t, nullptr, in_dtype, ldh, h->seq_N, h->seq_nocc, h->seq_tol, dD_t, nullptr, out_dtype, ldd,
+  st = enqueue_solve(h, dH_t, none, in_dtype, ldh, h->seq_N, h->seq_nocc, h->seq_tol, dD_t, out_dtype, ldd,
                      h->seq_steps, h->seq_stream, effective_max_layers(h->opt), nullptr);
   if (st == SP2_OK) ++h->seq_steps;
   return st;
@@ -783,7 +844,7 @@ sp2_status_t sp2_debug_plane(sp2_handle_t h, int which, size_t* offset, long* pi
   const int buf = (host_ctrl.n & 1) ^ prev;
   if (offset) *offset = (size_t)(reinterpret_cast<uint8_t*>(h->plane(which, buf)) - h->ws);
   if (pitch) *pitch = host_ctrl.npad;
-  if (exponent) *exponent = which < 2 ? host_ctrl.t : host_ctrl.u;
+  if (exponent) *exponent = which < 2 ? host_ctrl.t : host_ctrl.u[0];
   if (shift) *shift = host_ctrl.c;
   return SP2_OK;
 }

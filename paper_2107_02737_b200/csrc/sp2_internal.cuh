@@ -14,6 +14,7 @@
 #define SP2_INTERNAL_INCOMPLETE 100  // ring status: the enqueued layer launches ran out before the controller stopped
 #define SP2_LAYER_CAP 128          // size of the per-layer history arrays (max_layers <= 126)
 #define SP2_FP16_TARGET_LOG2 15    // planes are scaled so that (bound on max|.|) * 2^t <= 2^15 < 65504
+#define SP2_NB SP2_MAX_BATCH       // perturbations one layer stack can carry (sp2_response_batch)
 
 struct Sp2Slot {      // one partial per producer (block / epilogue warp); reduced in index order
   double tr;          // sum of stored diagonal values (scaled units)
@@ -32,23 +33,23 @@ struct Sp2BoundSlot { // per block of the bounds kernel
 
 struct Sp2Coef {      // epilogue coefficients of the layer about to run (scaled units)
   float a1y_hi, a1y_lo, a2y;   // Y' = (a1y_hi + a1y_lo) * (Yh+Ym) + a2y * acc
-  float a1z_hi, a1z_lo, a2z;   // Z' likewise with the (YZ+ZY) accumulator
+  float a1z_hi[SP2_NB], a1z_lo[SP2_NB], a2z[SP2_NB];   // Z_b' likewise with the (Y Z_b + Z_b Y) accumulator
   float dsh_hi, dsh_lo;        // added to the diagonal of Y' (re-centring of the shift c), scaled units
 };
 
 struct Sp2Ctrl {
   // problem (written by k_init)
-  int N, n_occ, npad, with_response;
+  int N, n_occ, npad, with_response;   // with_response = number of perturbations carried (0 .. SP2_NB)
   int max_layers, user_bounds, forced_layers, no_recentre;
   unsigned long long forced_signs;
   double tol, user_eps_min, user_eps_max;
   // input layer (written by k_setup)
-  double eps_min, eps_max, delta, tr_h, maxabs_h, maxabs_h1;
+  double eps_min, eps_max, delta, tr_h, maxabs_h, maxabs_h1[SP2_NB];
   // iterate state
   double c;             // shift of the current iterate
-  int t, u;             // plane exponents of the current iterate (Y, Z)
+  int t;                // plane exponent of the current iterate Y
   int t_in;             // exponent of the Y planes the running layer READS (for the trace identity)
-  int pad2;
+  int u[SP2_NB];        // plane exponents of the current first-order iterates Z_b
   double sigma_last;    // +1 / -1: branch of the layer that is running / ran last
   double fro_in;        // ||Y||_F^2 (TRUE units) of the iterate the running layer reads
   int n;                // index of the layer about to run = number of layers applied so far
@@ -57,13 +58,14 @@ struct Sp2Ctrl {
   int stop_reason;
   unsigned int ticket;  // last-block election of the layer kernel
   int pad1;
-  double tr_y, fro_y, max_y, tr_z, fro_z, max_z;  // reduced partials of the current iterate, TRUE units
+  double tr_y, fro_y, max_y;                              // reduced partials of the current iterate, TRUE units
+  double tr_z[SP2_NB], fro_z[SP2_NB], max_z[SP2_NB];
   Sp2Coef coef;
   unsigned long long sign_mask[2];
   double tr_x[SP2_LAYER_CAP];
   double e[SP2_LAYER_CAP];
   // finalise
-  double tr_d, tr_dh, tr_d1;
+  double tr_d, tr_dh, tr_d1[SP2_NB];
   // plane exponents of the congruence products (sp2_congruence): operands A, B and the intermediate T
   int g_ea, g_eb, g_et;      // exponents the running product reads: A operand, B operand, plane output
   int g_el, g_ex, g_pad;     // exponents of the L (= Z or Z^T) planes and of the transformed matrix X
@@ -125,8 +127,9 @@ __device__ inline void sp2_controller(Sp2Ctrl* c) {
   const int n = c->n;
   const double N = (double)c->N;
   const double cc = c->c;
-  if (!isfinite(c->fro_y) || !isfinite(c->tr_y) || !isfinite(c->max_y) ||
-      (c->with_response && (!isfinite(c->fro_z) || !isfinite(c->max_z)))) {
+  bool finite = isfinite(c->fro_y) && isfinite(c->tr_y) && isfinite(c->max_y);
+  for (int b = 0; b < c->with_response; ++b) finite = finite && isfinite(c->fro_z[b]) && isfinite(c->max_z[b]);
+  if (!finite) {
     c->done = 1; c->status = SP2_ERR_NONFINITE; c->stop_reason = 0;
     return;
   }
@@ -172,13 +175,13 @@ __device__ inline void sp2_controller(Sp2Ctrl* c) {
   sp2_split_f32(alpha * sp2_exp2i(t_next - t), c->coef.a1y_hi, c->coef.a1y_lo);
   c->coef.a2y = (float)(sigma * sp2_exp2i(t_next - 2 * t));
   sp2_split_f32(dshift * sp2_exp2i(t_next), c->coef.dsh_hi, c->coef.dsh_lo);
-  if (c->with_response) {
-    const double bz = fabs(alpha) * c->max_z + 2.0 * sqrt(y2) * sqrt(c->fro_z);
+  for (int b = 0; b < c->with_response; ++b) {   // every perturbation keeps its own exponent
+    const double bz = fabs(alpha) * c->max_z[b] + 2.0 * sqrt(y2) * sqrt(c->fro_z[b]);
     const int u_next = sp2_pick_exponent(bz);
-    const int u = c->u;
-    sp2_split_f32(alpha * sp2_exp2i(u_next - u), c->coef.a1z_hi, c->coef.a1z_lo);
-    c->coef.a2z = (float)(sigma * sp2_exp2i(u_next - t - u));
-    c->u = u_next;    // exponents describe the iterate the layer WRITES; the layer itself only
+    const int u = c->u[b];
+    sp2_split_f32(alpha * sp2_exp2i(u_next - u), c->coef.a1z_hi[b], c->coef.a1z_lo[b]);
+    c->coef.a2z[b] = (float)(sigma * sp2_exp2i(u_next - t - u));
+    c->u[b] = u_next; // exponents describe the iterate the layer WRITES; the layer itself only
   }                   // needs coef, so they can be advanced here
   c->t_in = t;
   c->sigma_last = sigma;

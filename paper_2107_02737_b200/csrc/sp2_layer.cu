@@ -218,7 +218,8 @@ __device__ __forceinline__ uint32_t u4_word(const uint4& v, int i) {
 
 // ----------------------------------------------------------------------------------------------
 // shared tail of both engines: last block reduces the slots (index order) and runs the controller
-__device__ inline void layer_tail(Sp2Ctrl* ctrl, const Sp2Slot* slots, int n_y, int n_z, int y_first,
+// slot array: [z slots of perturbation 0 (n_z)] ... [z slots of perturbation nb - 1][y slots (n_y)]
+__device__ inline void layer_tail(Sp2Ctrl* ctrl, const Sp2Slot* slots, int n_y, int n_z, int nb,
                                   unsigned int n_blocks, uint32_t* is_last_smem, double* red,
                                   unsigned int* flags = nullptr, int n_flags = 0) {
   __syncthreads();
@@ -231,15 +232,20 @@ __device__ inline void layer_tail(Sp2Ctrl* ctrl, const Sp2Slot* slots, int n_y, 
   if (!*is_last_smem) return;
   __threadfence();
   for (int i = threadIdx.x; i < n_flags; i += blockDim.x) flags[i] = 0u;   // every split unit was consumed
-  double tr, fro, mx, tracc, trz = 0.0, froz = 0.0, mxz = 0.0, unused;
-  // slot array: [z slots (n_z)][y slots (n_y)] when y_first == n_z
-  sp2_reduce_slots(slots + y_first, n_y, red, tr, fro, mx, tracc);
-  if (n_z > 0) sp2_reduce_slots(slots, n_z, red, trz, froz, mxz, unused);
+  double tr, fro, mx, tracc, unused;
+  sp2_reduce_slots(slots + (size_t)nb * n_z, n_y, red, tr, fro, mx, tracc);
+  for (int b = 0; b < nb; ++b) {
+    double trz, froz, mxz;
+    sp2_reduce_slots(slots + (size_t)b * n_z, n_z, red, trz, froz, mxz, unused);
+    if (threadIdx.x == 0) {
+      const double sz = sp2_exp2i(-ctrl->u[b]);
+      ctrl->tr_z[b] = trz * sz; ctrl->fro_z[b] = froz * sz * sz; ctrl->max_z[b] = mxz * sz;
+    }
+  }
   if (threadIdx.x == 0) {
     sp2_trace_identity(ctrl, tracc);
-    const double sy = sp2_exp2i(-ctrl->t), sz = sp2_exp2i(-ctrl->u);
+    const double sy = sp2_exp2i(-ctrl->t);
     ctrl->tr_y = tr * sy; ctrl->fro_y = fro * sy * sy; ctrl->max_y = mx * sy;
-    ctrl->tr_z = trz * sz; ctrl->fro_z = froz * sz * sz; ctrl->max_z = mxz * sz;
     ctrl->ticket = 0;
     sp2_controller(ctrl);
   }
@@ -453,9 +459,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   const int KB = a.npad / kBK;            // ring stages per k sweep
   const int seg_kb = a.seg_kb * (64 / kBK);   // ring stages per TMEM accumulation segment (divides KB)
   const int item_lo = a.item_begin[cluster_id], item_hi = a.item_begin[cluster_id + 1];
+  const int nz_units = MODE == 1 ? 0 : a.with_response * n_tiles;   // units [0, nz_units): first-order, then the Y^2 units
 
   if (warp == kWarpTma && lane == 0) {
-    for (int i = 0; i < 4; ++i) asm volatile("prefetch.tensormap [%0];" ::"l"(&a.tm[i]) : "memory");
+    const int n_maps = MODE == 1 ? 4 : 2 + 2 * a.with_response;
+    for (int i = 0; i < n_maps; ++i) asm volatile("prefetch.tensormap [%0];" ::"l"(&a.tm[i]) : "memory");
   }
   if (warp == kWarpMma && lane == 0) {
     for (int s = 0; s < kStages; ++s) { mbar_init(smem_u32(&bars->full[s]), 1); mbar_init(smem_u32(&bars->empty[s]), 1); }
@@ -487,8 +495,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
         for (int iti = item_lo; iti < item_hi; ++iti) {
           const Sp2Item I = a.items[iti];
           const int u = I.unit;
-          const bool wunit = a.with_response && u < n_tiles;
-          const int2 tij = a.tiles[wunit ? u : (a.with_response ? u - n_tiles : u)];
+          const bool wunit = u < nz_units;           // Y Z_b + Z_b Y unit of perturbation b = u / n_tiles
+          const int zb = wunit ? u / n_tiles : 0;
+          const int2 tij = a.tiles[wunit ? u - zb * n_tiles : u - nz_units];
+          const int zpl = 2 + 2 * zb;                // planes of Z_b
           const int row_a = tij.x * TILE + (int)rank * kRows;
           const int row_b = tij.y * TILE + (int)rank * kRows;
           {
@@ -496,8 +506,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
               // Y^2: A = (Yh, Ym), B = (Yh, Ym).  W pass 0: A = (Yh, Ym), B = (Zh, Zm).  W pass 1: A = (Zh, Zm), B = (Yh, Ym).
               const int p = (g >= KB) ? 1 : 0;
               const int kb = g - p * KB;
-              const int ma = (wunit && p == 1) ? 2 : 0;
-              const int mb = (MODE == 1 || (wunit && p == 0)) ? 2 : 0;
+              const int ma = (wunit && p == 1) ? zpl : 0;
+              const int mb = (MODE == 1 || (wunit && p == 0)) ? zpl : 0;
               mbar_wait(smem_u32(&bars->empty[stage]), phase ^ 1u);
               const uint32_t dst = smem_u32(smem + stage * kStageBytes);
               if (CG == 1 || leader) mbar_expect_tx(smem_u32(&bars->full[stage]), (uint32_t)(CG * kStageBytes));
@@ -560,7 +570,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
     const int cw = warp;
     const int q = warp & 3;                       // TMEM lane quarter this warp may read
     const int hh = cw >> 2;                       // which half of the accumulator columns
-    const Sp2Coef cf = a.ctrl->coef;
+    const float cf_a1y_hi = a.ctrl->coef.a1y_hi, cf_a1y_lo = a.ctrl->coef.a1y_lo, cf_a2y = a.ctrl->coef.a2y;
+    const float cf_dsh_hi = a.ctrl->coef.dsh_hi, cf_dsh_lo = a.ctrl->coef.dsh_lo;
     const double gemm_scale = MODE == 1 ? sp2_exp2i((a.out_kind == 0 ? a.ctrl->g_et : 0) - a.ctrl->g_ea - a.ctrl->g_eb) : 0.0;
     // optional power saving: round the lo plane to lo_bits significant bits (fewer toggling multiplier inputs)
     const int drop = 11 - a.lo_bits;
@@ -570,10 +581,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
     for (int iti = item_lo; iti < item_hi; ++iti) {
       const Sp2Item I = a.items[iti];
       const int u = I.unit;
-      const bool wunit = a.with_response && u < n_tiles;
-      const int2 tij = a.tiles[wunit ? u : (a.with_response ? u - n_tiles : u)];
+      const bool wunit = u < nz_units;
+      const int zb = wunit ? u / n_tiles : 0;
+      const int2 tij = a.tiles[wunit ? u - zb * n_tiles : u - nz_units];
       float sums[WCOLS];
-      const int pl = wunit ? 2 : 0;
+      const int pl = wunit ? 2 + 2 * zb : 0;
       const int gi = tij.x * TILE + (int)rank * kRows + q * 32 + lane;   // global row of this thread
       const int j0 = tij.y * TILE + hh * WCOLS;
       EpiOld old;
@@ -640,10 +652,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
         continue;
       }
       // ---- fused epilogue from the register sums
-      const float a1hi = wunit ? cf.a1z_hi : cf.a1y_hi, a1lo = wunit ? cf.a1z_lo : cf.a1y_lo;
-      const float a2 = wunit ? cf.a2z : cf.a2y;
+      const Sp2Coef* cz = &a.ctrl->coef;
+      const float a1hi = wunit ? cz->a1z_hi[zb] : cf_a1y_hi, a1lo = wunit ? cz->a1z_lo[zb] : cf_a1y_lo;
+      const float a2 = wunit ? cz->a2z[zb] : cf_a2y;
       const bool shift_row = !wunit && gi < a.n;        // zero padding stays zero
-      const float dsh_hi = shift_row ? cf.dsh_hi : 0.f, dsh_lo = shift_row ? cf.dsh_lo : 0.f;
+      const float dsh_hi = shift_row ? cf_dsh_hi : 0.f, dsh_lo = shift_row ? cf_dsh_lo : 0.f;
       EpiPartials P; P.tr = 0.0; P.fro = 0.0; P.tracc = 0.0; P.mx = 0.f;
       if (a.debug_flags & 1) {
         float t = 0.f;
@@ -689,8 +702,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   }
 
   const int per_unit = CG * kConsumerWarps;
-  const int n_z = a.with_response ? n_tiles * per_unit : 0;
-  layer_tail(a.ctrl, a.slots, n_tiles * per_unit, n_z, n_z, gridDim.x, &bars->is_last, red, a.flags, a.n_flags);
+  layer_tail(a.ctrl, a.slots, n_tiles * per_unit, n_tiles * per_unit, a.with_response, gridDim.x, &bars->is_last, red,
+             a.flags, a.n_flags);
 }
 
 // ----------------------------------------------------------------------------------------------
@@ -704,7 +717,7 @@ __global__ void __launch_bounds__(256) k_layer_simt(Sp2LayerArgs a) {
   __shared__ float rm[8];
   const int nb = a.npad / 16;
   const int n_blk_tri = nb * (nb + 1) / 2;
-  const int cls = blockIdx.y;                  // 0: Y^2, 1: YZ + ZY
+  const int cls = blockIdx.y;                  // 0: Y^2, 1 + b: Y Z_b + Z_b Y
   int bi = 0, rem = blockIdx.x;
   while (rem >= nb - bi) { rem -= nb - bi; ++bi; }
   const int bj = bi + rem;
@@ -712,7 +725,7 @@ __global__ void __launch_bounds__(256) k_layer_simt(Sp2LayerArgs a) {
   const int gi = bi * 16 + r, gj = bj * 16 + cidx;
   const size_t npad = (size_t)a.npad;
   const __half* Yh = a.in[0]; const __half* Ym = a.in[1];
-  const __half* Zh = a.in[2]; const __half* Zm = a.in[3];
+  const __half* Zh = a.in[2 * cls]; const __half* Zm = a.in[2 * cls + 1];
   float acc = 0.f;
   if (cls == 0) {
     for (int k = 0; k < a.npad; ++k) {
@@ -730,9 +743,10 @@ __global__ void __launch_bounds__(256) k_layer_simt(Sp2LayerArgs a) {
       acc = fmaf(pi_, hj, acc); acc = fmaf(pi_, mj, acc); acc = fmaf(qi, hj, acc);
     }
   }
-  const Sp2Coef cf = a.ctrl->coef;
-  const int pl = cls ? 2 : 0;
-  const float a1hi = cls ? cf.a1z_hi : cf.a1y_hi, a1lo = cls ? cf.a1z_lo : cf.a1y_lo, a2 = cls ? cf.a2z : cf.a2y;
+  const Sp2Coef& cf = a.ctrl->coef;
+  const int pl = 2 * cls;
+  const int zb = cls ? cls - 1 : 0;
+  const float a1hi = cls ? cf.a1z_hi[zb] : cf.a1y_hi, a1lo = cls ? cf.a1z_lo[zb] : cf.a1y_lo, a2 = cls ? cf.a2z[zb] : cf.a2y;
   double tr = 0.0, fro = 0.0, tracc = 0.0;
   float mx = 0.f;
   if (gj >= gi) {
@@ -760,12 +774,10 @@ __global__ void __launch_bounds__(256) k_layer_simt(Sp2LayerArgs a) {
   if (threadIdx.x == 0) {
     Sp2Slot s; s.tr = 0; s.fro = 0; s.tracc = 0; s.mx = 0.f; s.pad = 0.f;
     for (int w = 0; w < 8; ++w) { s.tr += rs[0][w]; s.fro += rs[1][w]; s.tracc += rs[2][w]; s.mx = (rm[w] > s.mx || rm[w] != rm[w]) ? rm[w] : s.mx; }
-    // layout [z slots][y slots]
-    const int n_z = a.with_response ? n_blk_tri : 0;
-    a.slots[(cls ? 0 : n_z) + blockIdx.x] = s;
+    // layout [z slots of perturbation 0] ... [z slots of perturbation nb - 1][y slots]
+    a.slots[(size_t)(cls ? cls - 1 : a.with_response) * n_blk_tri + blockIdx.x] = s;
   }
-  const int n_z = a.with_response ? n_blk_tri : 0;
-  layer_tail(a.ctrl, a.slots, n_blk_tri, n_z, n_z, gridDim.x * gridDim.y, &is_last, red);
+  layer_tail(a.ctrl, a.slots, n_blk_tri, n_blk_tri, a.with_response, gridDim.x * gridDim.y, &is_last, red);
 }
 
 }  // namespace
@@ -778,10 +790,10 @@ size_t sp2_layer_smem_bytes() { return (size_t)kStages * kStageBytes + sizeof(Sm
 int sp2_layer_slots(int npad, int cta_group, int with_response, int engine) {
   if (engine == SP2_ENGINE_SIMT_DEBUG) {
     const int nb = npad / 16;
-    return nb * (nb + 1) / 2 * (with_response ? 2 : 1);
+    return nb * (nb + 1) / 2 * (1 + with_response);
   }
   const int nt = npad / (128 * cta_group);
-  return nt * (nt + 1) / 2 * cta_group * kConsumerWarps * (with_response ? 2 : 1);
+  return nt * (nt + 1) / 2 * cta_group * kConsumerWarps * (1 + with_response);
 }
 
 cudaError_t sp2_layer_configure() {
@@ -800,7 +812,7 @@ size_t sp2_layer_scratch_slot_bytes(int cta_group) {
 cudaError_t sp2_launch_layer(const Sp2LayerArgs& args, int engine, int cta_group, cudaStream_t s) {
   if (engine == SP2_ENGINE_SIMT_DEBUG) {
     const int nb = args.npad / 16;
-    dim3 grid(nb * (nb + 1) / 2, args.with_response ? 2 : 1);
+    dim3 grid(nb * (nb + 1) / 2, 1 + args.with_response);
     k_layer_simt<<<grid, 256, 0, s>>>(args);
     return cudaGetLastError();
   }

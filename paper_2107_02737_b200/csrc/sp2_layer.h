@@ -15,14 +15,15 @@ struct Sp2Item {
   int slot, nparts, flag_id, pad;
 };
 
-// Arguments of one layer launch.  tm[] are TMA descriptors of the INPUT planes (Yh, Ym, Zh, Zm):
-// 2-D FP16 tensors npad x npad, box sp2_layer_box_k() (k) x 128 (rows), swizzle = box row bytes.
+// Arguments of one layer launch.  tm[] are TMA descriptors of the INPUT planes (Yh, Ym, then Zh, Zm of every
+// perturbation b at 2 + 2b): 2-D FP16 tensors npad x npad, box sp2_layer_box_k() (k) x 128 (rows), swizzle = box row bytes.
+#define SP2_LAYER_PLANES (2 + 2 * SP2_NB)
 struct alignas(64) Sp2LayerArgs {
-  CUtensorMap tm[4];
-  const __half* in[4];   // the same input planes as raw pointers (epilogue reads the old tile)
-  __half* out[4];        // output planes Yh', Ym', Zh', Zm' (the other ping-pong buffer)
+  CUtensorMap tm[SP2_LAYER_PLANES];
+  const __half* in[SP2_LAYER_PLANES];   // the same input planes as raw pointers (epilogue reads the old tile)
+  __half* out[SP2_LAYER_PLANES];        // output planes Yh', Ym', Zh', Zm', ... (the other ping-pong buffer)
   Sp2Ctrl* ctrl;
-  Sp2Slot* slots;        // [z-class slots][y-class slots]
+  Sp2Slot* slots;        // [z slots of perturbation 0] ... [z slots of perturbation nb - 1][y slots]
   const int2* tiles;     // (ti, tj), ti <= tj, upper-triangular tile list in L2-friendly order
   const Sp2Item* items;  // work lists of all CTA(-pair)s, concatenated
   const int* item_begin; // [n_clusters + 1] offsets into items
@@ -41,7 +42,7 @@ struct alignas(64) Sp2LayerArgs {
   int n;                 // true dimension (rows/cols >= n are zero padding and stay zero)
   int npad;              // padded dimension (multiple of the tile edge)
   int n_tiles;           // number of upper-triangular tiles
-  int with_response;
+  int with_response;     // number of perturbations carried (0 .. SP2_NB)
   int seg_kb;            // k-blocks (of 64) per in-TMEM accumulation segment; divides npad/64
 };
 

@@ -92,12 +92,19 @@ __global__ void __launch_bounds__(256) k_setup(Sp2Ctrl* c, const Sp2BoundSlot* s
                                                const Sp2BoundSlot* s1_slots, int n_h1) {
   __shared__ double red[5][256];
   const int tid = threadIdx.x;
-  double lo = INFINITY, hi = -INFINITY, tr = 0.0, mx = 0.0, sum = 0.0, mx1 = 0.0, sum1 = 0.0;
+  double lo = INFINITY, hi = -INFINITY, tr = 0.0, mx = 0.0, sum = 0.0, sum1 = 0.0;
   for (int i = tid; i < n_h; i += 256) {
     lo = fmin(lo, sh_slots[i].lo); hi = fmax(hi, sh_slots[i].hi);
     tr += sh_slots[i].tr; mx = fmax(mx, sh_slots[i].mx); sum += sh_slots[i].sum;
   }
-  for (int i = tid; i < n_h1; i += 256) { mx1 = fmax(mx1, s1_slots[i].mx); sum1 += s1_slots[i].sum; }
+  const int nb = n_h1 > 0 ? c->with_response : 0;     // s1_slots = nb arrays of n_h1 slots, one per perturbation
+  double mx1[SP2_NB];
+  for (int b = 0; b < SP2_NB; ++b) mx1[b] = 0.0;
+  for (int b = 0; b < nb; ++b)
+    for (int i = tid; i < n_h1; i += 256) {
+      mx1[b] = fmax(mx1[b], s1_slots[(size_t)b * n_h1 + i].mx);
+      sum1 += s1_slots[(size_t)b * n_h1 + i].sum;
+    }
   red[0][tid] = lo; red[1][tid] = hi; red[2][tid] = tr; red[3][tid] = fmax(mx, 0.0); red[4][tid] = sum + sum1;
   __syncthreads();
   for (int w = 128; w > 0; w >>= 1) {
@@ -111,16 +118,19 @@ __global__ void __launch_bounds__(256) k_setup(Sp2Ctrl* c, const Sp2BoundSlot* s
     __syncthreads();
   }
   __shared__ double red1[256];
-  red1[tid] = mx1;
-  __syncthreads();
-  for (int w = 128; w > 0; w >>= 1) {
-    if (tid < w) red1[tid] = fmax(red1[tid], red1[tid + w]);
+  for (int b = 0; b < nb; ++b) {
+    red1[tid] = mx1[b];
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+      if (tid < w) red1[tid] = fmax(red1[tid], red1[tid + w]);
+      __syncthreads();
+    }
+    if (tid == 0) c->maxabs_h1[b] = red1[0];
     __syncthreads();
   }
   if (tid != 0) return;
   c->tr_h = red[2][0];
   c->maxabs_h = red[3][0];
-  c->maxabs_h1 = red1[0];
   double eps_min = red[0][0], eps_max = red[1][0];
   if (c->lanczos_steps > 0 && isfinite(c->lz_min) && isfinite(c->lz_max) && c->lz_max > c->lz_min) {
     // tighter bounds from k Lanczos steps, never wider than the Gershgorin discs
@@ -140,13 +150,13 @@ __global__ void __launch_bounds__(256) k_setup(Sp2Ctrl* c, const Sp2BoundSlot* s
   c->c = (eps_max - c->tr_h / N) / delta;
   // |Y0_ij| <= (max|H| + |tr H|/N) / Delta
   c->t = sp2_pick_exponent((c->maxabs_h + fabs(c->tr_h) / N) / delta);
-  c->u = sp2_pick_exponent(c->maxabs_h1 / delta);
+  for (int b = 0; b < nb; ++b) c->u[b] = sp2_pick_exponent(c->maxabs_h1[b] / delta);
 }
 
 // ------------------------------------------------------------------------------------------
 // a2: 32x32 tile pairs (bi <= bj).  Each block reads H tile (bi,bj) and (bj,bi), forms the
 // symmetrised value, and writes both mirror images of the hi/lo planes with coalesced rows, so
-// the planes are bit-symmetric by construction.  which = 0: Y from H, 1: Z from H1.
+// the planes are bit-symmetric by construction.  which = 0: Y from H, 1 + b: Z_b from H1_b.
 // Pads (rows/cols >= N up to npad) are written as zero.
 template <typename T>
 __global__ void __launch_bounds__(256) k_rescale(const T* __restrict__ H, long ld, const Sp2Ctrl* __restrict__ c,
@@ -175,7 +185,7 @@ __global__ void __launch_bounds__(256) k_rescale(const T* __restrict__ H, long l
   __syncthreads();
   const double inv_delta = 1.0 / c->delta;
   const double shift = which == 0 ? c->tr_h / (double)N : 0.0;   // Y0_ii = (tr H/N - H_ii)/Delta
-  const double scale = sp2_exp2i(which == 0 ? c->t : c->u);
+  const double scale = sp2_exp2i(which == 0 ? c->t : c->u[which - 1]);
   double tr = 0.0, fro = 0.0;
   float mx = 0.f;
   for (int r = ty; r < 32; r += 8) {
@@ -241,18 +251,24 @@ __global__ void __launch_bounds__(256) k_ctrl0(Sp2Ctrl* c, const Sp2Slot* ys, co
   __shared__ double red[4 * 256];
   double tr, fro, mx, unused;
   sp2_reduce_slots(ys, count, red, tr, fro, mx, unused);
-  double trz = 0.0, froz = 0.0, mxz = 0.0;
-  if (c->with_response) sp2_reduce_slots(zs, count, red, trz, froz, mxz, unused);
+  for (int b = 0; b < c->with_response; ++b) {       // zs = one slot array of `count` per perturbation
+    double trz, froz, mxz;
+    sp2_reduce_slots(zs + (size_t)b * count, count, red, trz, froz, mxz, unused);
+    if (threadIdx.x == 0) {
+      const double sz = sp2_exp2i(-c->u[b]);
+      c->tr_z[b] = trz * sz; c->fro_z[b] = froz * sz * sz; c->max_z[b] = mxz * sz;
+    }
+  }
   if (threadIdx.x != 0) return;
-  const double sy = sp2_exp2i(-c->t), sz = sp2_exp2i(-c->u);
+  const double sy = sp2_exp2i(-c->t);
   c->tr_y = tr * sy; c->fro_y = fro * sy * sy; c->max_y = mx * sy;
-  c->tr_z = trz * sz; c->fro_z = froz * sz * sz; c->max_z = mxz * sz;
   sp2_controller(c);
 }
 
 // ------------------------------------------------------------------------------------------
 // a6: D = c I + (Yh+Ym) 2^-t, D1 = (Zh+Zm) 2^-u;  tr D, tr(DH), tr D1.  One warp per row.
-// The final iterate lives in buffer (layers & 1); both candidates are passed.
+// The final iterate lives in buffer (layers & 1); both candidates are passed.  Batched response: one launch
+// per perturbation zb with that perturbation's planes; launches zb > 0 pass D = nullptr and only write D1_zb.
 template <typename TI, typename TO>
 __global__ void __launch_bounds__(256) k_finalise(const Sp2Ctrl* __restrict__ c,
                                                   const __half* __restrict__ Yh0, const __half* __restrict__ Ym0,
@@ -260,7 +276,7 @@ __global__ void __launch_bounds__(256) k_finalise(const Sp2Ctrl* __restrict__ c,
                                                   const __half* __restrict__ Zh0, const __half* __restrict__ Zm0,
                                                   const __half* __restrict__ Zh1, const __half* __restrict__ Zm1,
                                                   int npad, const TI* __restrict__ H, long ldh,
-                                                  TO* __restrict__ D, TO* __restrict__ D1, long ldo,
+                                                  TO* __restrict__ D, TO* __restrict__ D1, long ldo, int zb,
                                                   double* __restrict__ slots /* 3 per block */) {
   const int st = c->status;
   if (!c->done || (st != SP2_OK && st != SP2_WARN_NOT_CONVERGED)) return;
@@ -271,7 +287,7 @@ __global__ void __launch_bounds__(256) k_finalise(const Sp2Ctrl* __restrict__ c,
   const __half* Zh = par ? Zh1 : Zh0;
   const __half* Zm = par ? Zm1 : Zm0;
   const bool resp = c->with_response && D1 != nullptr;
-  const double sy = sp2_exp2i(-c->t), sz = sp2_exp2i(-c->u), shift = c->c;
+  const double sy = sp2_exp2i(-c->t), sz = sp2_exp2i(-c->u[zb]), shift = c->c;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int row = blockIdx.x * 8 + warp;
   double trd = 0.0, trdh = 0.0, trd1 = 0.0;
@@ -281,22 +297,24 @@ __global__ void __launch_bounds__(256) k_finalise(const Sp2Ctrl* __restrict__ c,
     const __half2* zh = reinterpret_cast<const __half2*>(Zh + (size_t)row * npad);
     const __half2* zm = reinterpret_cast<const __half2*>(Zm + (size_t)row * npad);
     const TI* h = H + (size_t)row * ldh;
-    TO* d = D + (size_t)row * ldo;
+    TO* d = D ? D + (size_t)row * ldo : nullptr;
     TO* d1 = resp ? D1 + (size_t)row * ldo : nullptr;
     for (int j2 = lane; 2 * j2 < N; j2 += 32) {
-      const float2 a = __half22float2(yh[j2]);
-      const float2 b = __half22float2(ym[j2]);
+      float2 a = make_float2(0.f, 0.f), b = a;
+      if (d) { a = __half22float2(yh[j2]); b = __half22float2(ym[j2]); }
       float2 p = make_float2(0.f, 0.f), q = p;
       if (resp) { p = __half22float2(zh[j2]); q = __half22float2(zm[j2]); }
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
         const int j = 2 * j2 + e;
         if (j >= N) break;
-        const double y = (double)((e ? a.y : a.x) + (e ? b.y : b.x)) * sy;
-        const double x = y + (j == row ? shift : 0.0);
-        d[j] = (TO)x;
-        trdh += x * (double)__ldg(h + j);
-        if (j == row) trd += x;
+        if (d) {
+          const double y = (double)((e ? a.y : a.x) + (e ? b.y : b.x)) * sy;
+          const double x = y + (j == row ? shift : 0.0);
+          d[j] = (TO)x;
+          trdh += x * (double)__ldg(h + j);
+          if (j == row) trd += x;
+        }
         if (resp) {
           const double z = (double)((e ? p.y : p.x) + (e ? q.y : q.x)) * sz;
           d1[j] = (TO)z;
@@ -331,12 +349,23 @@ __global__ void __launch_bounds__(256) k_finalise_reduce(Sp2Ctrl* c, const doubl
     if (tid < w) { red[0][tid] += red[0][tid + w]; red[1][tid] += red[1][tid + w]; red[2][tid] += red[2][tid + w]; }
     __syncthreads();
   }
+  // perturbations b > 0 of a batched response: their finalise launches left tr D1_b in slot arrays b * count ..
+  for (int bb = 1; bb < c->with_response; ++bb) {
+    __shared__ double redb[256];
+    double eb = 0.0;
+    if (ok) for (int i = tid; i < count; i += 256) eb += slots[3 * ((size_t)bb * count + i) + 2];
+    redb[tid] = eb;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) { if (tid < w) redb[tid] += redb[tid + w]; __syncthreads(); }
+    if (tid == 0) c->tr_d1[bb] = redb[0];
+    __syncthreads();
+  }
   if (tid != 0) return;
-  c->tr_d = red[0][0]; c->tr_dh = red[1][0]; c->tr_d1 = red[2][0];
+  c->tr_d = red[0][0]; c->tr_dh = red[1][0]; c->tr_d1[0] = red[2][0];
   sp2_result_t r;
   r.status = st; r.layers = c->n; r.sign_mask[0] = c->sign_mask[0]; r.sign_mask[1] = c->sign_mask[1];
   r.stop_reason = c->stop_reason; r.reserved = 0;
-  r.tr_d = c->tr_d; r.tr_dh = c->tr_dh; r.tr_d1 = c->tr_d1;
+  r.tr_d = c->tr_d; r.tr_dh = c->tr_dh; r.tr_d1 = c->tr_d1[0];
   r.idem_est = ok ? c->e[c->n] : 0.0;
   r.eps_min = c->eps_min; r.eps_max = c->eps_max; r.gpu_ms = 0.f; r.layers_ms = 0.f; r.kernel_launches = 0; r.reserved2 = 0;
   *ring_entry = r;
@@ -575,19 +604,24 @@ void sp2_launch_ctrl0(Sp2Ctrl* c, const Sp2Slot* ys, const Sp2Slot* zs, int coun
 
 int sp2_finalise_blocks(int N) { return (N + 7) / 8; }
 
+// One launch for D (+ D1 of perturbation zb = 0, or none), or for D1_zb alone (D = nullptr, zb > 0).  planes[0..3] =
+// Yh, Ym of buffers 0, 1; planes[4..7] = Zh, Zm of perturbation zb, buffers 0, 1.  slots: 3 * blocks doubles per zb.
 void sp2_launch_finalise(Sp2Ctrl* c, __half* const planes[8], int npad, const void* H, sp2_dtype_t in_dt, long ldh,
-                         void* D, void* D1, sp2_dtype_t out_dt, long ldo, int N, double* slots,
-                         sp2_result_t* ring_entry, cudaStream_t s) {
+                         void* D, void* D1, sp2_dtype_t out_dt, long ldo, int N, int zb, double* slots, cudaStream_t s) {
   const int grid = sp2_finalise_blocks(N);
+  double* sl = slots + 3 * (size_t)grid * zb;
 #define SP2_FIN(TI, TO)                                                                                     \
   k_finalise<TI, TO><<<grid, 256, 0, s>>>(c, planes[0], planes[1], planes[2], planes[3], planes[4], planes[5], \
-                                          planes[6], planes[7], npad, (const TI*)H, ldh, (TO*)D, (TO*)D1, ldo, slots)
+                                          planes[6], planes[7], npad, (const TI*)H, ldh, (TO*)D, (TO*)D1, ldo, zb, sl)
   if (in_dt == SP2_F32 && out_dt == SP2_F32) SP2_FIN(float, float);
   else if (in_dt == SP2_F32 && out_dt == SP2_F64) SP2_FIN(float, double);
   else if (in_dt == SP2_F64 && out_dt == SP2_F32) SP2_FIN(double, float);
   else SP2_FIN(double, double);
 #undef SP2_FIN
-  k_finalise_reduce<<<1, 256, 0, s>>>(c, slots, grid, ring_entry);
+}
+
+void sp2_launch_finalise_reduce(Sp2Ctrl* c, int N, double* slots, sp2_result_t* ring_entry, cudaStream_t s) {
+  k_finalise_reduce<<<1, 256, 0, s>>>(c, slots, sp2_finalise_blocks(N), ring_entry);
 }
 
 void sp2_launch_trivial(Sp2Ctrl* c, void* D, void* D1, sp2_dtype_t out_dt, long ldo, int N,

@@ -30,11 +30,17 @@ SP2_WARN_NOT_CONVERGED = 7
 
 SP2_F32, SP2_F64 = 0, 1
 SP2_WITH_RESPONSE, SP2_WITH_HOST_STAGING, SP2_WITH_REFINEMENT = 1, 2, 4
+SP2_MAX_BATCH = 8
+
+
+def SP2_WITH_BATCH(nb: int) -> int:
+    return (int(nb) & 15) << 8
+
 SP2_ENGINE_TCGEN05, SP2_ENGINE_SIMT_DEBUG = 0, 1
 
 EXPORTS = [
     "sp2_workspace_bytes", "sp2_create", "sp2_destroy", "sp2_set_options", "sp2_get_options",
-    "sp2_density", "sp2_response", "sp2_density_host", "sp2_response_host",
+    "sp2_density", "sp2_response", "sp2_response_batch", "sp2_density_host", "sp2_response_host",
     "sp2_sequence_begin", "sp2_sequence_step", "sp2_sequence_end", "sp2_congruence",
     "sp2_status_string", "sp2_last_cuda_error", "sp2_launch_count",
     "sp2_debug_history", "sp2_debug_plane", "sp2_debug_schedule",
@@ -100,6 +106,9 @@ def _load():
         f = getattr(lib, name)
         f.restype = i
         f.argtypes = args
+    lib.sp2_response_batch.restype = i
+    lib.sp2_response_batch.argtypes = [vp, vp, C.POINTER(vp), i, i, l, i, i, d, vp, C.POINTER(vp), i, l, C.POINTER(d),
+                                       C.POINTER(Sp2Result), vp]
     lib.sp2_sequence_begin.restype = i
     lib.sp2_sequence_begin.argtypes = [vp, i, i, d, i, vp]
     lib.sp2_sequence_step.restype = i
@@ -128,7 +137,7 @@ lib = _load()
 
 def debug_schedule(n_tiles: int, with_response: bool, segs_per_pass: int, n_clusters: int):
     """Host-only: work lists of the layer kernel -> list (per cluster) of dicts."""
-    cap = 2 * n_tiles * 2 + 4 * n_clusters + 16
+    cap = (1 + int(with_response)) * n_tiles * 2 + 4 * n_clusters + 16   # with_response: bool or perturbation count
     buf = (C.c_int * (8 * cap))()
     begin = (C.c_int * (n_clusters + 1))()
     cnt = lib.sp2_debug_schedule(n_tiles, int(with_response), segs_per_pass, n_clusters, buf, cap, begin)
@@ -169,14 +178,14 @@ class Sp2Handle:
     """sp2_create / sp2_destroy over a torch-owned workspace on the current CUDA device."""
 
     def __init__(self, n_max: int, response: bool = False, host_staging: bool = False, device=None,
-                 refinement: bool = False):
+                 refinement: bool = False, batch: int = 0):
         import torch
 
         if not torch.cuda.is_available():
             raise RuntimeError("sp2-b200 needs a CUDA device (sm_100); there is no CPU fallback")
         self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
         self.flags = ((SP2_WITH_RESPONSE if response else 0) | (SP2_WITH_HOST_STAGING if host_staging else 0)
-                      | (SP2_WITH_REFINEMENT if refinement else 0))
+                      | (SP2_WITH_REFINEMENT if refinement else 0) | (SP2_WITH_BATCH(batch) if batch else 0))
         self.n_max = int(n_max)
         nbytes = workspace_bytes(self.n_max, self.flags)
         with torch.cuda.device(self.device):
@@ -280,6 +289,34 @@ class Sp2Handle:
                               _dtype_code(out), out.stride(0), C.byref(r), self._stream())
         self._raise(st)
         return out, out1, r.as_dict()
+
+    def response_batch(self, H, H1s, n_occ: int, tol: float = 0.0, out=None, out1s=None, out_dtype=None):
+        """sp2_response_batch: (H, [H1_b]) -> (D, [D1_b], [tr D1_b], result dict); one stack of layers for all b."""
+        import torch
+
+        n = H.shape[0]
+        nb = len(H1s)
+        self._check_dev(H, n)
+        for H1 in H1s:
+            self._check_dev(H1, n)
+            if H1.dtype != H.dtype or H1.stride(0) != H.stride(0):
+                raise ValueError("every H1 must have the dtype and pitch of H")
+        if out is None:
+            out = torch.empty((n, n), dtype=out_dtype or H.dtype, device=H.device)
+        if out1s is None:
+            out1s = [torch.empty_like(out) for _ in range(nb)]
+        for o in out1s:
+            if o.dtype != out.dtype or o.stride(0) != out.stride(0):
+                raise ValueError("every D1 must have the dtype and pitch of D")
+        pin = (C.c_void_p * max(nb, 1))(*[H1.data_ptr() for H1 in H1s])
+        pout = (C.c_void_p * max(nb, 1))(*[o.data_ptr() for o in out1s])
+        tr = (C.c_double * SP2_MAX_BATCH)()
+        r = Sp2Result()
+        st = lib.sp2_response_batch(self._h, C.c_void_p(H.data_ptr()), pin, nb, _dtype_code(H), H.stride(0), n, int(n_occ),
+                                    float(tol), C.c_void_p(out.data_ptr()), pout, _dtype_code(out), out.stride(0), tr,
+                                    C.byref(r), self._stream())
+        self._raise(st)
+        return out, list(out1s), [tr[b] for b in range(nb)], r.as_dict()
 
     # ------------------------------------------------------------------ host-buffer calls
     @staticmethod
