@@ -496,13 +496,82 @@ def run_congruence(args):
     return 0
 
 
+def run_batch(args):
+    """--workload batch --batch B: sp2_response_batch on config 4's H with B perturbations: one
+    stack of layers carries D and D1_0..D1_{B-1}.  Extra workload, not the headline.  value = effective Tflop/s with
+    (2 + 4 B) N^3 logical flops per layer; the layer kernel issues (3 + 6 B) N^3."""
+    import numpy as np
+    import torch
+
+    from paper_2107_02737_b200 import inputs, sp2
+
+    _, _, local = dist_env()
+    torch.cuda.set_device(local)
+    B = args.batch
+    cfg = inputs.CONFIGS[CONFIG_INDEX]
+    p = inputs.make_problem(cfg, device="cuda", want_h1=False)
+    n, n_occ = p["n"], p["n_occ"]
+    H = torch.from_numpy(p["H"]).cuda()
+    H1n = inputs.perturbations(n, B, seed=cfg.seed, decades=0.5)
+    H1s = [torch.from_numpy(a).cuda() for a in H1n]
+    D = torch.empty_like(H)
+    D1s = [torch.empty_like(H) for _ in range(B)]
+    h = sp2.Sp2Handle(n, batch=B)
+    if args.lanczos > 0:
+        h.set_options(lanczos_steps=args.lanczos)
+    for _ in range(max(args.warmup, 3)):
+        h.response_batch(H, H1s, n_occ, out=D, out1s=D1s)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local)
+    launches0 = h.launch_count
+    torch.cuda.synchronize()
+    sampler.start()
+    ev0.record()
+    res = [h.response_batch(H, H1s, n_occ, out=D, out1s=D1s)[3] for _ in range(args.steps)]
+    ev1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1)
+    layers = [r["layers"] for r in res]
+    flops = sum((2.0 + 4.0 * B) * float(n) ** 3 * L for L in layers)
+    layer_ms = sum(r["layers_ms"] for r in res) / sum(layers)
+    issued = (3.0 + 6.0 * B) * float(n) ** 3 / (layer_ms * 1e-3) / 1e12
+    peaks = read_peaks()
+    # parity at full size: sampled entries of D and of every D1_b against the closed forms the oracle evaluates one by one
+    import oracle
+
+    rng = np.random.default_rng(2)
+    rows, cols = rng.integers(0, n, 128), rng.integers(0, n, 128)
+    ri, ci = torch.from_numpy(rows).cuda(), torch.from_numpy(cols).cuda()
+    dD = float(np.abs(D[ri, ci].cpu().numpy() - oracle.density_from_eigenpairs(p["Q"], p["lam"], n_occ, rows, cols)).max())
+    d1 = []
+    for b in range(B):
+        want = oracle.response_closed_form_sampled(p["Q"], p["lam"], n_occ, H1n[b], rows, cols)
+        d1.append(float(np.abs(D1s[b][ri, ci].cpu().numpy() - want).max() / float(D1s[b].abs().max())))
+    line = {"metric": METRIC, "value": flops / (ms * 1e-3) / 1e12, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f16", "data": "synthetic",
+            "config": {"workload": f"config 4 H (N={n}, N_occ={n_occ}) with {B} perturbations -> D and {B} x D1 "
+                                   "(sp2_response_batch)", "batch": B, "lanczos_steps": args.lanczos, "layers_per_step": layers,
+                       },
+            "clocks": clocks, "gpu_launches": int(h.launch_count - launches0),
+            "roofline": {"bound": "tensor", "achieved": issued, "peak": peaks["sustained"], "unit": "TFLOP/s",
+                         "frac": issued / peaks["sustained"], "traffic": None, "ms_per_launch": layer_ms,
+                         "flops_per_launch": (3.0 + 6.0 * B) * float(n) ** 3, "peak_source": peaks["source"]},
+            "parity": {"max_abs_dD_sampled": dD, "max_rel_dD1_sampled": d1, "abs_trD_minus_nocc": abs(res[-1]["tr_d"] - n_occ)}}
+    print(json.dumps(line), flush=True)
+    h.close()
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--workload", choices=["response", "density", "sequence", "congruence"], default="response")
+    ap.add_argument("--workload", choices=["response", "density", "sequence", "congruence", "batch"], default="response")
+    ap.add_argument("--batch", type=int, default=4, help="perturbations per call of --workload batch (1..8)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--lanczos", type=int, default=0,
                     help="Lanczos steps for tighter spectral bounds (SURVEY 8(f) NEXT-3); extra, not the headline")
@@ -515,6 +584,8 @@ def main(argv=None):
         return run_sequence(args)
     if args.workload == "congruence":
         return run_congruence(args)
+    if args.workload == "batch":
+        return run_batch(args)
     return run_ours(args)
 
 

@@ -113,3 +113,34 @@ def test_batch_argument_errors(torch_cuda, sp2):
         h.response_batch(H, [H1s[0], H1s[1], bad], p["n_occ"])
     assert e.value.status == sp2.SP2_ERR_NONFINITE
     h.close()
+
+
+def test_batch_full_size_config4(torch_cuda, sp2):
+    """BASELINE.json config 4 (N = 8192, gap 0.05) with 3 perturbations, in the launch configuration
+    `bench.py --workload batch` times: sampled entries against the definitions the oracle evaluates one by one."""
+    import oracle
+
+    torch = torch_cuda
+    p = inputs.make_problem(inputs.CONFIGS[4], device="cuda", want_h1=False)
+    n, n_occ, nb = p["n"], p["n_occ"], 3
+    H1n = inputs.perturbations(n, nb, seed=4, decades=2.0)
+    H = torch.from_numpy(p["H"]).cuda()
+    h = sp2.Sp2Handle(n, batch=nb)
+    D, D1s, tr1, r = h.response_batch(H, [torch.from_numpy(a).cuda() for a in H1n], n_occ)
+    h.close()
+    rng = np.random.default_rng(3)
+    rows = np.concatenate([rng.integers(0, n, 1500), [0, n - 1, 17]])
+    cols = np.concatenate([rng.integers(0, n, 1500), [n - 1, n - 1, 17]])
+    ri, ci = torch.from_numpy(rows).cuda(), torch.from_numpy(cols).cuda()
+    De = oracle.density_from_eigenpairs(p["Q"], p["lam"], n_occ, rows, cols)
+    assert r["status"] == 0 and 35 <= r["layers"] <= 52
+    assert np.abs(D[ri, ci].cpu().numpy() - De).max() <= 1e-4
+    assert abs(r["tr_d"] - n_occ) <= 1e-3
+    E = inputs.band_energy_closed_form(p["lam"], n_occ)
+    assert abs(r["tr_dh"] - E) <= 1e-5 * abs(E)
+    for b in range(nb):
+        want = oracle.response_closed_form_sampled(p["Q"], p["lam"], n_occ, H1n[b], rows, cols)
+        s = float(D1s[b].abs().max())
+        assert np.abs(D1s[b][ri, ci].cpu().numpy() - want).max() <= 1e-3 * s, b
+        assert bool(torch.equal(D1s[b], D1s[b].T))
+        assert abs(tr1[b]) <= 1e-3 * s * n ** 0.5                          # particle number conserved to first order
