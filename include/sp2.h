@@ -119,7 +119,11 @@ typedef struct {
   int reserved2;
 } sp2_result_t;
 
-/* Bytes of device workspace needed for problems up to n_max (flags: SP2_WITH_*). 0 if n_max <= 0. */
+/* Largest supported dimension (the largest size the GPU parity tests cover; 32-bit index arithmetic in the
+ * kernels holds up to here). */
+#define SP2_MAX_N 32768
+
+/* Bytes of device workspace needed for problems up to n_max (flags: SP2_WITH_*). 0 if n_max <= 0 or > SP2_MAX_N. */
 SP2_API size_t sp2_workspace_bytes(int n_max, int flags);
 
 /* Create a handle on the CURRENT device over caller-owned device memory. */

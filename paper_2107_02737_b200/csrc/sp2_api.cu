@@ -304,8 +304,9 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   const int cg = pick_cta_group(h, npad, resp);
   int seg = h->opt.seg_kb;
   // default: 4 k-blocks per in-TMEM segment; the residual truncation bias in tr D grows ~ N * segment length
-  // (2.4e-4 at N = 16384 against the 1e-3 bar), so very large problems take shorter segments
-  if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = npad > 16384 ? 2 : 4;
+  // (measured at 2/3 filling, the worst case: 3.8e-4 at N = 24000, 6.1e-4 at N = 32768 against the 1e-3 bar), so the
+  // largest problems take shorter segments (1.5e-4 at N = 32768, at 15 % lower throughput)
+  if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = npad > 24576 ? 2 : 4;
   while ((npad / 64) % seg) seg >>= 1;
   if (h->cur_n == N && h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp && h->cur_seg == seg &&
       h->cur_dbg == h->opt.debug_flags && h->cur_first == h->opt.seg_first &&
@@ -567,12 +568,12 @@ sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dt
 extern "C" {
 
 size_t sp2_workspace_bytes(int n_max, int flags) {
-  if (n_max <= 0) return 0;
+  if (n_max <= 0 || n_max > SP2_MAX_N) return 0;
   return make_layout(n_max, flags).total;
 }
 
 sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_workspace, size_t bytes) {
-  if (!handle || n_max <= 0) return SP2_ERR_INVALID_ARG;
+  if (!handle || n_max <= 0 || n_max > SP2_MAX_N) return SP2_ERR_INVALID_ARG;
   *handle = nullptr;
   Layout L = make_layout(n_max, flags);
   if (!d_workspace || (reinterpret_cast<uintptr_t>(d_workspace) & 1023) || bytes < L.total) return SP2_ERR_WORKSPACE;

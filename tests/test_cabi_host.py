@@ -60,6 +60,11 @@ def test_workspace_bytes_and_status_strings(sp2):
     assert sp2.workspace_bytes(6000) >= 4 * 6144 * 6144 * 2
     # memory claim of DESIGN.md: N = 16384 density-only fits in ~2.2 GB of workspace
     assert sp2.workspace_bytes(16384) < 2.3 * 2 ** 30
+    # SP2_MAX_N = 32768 is the largest supported (and GPU-tested) dimension
+    assert sp2.workspace_bytes(32768) > 0 and sp2.workspace_bytes(32769) == 0
+    # batched response: 4 more planes per extra perturbation
+    b4 = sp2.workspace_bytes(1024, sp2.SP2_WITH_BATCH(4))
+    assert b4 - b2 >= 3 * 4 * plane and sp2.workspace_bytes(1024, sp2.SP2_WITH_BATCH(1)) == b2
     assert sp2.status_string(sp2.SP2_OK) == "ok"
     assert "degenerate" in sp2.status_string(sp2.SP2_ERR_DEGENERATE)
     assert "unknown" in sp2.status_string(99)

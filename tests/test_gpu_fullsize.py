@@ -129,3 +129,28 @@ def test_config5_md_sequence_n16384(torch_cuda, sp2):
     assert dE25 < 25 * d1 and dE49 < 49 * d1
     ratio = (dE49 - 49 * d1) / (dE25 - 25 * d1)
     assert 3.0 <= ratio <= 4.6                                   # (49/25)^2 = 3.84 for a pure t^2 law
+
+
+def test_maximum_size_n32768_f32(torch_cuda, sp2):
+    """SP2_MAX_N: the largest supported dimension (planes of 2 GiB each, 2^30 elements; seg_kb = 2 above N = 16384).
+    Same recipe as config 5, scaled."""
+    import oracle
+
+    torch = torch_cuda
+    n = sp2_max_n = 32768
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[5], n), device="cuda")
+    n_occ = p["n_occ"]
+    H = torch.from_numpy(p["H"]).cuda()
+    h = sp2.Sp2Handle(sp2_max_n)
+    D, r = h.density(H, n_occ)
+    h.close()
+    rows, cols = _samples(n, k=2000)
+    De = oracle.density_from_eigenpairs(p["Q"], p["lam"], n_occ, rows, cols)
+    assert r["status"] == 0 and 30 <= r["layers"] <= 55
+    assert np.abs(_gather(torch, D, rows, cols) - De).max() <= TOL_D
+    assert abs(r["tr_d"] - n_occ) <= TOL_TR
+    E = inputs.band_energy_closed_form(p["lam"], n_occ)
+    assert abs(r["tr_dh"] - E) <= TOL_E * abs(E)
+    assert bool(torch.equal(D, D.T))
+    with pytest.raises(sp2.Sp2Error):
+        sp2.Sp2Handle(sp2_max_n + 1)
