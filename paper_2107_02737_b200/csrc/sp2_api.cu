@@ -191,15 +191,18 @@ namespace {
   } while (0)
 
 // Upper-triangular tile list in an L2-friendly order: G x G groups of tiles, so that the tiles that
-// run concurrently (consecutive list entries) share row panels of the operand planes.
+// run concurrently (consecutive list entries) share row panels of the operand planes.  Consecutive groups share
+// their ROW panels (same gi), so inside a group the tiles go column by column: a wave of CTA(-pair)s that
+// straddles two groups then touches the next group's first columns only (1-2 new column panels instead of all G;
+// measured: 14 % fewer DRAM reads than row by row).
 void build_tiles(int nt, std::vector<int2>& out) {
   out.clear();
   const int G = 8;
   const int ng = (nt + G - 1) / G;
   for (int gi = 0; gi < ng; ++gi)
     for (int gj = gi; gj < ng; ++gj)
-      for (int ti = gi * G; ti < (gi + 1) * G && ti < nt; ++ti)
-        for (int tj = gj * G; tj < (gj + 1) * G && tj < nt; ++tj)
+      for (int tj = gj * G; tj < (gj + 1) * G && tj < nt; ++tj)
+        for (int ti = gi * G; ti < (gi + 1) * G && ti < nt; ++ti)
           if (tj >= ti) out.push_back(make_int2(ti, tj));
 }
 
@@ -305,8 +308,9 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   int seg = h->opt.seg_kb;
   // default: 4 k-blocks per in-TMEM segment; the residual truncation bias in tr D grows ~ N * segment length
   // (measured at 2/3 filling, the worst case: 3.8e-4 at N = 24000, 6.1e-4 at N = 32768 against the 1e-3 bar), so the
-  // largest problems take shorter segments (1.5e-4 at N = 32768, at 15 % lower throughput)
-  if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = npad > 24576 ? 2 : 4;
+  // largest problems take shorter segments (1.5e-4 at N = 32768, at 15 % lower throughput) and problems up to
+  // N = 8192 longer ones (8 k-blocks: 8e-5 at N = 8192, 2 % faster than 4)
+  if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = npad > 24576 ? 2 : (npad > 8192 ? 4 : 8);
   while ((npad / 64) % seg) seg >>= 1;
   if (h->cur_n == N && h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp && h->cur_seg == seg &&
       h->cur_dbg == h->opt.debug_flags && h->cur_first == h->opt.seg_first &&
@@ -734,8 +738,8 @@ sp2_status_t sp2_congruence(sp2_handle_t h, const void* dZ, const void* dX, sp2_
   const int G = 8;
   for (int gi = 0; gi < nt; gi += G)
     for (int gj = 0; gj < nt; gj += G)
-      for (int ti = gi; ti < gi + G && ti < nt; ++ti)
-        for (int tj = gj; tj < gj + G && tj < nt; ++tj) h->tiles_host.push_back(make_int2(ti, tj));
+      for (int tj = gj; tj < gj + G && tj < nt; ++tj)       // column by column inside a group, as build_tiles
+        for (int ti = gi; ti < gi + G && ti < nt; ++ti) h->tiles_host.push_back(make_int2(ti, tj));
   int seg = 4;
   while ((npad / 64) % seg) seg >>= 1;
   int nC = h->num_sms / cg;
