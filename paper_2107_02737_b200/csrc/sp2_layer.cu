@@ -195,6 +195,9 @@ struct alignas(8) SmemBarriers {
   uint64_t tmem_empty[2];
   uint32_t tmem_base;
   uint32_t is_last;
+  // partial sums of this CTA, per consumer warp and product class (0: Y^2, 1 + b: Y Z_b + Z_b Y): one writer each
+  // (lane 0 of the warp), reduced in fixed order at the end of the kernel into ONE slot per CTA and class
+  Sp2Slot acc[kConsumerWarps][1 + SP2_NB];
 };
 
 __device__ __forceinline__ uint4 ld_global_v4(const void* p) {
@@ -470,6 +473,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
     for (int s = 0; s < 2; ++s) { mbar_init(smem_u32(&bars->tmem_full[s]), 1); mbar_init(smem_u32(&bars->tmem_empty[s]), kConsumerWarps * CG); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  if (warp < kConsumerWarps && lane < 1 + SP2_NB) {
+    Sp2Slot z; z.tr = 0.0; z.fro = 0.0; z.tracc = 0.0; z.mx = 0.f; z.pad = 0.f;
+    bars->acc[warp][lane] = z;
+  }
   if (warp == kWarpAlloc) tmem_alloc<CG>(smem_u32(&bars->tmem_base), TMEM_COLS);
   tc_fence_before();
   if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
@@ -675,9 +682,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
         const float qv = __shfl_xor_sync(0xffffffffu, P.mx, o);
         P.mx = (qv > P.mx || qv != qv) ? qv : P.mx;
       }
-      if (lane == 0) {
-        Sp2Slot s; s.tr = P.tr; s.fro = P.fro; s.tracc = wunit ? 0.0 : P.tracc; s.mx = P.mx; s.pad = 0.f;
-        a.slots[((size_t)u * CG + rank) * kConsumerWarps + cw] = s;
+      if (lane == 0) {                           // fixed item order per warp: deterministic
+        Sp2Slot& s = bars->acc[cw][wunit ? 1 + zb : 0];
+        s.tr += P.tr; s.fro += P.fro;
+        if (!wunit) s.tracc += P.tracc;
+        s.mx = (P.mx > s.mx || P.mx != P.mx) ? P.mx : s.mx;   // NaN-propagating max
       }
     }
   }
@@ -701,9 +710,18 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
     return;
   }
 
-  const int per_unit = CG * kConsumerWarps;
-  layer_tail(a.ctrl, a.slots, n_tiles * per_unit, n_tiles * per_unit, a.with_response, gridDim.x, &bars->is_last, red,
-             a.flags, a.n_flags);
+  // one slot per CTA and class: [class z_0: gridDim.x slots] ... [class z_{nb-1}][class y]
+  if ((int)threadIdx.x < 1 + a.with_response) {
+    const int cls = threadIdx.x;               // 0: y, 1 + b: z_b
+    Sp2Slot t = bars->acc[0][cls];
+    for (int w = 1; w < kConsumerWarps; ++w) {
+      const Sp2Slot& o = bars->acc[w][cls];
+      t.tr += o.tr; t.fro += o.fro; t.tracc += o.tracc;
+      t.mx = (o.mx > t.mx || o.mx != o.mx) ? o.mx : t.mx;
+    }
+    a.slots[(size_t)(cls == 0 ? a.with_response : cls - 1) * gridDim.x + blockIdx.x] = t;
+  }
+  layer_tail(a.ctrl, a.slots, gridDim.x, gridDim.x, a.with_response, gridDim.x, &bars->is_last, red, a.flags, a.n_flags);
 }
 
 // ----------------------------------------------------------------------------------------------

@@ -100,27 +100,30 @@ def test_product_path_does_not_touch_the_oracle():
 
 @pytest.mark.parametrize("n_tiles, resp, segs, ncl", [(528, False, 32, 74), (528, True, 32, 74), (36, True, 4, 148),
                                                       (10, False, 4, 74), (3, True, 1, 3), (300, False, 24, 74),
-                                                      (2080, False, 64, 74), (1, False, 1, 1)])
+                                                      (2080, False, 64, 74), (1, False, 1, 1), (528, 4, 16, 74),
+                                                      (45, 8, 2, 148)])
 def test_work_schedule_covers_every_segment_once_and_is_balanced(sp2, n_tiles, resp, segs, ncl):
     lists = sp2.debug_schedule(n_tiles, resp, segs, ncl)
-    n_units = n_tiles * (2 if resp else 1)
-    cost = lambda u: 2 * segs if (resp and u < n_tiles) else segs
+    n_units = n_tiles * (1 + int(resp))                          # resp = number of perturbations carried
+    cost = lambda u: 2 * segs if u < int(resp) * n_tiles else segs
     cover = {u: [0] * cost(u) for u in range(n_units)}
     loads, owners, contribs = [], {}, {}
     for items in lists:
-        load, seen_owner = 0, False
+        load, seen_other = 0, False
         for it in items:
             assert 0 <= it["seg0"] < it["seg1"] <= cost(it["unit"])
             for sgm in range(it["seg0"], it["seg1"]):
                 cover[it["unit"]][sgm] += 1
             load += it["seg1"] - it["seg0"]
             if it["kind"] == 2:
-                seen_owner = True
                 owners[it["unit"]] = it
-            else:
-                assert not seen_owner              # owners (which wait) come last: no wait cycles
             if it["kind"] == 1:
+                assert not seen_other              # contributors (which never wait) head every list: no wait cycles
                 contribs.setdefault(it["unit"], []).append(it)
+            else:
+                seen_other = True
+        if any(it["kind"] == 0 for it in items):
+            assert items[-1]["kind"] == 0          # a list ends with a whole unit: only its epilogue follows the last MMA
             if it["kind"] == 0:
                 assert (it["seg0"], it["seg1"]) == (0, cost(it["unit"]))
         loads.append(load)
