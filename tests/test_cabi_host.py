@@ -109,21 +109,19 @@ def test_work_schedule_covers_every_segment_once_and_is_balanced(sp2, n_tiles, r
     cover = {u: [0] * cost(u) for u in range(n_units)}
     loads, owners, contribs = [], {}, {}
     for items in lists:
-        load, seen_other = 0, False
+        load, seen_owner = 0, False
         for it in items:
             assert 0 <= it["seg0"] < it["seg1"] <= cost(it["unit"])
             for sgm in range(it["seg0"], it["seg1"]):
                 cover[it["unit"]][sgm] += 1
             load += it["seg1"] - it["seg0"]
             if it["kind"] == 2:
+                seen_owner = True
                 owners[it["unit"]] = it
-            if it["kind"] == 1:
-                assert not seen_other              # contributors (which never wait) head every list: no wait cycles
-                contribs.setdefault(it["unit"], []).append(it)
             else:
-                seen_other = True
-        if any(it["kind"] == 0 for it in items):
-            assert items[-1]["kind"] == 0          # a list ends with a whole unit: only its epilogue follows the last MMA
+                assert not seen_owner              # owners (which wait) come last: no wait cycles
+            if it["kind"] == 1:
+                contribs.setdefault(it["unit"], []).append(it)
             if it["kind"] == 0:
                 assert (it["seg0"], it["seg1"]) == (0, cost(it["unit"]))
         loads.append(load)
