@@ -85,7 +85,15 @@ class ClockSampler:
         self.rows = []
         self.proc = None
 
+    def mark(self):
+        """Start of the timed region: wait (bounded) for the first sample, then drop what was sampled before it."""
+        t0 = time.perf_counter()
+        while self.proc is not None and not self.rows and time.perf_counter() - t0 < 1.0:
+            time.sleep(0.01)
+        self.skip = len(self.rows)
+
     def start(self):
+        self.skip = 0
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
@@ -110,7 +118,8 @@ class ClockSampler:
             self.proc.kill()
         sm, smax, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for row in self.rows:
+        rows = self.rows[self.skip:] or self.rows[-1:]      # a very short region may hold no sample of its own
+        for row in rows:
             parts = [s.strip() for s in row.split(",")]
             if len(parts) < 6:
                 continue
@@ -297,15 +306,16 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    sampler = ClockSampler(local)
+    sampler.start()                      # before the warm-up, so that samples are flowing when the timed region starts
     for _ in range(max(args.warmup, 3)):
         step()
     # ---- timed region: exactly K steps, CUDA events on the launching stream, barrier + sync both sides
     stream = torch.cuda.current_stream()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler = ClockSampler(local)
     launches0 = h.launch_count
     barrier()
-    sampler.start()
+    sampler.mark()
     ev0.record(stream)
     results = [step() for _ in range(args.steps)]
     ev1.record(stream)
