@@ -88,18 +88,14 @@ typedef struct {
                         fewer layers for dense matrices (the paper leaves accelerated variants aside) */
   int refine_layers; /* 0 = off (default); 1..4: float64 SP2 layers applied to the converged iterate before D is written
                         (the paper uses 2); D1 is not refined.  Needs SP2_WITH_REFINEMENT */
-  int seg_kb;       /* 0 = default (4); 1, 2, 4, 8, 16 or 32 (must divide npad/64): k-blocks of 64 accumulated inside
-                       the tensor core before the FP32 round-to-nearest add in registers (shorter = less
-                       truncation bias, more drains) */
-  int seg_first;    /* 0 = default (1 = off): segments merged into each of the first two TMEM hand-offs of a work
-                       unit (longer run-ahead during the previous epilogue; measured no gain, more truncation bias) */
+  int seg_kb;       /* 0 = default (8 up to N = 8192, 4 up to N = 24576, 2 above); 1, 2, 4, 8, 16 or 32 (must divide
+                       npad/64): k-blocks of 64 accumulated inside the tensor core before the FP32 round-to-nearest add in
+                       registers (shorter = less truncation bias, more drains) */
   int lo_bits;      /* 0 = default (11: full FP16 lo plane); 6..10: round the lo planes to that many significant bits.
                        The B200 is power-capped during the layer stack and multiplier inputs with fewer toggling bits
-                       draw less power: lo_bits = 8 measured 0-5 % faster (within the box-to-box noise) at ~3x larger max|dD|,
-                       still > 10x inside the bars; kept as an experiment knob, not a recommendation */
+                       draw less power: lo_bits = 8 measured 1.8 % faster at ~3x larger max|dD|, still > 1000x inside
+                       the bar; kept as an experiment knob, not a recommendation */
   int no_recentre;  /* debug, with forced_layers only: keep c on the scalar map instead of the cluster midpoint */
-  int debug_flags;  /* performance experiments only (results are WRONG): 1 = skip the epilogue's global loads/stores,
-                       2 = issue only the hi*hi product; bits 8-15 = cap on the number of CTA(-pair)s */
 } sp2_options_t;
 
 typedef struct {

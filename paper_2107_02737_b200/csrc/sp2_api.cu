@@ -143,7 +143,7 @@ struct sp2_handle_s {
   sp2_options_t opt;
   PFN_cuTensorMapEncodeTiled_v12000 encode;
   // per-(N, cta_group) cache
-  int cur_n, cur_npad, cur_cg, cur_resp, cur_seg, cur_dbg, cur_first, cur_lo;
+  int cur_n, cur_npad, cur_cg, cur_resp, cur_seg, cur_lo;
   Sp2LayerArgs args[2];          // parity 0: buffer 0 -> 1, parity 1: buffer 1 -> 0
   std::vector<int2> tiles_host;
   std::vector<Sp2Item> items_host;
@@ -316,7 +316,6 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = npad > 24576 ? 2 : (npad > 8192 ? 4 : 8);
   while ((npad / 64) % seg) seg >>= 1;
   if (h->cur_n == N && h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp && h->cur_seg == seg &&
-      h->cur_dbg == h->opt.debug_flags && h->cur_first == h->opt.seg_first &&
       h->cur_lo == h->opt.lo_bits) return SP2_OK;
   const int nt = npad / (128 * cg);
   build_tiles(nt, h->tiles_host);
@@ -326,7 +325,6 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   int nC = h->num_sms / cg;
   if (nC > kMaxClusters / cg) nC = kMaxClusters / cg;
   (void)n_units;   // fewer units than CTA(-pair)s: the schedule splits them along k, every SM gets work
-  if (h->opt.debug_flags >> 8) { int lim = h->opt.debug_flags >> 8; if (nC > lim) nC = lim; }   // experiments: fewer CTA(-pair)s
   int n_slots = 0;
   build_schedule((int)h->tiles_host.size(), resp, (npad / 64) / seg, nC, h->items_host, h->item_begin_host,
                  &h->n_flags, &n_slots);
@@ -353,13 +351,12 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
     }
     a.ctrl = h->ctrl(); a.slots = h->slots(); a.tiles = h->tiles();
     a.items = h->items(); a.item_begin = h->item_begin(); a.scratch = h->scratch(); a.flags = h->split_flags();
-    a.n_flags = h->n_flags; a.n_clusters = h->n_clusters; a.debug_flags = h->opt.debug_flags;
+    a.n_flags = h->n_flags; a.n_clusters = h->n_clusters;
     a.lo_bits = (h->opt.lo_bits >= 6 && h->opt.lo_bits <= 10) ? h->opt.lo_bits : 11;
-    a.seg_first = (h->opt.seg_first >= 1 && h->opt.seg_first <= 16) ? h->opt.seg_first : 1;
     a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = resp; a.seg_kb = seg;
   }
   h->layers_hint = 0;
-  h->cur_n = N; h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp; h->cur_seg = seg; h->cur_dbg = h->opt.debug_flags; h->cur_first = h->opt.seg_first; h->cur_lo = h->opt.lo_bits;
+  h->cur_n = N; h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp; h->cur_seg = seg; h->cur_lo = h->opt.lo_bits;
   return SP2_OK;
 }
 
@@ -775,7 +772,7 @@ sp2_status_t sp2_congruence(sp2_handle_t h, const void* dZ, const void* dX, sp2_
   memset(&a, 0, sizeof(a));
   a.ctrl = c; a.slots = h->slots(); a.tiles = h->tiles(); a.items = h->items(); a.item_begin = h->item_begin();
   a.scratch = h->scratch(); a.flags = h->split_flags(); a.n_flags = h->n_flags; a.n_clusters = nC;
-  a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = 0; a.seg_kb = seg; a.seg_first = 1;
+  a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = 0; a.seg_kb = seg;
   a.lo_bits = 11; a.gemm_mode = 1;
   sp2_status_t st;
   // T = L X^T (= L X): planes out

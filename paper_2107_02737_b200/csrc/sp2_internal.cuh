@@ -210,28 +210,13 @@ __device__ inline void sp2_reduce_slots(const Sp2Slot* slots, int count, double*
   const int nt = 256;             // blockDim.x >= 256; extra threads only join the barriers
   double a = 0.0, b = 0.0, m = 0.0, d = 0.0;
   if (tid < nt) {
-    // four independent chains (slots tid, tid + nt, ... taken four at a time) keep several loads in flight; the
-    // chains are combined in a fixed order, so the result does not depend on timing
-    double a4[4] = {0.0, 0.0, 0.0, 0.0}, b4[4] = {0.0, 0.0, 0.0, 0.0}, d4[4] = {0.0, 0.0, 0.0, 0.0}, m4[4] = {0.0, 0.0, 0.0, 0.0};
-    int i = tid;
-    for (; i + 3 * nt < count; i += 4 * nt) {
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const Sp2Slot s = slots[i + q * nt];
-        a4[q] += s.tr; b4[q] += s.fro; d4[q] += s.tracc;
-        const double v = (double)s.mx;
-        m4[q] = (v > m4[q] || v != v) ? v : m4[q];   // NaN-propagating max
-      }
+    for (int i = tid; i < count; i += nt) {
+      a += slots[i].tr;
+      b += slots[i].fro;
+      d += slots[i].tracc;
+      const double v = (double)slots[i].mx;
+      m = (v > m || v != v) ? v : m;   // NaN-propagating max
     }
-    for (; i < count; i += nt) {
-      const Sp2Slot s = slots[i];
-      a4[0] += s.tr; b4[0] += s.fro; d4[0] += s.tracc;
-      const double v = (double)s.mx;
-      m4[0] = (v > m4[0] || v != v) ? v : m4[0];
-    }
-    a = (a4[0] + a4[1]) + (a4[2] + a4[3]); b = (b4[0] + b4[1]) + (b4[2] + b4[3]); d = (d4[0] + d4[1]) + (d4[2] + d4[3]);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) m = (m4[q] > m || m4[q] != m4[q]) ? m4[q] : m;
     red[tid] = a; red[256 + tid] = b; red[512 + tid] = m; red[768 + tid] = d;
   }
   __syncthreads();

@@ -534,15 +534,11 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
         int as = 0; uint32_t aphase = 0;
         for (int iti = item_lo; iti < item_hi; ++iti) {
           const Sp2Item I = a.items[iti];
-          for (int sg = I.seg0, ho = 0; sg < I.seg1; ++ho) {
-            // the first two hand-offs of an item are longer, so that the tensor core has work while the
-            // consumers are still in the previous unit's epilogue
-            const int len = (ho < 2) ? min(a.seg_first, I.seg1 - sg) : 1;
-            sg += len;
+          for (int sg = I.seg0; sg < I.seg1; ++sg) {
             mbar_wait(smem_u32(&bars->tmem_empty[as]), aphase ^ 1u);
             tc_fence_after();
             const uint32_t acc = tmem_base + (uint32_t)(as * ACC_COLS);
-            for (int it = 0; it < len * seg_kb; ++it) {
+            for (int it = 0; it < seg_kb; ++it) {
               mbar_wait(smem_u32(&bars->full[stage]), phase);
               tc_fence_after();
               const uint32_t sa = smem_u32(smem + stage * kStageBytes);
@@ -554,13 +550,9 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
               for (int k = 0; k < kBK / 16; ++k) {
                 const uint64_t ko = (uint64_t)(k * 2);     // 16 elements * 2 B = 32 B -> >>4 = 2
                 // small cross terms first, the dominant hi*hi product last
-                if (!(a.debug_flags & 2)) {
-                  umma_f16<CG>(acc, dA0 + ko, dB1 + ko, IDESC, (it | k) ? 1u : 0u);
-                  umma_f16<CG>(acc, dA1 + ko, dB0 + ko, IDESC, 1u);
-                  umma_f16<CG>(acc, dA0 + ko, dB0 + ko, IDESC, 1u);
-                } else {
-                  umma_f16<CG>(acc, dA0 + ko, dB0 + ko, IDESC, (it | k) ? 1u : 0u);
-                }
+                umma_f16<CG>(acc, dA0 + ko, dB1 + ko, IDESC, (it | k) ? 1u : 0u);
+                umma_f16<CG>(acc, dA1 + ko, dB0 + ko, IDESC, 1u);
+                umma_f16<CG>(acc, dA0 + ko, dB0 + ko, IDESC, 1u);
               }
               umma_commit<CG>(smem_u32(&bars->empty[stage]));   // smem slot free when these MMAs retire
               if (++stage == kStages) { stage = 0; phase ^= 1u; }
@@ -596,11 +588,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
       const int gi = tij.x * TILE + (int)rank * kRows + q * 32 + lane;   // global row of this thread
       const int j0 = tij.y * TILE + hh * WCOLS;
       EpiOld old;
-      for (int sg = I.seg0, ho = 0; sg < I.seg1; ++ho) {
-        const int len = (ho < 2) ? min(a.seg_first, I.seg1 - sg) : 1;     // same hand-off lengths as the MMA issuer
-        sg += len;
-        // the old tile's first chunk is fetched under the last hand-off's MMAs
-        if (MODE == 0 && sg == I.seg1 && I.kind != 1) epilogue_prefetch(old, gi, j0, (size_t)a.npad, a.in[pl], a.in[pl + 1]);
+#pragma unroll 1
+      for (int sg = I.seg0, ho = 0; sg < I.seg1; ++sg, ++ho) {
+        // the old tile's first chunk is fetched under the last segment's MMAs
+        if (MODE == 0 && sg + 1 == I.seg1 && I.kind != 1) epilogue_prefetch(old, gi, j0, (size_t)a.npad, a.in[pl], a.in[pl + 1]);
         mbar_wait(smem_u32(&bars->tmem_full[as]), aphase);
         tc_fence_after();
         const uint32_t tcol = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * ACC_COLS + hh * WCOLS);
@@ -665,14 +656,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
       const bool shift_row = !wunit && gi < a.n;        // zero padding stays zero
       const float dsh_hi = shift_row ? cf_dsh_hi : 0.f, dsh_lo = shift_row ? cf_dsh_lo : 0.f;
       EpiPartials P; P.tr = 0.0; P.fro = 0.0; P.tracc = 0.0; P.mx = 0.f;
-      if (a.debug_flags & 1) {
-        float t = 0.f;
-#pragma unroll
-        for (int c = 0; c < WCOLS; ++c) t += sums[c];
-        P.fro = (double)t;
-      } else
-        epilogue_row<NCH>(sums, old, gi, j0, (size_t)a.npad, a.in[pl], a.in[pl + 1], a.out[pl], a.out[pl + 1],
-                          a1hi, a1lo, a2, dsh_hi, dsh_lo, lo_round, lo_mask, P);
+      epilogue_row<NCH>(sums, old, gi, j0, (size_t)a.npad, a.in[pl], a.in[pl + 1], a.out[pl], a.out[pl + 1],
+                        a1hi, a1lo, a2, dsh_hi, dsh_lo, lo_round, lo_mask, P);
       // warp partial -> slot (fixed shuffle tree: deterministic)
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {

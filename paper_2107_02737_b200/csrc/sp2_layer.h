@@ -30,14 +30,12 @@ struct alignas(64) Sp2LayerArgs {
   float* scratch;        // split-k partial sums
   unsigned int* flags;   // one arrival counter per split unit (zero between launches)
   int n_flags;
-  int seg_first;         // segments merged into each of the first two TMEM hand-offs of an item
   int lo_bits;           // significant bits kept in the lo planes (11 = all)
   // plain-product mode (sp2_congruence): C = A B^T, A = tm[0..1], B = tm[2..3]
   int gemm_mode;         // 0: SP2 layer, 1: plain product
   int out_kind;          // 0: hi/lo planes out[0], out[1]; 1: float matrix cout; 2: double matrix cout
   void* cout;            // caller's output matrix (out_kind 1, 2)
   long ldc;
-  int debug_flags;       // sp2_options_t.debug_flags
   int n_clusters;        // CTA(-pair)s the work lists were built for (= grid size / cta_group)
   int n;                 // true dimension (rows/cols >= n are zero padding and stay zero)
   int npad;              // padded dimension (multiple of the tile edge)

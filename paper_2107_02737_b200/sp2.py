@@ -53,7 +53,7 @@ class Sp2Options(C.Structure):
         ("eps_min", C.c_double), ("eps_max", C.c_double),
         ("engine", C.c_int), ("forced_layers", C.c_int),
         ("forced_signs", C.c_ulonglong), ("cta_group", C.c_int),
-        ("lanczos_steps", C.c_int), ("refine_layers", C.c_int), ("seg_kb", C.c_int), ("seg_first", C.c_int), ("lo_bits", C.c_int), ("no_recentre", C.c_int), ("debug_flags", C.c_int),
+        ("lanczos_steps", C.c_int), ("refine_layers", C.c_int), ("seg_kb", C.c_int), ("lo_bits", C.c_int), ("no_recentre", C.c_int),
     ]
 
 
