@@ -144,3 +144,27 @@ def test_batch_full_size_config4(torch_cuda, sp2):
         assert np.abs(D1s[b][ri, ci].cpu().numpy() - want).max() <= 1e-3 * s, b
         assert bool(torch.equal(D1s[b], D1s[b].T))
         assert abs(tr1[b]) <= 1e-3 * s * n ** 0.5                          # particle number conserved to first order
+
+
+def test_batch_with_lanczos_bounds_and_refinement(torch_cuda, sp2):
+    """The options compose: Lanczos bounds (fewer layers) and float64 refinement of D under a batched response."""
+    import oracle
+
+    torch = torch_cuda
+    n, nb = 384, 3
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[2], n), want_h1=False)
+    n_occ = p["n_occ"]
+    H1s = inputs.perturbations(n, nb, seed=21)
+    lo, hi = oracle.lanczos_bounds(p["H"], 10)
+    ref = oracle.sp2_response_batch(p["H"], n_occ, H1s, bounds=(lo, hi))
+    ref_g = oracle.sp2_response_batch(p["H"], n_occ, H1s[:1])
+    h = sp2.Sp2Handle(n, batch=nb, refinement=True)
+    h.set_options(lanczos_steps=10, refine_layers=2)
+    D, D1s, tr1, r = h.response_batch(torch.from_numpy(p["H"]).cuda(), [torch.from_numpy(a).cuda() for a in H1s], n_occ)
+    h.close()
+    assert r["status"] == 0 and r["refine_layers"] == 2 and r["layers"] <= ref_g["layers"] - 3
+    Dn = D.cpu().numpy()
+    assert np.abs(Dn - ref["D"]).max() <= 1e-6                        # refined: far inside the 1e-4 bar
+    assert np.abs(Dn @ Dn - Dn).max() <= 1e-9
+    for b in range(nb):
+        assert np.abs(D1s[b].cpu().numpy() - ref["D1"][b]).max() <= 1e-3 * np.abs(ref["D1"][b]).max()
