@@ -1,0 +1,49 @@
+"""Seeded random sweep of the GPU path against the oracle through the C ABI: N = 2..1500, any occupation, gaps
+0.02..1, f32 / f64 inputs, 0-3 perturbations (magnitudes up to 3 decades apart), every tile shape, with and without
+Lanczos bounds.  Tolerances [north_star]: max|dD| <= 1e-4, |tr D - N_occ| <= 1e-3, rel d tr(DH) <= 1e-5,
+max|dD1_b| <= 1e-3 max|D1_b|."""
+import numpy as np
+import pytest
+
+from paper_2107_02737_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("seed0", [1, 2])
+def test_random_sweep_against_oracle(torch_cuda, sp2, seed0):
+    import oracle
+
+    torch = torch_cuda
+    rng = np.random.default_rng(seed0)
+    for it in range(30):
+        n = int(rng.choice([rng.integers(2, 64), rng.integers(64, 400), rng.integers(400, 1500)]))
+        n_occ = int(rng.integers(1, n))
+        gap = float(rng.choice([0.02, 0.1, 0.5, 1.0]))
+        dt = str(rng.choice(["f32", "f64"]))
+        nb = int(rng.choice([0, 0, 1, 2, 3]))
+        cg = int(rng.choice([0, 1, 2]))
+        lz = int(rng.choice([0, 0, 8]))
+        lz = lz if n > lz else 0
+        cfg = inputs.Sp2Config("sweep", 2, n, n_occ, (-1.5, -gap / 2), (gap / 2, 1.5), dt, False)
+        p = inputs.make_problem(cfg, seed=seed0 * 1000 + it)
+        H1s = inputs.perturbations(n, nb, seed=it, dtype=p["H"].dtype, decades=float(rng.choice([0.0, 1.0, 3.0])))
+        H64 = p["H"].astype(np.float64)
+        bounds = oracle.lanczos_bounds(H64, lz) if lz else None
+        ref = oracle.sp2_response_batch(H64, n_occ, [a.astype(np.float64) for a in H1s], bounds=bounds)
+        h = sp2.Sp2Handle(n, batch=nb)
+        h.set_options(cta_group=cg, lanczos_steps=lz)
+        H = torch.from_numpy(p["H"]).cuda()
+        if nb:
+            D, D1s, _, r = h.response_batch(H, [torch.from_numpy(a).cuda() for a in H1s], n_occ)
+        else:
+            (D, r), D1s = h.density(H, n_occ), []
+        h.close()
+        case = f"case {seed0}/{it}: n={n} n_occ={n_occ} gap={gap} {dt} nb={nb} cta_group={cg} lanczos={lz}"
+        assert r["status"] == 0, case
+        assert np.abs(D.cpu().numpy().astype(np.float64) - ref["D"]).max() <= 1e-4, case
+        assert abs(r["tr_d"] - n_occ) <= 1e-3, case
+        if 3 < n_occ < n - 2:      # |tr(DH)| of one or two levels is no scale for a relative bar
+            assert abs(r["tr_dh"] - ref["tr_dh"]) <= 1e-5 * abs(ref["tr_dh"]), case
+        for b in range(nb):
+            assert np.abs(D1s[b].cpu().numpy().astype(np.float64) - ref["D1"][b]).max() <= 1e-3 * np.abs(ref["D1"][b]).max(), case
