@@ -18,7 +18,7 @@
  * Conventions
  *   - Matrices are dense, row-major, symmetric, `ld` = row pitch in ELEMENTS (ld >= N).
  *     Input symmetry: the library uses (H_ij + H_ji)/2, which is H itself when H is exactly symmetric.
- *   - sp2_density / sp2_response / sp2_sequence_*: every matrix pointer is a DEVICE pointer owned
+ *   - sp2_density / sp2_response / sp2_response_batch / sp2_sequence_* / sp2_congruence: every matrix pointer is a DEVICE pointer owned
  *     by the caller; H, H1 are never written; D, D1 must not alias H, H1 or the workspace.
  *     sp2_density_host / sp2_response_host: every matrix pointer is a HOST pointer (pinned memory
  *     is faster, pageable works); the copies to and from the device are part of the call.
