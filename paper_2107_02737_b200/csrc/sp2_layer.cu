@@ -126,23 +126,26 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
   else asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
 }
 
-// D[tmem] (+)= A[smem] * B[smem]^T, FP16 inputs, FP32 accumulate
-template <int CG>
+// D[tmem] (+)= A[smem] * B[smem]^T, FP16 inputs, FP32 accumulate.  COLL: use of the A collector buffer -- 0: none,
+// 1: fill (keep this A for the next MMA), 2: lastuse (take A from the collector: the previous MMA had the same A)
+#define SP2_UMMA_ASM(GROUP, COLLECTOR)                                                                     \
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"                                         \
+               "tcgen05.mma.cta_group::" GROUP ".kind::f16" COLLECTOR " [%0], %1, %2, %3, p;\n\t}"        \
+               ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)                        \
+               : "memory")
+template <int CG, int COLL = 0>
 __device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
   if constexpr (CG == 1) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-        : "memory");
+    if constexpr (COLL == 1) SP2_UMMA_ASM("1", ".collector::a::fill");
+    else if constexpr (COLL == 2) SP2_UMMA_ASM("1", ".collector::a::lastuse");
+    else SP2_UMMA_ASM("1", "");
   } else {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-        : "memory");
+    if constexpr (COLL == 1) SP2_UMMA_ASM("2", ".collector::a::fill");
+    else if constexpr (COLL == 2) SP2_UMMA_ASM("2", ".collector::a::lastuse");
+    else SP2_UMMA_ASM("2", "");
   }
 }
+#undef SP2_UMMA_ASM
 // all previously issued MMAs of this thread -> one arrival on `bar` (same offset in every CTA of the mask)
 template <int CG>
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
@@ -550,9 +553,10 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
               for (int k = 0; k < kBK / 16; ++k) {
                 const uint64_t ko = (uint64_t)(k * 2);     // 16 elements * 2 B = 32 B -> >>4 = 2
                 // small cross terms first, the dominant hi*hi product last
-                umma_f16<CG>(acc, dA0 + ko, dB1 + ko, IDESC, (it | k) ? 1u : 0u);
-                umma_f16<CG>(acc, dA1 + ko, dB0 + ko, IDESC, 1u);
-                umma_f16<CG>(acc, dA0 + ko, dB0 + ko, IDESC, 1u);
+                // the two products with A.hi are adjacent: A.hi is read from shared memory once (collector buffer)
+                umma_f16<CG>(acc, dA1 + ko, dB0 + ko, IDESC, (it | k) ? 1u : 0u);
+                umma_f16<CG, 1>(acc, dA0 + ko, dB1 + ko, IDESC, 1u);
+                umma_f16<CG, 2>(acc, dA0 + ko, dB0 + ko, IDESC, 1u);
               }
               umma_commit<CG>(smem_u32(&bars->empty[stage]));   // smem slot free when these MMAs retire
               if (++stage == kStages) { stage = 0; phase ^= 1u; }
