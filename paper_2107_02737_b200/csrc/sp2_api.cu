@@ -321,10 +321,9 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   build_tiles(nt, h->tiles_host);
   SP2_CUDA(h, cudaMemcpyAsync(h->tiles(), h->tiles_host.data(), h->tiles_host.size() * sizeof(int2),
                               cudaMemcpyHostToDevice, s));
-  int n_units = (int)h->tiles_host.size() * (1 + resp);
   int nC = h->num_sms / cg;
   if (nC > kMaxClusters / cg) nC = kMaxClusters / cg;
-  (void)n_units;   // fewer units than CTA(-pair)s: the schedule splits them along k, every SM gets work
+  // (fewer units than CTA(-pair)s is fine: the schedule splits them along k, every SM gets work)
   int n_slots = 0;
   build_schedule((int)h->tiles_host.size(), resp, (npad / 64) / seg, nC, h->items_host, h->item_begin_host,
                  &h->n_flags, &n_slots);
