@@ -102,7 +102,8 @@ typedef struct {
   int status;                        /* sp2_status_t of the solve */
   int layers;                        /* number of layers applied (paper: 14-16 for water) */
   unsigned long long sign_mask[2];   /* bit n = 1 if layer n was X^2 ('+'), 0 if 2X - X^2 ('-') */
-  int stop_reason;                   /* 1 tol, 2 floor (parameter-free), 3 idempotent on entry, 4 max_layers, 5 trivial N_occ, 6 forced */
+  int stop_reason;                   /* 1 tol, 2 floor (parameter-free), 3 idempotent on entry, 4 max_layers, 5 trivial N_occ, 6 forced,
+                                        7 a sequence step ran out of enqueued layer launches (status NOT_CONVERGED) */
   int reserved;                      /* number of float64 refinement layers applied */
   double tr_d;                       /* tr D (should be N_occ) */
   double tr_dh;                      /* sum_ij D_ij H_ij */
@@ -197,6 +198,14 @@ SP2_API int sp2_debug_history(sp2_handle_t handle, double* tr_x, double* e, int 
  * (X_L = c*I + (hi+lo)*2^-exp); which + 4 = the same plane of the previous iterate X_{L-1} (other
  * ping-pong buffer; exponent and shift are still those of X_L).  c is returned in *shift. */
 SP2_API sp2_status_t sp2_debug_plane(sp2_handle_t handle, int which, size_t* offset, long* pitch, int* exponent, double* shift);
+
+/* The carved regions of the workspace and how much of each the calls made through this handle so far were entitled
+ * to write (computed from the launch geometry, not from the allocation formulas).  index in [0, count): fills name24
+ * (24 bytes, NUL-terminated), byte offset inside the workspace, reserved bytes, used bytes; any pointer may be NULL.
+ * Returns the number of regions (also for an out-of-range index, e.g. -1).  tests/test_gpu_canary.py fills the
+ * workspace with a sentinel and checks that used <= reserved and that nothing outside [offset, offset + used) changed:
+ * the stand-in for compute-sanitizer, which is not available on the GPU pool. */
+SP2_API int sp2_debug_layout(sp2_handle_t handle, int index, char* name24, size_t* offset, size_t* reserved, size_t* used);
 
 /* Host-only: the static work lists of the layer kernel for n_tiles upper-triangular tiles,
  * segs_per_pass k-segments per product pass and n_clusters CTA(-pair)s.  Each item is 8 ints

@@ -9,6 +9,7 @@
 #include <cudaTypedefs.h>
 #include <cuda_runtime.h>
 #include <new>
+#include <stdio.h>
 #include <string.h>
 #include <utility>
 #include <vector>
@@ -39,11 +40,12 @@ void sp2_launch_gsetup(Sp2Ctrl* c, const Sp2BoundSlot* sz, const Sp2BoundSlot* s
 void sp2_launch_gswap(Sp2Ctrl* c, cudaStream_t s);
 void sp2_launch_split(const void* A, sp2_dtype_t dt, long ld, int N, int npad, int transpose, int which, const Sp2Ctrl* c,
                       __half* Ph, __half* Pm, cudaStream_t s);
+void sp2_launch_close(Sp2Ctrl* c, cudaStream_t s);
 void sp2_launch_lanczos(Sp2Ctrl* c, const void* H, sp2_dtype_t dt, long ld, int N, int steps, double* vecs, cudaStream_t s);
 // sp2_refine.cu
 cudaError_t sp2_refine_configure();
 int sp2_launch_refine(Sp2Ctrl* c, __half* const planes[4], int npad, int N, int n_layers, double* Xa, double* Xb,
-                      double* slots, unsigned int* ticket, const void* H, sp2_dtype_t in_dt, long ldh, void* D,
+                      double* slots, const void* H, sp2_dtype_t in_dt, long ldh, void* D,
                       sp2_dtype_t out_dt, long ldo, sp2_result_t* ring_entry, cudaStream_t s);
 
 namespace {
@@ -52,9 +54,19 @@ constexpr int kRingCap = 4096;
 constexpr int kPadTo = 256;          // npad is a multiple of the largest tile edge
 constexpr int kSimtMaxN = 4096;
 constexpr int kMaxClusters = 256;   // >= SM count of any sm_100 part
+constexpr int kSeqSlack = 8;        // extra layer launches per sequence step on top of the last finished step's count
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline int pad_n(int n) { return (int)align_up((size_t)n, kPadTo); }
+
+// One carved region of the caller's workspace.  `used` is the extent (bytes from `off`) the calls made through the
+// handle so far were entitled to write, computed from the launch geometry (NOT from the allocation formulas), so
+// that tests can check used <= reserved and that nothing outside [off, off + used) was ever written
+// (sp2_debug_layout; compute-sanitizer is not available on the GPU pool).
+struct Region {
+  char name[24];
+  size_t off, reserved, used;
+};
 
 struct Layout {
   size_t plane_bytes;     // one FP16 plane at n_max
@@ -68,14 +80,33 @@ struct Layout {
   size_t off_items, items_cap, off_item_begin, off_scratch, scratch_bytes, off_flags;
   size_t off_ctrl, off_ring;
   size_t off_staging, staging_each;
-  size_t off_refine, refine_each, off_refine_slots;
+  size_t off_refine, refine_each, off_refine_slots, refine_slots_count;
   size_t off_lanczos;
   size_t total;
+  std::vector<Region> regions;
+  int r_plane0, r_slots, r_slots2, r_bslots, r_fslots, r_tiles, r_items, r_item_begin, r_scratch, r_flags, r_ctrl, r_ring,
+      r_staging0, r_lanczos, r_refine0, r_refine_slots;
 };
+
+int add_region(Layout& L, const char* name, size_t off, size_t reserved) {
+  Region r;
+  memset(&r, 0, sizeof(r));
+  strncpy(r.name, name, sizeof(r.name) - 1);
+  r.off = off; r.reserved = reserved; r.used = 0;
+  L.regions.push_back(r);
+  return (int)L.regions.size() - 1;
+}
+
+// float64 refinement: k_refine_expand writes 2 doubles per row (npad rows), k_refine_layer 2 per upper-triangular
+// 128x128 tile, k_refine_finalise 1 per row
+size_t refine_slot_doubles(size_t npad) {
+  const size_t nb = npad / 128, grid = nb * (nb + 1) / 2;
+  return 2 * (grid > npad ? grid : npad);
+}
 
 Layout make_layout(int n_max, int flags) {
   Layout L;
-  memset(&L, 0, sizeof(L));
+  L.regions.clear();
   const size_t npad = (size_t)pad_n(n_max);
   int resp = (flags >> 8) & 15;                      // SP2_WITH_BATCH(nb)
   if (resp > SP2_MAX_BATCH) resp = SP2_MAX_BATCH;
@@ -84,42 +115,68 @@ Layout make_layout(int n_max, int flags) {
   L.plane_bytes = align_up(npad * npad * 2, 1024);
   size_t off = 0;
   L.off_planes = off; off += L.plane_bytes * (4 + 4 * (size_t)resp);
-  size_t s_tc = (size_t)sp2_layer_slots((int)npad, 1, resp, SP2_ENGINE_TCGEN05);
-  size_t s_tc2 = (size_t)sp2_layer_slots((int)npad, 2, resp, SP2_ENGINE_TCGEN05);
-  size_t s_simt = npad <= (size_t)kSimtMaxN ? (size_t)sp2_layer_slots((int)npad, 1, resp, SP2_ENGINE_SIMT_DEBUG) : 0;
+  L.r_plane0 = (int)L.regions.size();
+  for (int k = 0; k < 4 + 4 * resp; ++k) {
+    char nm[24];
+    snprintf(nm, sizeof(nm), "plane%d", k);
+    add_region(L, nm, L.off_planes + (size_t)k * L.plane_bytes, L.plane_bytes);
+  }
+  // the layer kernel writes one slot per CTA and product class (grid <= kMaxClusters CTAs); the prologue's
+  // k_rescale(H) and the SIMT scaffold use the same array with one slot per block
+  size_t s_tc = (size_t)sp2_layer_slots((int)npad, kMaxClusters, resp, SP2_ENGINE_TCGEN05);
+  size_t s_simt = npad <= (size_t)kSimtMaxN ? (size_t)sp2_layer_slots((int)npad, 0, resp, SP2_ENGINE_SIMT_DEBUG) : 0;
   size_t s_resc = (size_t)sp2_rescale_blocks((int)npad);
   L.slots_count = s_tc;
-  if (s_tc2 > L.slots_count) L.slots_count = s_tc2;
   if (s_simt > L.slots_count) L.slots_count = s_simt;
   if (s_resc > L.slots_count) L.slots_count = s_resc;
-  L.off_slots = off; off += align_up(L.slots_count * sizeof(Sp2Slot), 1024);
+  auto carve = [&](const char* name, size_t bytes, size_t* off_out) {
+    *off_out = off;
+    const size_t reserved = align_up(bytes, 1024);
+    const int id = add_region(L, name, off, reserved);
+    off += reserved;
+    return id;
+  };
+  L.r_slots = carve("slots", L.slots_count * sizeof(Sp2Slot), &L.off_slots);
   const size_t nb1 = resp > 1 ? (size_t)resp : 1;
-  L.off_slots2 = off; off += align_up(nb1 * s_resc * sizeof(Sp2Slot), 1024);
+  L.r_slots2 = carve("slots2", nb1 * s_resc * sizeof(Sp2Slot), &L.off_slots2);
   L.bslots_count = (size_t)sp2_bounds_blocks(n_max);
-  L.off_bslots = off; off += align_up((1 + nb1) * L.bslots_count * sizeof(Sp2BoundSlot), 1024);
-  L.off_fslots = off; off += align_up(3 * nb1 * (size_t)sp2_finalise_blocks(n_max) * sizeof(double), 1024);
+  L.r_bslots = carve("bslots", (1 + nb1) * L.bslots_count * sizeof(Sp2BoundSlot), &L.off_bslots);
+  L.r_fslots = carve("fslots", 3 * nb1 * (size_t)sp2_finalise_blocks(n_max) * sizeof(double), &L.off_fslots);
   const size_t nt1 = npad / 128;
   L.tiles_count = nt1 * nt1;                 // the congruence products use every tile, the layers the upper triangle
-  L.off_tiles = off; off += align_up(L.tiles_count * sizeof(int2), 1024);
+  L.r_tiles = carve("tiles", L.tiles_count * sizeof(int2), &L.off_tiles);
   L.items_cap = (1 + nb1) * L.tiles_count + 1024;
-  L.off_items = off; off += align_up(L.items_cap * sizeof(Sp2Item), 1024);
-  L.off_item_begin = off; off += align_up((kMaxClusters + 1) * sizeof(int), 1024);
+  L.r_items = carve("items", L.items_cap * sizeof(Sp2Item), &L.off_items);
+  L.r_item_begin = carve("item_begin", (kMaxClusters + 1) * sizeof(int), &L.off_item_begin);
   L.scratch_bytes = 2 * (size_t)kMaxClusters * sp2_layer_scratch_slot_bytes(1);
   if (2 * (size_t)(kMaxClusters / 2) * sp2_layer_scratch_slot_bytes(2) > L.scratch_bytes)
     L.scratch_bytes = 2 * (size_t)(kMaxClusters / 2) * sp2_layer_scratch_slot_bytes(2);
-  L.off_scratch = off; off += align_up(L.scratch_bytes, 1024);
-  L.off_flags = off; off += align_up(2 * kMaxClusters * sizeof(unsigned int), 1024);
-  L.off_ctrl = off; off += align_up(sizeof(Sp2Ctrl), 1024);
-  L.off_ring = off; off += align_up((size_t)kRingCap * sizeof(sp2_result_t), 1024);
+  L.r_scratch = carve("scratch", L.scratch_bytes, &L.off_scratch);
+  L.r_flags = carve("flags", 2 * kMaxClusters * sizeof(unsigned int), &L.off_flags);
+  L.r_ctrl = carve("ctrl", sizeof(Sp2Ctrl), &L.off_ctrl);
+  L.r_ring = carve("ring", (size_t)kRingCap * sizeof(sp2_result_t), &L.off_ring);
+  L.r_staging0 = -1; L.staging_each = 0; L.off_staging = 0;
   if (flags & SP2_WITH_HOST_STAGING) {
     L.staging_each = align_up((size_t)n_max * (size_t)n_max * 8, 1024);
-    L.off_staging = off; off += L.staging_each * (resp ? 4 : 2);
+    L.off_staging = off;
+    L.r_staging0 = (int)L.regions.size();
+    for (int k = 0; k < (resp ? 4 : 2); ++k) {
+      char nm[24];
+      snprintf(nm, sizeof(nm), "staging%d", k);
+      add_region(L, nm, off, L.staging_each);
+      off += L.staging_each;
+    }
   }
-  L.off_lanczos = off; off += align_up(3 * (size_t)n_max * sizeof(double), 1024);
+  L.r_lanczos = carve("lanczos", 3 * (size_t)n_max * sizeof(double), &L.off_lanczos);
+  L.r_refine0 = -1; L.r_refine_slots = -1; L.refine_each = 0; L.off_refine = 0; L.off_refine_slots = 0;
+  L.refine_slots_count = 0;
   if (flags & SP2_WITH_REFINEMENT) {
     L.refine_each = align_up(npad * npad * sizeof(double), 1024);
-    L.off_refine = off; off += 2 * L.refine_each;
-    L.off_refine_slots = off; off += align_up((2 * npad + 64) * sizeof(double), 1024);
+    L.off_refine = off;
+    L.r_refine0 = add_region(L, "refine0", off, L.refine_each); off += L.refine_each;
+    add_region(L, "refine1", off, L.refine_each); off += L.refine_each;
+    L.refine_slots_count = refine_slot_doubles(npad);
+    L.r_refine_slots = carve("refine_slots", L.refine_slots_count * sizeof(double), &L.off_refine_slots);
   }
   L.total = off;
   return L;
@@ -149,6 +206,7 @@ struct sp2_handle_s {
   std::vector<Sp2Item> items_host;
   std::vector<int> item_begin_host;
   int n_flags, n_clusters;
+  int max_clusters[3];           // co-resident CTAs (cta_group 1) / CTA pairs (cta_group 2) of the layer kernel on this device
   cudaEvent_t ev0, ev1, evl0, evl1;
   int time_layers;               // record evl0/evl1 around the layer launches of the next solve
   sp2_result_t* h_result;        // pinned
@@ -157,6 +215,7 @@ struct sp2_handle_s {
   unsigned long long launches;
   // sequence state
   int seq_active, seq_N, seq_nocc, seq_steps;
+  cudaEvent_t seq_ev[2];         // "step t finished" markers, polled (never waited on) by later steps
   double seq_tol;
   cudaStream_t seq_stream;
 
@@ -179,7 +238,14 @@ struct sp2_handle_s {
   double* lanczos_vecs() const { return reinterpret_cast<double*>(ws + L.off_lanczos); }
   double* refine_x(int i) const { return reinterpret_cast<double*>(ws + L.off_refine + (size_t)i * L.refine_each); }
   double* refine_slots() const { return reinterpret_cast<double*>(ws + L.off_refine_slots); }
-  unsigned int* refine_ticket() const { return reinterpret_cast<unsigned int*>(refine_slots() + 2 * (size_t)pad_n(n_max) + 32); }
+  // bookkeeping for sp2_debug_layout: this call may write [off, off + bytes) of region `id`
+  void touch(int id, size_t bytes) {
+    if (id >= 0 && id < (int)L.regions.size() && bytes > L.regions[id].used) L.regions[id].used = bytes;
+  }
+  void touch_plane(int which, int buf, size_t npad) {
+    const int idx = (which < 2) ? (buf * 2 + which) : (4 + 4 * ((which - 2) >> 1) + buf * 2 + (which & 1));
+    touch(L.r_plane0 + idx, npad * npad * 2);
+  }
 };
 
 namespace {
@@ -304,6 +370,15 @@ int pick_cta_group(sp2_handle_t h, int npad, int resp) {
   return npad >= (resp ? 4608 : 5632) ? 2 : 1;
 }
 
+// CTA(-pair)s of one layer launch: one per SM (pair of SMs), bounded by what the device can keep co-resident
+// (sp2_create queried it): the split-k owners of the last wave wait for contributors, which must be running.
+int layer_clusters(sp2_handle_t h, int cg) {
+  int nC = h->num_sms / cg;
+  if (nC > h->max_clusters[cg]) nC = h->max_clusters[cg];
+  if (nC > kMaxClusters / cg) nC = kMaxClusters / cg;
+  return nC < 1 ? 1 : nC;
+}
+
 // (re)build the per-problem launch state: tile list, TMA descriptors, ping-pong argument blocks
 sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   const int npad = pad_n(N);
@@ -321,16 +396,21 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   build_tiles(nt, h->tiles_host);
   SP2_CUDA(h, cudaMemcpyAsync(h->tiles(), h->tiles_host.data(), h->tiles_host.size() * sizeof(int2),
                               cudaMemcpyHostToDevice, s));
-  int nC = h->num_sms / cg;
-  if (nC > kMaxClusters / cg) nC = kMaxClusters / cg;
+  const int nC = layer_clusters(h, cg);
   // (fewer units than CTA(-pair)s is fine: the schedule splits them along k, every SM gets work)
   int n_slots = 0;
   build_schedule((int)h->tiles_host.size(), resp, (npad / 64) / seg, nC, h->items_host, h->item_begin_host,
                  &h->n_flags, &n_slots);
   h->n_clusters = nC;
-  if (h->items_host.size() > h->L.items_cap || (size_t)n_slots * sp2_layer_scratch_slot_bytes(cg) > h->L.scratch_bytes ||
-      h->n_flags > 2 * kMaxClusters)
+  if (h->items_host.size() > h->L.items_cap || h->tiles_host.size() > h->L.tiles_count ||
+      (size_t)n_slots * sp2_layer_scratch_slot_bytes(cg) > h->L.scratch_bytes || h->n_flags > 2 * kMaxClusters ||
+      (size_t)sp2_layer_slots(npad, cg * nC, resp, SP2_ENGINE_TCGEN05) > h->L.slots_count)
     return SP2_ERR_WORKSPACE;
+  h->touch(h->L.r_tiles, h->tiles_host.size() * sizeof(int2));
+  h->touch(h->L.r_items, h->items_host.size() * sizeof(Sp2Item));
+  h->touch(h->L.r_item_begin, h->item_begin_host.size() * sizeof(int));
+  h->touch(h->L.r_flags, 2 * kMaxClusters * sizeof(unsigned int));
+  h->touch(h->L.r_scratch, (size_t)n_slots * sp2_layer_scratch_slot_bytes(cg));
   SP2_CUDA(h, cudaMemcpyAsync(h->items(), h->items_host.data(), h->items_host.size() * sizeof(Sp2Item),
                               cudaMemcpyHostToDevice, s));
   SP2_CUDA(h, cudaMemcpyAsync(h->item_begin(), h->item_begin_host.data(), h->item_begin_host.size() * sizeof(int),
@@ -415,7 +495,7 @@ sp2_status_t enqueue_finalise(sp2_handle_t h, const void* H, sp2_dtype_t in_dt, 
   if (nref > 0) {   // float64 refinement layers on the converged iterate; overwrites D, tr D, tr(DH)
     __half* yp[4] = {h->plane(0, 0), h->plane(1, 0), h->plane(0, 1), h->plane(1, 1)};
     const int k = sp2_launch_refine(h->ctrl(), yp, h->cur_npad, N, nref, h->refine_x(0), h->refine_x(1), h->refine_slots(),
-                                    h->refine_ticket(), H, in_dt, ldh, D, out_dt, ldd, h->ring() + ring_idx, s);
+                                    H, in_dt, ldh, D, out_dt, ldd, h->ring() + ring_idx, s);
     *launches += k;
   }
   return SP2_OK;
@@ -431,7 +511,7 @@ int effective_max_layers(const sp2_options_t& o) {
 // k_finalise_reduce then reports SP2_INTERNAL_INCOMPLETE).
 sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dtype_t in_dt, long ldh, int N, int N_occ,
                            double tol, void* D, sp2_dtype_t out_dt, long ldd, int ring_idx, cudaStream_t s,
-                           int n_layers, int* launches_out) {
+                           int n_layers, int* launches_out, bool close_if_incomplete = false) {
   const int resp = P.nb;
   sp2_status_t st = prepare(h, N, resp, s);
   if (st != SP2_OK) return st;
@@ -441,6 +521,27 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dty
   const int forced = o.forced_layers > 0 ? max_layers : 0;
   int launches = 0;
   Sp2Ctrl* c = h->ctrl();
+  {   // what this solve may write (sp2_debug_layout)
+    const bool trivial = (N_occ == 0 || N_occ == N);
+    const size_t nbb = (size_t)sp2_bounds_blocks(N);
+    h->touch(h->L.r_ctrl, sizeof(Sp2Ctrl));
+    h->touch(h->L.r_ring, (size_t)(ring_idx + 1) * sizeof(sp2_result_t));
+    h->touch(h->L.r_bslots, (resp ? h->L.bslots_count + (size_t)resp * nbb : nbb) * sizeof(Sp2BoundSlot));
+    if (o.lanczos_steps > 0) h->touch(h->L.r_lanczos, 3 * (size_t)N * sizeof(double));
+    if (!trivial) {
+      const size_t s_resc = (size_t)sp2_rescale_blocks(npad);
+      size_t s_layer = (size_t)sp2_layer_slots(npad, h->cur_cg * h->n_clusters, resp, o.engine);
+      h->touch(h->L.r_slots, (s_layer > s_resc ? s_layer : s_resc) * sizeof(Sp2Slot));
+      if (resp) h->touch(h->L.r_slots2, (size_t)resp * s_resc * sizeof(Sp2Slot));
+      h->touch(h->L.r_fslots, 3 * (size_t)(resp > 1 ? resp : 1) * (size_t)sp2_finalise_blocks(N) * sizeof(double));
+      for (int w = 0; w < 2 + 2 * resp; ++w) { h->touch_plane(w, 0, (size_t)npad); h->touch_plane(w, 1, (size_t)npad); }
+      if (o.refine_layers > 0 && h->L.r_refine0 >= 0) {
+        h->touch(h->L.r_refine0, (size_t)npad * npad * sizeof(double));
+        h->touch(h->L.r_refine0 + 1, (size_t)npad * npad * sizeof(double));
+        h->touch(h->L.r_refine_slots, refine_slot_doubles((size_t)npad) * sizeof(double));
+      }
+    }
+  }
   sp2_launch_init(c, N, N_occ, npad, resp, max_layers, o.user_bounds, o.eps_min, o.eps_max, tol, forced, o.forced_signs, o.no_recentre, s);
   ++launches;
   sp2_launch_bounds(H, in_dt, ldh, N, 0, h->bslots(0), s); ++launches;
@@ -471,6 +572,9 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dty
     st = enqueue_layers(h, 0, n_layers, s, &launches);
     if (st != SP2_OK) return st;
     if (h->time_layers) SP2_CUDA(h, cudaEventRecord(h->evl1, s));
+    // no top-up is possible without a host round trip (sequence call): an unfinished stack is closed as
+    // "not converged, launch budget exhausted" and D is written from the iterate reached
+    if (close_if_incomplete && n_layers < max_layers) { sp2_launch_close(c, s); ++launches; }
     enqueue_finalise(h, H, in_dt, ldh, N, P, D, out_dt, ldd, ring_idx, s, &launches);
   }
   cudaError_t e = cudaGetLastError();
@@ -501,6 +605,9 @@ sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dt
     if (!(h->flags & SP2_WITH_HOST_STAGING)) return SP2_ERR_WORKSPACE;
     dH = h->staging(0); dD = h->staging(1);
     dld_in = N; dld_out = N;
+    h->touch(h->L.r_staging0, (size_t)N * N * in_sz);
+    h->touch(h->L.r_staging0 + 1, (size_t)N * N * out_sz);
+    if (want_resp) { h->touch(h->L.r_staging0 + 2, (size_t)N * N * in_sz); h->touch(h->L.r_staging0 + 3, (size_t)N * N * out_sz); }
     SP2_CUDA(h, cudaMemcpy2DAsync(h->staging(0), (size_t)N * in_sz, H, (size_t)ldh * in_sz, (size_t)N * in_sz, N,
                                   cudaMemcpyHostToDevice, s));
     if (want_resp) {
@@ -599,13 +706,22 @@ sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_work
   if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) { delete h; return SP2_ERR_CUDA; }
   h->encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(fn);
   if (sp2_layer_configure() != cudaSuccess || sp2_refine_configure() != cudaSuccess) { delete h; return SP2_ERR_CUDA; }
+  // The layer kernel is persistent and its last-wave units hand partial sums between CTAs, so every CTA(-pair) of a
+  // launch must be able to run at once: size the grid by what the device can keep co-resident, fail here (not
+  // with a device-side trap later) if the kernel does not fit at all.
+  h->max_clusters[0] = 0;
+  for (int cg = 1; cg <= 2; ++cg) {
+    cudaError_t oe = sp2_layer_max_coresident(cg, h->num_sms, &h->max_clusters[cg]);
+    if (oe != cudaSuccess || h->max_clusters[cg] < 1) { h->last_cuda_error = (int)oe; delete h; return SP2_ERR_CUDA; }
+  }
   if (cudaEventCreate(&h->ev0) != cudaSuccess || cudaEventCreate(&h->ev1) != cudaSuccess ||
-      cudaEventCreate(&h->evl0) != cudaSuccess || cudaEventCreate(&h->evl1) != cudaSuccess) { delete h; return SP2_ERR_CUDA; }
+      cudaEventCreate(&h->evl0) != cudaSuccess || cudaEventCreate(&h->evl1) != cudaSuccess ||
+      cudaEventCreateWithFlags(&h->seq_ev[0], cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&h->seq_ev[1], cudaEventDisableTiming) != cudaSuccess) { delete h; return SP2_ERR_CUDA; }
   h->time_layers = 0;
   if (cudaMallocHost(reinterpret_cast<void**>(&h->h_result), sizeof(sp2_result_t) * kRingCap) != cudaSuccess) {
     delete h; return SP2_ERR_CUDA;
   }
-  if (flags & SP2_WITH_REFINEMENT) cudaMemset(h->refine_slots(), 0, (2 * (size_t)pad_n(n_max) + 64) * sizeof(double));
   *handle = h;
   return SP2_OK;
 }
@@ -616,6 +732,8 @@ sp2_status_t sp2_destroy(sp2_handle_t h) {
   cudaEventDestroy(h->ev1);
   cudaEventDestroy(h->evl0);
   cudaEventDestroy(h->evl1);
+  cudaEventDestroy(h->seq_ev[0]);
+  cudaEventDestroy(h->seq_ev[1]);
   cudaFreeHost(h->h_result);
   delete h;
   return SP2_OK;
@@ -699,10 +817,30 @@ sp2_status_t sp2_sequence_step(sp2_handle_t h, const void* dH_t, sp2_dtype_t in_
   const Pert none = make_pert(nullptr, nullptr);
   sp2_status_t st = check_args(h, dH_t, none, in_dtype, ldh, h->seq_N, h->seq_nocc, dD_t, out_dtype, ldd);
   if (st != SP2_OK) return st;
+  // Layer launches per step: what the last FINISHED solve of this shape needed, plus slack (consecutive MD-step
+  // Hamiltonians differ little), instead of max_layers launches of which most exit at once.  The hint
+  // comes from a blocking call before begin, or from this sequence's own earlier steps: each step leaves an event
+  // and a copy of its result in pinned memory, polled here WITHOUT waiting.
+  const int max_layers = effective_max_layers(h->opt);
+  for (int back = 1; back <= 2 && back <= h->seq_steps; ++back) {   // the two youngest steps still own their events
+    const int i = h->seq_steps - back;
+    if (cudaEventQuery(h->seq_ev[i & 1]) == cudaSuccess) {
+      const sp2_result_t& r = h->h_result[i];
+      if (r.status == SP2_OK && r.layers > 0) h->layers_hint = r.layers + kSeqSlack;
+      break;
+    }
+  }
+  (void)cudaGetLastError();                                         // "not ready" is not an error
+  int n_layers = max_layers;
+  if (h->opt.forced_layers <= 0 && h->layers_hint > 0 && h->layers_hint < max_layers) n_layers = h->layers_hint;
   st = enqueue_solve(h, dH_t, none, in_dtype, ldh, h->seq_N, h->seq_nocc, h->seq_tol, dD_t, out_dtype, ldd,
-                     h->seq_steps, h->seq_stream, effective_max_layers(h->opt), nullptr);
-  if (st == SP2_OK) ++h->seq_steps;
-  return st;
+                     h->seq_steps, h->seq_stream, n_layers, nullptr, true);
+  if (st != SP2_OK) return st;
+  SP2_CUDA(h, cudaMemcpyAsync(h->h_result + h->seq_steps, h->ring() + h->seq_steps, sizeof(sp2_result_t),
+                              cudaMemcpyDeviceToHost, h->seq_stream));
+  SP2_CUDA(h, cudaEventRecord(h->seq_ev[h->seq_steps & 1], h->seq_stream));
+  ++h->seq_steps;
+  return SP2_OK;
 }
 
 sp2_status_t sp2_sequence_end(sp2_handle_t h, sp2_result_t* results, int* n_steps) {
@@ -718,6 +856,7 @@ sp2_status_t sp2_sequence_end(sp2_handle_t h, sp2_result_t* results, int* n_step
   for (int i = 0; i < n; ++i) {
     if (results) results[i] = h->h_result[i];
     if (h->h_result[i].status != SP2_OK && worst == SP2_OK) worst = (sp2_status_t)h->h_result[i].status;
+    if (h->h_result[i].status == SP2_OK && h->h_result[i].layers > 0) h->layers_hint = h->h_result[i].layers + kSeqSlack;
   }
   return worst;
 }
@@ -741,8 +880,7 @@ sp2_status_t sp2_congruence(sp2_handle_t h, const void* dZ, const void* dX, sp2_
         for (int ti = gi; ti < gi + G && ti < nt; ++ti) h->tiles_host.push_back(make_int2(ti, tj));
   int seg = 4;
   while ((npad / 64) % seg) seg >>= 1;
-  int nC = h->num_sms / cg;
-  if (nC > kMaxClusters / cg) nC = kMaxClusters / cg;
+  const int nC = layer_clusters(h, cg);
   int n_slots = 0;
   build_schedule((int)h->tiles_host.size(), 0, (npad / 64) / seg, nC, h->items_host, h->item_begin_host, &h->n_flags, &n_slots);
   h->n_clusters = nC;
@@ -750,6 +888,16 @@ sp2_status_t sp2_congruence(sp2_handle_t h, const void* dZ, const void* dX, sp2_
   if (h->items_host.size() > h->L.items_cap || h->tiles_host.size() > h->L.tiles_count ||
       (size_t)n_slots * sp2_layer_scratch_slot_bytes(cg) > h->L.scratch_bytes || h->n_flags > 2 * kMaxClusters)
     return SP2_ERR_WORKSPACE;
+  h->touch(h->L.r_tiles, h->tiles_host.size() * sizeof(int2));
+  h->touch(h->L.r_items, h->items_host.size() * sizeof(Sp2Item));
+  h->touch(h->L.r_item_begin, h->item_begin_host.size() * sizeof(int));
+  h->touch(h->L.r_flags, 2 * kMaxClusters * sizeof(unsigned int));
+  h->touch(h->L.r_scratch, (size_t)n_slots * sp2_layer_scratch_slot_bytes(cg));
+  h->touch(h->L.r_ctrl, sizeof(Sp2Ctrl));
+  h->touch(h->L.r_ring, sizeof(sp2_result_t));
+  h->touch(h->L.r_bslots, (h->L.bslots_count + (size_t)sp2_bounds_blocks(N)) * sizeof(Sp2BoundSlot));
+  for (int w = 0; w < 4; ++w) h->touch_plane(w, 0, (size_t)npad);
+  h->touch_plane(2, 1, (size_t)npad); h->touch_plane(3, 1, (size_t)npad);
   SP2_CUDA(h, cudaMemcpyAsync(h->tiles(), h->tiles_host.data(), h->tiles_host.size() * sizeof(int2), cudaMemcpyHostToDevice, s));
   SP2_CUDA(h, cudaMemcpyAsync(h->items(), h->items_host.data(), h->items_host.size() * sizeof(Sp2Item), cudaMemcpyHostToDevice, s));
   SP2_CUDA(h, cudaMemcpyAsync(h->item_begin(), h->item_begin_host.data(), h->item_begin_host.size() * sizeof(int),
@@ -827,7 +975,7 @@ int sp2_debug_schedule(int n_tiles, int with_response, int segs_per_pass, int n_
 
 int sp2_debug_history(sp2_handle_t h, double* tr_x, double* e, int capacity) {
   if (!h) return -1;
-  static Sp2Ctrl host_ctrl;
+  Sp2Ctrl host_ctrl;
   if (cudaMemcpy(&host_ctrl, h->ctrl(), sizeof(Sp2Ctrl), cudaMemcpyDeviceToHost) != cudaSuccess) return -1;
   int cnt = host_ctrl.n + 1;
   if (cnt > SP2_LAYER_CAP) cnt = SP2_LAYER_CAP;
@@ -843,7 +991,7 @@ sp2_status_t sp2_debug_plane(sp2_handle_t h, int which, size_t* offset, long* pi
   const int prev = which >> 2;      // 4..7: the same planes of the PREVIOUS iterate (other ping-pong buffer)
   which &= 3;
   if (which >= 2 && !(h->flags & SP2_WITH_RESPONSE)) return SP2_ERR_INVALID_ARG;
-  static Sp2Ctrl host_ctrl;
+  Sp2Ctrl host_ctrl;
   if (cudaMemcpy(&host_ctrl, h->ctrl(), sizeof(Sp2Ctrl), cudaMemcpyDeviceToHost) != cudaSuccess) return SP2_ERR_CUDA;
   const int buf = (host_ctrl.n & 1) ^ prev;
   if (offset) *offset = (size_t)(reinterpret_cast<uint8_t*>(h->plane(which, buf)) - h->ws);
@@ -851,6 +999,18 @@ sp2_status_t sp2_debug_plane(sp2_handle_t h, int which, size_t* offset, long* pi
   if (exponent) *exponent = which < 2 ? host_ctrl.t : host_ctrl.u[0];
   if (shift) *shift = host_ctrl.c;
   return SP2_OK;
+}
+
+int sp2_debug_layout(sp2_handle_t h, int index, char* name24, size_t* offset, size_t* reserved, size_t* used) {
+  if (!h) return -1;
+  const int n = (int)h->L.regions.size();
+  if (index < 0 || index >= n) return n;
+  const Region& r = h->L.regions[index];
+  if (name24) memcpy(name24, r.name, sizeof(r.name));
+  if (offset) *offset = r.off;
+  if (reserved) *reserved = r.reserved;
+  if (used) *used = r.used;
+  return n;
 }
 
 }  // extern "C"

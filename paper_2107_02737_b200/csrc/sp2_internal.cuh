@@ -76,6 +76,8 @@ struct Sp2Ctrl {
   // float64 refinement layers (sp2_refine.cu)
   double ref_tr, ref_fro;   // tr X and ||X||_F^2 of the current float64 iterate
   int ref_plus, ref_done;   // branch of the next refinement layer; layers applied
+  unsigned int ref_ticket;  // last-block election of the refinement layer kernel (zero between launches)
+  int ref_pad;
 };
 
 // ----------------------------------------------------------------------------------------------

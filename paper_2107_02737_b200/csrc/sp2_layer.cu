@@ -794,13 +794,15 @@ int sp2_layer_box_k() { return kBK; }
 
 size_t sp2_layer_smem_bytes() { return (size_t)kStages * kStageBytes + sizeof(SmemBarriers) + 1024; }
 
-int sp2_layer_slots(int npad, int cta_group, int with_response, int engine) {
+// Partial-sum slots one layer launch writes: the tcgen05 engine writes ONE slot per CTA and product class at
+// class * gridDim.x + blockIdx.x (k_layer_tc, end of the kernel), so it needs (1 + nb) * grid_ctas; the SIMT
+// scaffold writes one per 16x16 block and class.
+int sp2_layer_slots(int npad, int grid_ctas, int with_response, int engine) {
   if (engine == SP2_ENGINE_SIMT_DEBUG) {
     const int nb = npad / 16;
     return nb * (nb + 1) / 2 * (1 + with_response);
   }
-  const int nt = npad / (128 * cta_group);
-  return nt * (nt + 1) / 2 * cta_group * kConsumerWarps * (1 + with_response);
+  return grid_ctas * (1 + with_response);
 }
 
 cudaError_t sp2_layer_configure() {
@@ -809,6 +811,27 @@ cudaError_t sp2_layer_configure() {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_layer_tc<2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_layer_tc<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_layer_tc<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  return e;
+}
+
+// CTAs (cta_group 1) or CTA pairs (cta_group 2) of the layer kernel the current device can keep resident at once
+// (static resources only: registers, 200 KB of shared memory, cluster placement inside the GPCs).
+cudaError_t sp2_layer_max_coresident(int cta_group, int num_sms, int* out) {
+  *out = 0;
+  if (cta_group == 2) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.blockDim = dim3(kThreads);
+    cfg.gridDim = dim3(2 * (num_sms / 2));
+    cfg.dynamicSmemBytes = sp2_layer_smem_bytes();
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaOccupancyMaxActiveClusters(out, k_layer_tc<2, 0>, &cfg);
+  }
+  int per_sm = 0;
+  cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_layer_tc<1, 0>, kThreads, sp2_layer_smem_bytes());
+  *out = per_sm * num_sms;
   return e;
 }
 

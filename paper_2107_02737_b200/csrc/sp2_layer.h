@@ -46,7 +46,8 @@ struct alignas(64) Sp2LayerArgs {
 
 size_t sp2_layer_smem_bytes();
 int sp2_layer_box_k();   // k extent of the TMA box (32: SWIZZLE_64B, 64: SWIZZLE_128B)
-int sp2_layer_slots(int npad, int cta_group, int with_response, int engine);
+int sp2_layer_slots(int npad, int grid_ctas, int with_response, int engine);   // Sp2Slot entries one launch writes
 cudaError_t sp2_layer_configure();
+cudaError_t sp2_layer_max_coresident(int cta_group, int num_sms, int* out);
 cudaError_t sp2_launch_layer(const Sp2LayerArgs& args, int engine, int cta_group, cudaStream_t s);
 size_t sp2_layer_scratch_slot_bytes(int cta_group);

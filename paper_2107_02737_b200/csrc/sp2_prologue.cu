@@ -551,6 +551,13 @@ __global__ void __launch_bounds__(256) k_trivial(Sp2Ctrl* c, TO* __restrict__ D,
   }
 }
 
+// Sequence steps enqueue a bounded number of layer launches and cannot top up without a host round trip: a stack
+// that has not stopped by then is closed here (D is written from the iterate reached, as for max_layers).
+__global__ void k_close(Sp2Ctrl* c) {
+  if (c->done) return;
+  c->done = 1; c->status = SP2_WARN_NOT_CONVERGED; c->stop_reason = 7;
+}
+
 __global__ void k_init(Sp2Ctrl* c, int N, int n_occ, int npad, int with_response, int max_layers,
                        int user_bounds, double eps_min, double eps_max, double tol,
                        int forced_layers, unsigned long long forced_signs, int no_recentre) {
@@ -576,6 +583,8 @@ void sp2_launch_init(Sp2Ctrl* c, int N, int n_occ, int npad, int with_response, 
   k_init<<<1, 1, 0, s>>>(c, N, n_occ, npad, with_response, max_layers, user_bounds, eps_min, eps_max, tol,
                          forced_layers, forced_signs, no_recentre);
 }
+
+void sp2_launch_close(Sp2Ctrl* c, cudaStream_t s) { k_close<<<1, 1, 0, s>>>(c); }
 
 int sp2_bounds_blocks(int N) { return (N + 7) / 8; }
 

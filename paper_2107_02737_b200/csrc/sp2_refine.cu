@@ -244,7 +244,7 @@ cudaError_t sp2_refine_configure() {
 
 // enqueue expand + n_layers float64 layers + finalise; returns the number of kernels launched
 int sp2_launch_refine(Sp2Ctrl* c, __half* const planes[4] /* Yh0, Ym0, Yh1, Ym1 */, int npad, int N, int n_layers,
-                      double* Xa, double* Xb, double* slots, unsigned int* ticket, const void* H, sp2_dtype_t in_dt, long ldh,
+                      double* Xa, double* Xb, double* slots, const void* H, sp2_dtype_t in_dt, long ldh,
                       void* D, sp2_dtype_t out_dt, long ldo, sp2_result_t* ring_entry, cudaStream_t s) {
   int launches = 0;
   k_refine_expand<<<npad, 256, 0, s>>>(c, planes[0], planes[1], planes[2], planes[3], npad, Xa, slots); ++launches;
@@ -253,7 +253,7 @@ int sp2_launch_refine(Sp2Ctrl* c, __half* const planes[4] /* Yh0, Ym0, Yh1, Ym1 
   const int grid = nb * (nb + 1) / 2;
   double* in = Xa; double* out = Xb;
   for (int r = 0; r < n_layers; ++r) {
-    k_refine_layer<<<grid, 256, sp2_refine_smem_bytes(), s>>>(c, in, out, npad, slots, ticket); ++launches;
+    k_refine_layer<<<grid, 256, sp2_refine_smem_bytes(), s>>>(c, in, out, npad, slots, &c->ref_ticket); ++launches;
     double* t = in; in = out; out = t;
   }
 #define SP2_RFIN(TI, TO) k_refine_finalise<TI, TO><<<N, 256, 0, s>>>(c, in, npad, (const TI*)H, ldh, (TO*)D, ldo, slots)

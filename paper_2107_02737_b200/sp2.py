@@ -43,7 +43,7 @@ EXPORTS = [
     "sp2_density", "sp2_response", "sp2_response_batch", "sp2_density_host", "sp2_response_host",
     "sp2_sequence_begin", "sp2_sequence_step", "sp2_sequence_end", "sp2_congruence",
     "sp2_status_string", "sp2_last_cuda_error", "sp2_launch_count",
-    "sp2_debug_history", "sp2_debug_plane", "sp2_debug_schedule",
+    "sp2_debug_history", "sp2_debug_plane", "sp2_debug_schedule", "sp2_debug_layout",
 ]
 
 
@@ -127,6 +127,8 @@ def _load():
     lib.sp2_debug_history.argtypes = [vp, C.POINTER(d), C.POINTER(d), i]
     lib.sp2_debug_plane.restype = i
     lib.sp2_debug_plane.argtypes = [vp, i, C.POINTER(sz), C.POINTER(l), C.POINTER(i), C.POINTER(d)]
+    lib.sp2_debug_layout.restype = i
+    lib.sp2_debug_layout.argtypes = [vp, i, C.c_char_p, C.POINTER(sz), C.POINTER(sz), C.POINTER(sz)]
     lib.sp2_debug_schedule.restype = i
     lib.sp2_debug_schedule.argtypes = [i, i, i, i, C.POINTER(i), i, C.POINTER(i)]
     return lib
@@ -177,8 +179,12 @@ def _np_dtype_code(a):
 class Sp2Handle:
     """sp2_create / sp2_destroy over a torch-owned workspace on the current CUDA device."""
 
+    GUARD = 4096   # bytes either side of the workspace when a sentinel is asked for (tests)
+
     def __init__(self, n_max: int, response: bool = False, host_staging: bool = False, device=None,
-                 refinement: bool = False, batch: int = 0):
+                 refinement: bool = False, batch: int = 0, sentinel: int | None = None):
+        """sentinel (tests only): fill the workspace and a guard band either side of it with this byte BEFORE
+        sp2_create, so that ``debug_layout`` / ``check_canary`` can tell which bytes the library ever wrote."""
         import torch
 
         if not torch.cuda.is_available():
@@ -188,11 +194,16 @@ class Sp2Handle:
                       | (SP2_WITH_REFINEMENT if refinement else 0) | (SP2_WITH_BATCH(batch) if batch else 0))
         self.n_max = int(n_max)
         nbytes = workspace_bytes(self.n_max, self.flags)
+        self.sentinel = sentinel
+        guard = self.GUARD if sentinel is not None else 0
         with torch.cuda.device(self.device):
-            self.workspace = torch.empty(nbytes + 1024, dtype=torch.uint8, device=self.device)
+            self.workspace = torch.empty(nbytes + 1024 + 2 * guard, dtype=torch.uint8, device=self.device)
+            if sentinel is not None:
+                self.workspace.fill_(int(sentinel))
             base = self.workspace.data_ptr()
-            self._ws_ptr = (base + 1023) // 1024 * 1024
+            self._ws_ptr = (base + guard + 1023) // 1024 * 1024
             self._ws_off = self._ws_ptr - base
+            self._ws_bytes = nbytes
             h = C.c_void_p()
             st = lib.sp2_create(C.byref(h), self.n_max, self.flags, C.c_void_p(self._ws_ptr), nbytes)
         if st != SP2_OK:
@@ -394,6 +405,46 @@ class Sp2Handle:
         return out
 
     # ------------------------------------------------------------------ test hooks
+    def debug_layout(self):
+        """sp2_debug_layout: list of dicts name / offset / reserved / used (bytes) of the workspace regions."""
+        n = lib.sp2_debug_layout(self._h, -1, None, None, None, None)
+        out = []
+        for k in range(n):
+            name = C.create_string_buffer(24)
+            off, res, used = C.c_size_t(0), C.c_size_t(0), C.c_size_t(0)
+            lib.sp2_debug_layout(self._h, k, name, C.byref(off), C.byref(res), C.byref(used))
+            out.append(dict(name=name.value.decode(), offset=off.value, reserved=res.value, used=used.value))
+        return out
+
+    def check_canary(self):
+        """With a sentinel-filled workspace: every region's used extent fits its reservation, and every byte the
+        calls so far were NOT entitled to write (tails of the regions, padding between them, both guard bands)
+        still holds the sentinel.  Returns the list of violations (empty = clean)."""
+        import torch
+
+        assert self.sentinel is not None, "create the handle with sentinel=<byte>"
+        torch.cuda.synchronize(self.device)
+        bad = []
+        ws = self.workspace
+        regions = sorted(self.debug_layout(), key=lambda r: r["offset"])
+
+        def intact(lo, hi, what):     # [lo, hi) relative to the tensor start
+            if hi > lo and not bool((ws[lo:hi] == self.sentinel).all()):
+                first = int((ws[lo:hi] != self.sentinel).nonzero()[0]) + lo
+                bad.append(f"{what}: byte {first - self._ws_off} of the workspace was written")
+
+        intact(0, self._ws_off, "guard band before the workspace")
+        cursor = 0
+        for r in regions:
+            if r["used"] > r["reserved"]:
+                bad.append(f"{r['name']}: used {r['used']} > reserved {r['reserved']}")
+            intact(self._ws_off + cursor, self._ws_off + r["offset"], f"gap before {r['name']}")
+            intact(self._ws_off + r["offset"] + min(r["used"], r["reserved"]), self._ws_off + r["offset"] + r["reserved"],
+                   f"tail of {r['name']}")
+            cursor = r["offset"] + r["reserved"]
+        intact(self._ws_off + cursor, ws.numel(), "after the last region")
+        return bad
+
     def debug_history(self):
         tr = (C.c_double * 128)()
         e = (C.c_double * 128)()
