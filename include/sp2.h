@@ -59,7 +59,11 @@ typedef enum {
   SP2_ERR_ARCH = 4,          /* device is not sm_100 */
   SP2_ERR_NONFINITE = 5,     /* H (or H1) holds NaN/Inf, or the iterate became non-finite */
   SP2_ERR_DEGENERATE = 6,    /* eps_max == eps_min (H = c*I): no spectral width to rescale */
-  SP2_WARN_NOT_CONVERGED = 7 /* max_layers reached; D (and D1) are still written */
+  SP2_WARN_NOT_CONVERGED = 7, /* max_layers reached; D (and D1) are still written */
+  SP2_ERR_BOUNDS = 8         /* an eigenvalue of X left [0,1]: the spectral bounds (user_bounds, or a Lanczos estimate in a
+                                sequence step) do not enclose the spectrum of H; detected on the device from
+                                tr X - tr X^2 < 0 far from convergence; D is not written.  The blocking calls re-run a
+                                solve whose LANCZOS bounds fail this check with Gershgorin discs (result.bounds_fallback) */
 } sp2_status_t;
 
 typedef enum { SP2_F32 = 0, SP2_F64 = 1 } sp2_dtype_t;
@@ -85,7 +89,10 @@ typedef struct {
   int cta_group;    /* 0 = auto; 1 = 128x128 tiles, one CTA; 2 = 256x256 tiles on a CTA pair (cta_group::2) */
   int lanczos_steps; /* 0 = off (default: Gershgorin bounds only); 1..32: that many Lanczos steps on H tighten the spectral
                         bounds to [theta_min - beta_k, theta_max + beta_k] where that is inside the Gershgorin interval:
-                        fewer layers for dense matrices (the paper leaves accelerated variants aside) */
+                        fewer layers for dense matrices (the paper leaves accelerated variants aside).
+                        This interval is a HEURISTIC, not an enclosure (a start vector orthogonal to an extreme
+                        eigenvector never sees it): the device guards every solve (SP2_ERR_BOUNDS) and the blocking calls
+                        fall back to Gershgorin discs on their own.  Ignored when N <= 2 * lanczos_steps */
   int refine_layers; /* 0 = off (default); 1..4: float64 SP2 layers applied to the converged iterate before D is written
                         (the paper uses 2); D1 is not refined.  Needs SP2_WITH_REFINEMENT */
   int seg_kb;       /* 0 = default (8 up to N = 8192, 4 up to N = 24576, 2 above); 1, 2, 4, 8, 16 or 32 (must divide
@@ -113,7 +120,7 @@ typedef struct {
   float gpu_ms;                      /* device time of the call (CUDA events on `stream`), blocking calls only */
   float layers_ms;                   /* device time of the layer-kernel launches alone (a3-a5), blocking calls only */
   int kernel_launches;               /* kernels of this library launched by the call */
-  int reserved2;
+  int bounds_fallback;               /* 1: the Lanczos bounds failed the device guard and the solve was re-run with Gershgorin discs */
 } sp2_result_t;
 
 /* Largest supported dimension (the largest size the GPU parity tests cover; 32-bit index arithmetic in the

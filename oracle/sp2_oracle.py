@@ -100,7 +100,9 @@ def lanczos_bounds(H, steps=12):
     spectral estimates aside): ``steps`` iterations of the Lanczos process on H from the fixed start
     vector v_i = cos(0.7 i + 0.3); with T_k the tridiagonal matrix of the alphas and betas and beta_k the norm of
     the last residual, returns (theta_min - beta_k, theta_max + beta_k) intersected with the Gershgorin interval.
-    The extreme Ritz values lie inside the spectrum; widening by the residual norm is the usual safe bound."""
+    The extreme Ritz values lie inside the spectrum; widening by the residual norm is the usual "safe" bound, but it
+    is a HEURISTIC, not an enclosure: an extreme eigenvector orthogonal to the start vector is never seen
+    (pinned both ways: enclosure on ordinary matrices, a miss by > 1 on the adversarial one)."""
     H = np.asarray(H, dtype=np.float64)
     n = H.shape[0]
     k = max(1, min(steps, n - 1))

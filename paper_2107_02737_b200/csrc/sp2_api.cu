@@ -212,6 +212,7 @@ struct sp2_handle_s {
   sp2_result_t* h_result;        // pinned
   int last_cuda_error;
   int layers_hint;               // layers + slack of the last converged solve of the current shape (0 = unknown)
+  int no_lanczos;                // this solve is the Gershgorin re-run after the device guard rejected the Lanczos bounds
   unsigned long long launches;
   // sequence state
   int seq_active, seq_N, seq_nocc, seq_steps;
@@ -501,6 +502,11 @@ sp2_status_t enqueue_finalise(sp2_handle_t h, const void* H, sp2_dtype_t in_dt, 
   return SP2_OK;
 }
 
+bool lanczos_active(sp2_handle_t h, int N, int N_occ) {
+  const sp2_options_t& o = h->opt;
+  return o.lanczos_steps > 0 && !o.user_bounds && !h->no_lanczos && N > 2 * o.lanczos_steps && N_occ > 0 && N_occ < N;
+}
+
 int effective_max_layers(const sp2_options_t& o) {
   if (o.forced_layers > 0) return o.forced_layers > 64 ? 64 : o.forced_layers;
   return o.max_layers <= 0 ? 100 : (o.max_layers > 126 ? 126 : o.max_layers);
@@ -549,10 +555,11 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dty
     sp2_launch_bounds(P.H1[b], in_dt, ldh, N, 1, h->bslots(1) + (size_t)b * sp2_bounds_blocks(N), s);
     ++launches;
   }
-  if (o.lanczos_steps > 0 && !o.user_bounds && N_occ > 0 && N_occ < N) {
-    const int k = o.lanczos_steps < N ? o.lanczos_steps : N - 1 > 0 ? N - 1 : 1;
-    sp2_launch_lanczos(c, H, in_dt, ldh, N, k, h->lanczos_vecs(), s);
-    launches += 2 + 2 * k;
+  // Lanczos bounds are an estimate (include/sp2.h): skipped for matrices no larger than the Krylov space asked for
+  // and on the re-run after the device guard rejected them (SP2_ERR_BOUNDS)
+  if (lanczos_active(h, N, N_occ)) {
+    sp2_launch_lanczos(c, H, in_dt, ldh, N, o.lanczos_steps, h->lanczos_vecs(), s);
+    launches += 2 + 2 * o.lanczos_steps;
   }
   sp2_launch_setup(c, h->bslots(0), sp2_bounds_blocks(N), h->bslots(1), resp ? sp2_bounds_blocks(N) : 0, s); ++launches;
   if (N_occ == 0 || N_occ == N) {
@@ -622,39 +629,53 @@ sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dt
   // shape needed (+ slack) instead of max_layers early-exit launches; if the solve turns out unfinished,
   // top up once with the rest (the answer is the same: the device controller decides when to stop).
   const int max_layers = effective_max_layers(h->opt);
-  int n_first = max_layers;
-  if (h->opt.forced_layers <= 0 && h->layers_hint > 0 && h->layers_hint < max_layers) n_first = h->layers_hint;
-  h->time_layers = 1;
-  st = enqueue_solve(h, dH, dP, in_dt, dld_in, N, N_occ, tol, dD, out_dt, dld_out, 0, s, n_first, &launches);
-  h->time_layers = 0;
-  if (st != SP2_OK) return st;
   float layers_ms = 0.f;
-  for (int pass = 0; pass < 2; ++pass) {
-    if (host_buffers) {
-      SP2_CUDA(h, cudaMemcpy2DAsync(D, (size_t)ldd * out_sz, dD, (size_t)N * out_sz, (size_t)N * out_sz, N,
-                                    cudaMemcpyDeviceToHost, s));
-      if (want_resp)
-        SP2_CUDA(h, cudaMemcpy2DAsync(D1, (size_t)ldd * out_sz, dD1, (size_t)N * out_sz, (size_t)N * out_sz, N,
+  int bounds_fallback = 0;
+  for (int attempt = 0; attempt < 2; ++attempt) {
+    int n_first = max_layers;
+    if (h->opt.forced_layers <= 0 && h->layers_hint > 0 && h->layers_hint < max_layers) n_first = h->layers_hint;
+    h->time_layers = 1;
+    int l0 = 0;
+    st = enqueue_solve(h, dH, dP, in_dt, dld_in, N, N_occ, tol, dD, out_dt, dld_out, 0, s, n_first, &l0);
+    launches += l0;
+    h->time_layers = 0;
+    if (st != SP2_OK) { h->no_lanczos = 0; return st; }
+    for (int pass = 0; pass < 2; ++pass) {
+      if (host_buffers) {
+        SP2_CUDA(h, cudaMemcpy2DAsync(D, (size_t)ldd * out_sz, dD, (size_t)N * out_sz, (size_t)N * out_sz, N,
                                       cudaMemcpyDeviceToHost, s));
+        if (want_resp)
+          SP2_CUDA(h, cudaMemcpy2DAsync(D1, (size_t)ldd * out_sz, dD1, (size_t)N * out_sz, (size_t)N * out_sz, N,
+                                        cudaMemcpyDeviceToHost, s));
+      }
+      SP2_CUDA(h, cudaMemcpyAsync(h->h_result, h->ring(), sizeof(sp2_result_t), cudaMemcpyDeviceToHost, s));
+      if (tr_d1)    // the pinned result ring is idle outside a sequence: entry 1.. carries tr D1_b
+        SP2_CUDA(h, cudaMemcpyAsync(h->h_result + 1, h->ctrl()->tr_d1, sizeof(double) * SP2_MAX_BATCH, cudaMemcpyDeviceToHost, s));
+      SP2_CUDA(h, cudaEventRecord(h->ev1, s));
+      SP2_CUDA(h, cudaStreamSynchronize(s));
+      if (layers_timed) {
+        float t = 0.f;
+        SP2_CUDA(h, cudaEventElapsedTime(&t, h->evl0, h->evl1));
+        layers_ms += t;
+      }
+      if (h->h_result->status != SP2_INTERNAL_INCOMPLETE || pass == 1) break;
+      SP2_CUDA(h, cudaEventRecord(h->evl0, s));                   // top-up: the remaining layer launches
+      st = enqueue_layers(h, n_first, max_layers - n_first, s, &launches);
+      if (st != SP2_OK) { h->no_lanczos = 0; return st; }
+      SP2_CUDA(h, cudaEventRecord(h->evl1, s));
+      enqueue_finalise(h, dH, in_dt, dld_in, N, dP, dD, out_dt, dld_out, 0, s, &launches);
+      h->launches += (unsigned long long)(max_layers - n_first + 1 + (want_resp > 1 ? want_resp : 1));
     }
-    SP2_CUDA(h, cudaMemcpyAsync(h->h_result, h->ring(), sizeof(sp2_result_t), cudaMemcpyDeviceToHost, s));
-    if (tr_d1)    // the pinned result ring is idle outside a sequence: entry 1.. carries tr D1_b
-      SP2_CUDA(h, cudaMemcpyAsync(h->h_result + 1, h->ctrl()->tr_d1, sizeof(double) * SP2_MAX_BATCH, cudaMemcpyDeviceToHost, s));
-    SP2_CUDA(h, cudaEventRecord(h->ev1, s));
-    SP2_CUDA(h, cudaStreamSynchronize(s));
-    if (layers_timed) {
-      float t = 0.f;
-      SP2_CUDA(h, cudaEventElapsedTime(&t, h->evl0, h->evl1));
-      layers_ms += t;
+    // The Lanczos interval is an estimate.  If the device guard saw an eigenvalue of X leave [0, 1] (or the iterate
+    // blow up), solve again with the rigorous Gershgorin discs: same answer as lanczos_steps = 0, one extra pass.
+    const int stt = h->h_result->status;
+    if (attempt == 0 && lanczos_active(h, N, N_occ) && (stt == SP2_ERR_BOUNDS || stt == SP2_ERR_NONFINITE)) {
+      h->no_lanczos = 1; bounds_fallback = 1; h->layers_hint = 0;
+      continue;
     }
-    if (h->h_result->status != SP2_INTERNAL_INCOMPLETE || pass == 1) break;
-    SP2_CUDA(h, cudaEventRecord(h->evl0, s));                   // top-up: the remaining layer launches
-    st = enqueue_layers(h, n_first, max_layers - n_first, s, &launches);
-    if (st != SP2_OK) return st;
-    SP2_CUDA(h, cudaEventRecord(h->evl1, s));
-    enqueue_finalise(h, dH, in_dt, dld_in, N, dP, dD, out_dt, dld_out, 0, s, &launches);
-    h->launches += (unsigned long long)(max_layers - n_first + 1 + (want_resp > 1 ? want_resp : 1));
+    break;
   }
+  h->no_lanczos = 0;
   float ms = 0.f;
   SP2_CUDA(h, cudaEventElapsedTime(&ms, h->ev0, h->ev1));
   sp2_result_t r = *h->h_result;
@@ -663,6 +684,8 @@ sp2_status_t blocking_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dt
   r.gpu_ms = ms;
   r.layers_ms = layers_ms;
   r.kernel_launches = launches;
+  r.bounds_fallback = bounds_fallback;
+  if (bounds_fallback) h->layers_hint = 0;       // the Gershgorin re-run's layer count says nothing about the next Lanczos solve
   if (out) *out = r;
   if (tr_d1) {
     const bool trivial = (N_occ == 0 || N_occ == N);
@@ -699,7 +722,7 @@ sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_work
   h->ws = static_cast<uint8_t*>(d_workspace); h->ws_bytes = bytes; h->L = L;
   default_options(&h->opt);
   h->cur_n = -1; h->cur_npad = -1; h->cur_cg = -1; h->cur_resp = -1; h->cur_seg = -1;
-  h->last_cuda_error = 0; h->launches = 0; h->seq_active = 0; h->layers_hint = 0;
+  h->last_cuda_error = 0; h->launches = 0; h->seq_active = 0; h->layers_hint = 0; h->no_lanczos = 0;
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
@@ -954,6 +977,7 @@ const char* sp2_status_string(sp2_status_t s) {
     case SP2_ERR_NONFINITE: return "non-finite input or iterate";
     case SP2_ERR_DEGENERATE: return "degenerate spectral bounds (eps_max == eps_min)";
     case SP2_WARN_NOT_CONVERGED: return "not converged within max_layers";
+    case SP2_ERR_BOUNDS: return "spectral bounds do not enclose the spectrum";
   }
   return "unknown status";
 }

@@ -139,6 +139,16 @@ __device__ inline void sp2_controller(Sp2Ctrl* c) {
   const double tr_x2 = N * cc * cc + 2.0 * cc * c->tr_y + c->fro_y;
   c->tr_x[n] = tr_x;
   c->e[n] = tr_x - tr_x2;
+  // Guard on the spectral bounds: spec(X) inside [0, 1] gives tr X^2 <= tr X and 0 <= tr X <= N.  An eigenvalue outside
+  // [0, 1] (bounds that miss part of the spectrum: user_bounds, or the Lanczos estimate) is driven away from the
+  // interval by one of the two branches, doubly exponentially, so e_n turns negative far beyond rounding (which
+  // is ~1e-7 N at convergence) within a few layers.  Every assumption downstream (plane exponents, convergence)
+  // rests on [0, 1], so the solve stops here.
+  const double guard = 1e-2 + 1e-5 * N;
+  if (c->forced_layers <= 0 && (c->e[n] < -guard || tr_x < -guard || tr_x > N + guard)) {
+    c->done = 1; c->status = SP2_ERR_BOUNDS; c->stop_reason = 0;
+    return;
+  }
   const int stop = sp2_stop_rule(c, n, tr_x);
   if (stop) {
     c->done = 1; c->stop_reason = stop;

@@ -367,7 +367,7 @@ __global__ void __launch_bounds__(256) k_finalise_reduce(Sp2Ctrl* c, const doubl
   r.stop_reason = c->stop_reason; r.reserved = 0;
   r.tr_d = c->tr_d; r.tr_dh = c->tr_dh; r.tr_d1 = c->tr_d1[0];
   r.idem_est = ok ? c->e[c->n] : 0.0;
-  r.eps_min = c->eps_min; r.eps_max = c->eps_max; r.gpu_ms = 0.f; r.layers_ms = 0.f; r.kernel_launches = 0; r.reserved2 = 0;
+  r.eps_min = c->eps_min; r.eps_max = c->eps_max; r.gpu_ms = 0.f; r.layers_ms = 0.f; r.kernel_launches = 0; r.bounds_fallback = 0;
   *ring_entry = r;
 }
 
@@ -546,7 +546,7 @@ __global__ void __launch_bounds__(256) k_trivial(Sp2Ctrl* c, TO* __restrict__ D,
     r.status = (st == SP2_ERR_NONFINITE) ? st : SP2_OK;
     r.layers = 0; r.sign_mask[0] = r.sign_mask[1] = 0; r.stop_reason = 5; r.reserved = 0;
     r.tr_d = diag * N; r.tr_dh = diag * c->tr_h; r.tr_d1 = 0.0; r.idem_est = 0.0;
-    r.eps_min = c->eps_min; r.eps_max = c->eps_max; r.gpu_ms = 0.f; r.layers_ms = 0.f; r.kernel_launches = 0; r.reserved2 = 0;
+    r.eps_min = c->eps_min; r.eps_max = c->eps_max; r.gpu_ms = 0.f; r.layers_ms = 0.f; r.kernel_launches = 0; r.bounds_fallback = 0;
     *ring_entry = r;
   }
 }

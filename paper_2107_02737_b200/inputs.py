@@ -186,3 +186,25 @@ def overlap_problem(n: int, n_occ: int, seed: int = 7, gap: float = 0.4):
     Horth = (Q * lam) @ Q.T
     H = Zinv @ (0.5 * (Horth + Horth.T)) @ Zinv
     return dict(H=0.5 * (H + H.T), S=0.5 * (S + S.T), Z=0.5 * (Z + Z.T), lam=lam, Q=Q, n=n, n_occ=n_occ)
+
+
+def hidden_eigenvector_problem(n: int, n_occ: int, hidden: float, orth_to, seed: int = 11, gap: float = 0.4):
+    """Adversarial input for any Krylov spectral estimate started from the vector ``orth_to``: a gapped spectrum in
+    [-1, 1] plus ONE outlier eigenvalue ``hidden`` (< -1: the lowest, occupied state; > 1: the highest, empty state) whose
+    eigenvector is exactly orthogonal to ``orth_to``, so that in exact arithmetic the Krylov space never contains it.
+    Returns (H, lam) with lam[k] the eigenvalue of column k of the (discarded) eigenvector matrix."""
+    rng = np.random.default_rng(seed)
+    v0 = np.asarray(orth_to, dtype=np.float64)
+    v0 = v0 / np.linalg.norm(v0)
+    q1 = rng.standard_normal(n)
+    q1 -= (q1 @ v0) * v0
+    q1 /= np.linalg.norm(q1)
+    A = rng.standard_normal((n, n))
+    A[:, 0] = q1
+    Q, _ = np.linalg.qr(A)                          # column 0 = +-q1, the rest an orthonormal completion
+    if hidden < 0:
+        lam = np.concatenate([[hidden], rng.uniform(-1.0, -gap / 2, n_occ - 1), rng.uniform(gap / 2, 1.0, n - n_occ)])
+    else:
+        lam = np.concatenate([[hidden], rng.uniform(-1.0, -gap / 2, n_occ), rng.uniform(gap / 2, 1.0, n - n_occ - 1)])
+    H = (Q * lam[None, :]) @ Q.T
+    return np.ascontiguousarray(0.5 * (H + H.T)), lam

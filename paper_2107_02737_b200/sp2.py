@@ -27,6 +27,7 @@ SP2_ERR_ARCH = 4
 SP2_ERR_NONFINITE = 5
 SP2_ERR_DEGENERATE = 6
 SP2_WARN_NOT_CONVERGED = 7
+SP2_ERR_BOUNDS = 8
 
 SP2_F32, SP2_F64 = 0, 1
 SP2_WITH_RESPONSE, SP2_WITH_HOST_STAGING, SP2_WITH_REFINEMENT = 1, 2, 4
@@ -64,7 +65,7 @@ class Sp2Result(C.Structure):
         ("stop_reason", C.c_int), ("reserved", C.c_int),
         ("tr_d", C.c_double), ("tr_dh", C.c_double), ("tr_d1", C.c_double),
         ("idem_est", C.c_double), ("eps_min", C.c_double), ("eps_max", C.c_double),
-        ("gpu_ms", C.c_float), ("layers_ms", C.c_float), ("kernel_launches", C.c_int), ("reserved2", C.c_int),
+        ("gpu_ms", C.c_float), ("layers_ms", C.c_float), ("kernel_launches", C.c_int), ("bounds_fallback", C.c_int),
     ]
 
     def as_dict(self):
@@ -73,7 +74,7 @@ class Sp2Result(C.Structure):
         return dict(status=self.status, layers=self.layers, signs=signs, stop_reason=self.stop_reason,
                     refine_layers=self.reserved, tr_d=self.tr_d, tr_dh=self.tr_dh, tr_d1=self.tr_d1, idem_est=self.idem_est,
                     eps_min=self.eps_min, eps_max=self.eps_max, gpu_ms=self.gpu_ms, layers_ms=self.layers_ms,
-                    kernel_launches=self.kernel_launches)
+                    kernel_launches=self.kernel_launches, bounds_fallback=self.bounds_fallback)
 
 
 class Sp2Error(RuntimeError):

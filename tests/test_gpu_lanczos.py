@@ -52,3 +52,40 @@ def test_lanczos_is_ignored_with_user_bounds_and_sparse_tight_case(torch_cuda, s
     D2, r2 = h.density(H, 256)
     assert (r2["eps_min"], r2["eps_max"]) == (-2.0, 2.0)
     h.close()
+
+
+@pytest.mark.parametrize("n_occ, hidden", [(40, -3.0), (150, 3.0)])
+def test_lanczos_bounds_that_miss_an_eigenvalue_fall_back_to_gershgorin(torch_cuda, sp2, n_occ, hidden):
+    """Adversarial input: an outlier eigenvalue whose eigenvector is orthogonal to the Lanczos start vector, so the
+    Lanczos interval misses it by > 1 (tests/test_oracle_pins.py shows the oracle's own Lanczos bounds do too and that SP2
+    with them returns garbage).  The device guard must see an eigenvalue of X leave [0, 1] (SP2_ERR_BOUNDS inside the
+    call) and the blocking call must re-run with the Gershgorin discs: right answer, flagged."""
+    import oracle
+
+    torch = torch_cuda
+    n = 300
+    H, lam = inputs.hidden_eigenvector_problem(n, n_occ, hidden, np.cos(0.7 * np.arange(n) + 0.3))
+    ref = oracle.sp2_density(H, n_occ)
+    lo, hi = oracle.lanczos_bounds(H, 12)
+    assert (lo > -2.0) if hidden < 0 else (hi < 2.0)
+    h = sp2.Sp2Handle(n)
+    h.set_options(lanczos_steps=12)
+    D, r = h.density(torch.from_numpy(H).cuda(), n_occ)
+    assert r["status"] == 0 and r["bounds_fallback"] == 1
+    assert r["eps_min"] == pytest.approx(ref["eps_min"], rel=1e-12) and r["eps_max"] == pytest.approx(ref["eps_max"], rel=1e-12)
+    assert np.abs(D.cpu().numpy() - ref["D"]).max() <= 1e-4
+    assert abs(r["tr_d"] - n_occ) <= 1e-3 and abs(r["tr_dh"] - ref["tr_dh"]) <= 1e-5 * abs(ref["tr_dh"])
+    # the same matrix with wrong USER bounds is the caller's error: reported, not repaired
+    h.set_options(lanczos_steps=0, user_bounds=(lo, hi))
+    with pytest.raises(sp2.Sp2Error) as ei:
+        h.density(torch.from_numpy(H).cuda(), n_occ)
+    assert ei.value.status == sp2.SP2_ERR_BOUNDS
+    # and in a sequence step (no host round trip, so no re-run) the step reports SP2_ERR_BOUNDS
+    h.set_options(lanczos_steps=12, user_bounds=None)
+    h.sequence_begin(n, n_occ, n_steps_hint=1)
+    Dt = torch.empty(n, n, dtype=torch.float64, device="cuda")
+    h.sequence_step(torch.from_numpy(H).cuda(), Dt)
+    with pytest.raises(sp2.Sp2Error) as ei:
+        h.sequence_end()
+    assert ei.value.status == sp2.SP2_ERR_BOUNDS
+    h.close()

@@ -378,6 +378,33 @@ def test_lanczos_bounds_enclose_the_spectrum_and_are_tighter(cfg1):
     assert np.abs(r_g["D"] - r_l["D"]).max() < 1e-12 and r_l["layers"] <= r_g["layers"] - 3
 
 
+def test_lanczos_bounds_are_a_heuristic_not_an_enclosure():
+    """The other side of the pin above: the Lanczos interval is NOT rigorous.  With an extreme eigenvector exactly
+    orthogonal to the start vector v_i = cos(0.7 i + 0.3), the Krylov space never contains it, the interval misses the
+    outlier eigenvalue by more than the whole remaining spectrum, and the SP2 loop run with those bounds maps that
+    eigenvalue outside [0, 1] and returns garbage -- which is why the GPU path guards every solve
+    (SP2_ERR_BOUNDS) and falls back to the Gershgorin discs (tests/test_gpu_lanczos.py)."""
+    n = 300
+    v0 = np.cos(0.7 * np.arange(n) + 0.3)
+    for n_occ, hidden in ((40, -3.0), (150, 3.0)):
+        H, lam = inputs.hidden_eigenvector_problem(n, n_occ, hidden, v0)
+        w = np.linalg.eigvalsh(H)
+        assert w[0 if hidden < 0 else -1] == pytest.approx(hidden, abs=1e-12)
+        lo, hi = oracle.lanczos_bounds(H, 12)
+        if hidden < 0:
+            assert lo > w[0] + 1.0 and hi >= w[-1]                    # misses the lowest eigenvalue by > 1
+        else:
+            assert hi < w[-1] - 1.0 and lo <= w[0]                    # misses the highest eigenvalue by > 1
+        g_lo, g_hi = oracle.gershgorin_bounds(H)
+        assert g_lo <= w[0] and g_hi >= w[-1]                         # the discs are rigorous
+        D_eig, _ = oracle.density_eigh(H, n_occ)
+        bad = oracle.sp2_density(H, n_occ, bounds=(lo, hi), max_layers=60)
+        assert min(bad["e"]) < -1.0                                   # tr X - tr X^2 < 0: an eigenvalue left [0, 1]
+        assert not np.abs(bad["D"] - D_eig).max() < 1.0
+        good = oracle.sp2_density(H, n_occ)
+        assert np.abs(good["D"] - D_eig).max() < 1e-11
+
+
 def test_batched_response_vs_perturbation_theory_and_linearity():
     """NEXT-4: every D1_b of the one-stack loop equals first-order perturbation theory for its own H1_b (an
     index mix-up between the Z_b, a dropped factor or a shared update fails this), and the map H1 -> D1 is linear."""
