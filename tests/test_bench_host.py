@@ -1,6 +1,8 @@
 """CPU tests of bench.py's host logic: the N > 1 aggregation (gloo, world size 2: timing = max over
-ranks, work = sum over ranks -- the path does not shard, ranks are independent replicas), the oracle
-sample plan and the flop accounting."""
+ranks, work = sum over ranks -- the path does not shard, ranks are independent replicas), the replica launcher of
+`bench.py --gpus N` (the real entry point with a stubbed step), the oracle sample plan and the flop accounting."""
+import json
+import subprocess
 import os
 import socket
 import sys
@@ -91,3 +93,54 @@ def test_oracle_sample_plan_is_bounded():
         r = oracle.sp2_density(H, 6, H1=H if resp else None, max_layers=k)
         assert r["layers"] == k and r["stop"] == "max_layers"
         assert bench.sample_text(dict(response=resp, max_layers=k, products=n_mm), 12).count(f"{n_mm} float64") == 1
+
+
+def _run_bench(argv, env_extra=None):
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    env.update(env_extra or {})
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py")] + argv, capture_output=True, text=True, env=env,
+                       timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout                          # rank 0 alone prints, exactly one JSON line
+    return json.loads(lines[0])
+
+
+def test_gpus_n_without_torchrun_starts_n_replicas():
+    """`python bench.py --gpus 2` (no torchrun, as a user or the driver may start it) must run TWO ranks, not silently
+    time one: main() re-launches itself under torch.distributed.run.  The step is stubbed (a sleep; rank 1 is 10 %
+    slower), so this runs on CPU with gloo; everything else is the real entry point."""
+    line = _run_bench(["--gpus", "2", "--steps", "4", "--warmup", "1", "--stub-ms", "25"])
+    assert line["n_gpus"] == 2 and line["gpus_active"] == 2 and line["steps"] == 4
+    assert 27.0 <= line["ms_per_step"] <= 60.0                # the slower rank (27.5 ms per step) sets the time
+    assert line["value"] == pytest.approx(2 * 4 * 1e12 / (line["ms_per_step"] * 4e-3) / 1e12, rel=1e-9)   # work of BOTH ranks
+    one = _run_bench(["--gpus", "1", "--steps", "4", "--warmup", "1", "--stub-ms", "25"])
+    assert one["n_gpus"] == 1 and one["gpus_active"] == 1 and 24.0 <= one["ms_per_step"] <= 50.0
+
+
+def test_workload_table_names_all_five_configs():
+    import bench
+    from paper_2107_02737_b200 import inputs
+
+    for k in range(1, 6):
+        idx, call = bench.WORKLOADS[f"config{k}"]
+        assert idx == k and call == ("sequence" if k == 5 else "response" if inputs.CONFIGS[k].response else "density")
+        assert f"N={inputs.CONFIGS[k].n}" in bench.config_text(inputs.CONFIGS[k], call)
+    assert bench.WORKLOADS["response"] == bench.WORKLOADS["config4"] and bench.WORKLOADS["density"] == (4, "density")
+
+
+def test_full_oracle_loop_is_chosen_when_it_fits_and_stale_traffic_is_not_reported(tmp_path):
+    import bench
+
+    plan = bench.oracle_sample_plan(128, False, layers=24)             # config 1: 25 tiny products: the full loop
+    assert plan["max_layers"] is None and plan["products"] == 25
+    plan = bench.oracle_sample_plan(16384, False, budget_s=0.0, layers=38, full_budget_s=1.0)   # config 5: a bounded sample
+    assert plan["max_layers"] == 0
+    assert "FULL loop" in bench.sample_text(dict(response=False, max_layers=None, products=25), 128, 1)
+    # roofline.traffic is the committed ncu constant only while sp2_layer.cu is the file the capture was taken at
+    val, src = bench.read_profile_traffic("response")
+    blob = bench.git_blob_hash(os.path.join(ROOT, "paper_2107_02737_b200", "csrc", "sp2_layer.cu"))
+    if blob in src and "STALE" not in src:
+        assert val is not None and val > 1e8
+    else:
+        assert val is None and "STALE" in src

@@ -89,46 +89,80 @@ def test_config4_smallgap_n8192_response(torch_cuda, sp2):
     assert resid <= TOL_D1 * scale1
 
 
-def test_config5_md_sequence_n16384(torch_cuda, sp2):
-    """H_t = H_0 + t*1e-3*P formed on the device by the harness; steps t = 0, 25, 49 of the 50-step
-    sweep go through sp2_sequence_* without a host synchronisation in between."""
+def test_config5_all_50_steps_n16384(torch_cuda, sp2):
+    """The whole 50-step sweep of config 5 at full size through sp2_sequence_* (one host synchronisation, at the end):
+    status, trace and band-energy law for EVERY step from the per-step results; bit-symmetry, idempotency and commutator
+    (float64 on the GPU, cross-check) on the steps whose D is kept (0, 25, 49; the others share one output buffer);
+    t = 0 against the exact projector.  The oracle comparison for t > 0 is test_config5_shape_n4096_steps_against_oracle."""
     import oracle
 
     torch = torch_cuda
     p = inputs.make_problem(inputs.CONFIGS[5], device="cuda", want_p=True)
-    n, n_occ = p["n"], p["n_occ"]
-    assert (n, n_occ, p["H"].dtype) == (16384, 8192, np.float32)
+    n, n_occ, n_steps = p["n"], p["n_occ"], inputs.CONFIGS[5].n_steps
+    assert n_steps == 50
     H0 = torch.from_numpy(p["H"]).cuda()
     P = torch.from_numpy(p["P"]).cuda()
-    steps = [0, 25, 49]
+    keep = {0: torch.empty_like(H0), 25: torch.empty_like(H0), 49: torch.empty_like(H0)}
+    scratch_D = torch.empty_like(H0)
+    Ht = torch.empty_like(H0)
     h = sp2.Sp2Handle(n)
-    Ht = [H0 + float(t) * 1e-3 * P for t in steps]
-    Dt = [torch.empty_like(H0) for _ in steps]
-    h.sequence_begin(n, n_occ, n_steps_hint=len(steps))
-    for a, b in zip(Ht, Dt):
+    h.density(H0, n_occ, out=scratch_D)                      # warm-up: gives the sequence its layer-count hint
+    h.sequence_begin(n, n_occ, n_steps_hint=n_steps)
+    for t in range(n_steps):
+        torch.add(H0, P, alpha=1e-3 * t, out=Ht)             # stream-ordered: the previous step has read Ht by then
+        h.sequence_step(Ht, keep.get(t, scratch_D))
+    res = h.sequence_end()
+    h.close()
+    assert len(res) == n_steps and [r["status"] for r in res] == [0] * n_steps
+    E0 = inputs.band_energy_closed_form(p["lam"], n_occ)
+    assert abs(res[0]["tr_dh"] - E0) <= TOL_E * abs(E0)
+    d1 = 1e-3 * float((keep[0].double() * P.double()).sum())   # first-order slope dE/dt = eps tr(D_0 P)
+    # E(t) = E_0 + t d1 - c t^2 + O(t^3), c > 0: second-order perturbation theory lowers the occupied sum, so every
+    # step lies below the first-order line and the drop follows one t^2 law along the whole sweep
+    curv = {t: (t * d1 - (res[t]["tr_dh"] - res[0]["tr_dh"])) / t ** 2 for t in range(5, n_steps)}
+    for t, r in enumerate(res):
+        assert 30 <= r["layers"] <= 50 and abs(r["tr_d"] - n_occ) <= TOL_TR, t
+    for t, c in curv.items():
+        assert c > 0 and 0.6 * curv[49] <= c <= 1.6 * curv[49], (t, c, curv[49])
+    rows, cols = _samples(n, k=2000)
+    De = oracle.density_from_eigenpairs(p["Q"], p["lam"], n_occ, rows, cols)
+    assert np.abs(_gather(torch, keep[0], rows, cols) - De).max() <= TOL_D
+    for t, D in keep.items():
+        assert bool(torch.equal(D, D.T)), t
+        idem, comm = _crosscheck_projector(torch, D, torch.add(H0, P, alpha=1e-3 * t), n_occ)
+        assert idem < 1e-4 and comm < 1e-5, t
+
+
+def test_config5_shape_n4096_steps_against_oracle(torch_cuda, sp2):
+    """Config 5's recipe at N = 4096 (f32, gap 0.2, H_t = H_0 + t 1e-3 P): all 50 steps through the sequence call, every
+    step's status and trace, and steps 0, 12, 25, 37, 49 element by element against the oracle's DEFINITION
+    (oracle.density_eigh of the same H_t in float64: a full eigendecomposition per compared step)."""
+    import oracle
+
+    torch = torch_cuda
+    n = 4096
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[5], n), device="cuda", want_p=True)
+    n_occ = p["n_occ"]
+    H0 = torch.from_numpy(p["H"]).cuda()
+    P = torch.from_numpy(p["P"]).cuda()
+    Hs = [torch.add(H0, P, alpha=1e-3 * t) for t in range(50)]
+    Ds = [torch.empty_like(H0) for _ in range(50)]
+    h = sp2.Sp2Handle(n)
+    h.sequence_begin(n, n_occ, n_steps_hint=50)
+    for a, b in zip(Hs, Ds):
         h.sequence_step(a, b)
     res = h.sequence_end()
     h.close()
-    assert [r["status"] for r in res] == [0, 0, 0]
-    rows, cols = _samples(n, k=2000)
-    De = oracle.density_from_eigenpairs(p["Q"], p["lam"], n_occ, rows, cols)
-    assert np.abs(_gather(torch, Dt[0], rows, cols) - De).max() <= TOL_D          # t = 0: exact projector
-    E0 = inputs.band_energy_closed_form(p["lam"], n_occ)
-    assert abs(res[0]["tr_dh"] - E0) <= TOL_E * abs(E0)
-    for a, b, r in zip(Ht, Dt, res):
-        assert 30 <= r["layers"] <= 50
-        assert abs(r["tr_d"] - n_occ) <= TOL_TR
-        assert bool(torch.equal(b, b.T))
-        idem, comm = _crosscheck_projector(torch, b, a, n_occ)                     # t > 0: invariants (cross-check)
-        assert idem < 1e-4 and comm < 1e-5
-    # band energy along the sweep E(t) = E_0 + t eps tr(D_0 P) - O(t^2): it lies below its first-order
-    # line (second-order perturbation theory lowers the occupied sum) and the drop grows ~ t^2
-    d1 = 1e-3 * float((Dt[0].double() * P.double()).sum())
-    dE25 = res[1]["tr_dh"] - res[0]["tr_dh"]
-    dE49 = res[2]["tr_dh"] - res[0]["tr_dh"]
-    assert dE25 < 25 * d1 and dE49 < 49 * d1
-    ratio = (dE49 - 49 * d1) / (dE25 - 25 * d1)
-    assert 3.0 <= ratio <= 4.6                                   # (49/25)^2 = 3.84 for a pure t^2 law
+    assert [r["status"] for r in res] == [0] * 50
+    for t, r in enumerate(res):
+        assert abs(r["tr_d"] - n_occ) <= TOL_TR, t
+    for t in (0, 12, 25, 37, 49):
+        H64 = Hs[t].double().cpu().numpy()
+        H64 = 0.5 * (H64 + H64.T)
+        De, w = oracle.density_eigh(H64, n_occ)
+        assert np.abs(Ds[t].double().cpu().numpy() - De).max() <= TOL_D, t
+        E = float(w[:n_occ].sum())
+        assert abs(res[t]["tr_dh"] - E) <= TOL_E * abs(E), t
 
 
 def test_maximum_size_n32768_f32(torch_cuda, sp2):

@@ -43,7 +43,14 @@ def test_random_sweep_against_oracle(torch_cuda, sp2, seed0):
         assert r["status"] == 0, case
         assert np.abs(D.cpu().numpy().astype(np.float64) - ref["D"]).max() <= 1e-4, case
         assert abs(r["tr_d"] - n_occ) <= 1e-3, case
-        if 3 < n_occ < n - 2:      # |tr(DH)| of one or two levels is no scale for a relative bar
-            assert abs(r["tr_dh"] - ref["tr_dh"]) <= 1e-5 * abs(ref["tr_dh"]), case
+        # Energy: north_star's relative bar wherever tr(DH) is an extensive sum (more than 3 levels on either side).
+        # With one to three occupied (or empty) levels |tr(DH)| is a single eigenvalue, possibly near zero, and no scale
+        # for a relative error; the test was shaped around that known miss in round 1 (12 of 200 such cases exceed
+        # 1e-5 relative, worst 1.8e-4), so EVERY case is now also held to the absolute form of the same bar,
+        # |d tr(DH)| <= 1e-5 max(|tr(DH)|, ||H||_F)  (reading R14) -- nothing is left unasserted.
+        dE = abs(r["tr_dh"] - ref["tr_dh"])
+        assert dE <= 1e-5 * max(abs(ref["tr_dh"]), float(np.linalg.norm(H64))), case
+        if 3 < n_occ < n - 2:
+            assert dE <= 1e-5 * abs(ref["tr_dh"]), case
         for b in range(nb):
             assert np.abs(D1s[b].cpu().numpy().astype(np.float64) - ref["D1"][b]).max() <= 1e-3 * np.abs(ref["D1"][b]).max(), case
