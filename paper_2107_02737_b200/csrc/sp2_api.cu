@@ -78,13 +78,13 @@ struct Layout {
   size_t off_fslots;
   size_t off_tiles, tiles_count;
   size_t off_items, items_cap, off_item_begin, off_scratch, scratch_bytes, off_flags;
-  size_t off_ctrl, off_ring;
+  size_t off_ctrl, off_ring, off_args;
   size_t off_staging, staging_each;
   size_t off_refine, refine_each, off_refine_slots, refine_slots_count;
   size_t off_lanczos;
   size_t total;
   std::vector<Region> regions;
-  int r_plane0, r_slots, r_slots2, r_bslots, r_fslots, r_tiles, r_items, r_item_begin, r_scratch, r_flags, r_ctrl, r_ring,
+  int r_plane0, r_slots, r_slots2, r_bslots, r_fslots, r_tiles, r_items, r_item_begin, r_scratch, r_flags, r_ctrl, r_args, r_ring,
       r_staging0, r_lanczos, r_refine0, r_refine_slots;
 };
 
@@ -154,6 +154,7 @@ Layout make_layout(int n_max, int flags) {
   L.r_scratch = carve("scratch", L.scratch_bytes, &L.off_scratch);
   L.r_flags = carve("flags", 2 * kMaxClusters * sizeof(unsigned int), &L.off_flags);
   L.r_ctrl = carve("ctrl", sizeof(Sp2Ctrl), &L.off_ctrl);
+  L.r_args = carve("args", 2 * sizeof(Sp2LayerArgs), &L.off_args);
   L.r_ring = carve("ring", (size_t)kRingCap * sizeof(sp2_result_t), &L.off_ring);
   L.r_staging0 = -1; L.staging_each = 0; L.off_staging = 0;
   if (flags & SP2_WITH_HOST_STAGING) {
@@ -200,7 +201,8 @@ struct sp2_handle_s {
   sp2_options_t opt;
   PFN_cuTensorMapEncodeTiled_v12000 encode;
   // per-(N, cta_group) cache
-  int cur_n, cur_npad, cur_cg, cur_resp, cur_seg, cur_lo;
+  int cur_n, cur_npad, cur_cg, cur_resp, cur_seg, cur_lo, cur_maxctas;
+  int n_active;                  // CTA(-pair)s whose work list is not empty (grid of the persistent multi-layer launch)
   Sp2LayerArgs args[2];          // parity 0: buffer 0 -> 1, parity 1: buffer 1 -> 0
   std::vector<int2> tiles_host;
   std::vector<Sp2Item> items_host;
@@ -234,6 +236,7 @@ struct sp2_handle_s {
   float* scratch() const { return reinterpret_cast<float*>(ws + L.off_scratch); }
   unsigned int* split_flags() const { return reinterpret_cast<unsigned int*>(ws + L.off_flags); }
   Sp2Ctrl* ctrl() const { return reinterpret_cast<Sp2Ctrl*>(ws + L.off_ctrl); }
+  Sp2LayerArgs* d_args() const { return reinterpret_cast<Sp2LayerArgs*>(ws + L.off_args); }   // copy of args[] for the persistent kernel
   sp2_result_t* ring() const { return reinterpret_cast<sp2_result_t*>(ws + L.off_ring); }
   void* staging(int i) const { return ws + L.off_staging + (size_t)i * L.staging_each; }
   double* lanczos_vecs() const { return reinterpret_cast<double*>(ws + L.off_lanczos); }
@@ -376,6 +379,7 @@ int pick_cta_group(sp2_handle_t h, int npad, int resp) {
 int layer_clusters(sp2_handle_t h, int cg) {
   int nC = h->num_sms / cg;
   if (nC > h->max_clusters[cg]) nC = h->max_clusters[cg];
+  if (h->opt.max_ctas > 0 && nC > h->opt.max_ctas / cg) nC = h->opt.max_ctas / cg;
   if (nC > kMaxClusters / cg) nC = kMaxClusters / cg;
   return nC < 1 ? 1 : nC;
 }
@@ -392,7 +396,7 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = npad > 24576 ? 2 : (npad > 8192 ? 4 : 8);
   while ((npad / 64) % seg) seg >>= 1;
   if (h->cur_n == N && h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp && h->cur_seg == seg &&
-      h->cur_lo == h->opt.lo_bits) return SP2_OK;
+      h->cur_lo == h->opt.lo_bits && h->cur_maxctas == h->opt.max_ctas) return SP2_OK;
   const int nt = npad / (128 * cg);
   build_tiles(nt, h->tiles_host);
   SP2_CUDA(h, cudaMemcpyAsync(h->tiles(), h->tiles_host.data(), h->tiles_host.size() * sizeof(int2),
@@ -403,6 +407,8 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   build_schedule((int)h->tiles_host.size(), resp, (npad / 64) / seg, nC, h->items_host, h->item_begin_host,
                  &h->n_flags, &n_slots);
   h->n_clusters = nC;
+  h->n_active = 1;
+  for (int c = 0; c < nC; ++c) if (h->item_begin_host[c + 1] > h->item_begin_host[c]) h->n_active = c + 1;
   if (h->items_host.size() > h->L.items_cap || h->tiles_host.size() > h->L.tiles_count ||
       (size_t)n_slots * sp2_layer_scratch_slot_bytes(cg) > h->L.scratch_bytes || h->n_flags > 2 * kMaxClusters ||
       (size_t)sp2_layer_slots(npad, cg * nC, resp, SP2_ENGINE_TCGEN05) > h->L.slots_count)
@@ -435,8 +441,12 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
     a.lo_bits = (h->opt.lo_bits >= 6 && h->opt.lo_bits <= 10) ? h->opt.lo_bits : 11;
     a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = resp; a.seg_kb = seg;
   }
+  SP2_CUDA(h, cudaMemcpyAsync(h->d_args(), h->args, 2 * sizeof(Sp2LayerArgs), cudaMemcpyHostToDevice, s));
+  SP2_CUDA(h, cudaStreamSynchronize(s));
+  h->touch(h->L.r_args, 2 * sizeof(Sp2LayerArgs));
   h->layers_hint = 0;
   h->cur_n = N; h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp; h->cur_seg = seg; h->cur_lo = h->opt.lo_bits;
+  h->cur_maxctas = h->opt.max_ctas;
   return SP2_OK;
 }
 
@@ -470,8 +480,22 @@ sp2_status_t check_args(sp2_handle_t h, const void* H, const Pert& P, sp2_dtype_
   return SP2_OK;
 }
 
+// One persistent launch for the whole stack?  Small problems: a layer is shorter than a launch and its tail.
+constexpr int kPersistMaxNpad = 2048;
+bool use_persistent(sp2_handle_t h) {
+  if (h->opt.engine != SP2_ENGINE_TCGEN05 || h->opt.persistent == 2) return false;
+  return h->opt.persistent == 1 || h->cur_npad <= kPersistMaxNpad;
+}
+
 // enqueue layer launches [first, first + count) on `s`
 sp2_status_t enqueue_layers(sp2_handle_t h, int first, int count, cudaStream_t s, int* launches) {
+  if (use_persistent(h)) {       // the kernel loops until the device controller stops (it starts at layer ctrl->n)
+    if (count <= 0) return SP2_OK;
+    cudaError_t e = sp2_launch_layers_persistent(h->d_args(), h->cur_cg, h->n_active, s);
+    if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
+    ++*launches;
+    return SP2_OK;
+  }
   for (int n = first; n < first + count; ++n) {
     cudaError_t e = sp2_launch_layer(h->args[n & 1], h->opt.engine, h->cur_cg, s);
     if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
@@ -721,7 +745,7 @@ sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_work
   h->n_max = n_max; h->flags = flags; h->device = dev; h->num_sms = prop.multiProcessorCount; h->nb_max = L.nb_max;
   h->ws = static_cast<uint8_t*>(d_workspace); h->ws_bytes = bytes; h->L = L;
   default_options(&h->opt);
-  h->cur_n = -1; h->cur_npad = -1; h->cur_cg = -1; h->cur_resp = -1; h->cur_seg = -1;
+  h->cur_n = -1; h->cur_npad = -1; h->cur_cg = -1; h->cur_resp = -1; h->cur_seg = -1; h->cur_maxctas = -1; h->n_active = 1;
   h->last_cuda_error = 0; h->launches = 0; h->seq_active = 0; h->layers_hint = 0; h->no_lanczos = 0;
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
@@ -773,6 +797,7 @@ sp2_status_t sp2_set_options(sp2_handle_t h, const sp2_options_t* opt) {
   if (opt->seg_kb != 0 && opt->seg_kb != 1 && opt->seg_kb != 2 && opt->seg_kb != 4 && opt->seg_kb != 8 &&
       opt->seg_kb != 16 && opt->seg_kb != 32) return SP2_ERR_INVALID_ARG;
   if (opt->user_bounds && !(opt->eps_max > opt->eps_min)) return SP2_ERR_INVALID_ARG;
+  if (opt->persistent < 0 || opt->persistent > 2 || opt->max_ctas < 0) return SP2_ERR_INVALID_ARG;
   h->opt = *opt;
   h->layers_hint = 0;
   return SP2_OK;

@@ -8,6 +8,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <cuda_fp16.h>
+#include <stddef.h>
 #include <stdint.h>
 #include "sp2.h"
 
@@ -57,13 +58,11 @@ struct Sp2Ctrl {
   int status;           // sp2_status_t
   int stop_reason;
   unsigned int ticket;  // last-block election of the layer kernel
-  int pad1;
+  unsigned int epoch;   // persistent multi-layer kernel: number of grid barriers passed (published by the last CTA)
   double tr_y, fro_y, max_y;                              // reduced partials of the current iterate, TRUE units
   double tr_z[SP2_NB], fro_z[SP2_NB], max_z[SP2_NB];
   Sp2Coef coef;
   unsigned long long sign_mask[2];
-  double tr_x[SP2_LAYER_CAP];
-  double e[SP2_LAYER_CAP];
   // finalise
   double tr_d, tr_dh, tr_d1[SP2_NB];
   // plane exponents of the congruence products (sp2_congruence): operands A, B and the intermediate T
@@ -78,7 +77,12 @@ struct Sp2Ctrl {
   int ref_plus, ref_done;   // branch of the next refinement layer; layers applied
   unsigned int ref_ticket;  // last-block election of the refinement layer kernel (zero between launches)
   int ref_pad;
+  // per-layer history, LAST in the block: the persistent kernel copies everything before it (the "head") through
+  // shared memory at every layer boundary and touches only the entries of the current layer here
+  double tr_x[SP2_LAYER_CAP];
+  double e[SP2_LAYER_CAP];
 };
+#define SP2_CTRL_HEAD_BYTES (offsetof(Sp2Ctrl, tr_x))
 
 // ----------------------------------------------------------------------------------------------
 // small device helpers

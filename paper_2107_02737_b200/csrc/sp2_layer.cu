@@ -198,14 +198,25 @@ struct alignas(8) SmemBarriers {
   uint64_t tmem_empty[2];
   uint32_t tmem_base;
   uint32_t is_last;
+  // persistent mode: stop = the consumers saw the controller's done flag; prod_layers = layers the TMA producer has
+  // started; prod_final = it will start no more (the MMA issuer follows the producer)
+  uint32_t stop, prod_layers, prod_final, pad0;
+  double red[32];         // persistent mode: warp partials of the slot reduction
+  // persistent mode: the last CTA's working copy of the control block (head + the history entries it touches)
+  alignas(8) uint8_t ctrl_copy[sizeof(Sp2Ctrl)];
+  // 32x32 diagonal blocks in flight, one per TMEM lane quarter (of the two warps of a quarter only one holds the
+  // diagonal): packed hi | lo << 16 per element, rows padded to 33 words (conflict-free row and column reads)
+  uint32_t diag_t[4][32 * 33];
   // partial sums of this CTA, per consumer warp and product class (0: Y^2, 1 + b: Y Z_b + Z_b Y): one writer each
   // (lane 0 of the warp), reduced in fixed order at the end of the kernel into ONE slot per CTA and class
   Sp2Slot acc[kConsumerWarps][1 + SP2_NB];
 };
 
+// (.cg: L2 only.  In the persistent mode other CTAs rewrite these planes between layers of the SAME kernel, so a line
+// left in this SM's L1 by an earlier layer would be stale; the reads have no L1 reuse anyway.)
 __device__ __forceinline__ uint4 ld_global_v4(const void* p) {
   uint4 r;
-  asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  asm volatile("ld.global.cg.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
   return r;
 }
 
@@ -283,17 +294,15 @@ __device__ __forceinline__ uint32_t f2_to_h2(float a, float b) {
   return *reinterpret_cast<const uint32_t*>(&h);
 }
 
-// One 32-column chunk.  FULL = the chunk lies entirely above the diagonal (the common case: no
-// diagonal element, every element counts twice in ||.||_F^2 and is stored twice); the statistics
-// then use the FP32 value before the split (it differs from the stored hi+lo by an unbiased 2^-22
-// relative rounding; a non-finite value still reaches the controller through the Frobenius sum).
-// !FULL = the chunk that holds the diagonal: exact stored values, gj >= gi only, diagonal shift.
-template <bool FULL>
-__device__ __forceinline__ void epilogue_chunk(const float* acc, EpiOld& old, const uint4* next_h, const uint4* next_m,
-                                               int gi, int gj0,
-                                               size_t npad, __half* __restrict__ out_h, __half* __restrict__ out_m,
-                                               float a1hi, float a1lo, float a2, float dsh_hi, float dsh_lo,
-                                               uint32_t lo_round, uint32_t lo_mask, EpiPartials& P) {
+// One 32-column chunk that lies entirely above the diagonal (the common case: no diagonal element, every element
+// counts twice in ||.||_F^2 and is stored twice).  The statistics use the FP32 value before the split (it differs
+// from the stored hi+lo by an unbiased 2^-22 relative rounding; a non-finite value still reaches the controller
+// through the Frobenius sum).
+__device__ __forceinline__ void epilogue_chunk_full(const float* acc, EpiOld& old, const uint4* next_h, const uint4* next_m,
+                                                    int gi, int gj0,
+                                                    size_t npad, __half* __restrict__ out_h, __half* __restrict__ out_m,
+                                                    float a1hi, float a1lo, float a2,
+                                                    uint32_t lo_round, uint32_t lo_mask, EpiPartials& P) {
   unsigned short* th = reinterpret_cast<unsigned short*>(out_h) + (size_t)gj0 * npad + gi;   // mirrored image
   unsigned short* tm = reinterpret_cast<unsigned short*>(out_m) + (size_t)gj0 * npad + gi;
   float fsum = 0.f, mx = P.mx;
@@ -307,62 +316,93 @@ __device__ __forceinline__ void epilogue_chunk(const float* acc, EpiOld& old, co
       const float2 fh = h2_to_f2(u4_word(oh, pr)), fm = h2_to_f2(u4_word(om, pr));
       const float old0 = fh.x + fm.x, old1 = fh.y + fm.y;
       const int ci = 8 * w + 2 * pr;
-      float y0 = fmaf(a1hi, old0, fmaf(a1lo, old0, a2 * acc[ci]));
-      float y1 = fmaf(a1hi, old1, fmaf(a1lo, old1, a2 * acc[ci + 1]));
-      if (!FULL) {
-        if (gj0 + ci == gi) y0 = (y0 + dsh_lo) + dsh_hi;
-        if (gj0 + ci + 1 == gi) y1 = (y1 + dsh_lo) + dsh_hi;
-      }
+      const float y0 = fmaf(a1hi, old0, fmaf(a1lo, old0, a2 * acc[ci]));
+      const float y1 = fmaf(a1hi, old1, fmaf(a1lo, old1, a2 * acc[ci + 1]));
       nh[pr] = f2_to_h2(y0, y1);
       const float2 hb = h2_to_f2(nh[pr]);
       nm[pr] = (f2_to_h2(y0 - hb.x, y1 - hb.y) + lo_round) & lo_mask;   // lo_mask = ~0: all 11 bits of the lo plane
-      if (FULL) {
-        fsum = fmaf(y0, y0, fsum);
-        fsum = fmaf(y1, y1, fsum);
-        mx = fmaxf(mx, fmaxf(fabsf(y0), fabsf(y1)));
-      } else {
-        const float2 mb = h2_to_f2(nm[pr]);
-        const float s0 = hb.x + mb.x, s1 = hb.y + mb.y;
-        const int gja = gj0 + ci, gjb = gja + 1;
-        const float wa = (gja > gi) ? 2.f : (gja == gi ? 1.f : 0.f);
-        const float wb = (gjb > gi) ? 2.f : (gjb == gi ? 1.f : 0.f);
-        fsum = fmaf(wa * s0, s0, fsum);
-        fsum = fmaf(wb * s1, s1, fsum);
-        if (gja == gi) { P.tr += (double)s0; P.tracc += (double)acc[ci]; }
-        if (gjb == gi) { P.tr += (double)s1; P.tracc += (double)acc[ci + 1]; }
-        if (gja >= gi) mx = fmaxf(mx, fabsf(s0));
-        if (gjb >= gi) mx = fmaxf(mx, fabsf(s1));
-      }
+      fsum = fmaf(y0, y0, fsum);
+      fsum = fmaf(y1, y1, fsum);
+      mx = fmaxf(mx, fmaxf(fabsf(y0), fabsf(y1)));
     }
-    if (FULL) {
-      st_cs_v4(out_h + (size_t)gi * npad + gj0 + 8 * w, nh[0], nh[1], nh[2], nh[3]);
-      st_cs_v4(out_m + (size_t)gi * npad + gj0 + 8 * w, nm[0], nm[1], nm[2], nm[3]);
+    st_cs_v4(out_h + (size_t)gi * npad + gj0 + 8 * w, nh[0], nh[1], nh[2], nh[3]);
+    st_cs_v4(out_m + (size_t)gi * npad + gj0 + 8 * w, nm[0], nm[1], nm[2], nm[3]);
 #pragma unroll
-      for (int pr = 0; pr < 4; ++pr) {        // lanes = consecutive rows -> 64 contiguous bytes per warp store
-        st_cs_u16(th, nh[pr] & 0xffffu);
-        st_cs_u16(tm, nm[pr] & 0xffffu);
-        st_cs_u16(th + npad, nh[pr] >> 16);
-        st_cs_u16(tm + npad, nm[pr] >> 16);
-        th += 2 * npad; tm += 2 * npad;
-      }
-    } else {
-      unsigned short* oh16 = reinterpret_cast<unsigned short*>(out_h);
-      unsigned short* om16 = reinterpret_cast<unsigned short*>(out_m);
-#pragma unroll
-      for (int pr = 0; pr < 4; ++pr) {
-#pragma unroll
-        for (int e = 0; e < 2; ++e) {
-          const int gj = gj0 + 8 * w + 2 * pr + e;
-          const unsigned short hv = (unsigned short)(e ? (nh[pr] >> 16) : (nh[pr] & 0xffffu));
-          const unsigned short mv = (unsigned short)(e ? (nm[pr] >> 16) : (nm[pr] & 0xffffu));
-          if (gj >= gi) { oh16[(size_t)gi * npad + gj] = hv; om16[(size_t)gi * npad + gj] = mv; }
-          if (gj > gi) { oh16[(size_t)gj * npad + gi] = hv; om16[(size_t)gj * npad + gi] = mv; }
-        }
-      }
+    for (int pr = 0; pr < 4; ++pr) {        // lanes = consecutive rows -> 64 contiguous bytes per warp store
+      st_cs_u16(th, nh[pr] & 0xffffu);
+      st_cs_u16(tm, nm[pr] & 0xffffu);
+      st_cs_u16(th + npad, nh[pr] >> 16);
+      st_cs_u16(tm + npad, nm[pr] >> 16);
+      th += 2 * npad; tm += 2 * npad;
     }
   }
   P.mx = mx;
-  P.fro += (double)(FULL ? 2.f * fsum : fsum);
+  P.fro += (double)(2.f * fsum);
+}
+
+// The 32-column chunk that holds the diagonal: the 32 x 32 block rows gj0 .. gj0 + 31 (one row per lane) by the same
+// columns.  Only elements on or above the diagonal are COMPUTED (hi*lo and lo*hi cross terms add in a different order
+// for (i,j) and (j,i), so the two accumulators may differ in the last bit); they go through a shared-memory tile, and
+// every lane then assembles its whole row -- its own values right of the diagonal, the other lanes' values left of
+// it -- and stores it with 16-byte vectors: the block is bit-symmetric by construction and no store is narrower than
+// 16 bytes (element-wise 2-byte stores, 32 rows apart per lane, made this chunk cost 8 us: the floor of small N).
+// T: this warp's tile (32 x 33 words, hi | lo << 16).  The statistics use the exact stored values.
+__device__ __forceinline__ void epilogue_chunk_diag(const float* acc, EpiOld& old, const uint4* next_h, const uint4* next_m,
+                                                    int gi, int gj0,
+                                                    size_t npad, __half* __restrict__ out_h, __half* __restrict__ out_m,
+                                                    float a1hi, float a1lo, float a2, float dsh_hi, float dsh_lo,
+                                                    uint32_t lo_round, uint32_t lo_mask, uint32_t* __restrict__ T, EpiPartials& P) {
+  const int r = gi - gj0;                     // row inside the block = lane
+  uint32_t* Trow = T + r * 33;
+  float dacc = 0.f, dval = 0.f;               // this row's diagonal accumulator and stored diagonal value
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    const uint4 oh = old.h[w], om = old.m[w];
+    if (next_h) { old.h[w] = ld_global_v4(next_h + w); old.m[w] = ld_global_v4(next_m + w); }   // one chunk ahead
+#pragma unroll
+    for (int pr = 0; pr < 4; ++pr) {
+      const float2 fh = h2_to_f2(u4_word(oh, pr)), fm = h2_to_f2(u4_word(om, pr));
+      const float old0 = fh.x + fm.x, old1 = fh.y + fm.y;
+      const int ci = 8 * w + 2 * pr;
+      float y0 = fmaf(a1hi, old0, fmaf(a1lo, old0, a2 * acc[ci]));
+      float y1 = fmaf(a1hi, old1, fmaf(a1lo, old1, a2 * acc[ci + 1]));
+      if (ci == r) { y0 = (y0 + dsh_lo) + dsh_hi; dacc = acc[ci]; }
+      if (ci + 1 == r) { y1 = (y1 + dsh_lo) + dsh_hi; dacc = acc[ci + 1]; }
+      const uint32_t nh = f2_to_h2(y0, y1);
+      const float2 hb = h2_to_f2(nh);
+      const uint32_t nm = (f2_to_h2(y0 - hb.x, y1 - hb.y) + lo_round) & lo_mask;
+      Trow[ci] = (nh & 0xffffu) | (nm << 16);
+      Trow[ci + 1] = (nh >> 16) | (nm & 0xffff0000u);
+    }
+  }
+  __syncwarp();
+  float fsum = 0.f, mx = P.mx;
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    uint32_t nh[4], nm[4];
+#pragma unroll
+    for (int pr = 0; pr < 4; ++pr) {
+      const int c0 = 8 * w + 2 * pr, c1 = c0 + 1;
+      const uint32_t e0 = T[(c0 >= r) ? r * 33 + c0 : c0 * 33 + r];  // left of the diagonal: the mirror image
+      const uint32_t e1 = T[(c1 >= r) ? r * 33 + c1 : c1 * 33 + r];
+      nh[pr] = (e0 & 0xffffu) | (e1 << 16);
+      nm[pr] = (e0 >> 16) | (e1 & 0xffff0000u);
+      const float2 hv = h2_to_f2(nh[pr]), mv = h2_to_f2(nm[pr]);
+      const float s0 = hv.x + mv.x, s1 = hv.y + mv.y;
+      fsum = fmaf(s0, s0, fsum);              // the whole symmetric row: off-diagonal elements of the block count twice
+      fsum = fmaf(s1, s1, fsum);
+      mx = fmaxf(mx, fmaxf(fabsf(s0), fabsf(s1)));
+      if (c0 == r) dval = s0;
+      if (c1 == r) dval = s1;
+    }
+    st_cs_v4(out_h + (size_t)gi * npad + gj0 + 8 * w, nh[0], nh[1], nh[2], nh[3]);
+    st_cs_v4(out_m + (size_t)gi * npad + gj0 + 8 * w, nm[0], nm[1], nm[2], nm[3]);
+  }
+  __syncwarp();                               // the tile is free for this warp's next diagonal block
+  P.mx = mx;
+  P.fro += (double)fsum;
+  P.tr += (double)dval;
+  P.tracc += (double)dacc;
 }
 
 // Fused epilogue of this thread's row over NCH chunks of 32 columns held in registers
@@ -373,7 +413,7 @@ __device__ __forceinline__ void epilogue_row(const float* acc, EpiOld& old, int 
                                              const __half* __restrict__ in_h, const __half* __restrict__ in_m,
                                              __half* __restrict__ out_h, __half* __restrict__ out_m,
                                              float a1hi, float a1lo, float a2, float dsh_hi, float dsh_lo,
-                                             uint32_t lo_round, uint32_t lo_mask, EpiPartials& P) {
+                                             uint32_t lo_round, uint32_t lo_mask, uint32_t* __restrict__ T, EpiPartials& P) {
 #pragma unroll
   for (int ch = 0; ch < NCH; ++ch) {
     const int gj0 = j0 + ch * 32;
@@ -381,9 +421,10 @@ __device__ __forceinline__ void epilogue_row(const float* acc, EpiOld& old, int 
     const uint4* nxm = (ch + 1 < NCH) ? reinterpret_cast<const uint4*>(in_m + (size_t)gi * npad + gj0 + 32) : nullptr;
     // gi = 32-aligned base + lane and gj0 is 32-aligned, so both tests are warp-uniform
     if (gj0 > gi) {                           // entirely above the diagonal
-      epilogue_chunk<true>(&acc[ch * 32], old, nxh, nxm, gi, gj0, npad, out_h, out_m, a1hi, a1lo, a2, dsh_hi, dsh_lo, lo_round, lo_mask, P);
+      epilogue_chunk_full(&acc[ch * 32], old, nxh, nxm, gi, gj0, npad, out_h, out_m, a1hi, a1lo, a2, lo_round, lo_mask, P);
     } else if (gj0 + 31 >= gi) {              // holds the diagonal
-      epilogue_chunk<false>(&acc[ch * 32], old, nxh, nxm, gi, gj0, npad, out_h, out_m, a1hi, a1lo, a2, dsh_hi, dsh_lo, lo_round, lo_mask, P);
+      epilogue_chunk_diag(&acc[ch * 32], old, nxh, nxm, gi, gj0, npad, out_h, out_m, a1hi, a1lo, a2, dsh_hi, dsh_lo,
+                          lo_round, lo_mask, T, P);
     } else if (nxh) {                         // entirely below: mirrored by its transpose; keep the prefetch rolling
       epilogue_prefetch(old, gi, gj0 + 32, npad, in_h, in_m);
     }
@@ -428,6 +469,64 @@ __device__ __forceinline__ void gemm_epilogue(const float* acc, int gi, int j0, 
 }
 
 // ----------------------------------------------------------------------------------------------
+// Persistent multi-layer mode (small and medium N, where a layer is shorter than a kernel launch and its tail):
+// ONE launch runs the whole stack.  Between layers the CTAs meet at a grid-wide barrier (every CTA of the grid is
+// resident: the grid is bounded by the co-residency query of sp2_create) that has two halves:
+//   arrive   each CTA stores its planes and its partial sums and takes a ticket (a counter that only grows);
+//   release  the CTA that draws the last ticket of the layer reduces the slots, runs the controller for the next
+//            layer and publishes the new epoch; the consumer warps of every CTA wait for that epoch.
+// The MMAs of layer n + 1 need the planes of layer n but NOT the controller's decision (branch and coefficients only
+// enter the epilogue), so the TMA producer waits for the arrive half alone (ticket count) and the tensor core runs
+// layer n + 1 while the controller of layer n is still at work.  When the controller says stop, that one layer has
+// been started in vain: the consumers drain its accumulators without an epilogue.  Barriers, TMEM and the pipeline
+// phases live across layers; the ping-pong planes swap by layer parity (both argument blocks live in global memory).
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+  asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+// generic-proxy global writes of this thread -> visible to later async-proxy (TMA) reads
+__device__ __forceinline__ void fence_proxy_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
+
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
+  unsigned int v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_u32(unsigned int* p, unsigned int v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// Reduce the per-CTA slots of one class with the 256 consumer threads (count <= 256): one slot per thread, fixed
+// shuffle tree, eight warp partials added in index order by thread 0.  Deterministic.  Result valid in thread 0.
+__device__ __forceinline__ void reduce_slots_fast(const Sp2Slot* slots, int count, double* red /* smem 4 x 8 */,
+                                                  double& tr, double& fro, double& mx, double& tracc) {
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  double a = 0.0, b = 0.0, d = 0.0, m = 0.0;
+  if (tid < count) {         // past L1: written by other CTAs of this kernel
+    a = __ldcg(&slots[tid].tr); b = __ldcg(&slots[tid].fro); d = __ldcg(&slots[tid].tracc); m = (double)__ldcg(&slots[tid].mx);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    a += __shfl_xor_sync(0xffffffffu, a, o);
+    b += __shfl_xor_sync(0xffffffffu, b, o);
+    d += __shfl_xor_sync(0xffffffffu, d, o);
+    const double q = __shfl_xor_sync(0xffffffffu, m, o);
+    m = (q > m || q != q) ? q : m;
+  }
+  if (lane == 0) { red[w] = a; red[8 + w] = b; red[16 + w] = d; red[24 + w] = m; }
+  named_bar_sync(1, kConsumerWarps * 32);
+  if (tid == 0) {
+    a = red[0]; b = red[8]; d = red[16]; m = red[24];
+    for (int k = 1; k < kConsumerWarps; ++k) {
+      a += red[k]; b += red[8 + k]; d += red[16 + k];
+      const double q = red[24 + k];
+      m = (q > m || q != q) ? q : m;
+    }
+    tr = a; fro = b; tracc = d; mx = m;
+  }
+  named_bar_sync(1, kConsumerWarps * 32);
+}
+
+// ----------------------------------------------------------------------------------------------
 // Warp roles (384 threads): warps 0..7 consumers; warp 8 TMA producer, warp 9 MMA issuer, warp 10 TMEM
 // allocator, warp 11 idle.  The k range of a unit is cut into segments of seg_kb k-blocks; each
 // segment is accumulated by the tensor core into a fresh TMEM buffer (2 buffers, ping-pong) and
@@ -436,8 +535,9 @@ __device__ __forceinline__ void gemm_epilogue(const float* acc, int gi, int j0, 
 // truncation bias") and costs no tensor time: the drain overlaps the next segment's MMAs.
 // MODE 0: one SP2 layer.  MODE 1: the same mainloop as a plain product C = A B^T of two hi/lo plane pairs (A = tm[0..1],
 // B = tm[2..3]; every tile, no mirror, no controller) for the congruence transforms of sp2_congruence.
-template <int CG, int MODE>
-__global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant__ Sp2LayerArgs a) {
+// PERSIST: the whole layer stack in one launch (see above); args[0] reads buffer 0 and writes buffer 1, args[1] the reverse.
+template <int CG, int MODE, bool PERSIST>
+__device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args) {
   constexpr int TILE = 128 * CG;          // output tile edge
   constexpr int UM = 128 * CG, UN = 128 * CG;
   constexpr int ACC_COLS = UN;            // FP32 accumulator columns per TMEM buffer
@@ -445,6 +545,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   constexpr int NCH = WCOLS / 32;         // 32-column chunks per consumer warp
   constexpr uint32_t TMEM_COLS = 2 * ACC_COLS;
   constexpr uint32_t IDESC = make_idesc(UM, UN);
+  static_assert(!(PERSIST && MODE == 1), "the plain-product mode is a single launch");
 
   // Programmatic dependent launch: let the next layer's CTAs be scheduled as soon as SMs free up; everything
   // up to griddepcontrol.wait below (barrier init, TMEM allocation, work-list offsets) then overlaps the tail
@@ -461,19 +562,24 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   const int cluster_id = blockIdx.x / CG;
   const bool leader = (rank == 0);
 
-  const int n_tiles = a.n_tiles;
-  const int KB = a.npad / kBK;            // ring stages per k sweep
-  const int seg_kb = a.seg_kb * (64 / kBK);   // ring stages per TMEM accumulation segment (divides KB)
-  const int item_lo = a.item_begin[cluster_id], item_hi = a.item_begin[cluster_id + 1];
-  const int nz_units = MODE == 1 ? 0 : a.with_response * n_tiles;   // units [0, nz_units): first-order, then the Y^2 units
+  const Sp2LayerArgs& a0 = args[0];       // everything but the planes / tensor maps is the same in both blocks
+  const int n_tiles = a0.n_tiles;
+  const int KB = a0.npad / kBK;            // ring stages per k sweep
+  const int seg_kb = a0.seg_kb * (64 / kBK);   // ring stages per TMEM accumulation segment (divides KB)
+  const int item_lo = a0.item_begin[cluster_id], item_hi = a0.item_begin[cluster_id + 1];
+  const int nz_units = MODE == 1 ? 0 : a0.with_response * n_tiles;   // units [0, nz_units): first-order, then the Y^2 units
 
   if (warp == kWarpTma && lane == 0) {
-    const int n_maps = MODE == 1 ? 4 : 2 + 2 * a.with_response;
-    for (int i = 0; i < n_maps; ++i) asm volatile("prefetch.tensormap [%0];" ::"l"(&a.tm[i]) : "memory");
+    const int n_maps = MODE == 1 ? 4 : 2 + 2 * a0.with_response;
+    for (int i = 0; i < n_maps; ++i) {
+      asm volatile("prefetch.tensormap [%0];" ::"l"(&args[0].tm[i]) : "memory");
+      if (PERSIST) asm volatile("prefetch.tensormap [%0];" ::"l"(&args[1].tm[i]) : "memory");
+    }
   }
   if (warp == kWarpMma && lane == 0) {
     for (int s = 0; s < kStages; ++s) { mbar_init(smem_u32(&bars->full[s]), 1); mbar_init(smem_u32(&bars->empty[s]), 1); }
     for (int s = 0; s < 2; ++s) { mbar_init(smem_u32(&bars->tmem_full[s]), 1); mbar_init(smem_u32(&bars->tmem_empty[s]), kConsumerWarps * CG); }
+    bars->stop = 0u; bars->prod_layers = 1u; bars->prod_final = 0u;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp < kConsumerWarps && lane < 1 + SP2_NB) {
@@ -487,7 +593,12 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
   const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(&bars->tmem_base);
 
   asm volatile("griddepcontrol.wait;" ::: "memory");    // previous layer complete, its writes visible
-  const bool active = MODE == 1 || *reinterpret_cast<volatile const int*>(&a.ctrl->done) == 0;   // uniform over the grid
+  const bool active = MODE == 1 || *reinterpret_cast<volatile const int*>(&a0.ctrl->done) == 0;   // uniform over the grid
+  // persistent mode: the layer about to run fixes which buffer is read.  The controller has already counted it
+  // (ctrl->n = its index + 1 while done == 0), so layer ctrl->n - 1 reads buffer (ctrl->n - 1) & 1.
+  int par = PERSIST ? ((*reinterpret_cast<volatile const int*>(&a0.ctrl->n) + 1) & 1) : 0;
+  // persistent mode: grid barriers passed before this launch (0 for the one launch of a solve: k_init clears the block)
+  const unsigned int epoch0 = PERSIST ? ld_acquire_u32(&a0.ctrl->epoch) : 0u;
 
   if (!active) {
     // converged (or failed) before this launch: nothing to do but release the TMEM columns
@@ -497,21 +608,23 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
       // =================================== TMA producer (one lane, every CTA) ==================
       if (elect_one()) {
         int stage = 0; uint32_t phase = 0;
+        unsigned int layers_loaded = 0;
         uint32_t full_bar[kStages];
         for (int s = 0; s < kStages; ++s) {
           full_bar[s] = smem_u32(&bars->full[s]);
           if constexpr (CG == 2) asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(full_bar[s]) : "r"(full_bar[s]), "r"(0));
         }
-        for (int iti = item_lo; iti < item_hi; ++iti) {
-          const Sp2Item I = a.items[iti];
-          const int u = I.unit;
-          const bool wunit = u < nz_units;           // Y Z_b + Z_b Y unit of perturbation b = u / n_tiles
-          const int zb = wunit ? u / n_tiles : 0;
-          const int2 tij = a.tiles[wunit ? u - zb * n_tiles : u - nz_units];
-          const int zpl = 2 + 2 * zb;                // planes of Z_b
-          const int row_a = tij.x * TILE + (int)rank * kRows;
-          const int row_b = tij.y * TILE + (int)rank * kRows;
-          {
+        for (;;) {
+          const Sp2LayerArgs& a = args[par];
+          for (int iti = item_lo; iti < item_hi; ++iti) {
+            const Sp2Item I = a.items[iti];
+            const int u = I.unit;
+            const bool wunit = u < nz_units;           // Y Z_b + Z_b Y unit of perturbation b = u / n_tiles
+            const int zb = wunit ? u / n_tiles : 0;
+            const int2 tij = a.tiles[wunit ? u - zb * n_tiles : u - nz_units];
+            const int zpl = 2 + 2 * zb;                // planes of Z_b
+            const int row_a = tij.x * TILE + (int)rank * kRows;
+            const int row_b = tij.y * TILE + (int)rank * kRows;
             for (int g = I.seg0 * seg_kb; g < I.seg1 * seg_kb; ++g) {
               // Y^2: A = (Yh, Ym), B = (Yh, Ym).  W pass 0: A = (Yh, Ym), B = (Zh, Zm).  W pass 1: A = (Zh, Zm), B = (Yh, Ym).
               const int p = (g >= KB) ? 1 : 0;
@@ -528,42 +641,69 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
               if (++stage == kStages) { stage = 0; phase ^= 1u; }
             }
           }
+          if (!PERSIST) break;
+          // arrive half of the grid barrier: every CTA has stored its planes of the layer just loaded.  (When the
+          // controller stops, no CTA arrives for the layer after: the consumers raise `stop` instead.  The ticket is
+          // tested first, so the one speculative layer is ALWAYS started and the consumers always drain exactly one.)
+          ++layers_loaded;
+          bool more = false;
+          for (long long spins = 0;; ++spins) {
+            if (ld_acquire_u32(&a.ctrl->ticket) >= (epoch0 + layers_loaded) * gridDim.x) { more = true; break; }
+            if (*reinterpret_cast<volatile const uint32_t*>(&bars->stop)) break;
+            if (spins > kSpinLimit) __trap();
+          }
+          if (!more) { *reinterpret_cast<volatile uint32_t*>(&bars->prod_final) = 1u; break; }
+          fence_proxy_async_global();
+          *reinterpret_cast<volatile uint32_t*>(&bars->prod_layers) = layers_loaded + 1u;
+          par ^= 1;
         }
       }
     } else if (warp == kWarpMma) {
       // =================================== MMA issuer (one lane of the leader CTA) ==============
       if (leader && elect_one()) {
         int stage = 0; uint32_t phase = 0;
+        unsigned int layers_issued = 0;
         int as = 0; uint32_t aphase = 0;
-        for (int iti = item_lo; iti < item_hi; ++iti) {
-          const Sp2Item I = a.items[iti];
-          for (int sg = I.seg0; sg < I.seg1; ++sg) {
-            mbar_wait(smem_u32(&bars->tmem_empty[as]), aphase ^ 1u);
-            tc_fence_after();
-            const uint32_t acc = tmem_base + (uint32_t)(as * ACC_COLS);
-            for (int it = 0; it < seg_kb; ++it) {
-              mbar_wait(smem_u32(&bars->full[stage]), phase);
+        for (;;) {
+          for (int iti = item_lo; iti < item_hi; ++iti) {
+            const Sp2Item I = a0.items[iti];
+            for (int sg = I.seg0; sg < I.seg1; ++sg) {
+              mbar_wait(smem_u32(&bars->tmem_empty[as]), aphase ^ 1u);
               tc_fence_after();
-              const uint32_t sa = smem_u32(smem + stage * kStageBytes);
-              const uint64_t dA0 = make_smem_desc(sa + 0 * kPlaneTileBytes);
-              const uint64_t dA1 = make_smem_desc(sa + 1 * kPlaneTileBytes);
-              const uint64_t dB0 = make_smem_desc(sa + 2 * kPlaneTileBytes);
-              const uint64_t dB1 = make_smem_desc(sa + 3 * kPlaneTileBytes);
+              const uint32_t acc = tmem_base + (uint32_t)(as * ACC_COLS);
+              for (int it = 0; it < seg_kb; ++it) {
+                mbar_wait(smem_u32(&bars->full[stage]), phase);
+                tc_fence_after();
+                const uint32_t sa = smem_u32(smem + stage * kStageBytes);
+                const uint64_t dA0 = make_smem_desc(sa + 0 * kPlaneTileBytes);
+                const uint64_t dA1 = make_smem_desc(sa + 1 * kPlaneTileBytes);
+                const uint64_t dB0 = make_smem_desc(sa + 2 * kPlaneTileBytes);
+                const uint64_t dB1 = make_smem_desc(sa + 3 * kPlaneTileBytes);
 #pragma unroll
-              for (int k = 0; k < kBK / 16; ++k) {
-                const uint64_t ko = (uint64_t)(k * 2);     // 16 elements * 2 B = 32 B -> >>4 = 2
-                // small cross terms first, the dominant hi*hi product last
-                // the two products with A.hi are adjacent: A.hi is read from shared memory once (collector buffer)
-                umma_f16<CG>(acc, dA1 + ko, dB0 + ko, IDESC, (it | k) ? 1u : 0u);
-                umma_f16<CG, 1>(acc, dA0 + ko, dB1 + ko, IDESC, 1u);
-                umma_f16<CG, 2>(acc, dA0 + ko, dB0 + ko, IDESC, 1u);
+                for (int k = 0; k < kBK / 16; ++k) {
+                  const uint64_t ko = (uint64_t)(k * 2);     // 16 elements * 2 B = 32 B -> >>4 = 2
+                  // small cross terms first, the dominant hi*hi product last
+                  // the two products with A.hi are adjacent: A.hi is read from shared memory once (collector buffer)
+                  umma_f16<CG>(acc, dA1 + ko, dB0 + ko, IDESC, (it | k) ? 1u : 0u);
+                  umma_f16<CG, 1>(acc, dA0 + ko, dB1 + ko, IDESC, 1u);
+                  umma_f16<CG, 2>(acc, dA0 + ko, dB0 + ko, IDESC, 1u);
+                }
+                umma_commit<CG>(smem_u32(&bars->empty[stage]));   // smem slot free when these MMAs retire
+                if (++stage == kStages) { stage = 0; phase ^= 1u; }
               }
-              umma_commit<CG>(smem_u32(&bars->empty[stage]));   // smem slot free when these MMAs retire
-              if (++stage == kStages) { stage = 0; phase ^= 1u; }
+              umma_commit<CG>(smem_u32(&bars->tmem_full[as]));     // segment accumulator complete
+              if (++as == 2) { as = 0; aphase ^= 1u; }
             }
-            umma_commit<CG>(smem_u32(&bars->tmem_full[as]));     // segment accumulator complete
-            if (++as == 2) { as = 0; aphase ^= 1u; }
           }
+          if (!PERSIST) break;
+          ++layers_issued;                         // follow the producer: another layer, or the end
+          bool more = false;
+          for (long long spins = 0;; ++spins) {
+            if (*reinterpret_cast<volatile const uint32_t*>(&bars->prod_layers) > layers_issued) { more = true; break; }
+            if (*reinterpret_cast<volatile const uint32_t*>(&bars->prod_final)) break;
+            if (spins > kSpinLimit) __trap();
+          }
+          if (!more) break;
         }
       }
     }
@@ -573,14 +713,18 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
     const int cw = warp;
     const int q = warp & 3;                       // TMEM lane quarter this warp may read
     const int hh = cw >> 2;                       // which half of the accumulator columns
-    const float cf_a1y_hi = a.ctrl->coef.a1y_hi, cf_a1y_lo = a.ctrl->coef.a1y_lo, cf_a2y = a.ctrl->coef.a2y;
-    const float cf_dsh_hi = a.ctrl->coef.dsh_hi, cf_dsh_lo = a.ctrl->coef.dsh_lo;
-    const double gemm_scale = MODE == 1 ? sp2_exp2i((a.out_kind == 0 ? a.ctrl->g_et : 0) - a.ctrl->g_ea - a.ctrl->g_eb) : 0.0;
+    const double gemm_scale = MODE == 1 ? sp2_exp2i((a0.out_kind == 0 ? a0.ctrl->g_et : 0) - a0.ctrl->g_ea - a0.ctrl->g_eb) : 0.0;
     // optional power saving: round the lo plane to lo_bits significant bits (fewer toggling multiplier inputs)
-    const int drop = 11 - a.lo_bits;
+    const int drop = 11 - a0.lo_bits;
     const uint32_t lo_mask = drop > 0 ? ~(((1u << drop) - 1u) * 0x00010001u) : 0xffffffffu;
     const uint32_t lo_round = drop > 0 ? (1u << (drop - 1)) * 0x00010001u : 0u;
     int as = 0; uint32_t aphase = 0;
+    unsigned int epoch = epoch0;
+    for (;;) {
+    const Sp2LayerArgs& a = args[par];
+    const volatile Sp2Coef* cz = &a.ctrl->coef;   // volatile: rewritten by another CTA between layers (persistent mode)
+    const float cf_a1y_hi = cz->a1y_hi, cf_a1y_lo = cz->a1y_lo, cf_a2y = cz->a2y;
+    const float cf_dsh_hi = cz->dsh_hi, cf_dsh_lo = cz->dsh_lo;
     for (int iti = item_lo; iti < item_hi; ++iti) {
       const Sp2Item I = a.items[iti];
       const int u = I.unit;
@@ -654,14 +798,13 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
         continue;
       }
       // ---- fused epilogue from the register sums
-      const Sp2Coef* cz = &a.ctrl->coef;
       const float a1hi = wunit ? cz->a1z_hi[zb] : cf_a1y_hi, a1lo = wunit ? cz->a1z_lo[zb] : cf_a1y_lo;
       const float a2 = wunit ? cz->a2z[zb] : cf_a2y;
       const bool shift_row = !wunit && gi < a.n;        // zero padding stays zero
       const float dsh_hi = shift_row ? cf_dsh_hi : 0.f, dsh_lo = shift_row ? cf_dsh_lo : 0.f;
       EpiPartials P; P.tr = 0.0; P.fro = 0.0; P.tracc = 0.0; P.mx = 0.f;
       epilogue_row<NCH>(sums, old, gi, j0, (size_t)a.npad, a.in[pl], a.in[pl + 1], a.out[pl], a.out[pl + 1],
-                        a1hi, a1lo, a2, dsh_hi, dsh_lo, lo_round, lo_mask, P);
+                        a1hi, a1lo, a2, dsh_hi, dsh_lo, lo_round, lo_mask, bars->diag_t[q], P);
       // warp partial -> slot (fixed shuffle tree: deterministic)
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {
@@ -678,13 +821,118 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
         s.mx = (P.mx > s.mx || P.mx != P.mx) ? P.mx : s.mx;   // NaN-propagating max
       }
     }
+    if constexpr (!PERSIST) {
+      break;
+    } else {
+      // ================================ end of a layer: grid-wide barrier ======================
+      constexpr int NT = kConsumerWarps * 32;
+      const int nb = a.with_response;
+      const int nblk = (int)gridDim.x;
+      fence_proxy_async_global();                  // this thread's plane stores -> visible to the next layer's TMA loads
+      __threadfence();
+      named_bar_sync(1, NT);
+      if ((int)threadIdx.x < 1 + nb) {             // one slot per CTA and class: [z_0 .. z_{nb-1}][y], gridDim.x each
+        const int cls = threadIdx.x;
+        Sp2Slot t = bars->acc[0][cls];
+        for (int w = 1; w < kConsumerWarps; ++w) {
+          const Sp2Slot& o = bars->acc[w][cls];
+          t.tr += o.tr; t.fro += o.fro; t.tracc += o.tracc;
+          t.mx = (o.mx > t.mx || o.mx != o.mx) ? o.mx : t.mx;
+        }
+        a.slots[(size_t)(cls == 0 ? nb : cls - 1) * nblk + blockIdx.x] = t;
+        Sp2Slot z; z.tr = 0.0; z.fro = 0.0; z.tracc = 0.0; z.mx = 0.f; z.pad = 0.f;
+        for (int w = 0; w < kConsumerWarps; ++w) bars->acc[w][cls] = z;
+        __threadfence();
+      }
+      named_bar_sync(1, NT);
+      ++epoch;
+      if (threadIdx.x == 0) {                      // arrive: the ticket only grows, epoch * nblk tickets end layer `epoch`
+        const unsigned int old_t = atomicAdd(&a.ctrl->ticket, 1u);
+        bars->is_last = (old_t == epoch * (unsigned int)nblk - 1u) ? 1u : 0u;
+      }
+      named_bar_sync(1, NT);
+      if (bars->is_last) {
+        __threadfence();
+        // The control block and the slots were last written by OTHER CTAs of this kernel, and this SM may hold stale
+        // copies of those lines in L1 from an earlier layer: read them past L1 (ld.cg), run the controller on a
+        // copy (below the ring's first stage would be busy with the next layer's loads: the copy lives next to the
+        // barriers) and write the changed part back.  Only the head of the block and the history entries of this
+        // layer move.
+        Sp2Ctrl* gctrl = a.ctrl;
+        Sp2Ctrl* ctrl = reinterpret_cast<Sp2Ctrl*>(bars->ctrl_copy);
+        {
+          const uint32_t* src = reinterpret_cast<const uint32_t*>(gctrl);
+          uint32_t* dst = reinterpret_cast<uint32_t*>(ctrl);
+          for (int i = threadIdx.x; i < (int)(SP2_CTRL_HEAD_BYTES / 4); i += NT) dst[i] = __ldcg(src + i);
+        }
+        for (int i = threadIdx.x; i < a.n_flags; i += NT) a.flags[i] = 0u;   // every split unit was consumed
+        named_bar_sync(1, NT);
+        double* redf = reinterpret_cast<double*>(bars->red);
+        double tr, fro, mx, tracc, unused;
+        reduce_slots_fast(a.slots + (size_t)nb * nblk, nblk, redf, tr, fro, mx, tracc);
+        for (int b = 0; b < nb; ++b) {
+          double trz, froz, mxz;
+          reduce_slots_fast(a.slots + (size_t)b * nblk, nblk, redf, trz, froz, mxz, unused);
+          if (threadIdx.x == 0) {
+            const double sz = sp2_exp2i(-ctrl->u[b]);
+            ctrl->tr_z[b] = trz * sz; ctrl->fro_z[b] = froz * sz * sz; ctrl->max_z[b] = mxz * sz;
+          }
+        }
+        if (threadIdx.x == 0) {
+          const int n = ctrl->n;                   // the controller reads e[n - 2] and writes tr_x[n], e[n]
+          if (n >= 2 && n < SP2_LAYER_CAP) ctrl->e[n - 2] = __ldcg(&gctrl->e[n - 2]);
+          sp2_trace_identity(ctrl, tracc);
+          const double sy = sp2_exp2i(-ctrl->t);
+          ctrl->tr_y = tr * sy; ctrl->fro_y = fro * sy * sy; ctrl->max_y = mx * sy;
+          sp2_controller(ctrl);
+          if (n < SP2_LAYER_CAP) { gctrl->tr_x[n] = ctrl->tr_x[n]; gctrl->e[n] = ctrl->e[n]; }
+        }
+        named_bar_sync(1, NT);
+        {
+          const uint32_t* src = reinterpret_cast<const uint32_t*>(ctrl);
+          uint32_t* dst = reinterpret_cast<uint32_t*>(gctrl);
+          for (int i = threadIdx.x; i < (int)(SP2_CTRL_HEAD_BYTES / 4); i += NT) dst[i] = src[i];   // (ticket, epoch: unchanged values)
+        }
+        __threadfence();
+        named_bar_sync(1, NT);
+        if (threadIdx.x == 0) st_release_u32(&gctrl->epoch, epoch);       // release half of the barrier
+      } else if (threadIdx.x == 0) {
+        long long spins = 0;
+        while ((int)(ld_acquire_u32(&a.ctrl->epoch) - epoch) < 0)
+          if (++spins > kSpinLimit) __trap();
+      }
+      named_bar_sync(1, NT);
+      const int done = *reinterpret_cast<volatile const int*>(&a.ctrl->done);
+      if (done) {
+        // the producer and the tensor core have started one more layer (see above): drain it, no epilogue
+        if (threadIdx.x == 0) *reinterpret_cast<volatile uint32_t*>(&bars->stop) = 1u;
+        for (int iti = item_lo; iti < item_hi; ++iti) {
+          const Sp2Item I = a.items[iti];
+          for (int sg = I.seg0; sg < I.seg1; ++sg) {
+            mbar_wait(smem_u32(&bars->tmem_full[as]), aphase);
+            tc_fence_after();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) {
+              if constexpr (CG == 2) mbar_arrive_cluster(smem_u32(&bars->tmem_empty[as]), 0);
+              else mbar_arrive(smem_u32(&bars->tmem_empty[as]));
+            }
+            if (++as == 2) { as = 0; aphase ^= 1u; }
+          }
+        }
+        break;
+      }
+      par ^= 1;
+    }
+    }
   }
 
   // ===================================== teardown ==============================================
   tc_fence_before();
   if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
   if (warp == kWarpAlloc) tmem_dealloc<CG>(tmem_base, TMEM_COLS);
-  if (!active) return;
+  if (!active || PERSIST) return;
+  const Sp2LayerArgs& a = a0;
   if constexpr (MODE == 1) {                     // last CTA re-arms the split-k flags; no controller
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -711,6 +959,18 @@ __global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant_
     a.slots[(size_t)(cls == 0 ? a.with_response : cls - 1) * gridDim.x + blockIdx.x] = t;
   }
   layer_tail(a.ctrl, a.slots, gridDim.x, gridDim.x, a.with_response, gridDim.x, &bars->is_last, red, a.flags, a.n_flags);
+}
+
+
+template <int CG, int MODE>
+__global__ void __launch_bounds__(kThreads, 1) k_layer_tc(const __grid_constant__ Sp2LayerArgs a) {
+  layer_body<CG, MODE, false>(&a);
+}
+
+// args: the two argument blocks (TMA descriptors included) in GLOBAL memory, written by the host before the launch
+template <int CG>
+__global__ void __launch_bounds__(kThreads, 1) k_layers_persist(const Sp2LayerArgs* __restrict__ args) {
+  layer_body<CG, 0, true>(args);
 }
 
 // ----------------------------------------------------------------------------------------------
@@ -811,6 +1071,8 @@ cudaError_t sp2_layer_configure() {
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_layer_tc<2, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_layer_tc<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(k_layer_tc<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_layers_persist<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(k_layers_persist<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   return e;
 }
 
@@ -863,4 +1125,25 @@ cudaError_t sp2_launch_layer(const Sp2LayerArgs& args, int engine, int cta_group
   }
   cfg.gridDim = dim3(args.n_clusters);
   return args.gemm_mode ? cudaLaunchKernelEx(&cfg, k_layer_tc<1, 1>, args) : cudaLaunchKernelEx(&cfg, k_layer_tc<1, 0>, args);
+}
+
+// The whole layer stack in ONE launch (persistent multi-layer mode): d_args = two argument blocks in DEVICE memory
+// (d_args[0] reads buffer 0 and writes buffer 1, d_args[1] the reverse); `grid_clusters` CTA(-pair)s (those with
+// work), all of which must be co-resident.
+cudaError_t sp2_launch_layers_persistent(const Sp2LayerArgs* d_args, int cta_group, int grid_clusters, cudaStream_t s) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = sp2_layer_smem_bytes();
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  cfg.attrs = attr; cfg.numAttrs = 0;
+  if (cta_group == 2) {
+    cfg.gridDim = dim3(2 * grid_clusters);
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, k_layers_persist<2>, d_args);
+  }
+  cfg.gridDim = dim3(grid_clusters);
+  return cudaLaunchKernelEx(&cfg, k_layers_persist<1>, d_args);
 }

@@ -51,3 +51,4 @@ cudaError_t sp2_layer_configure();
 cudaError_t sp2_layer_max_coresident(int cta_group, int num_sms, int* out);
 cudaError_t sp2_launch_layer(const Sp2LayerArgs& args, int engine, int cta_group, cudaStream_t s);
 size_t sp2_layer_scratch_slot_bytes(int cta_group);
+cudaError_t sp2_launch_layers_persistent(const Sp2LayerArgs* d_args, int cta_group, int grid_clusters, cudaStream_t s);

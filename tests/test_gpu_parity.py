@@ -91,16 +91,40 @@ def test_config2_n1024_response(sp2, torch_mod):
     assert np.abs(D1 - D1_pt).max() <= TOL_D1 * np.abs(D1_pt).max()
 
 
+@pytest.mark.parametrize("persistent", [1, 2])
 @pytest.mark.parametrize("cta_group", [1, 2])
 @pytest.mark.parametrize("n, base, response", [(300, 2, True), (77, 1, False), (520, 3, False), (641, 4, True)])
-def test_ragged_sizes_both_tile_shapes(sp2, torch_mod, n, base, response, cta_group):
+def test_ragged_sizes_both_tile_shapes(sp2, torch_mod, n, base, response, cta_group, persistent):
     """Sizes that are not tile multiples (zero padding must stay inert), several tiles, f32 and f64
-    inputs, 1/2 and 2/3 filling, both CTA-group code paths."""
+    inputs, 1/2 and 2/3 filling, both CTA-group code paths, and both ways of running the stack: ONE persistent launch
+    with a grid-wide barrier between layers (persistent = 1, the default up to N = 2048) or one launch per layer (2)."""
     import oracle
 
     p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[base], n), want_h1=response)
-    D, D1, r = _solve(sp2, torch_mod, p, response=response, cta_group=cta_group)
+    D, D1, r = _solve(sp2, torch_mod, p, response=response, cta_group=cta_group, persistent=persistent)
     _check_against_oracle(p, D, D1, r, oracle)
+    if persistent == 1:
+        assert r["kernel_launches"] <= 12            # prologue + ONE layer-stack launch + finalise
+
+
+def test_persistent_stack_matches_per_layer_launches(sp2, torch_mod):
+    """The persistent multi-layer kernel and the launch-per-layer path run the same layers (same branches; the
+    grid-wide reductions add in a different order, so the last bits may differ): N = 1100 response (81 + 162 work
+    units over every SM, split-k tails, ~30 grid barriers), and a size above the automatic switch forced on."""
+    import oracle
+
+    for n, base in ((1100, 2), (2304, 2)):
+        p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[base], n), device="cuda" if n > 2048 else "cpu")
+        a = _solve(sp2, torch_mod, p, persistent=1)
+        b = _solve(sp2, torch_mod, p, persistent=2)
+        assert a[2]["status"] == 0 and b[2]["status"] == 0
+        assert a[2]["layers"] == b[2]["layers"] and a[2]["signs"] == b[2]["signs"]
+        assert np.abs(a[0] - b[0]).max() <= 1e-6 and np.abs(a[1] - b[1]).max() <= 1e-6 * np.abs(b[1]).max()
+        assert a[2]["kernel_launches"] <= 12 < b[2]["kernel_launches"]
+        if n <= 1100:
+            _check_against_oracle(p, a[0], a[1], a[2], oracle)
+        again = _solve(sp2, torch_mod, p, persistent=1)                  # deterministic: bitwise reproducible
+        assert np.array_equal(a[0], again[0]) and np.array_equal(a[1], again[1])
 
 
 def test_segment_lengths_and_simt_scaffold_agree(sp2, torch_mod):
@@ -320,6 +344,7 @@ def test_layer_count_hint_and_top_up(sp2, torch_mod):
     easy = inputs.make_problem(inputs.Sp2Config("easy", 1, 256, 128, (-2.0, -1.0), (1.0, 2.0), "f64", False))
     hard = inputs.make_problem(inputs.Sp2Config("hard", 4, 256, 128, (-1.0, -0.004), (0.004, 1.0), "f64", False))
     h = sp2.Sp2Handle(256)
+    h.set_options(persistent=2)                       # one launch per layer (the path every N > 2048 takes)
     He, Hh = torch.from_numpy(easy["H"]).cuda(), torch.from_numpy(hard["H"]).cuda()
     D1, r1 = h.density(He, 128)                       # no hint yet: max_layers launches
     D2, r2 = h.density(He, 128)                       # hint = layers + 6
