@@ -103,9 +103,10 @@ typedef struct {
                        draw less power: lo_bits = 8 measured 1.8 % faster at ~3x larger max|dD|, still > 1000x inside
                        the bar; kept as an experiment knob, not a recommendation */
   int no_recentre;  /* debug, with forced_layers only: keep c on the scalar map instead of the cluster midpoint */
-  int persistent;   /* 0 = auto (on up to N = 2048); 1 = on; 2 = off.  On: the whole layer stack runs in ONE persistent
-                       launch with a grid-wide barrier between layers (no launch, no kernel prologue and a much shorter
-                       tail per layer: what bounds small problems); off: one launch per layer */
+  int persistent;   /* how the layer stack is launched.  0 = auto: N <= 128 (and at most 2 perturbations): ONE CTA with the
+                       iterate resident in shared memory, nothing leaves the SM between layers; N <= 2048: ONE persistent
+                       launch of the multi-CTA kernel with a grid-wide barrier between layers; above: one launch per layer.
+                       1 = the persistent multi-CTA kernel at any size; 2 = one launch per layer at any size */
   int max_ctas;     /* 0 = one CTA per SM (default); > 0: use at most this many CTAs for the layer kernel, e.g. to leave SMs
                        to other work on the same GPU (the layer grid must be co-resident, see "Conventions") */
 } sp2_options_t;

@@ -17,8 +17,8 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(PKG, "libsp2_b200.so")
-SOURCES = ["sp2_api.cu", "sp2_prologue.cu", "sp2_layer.cu", "sp2_refine.cu"]
-HEADERS = [os.path.join(CSRC, "sp2_internal.cuh"), os.path.join(CSRC, "sp2_layer.h"), os.path.join(INCLUDE, "sp2.h")]
+SOURCES = ["sp2_api.cu", "sp2_prologue.cu", "sp2_layer.cu", "sp2_small.cu", "sp2_refine.cu"]
+HEADERS = [os.path.join(CSRC, "sp2_internal.cuh"), os.path.join(CSRC, "sp2_layer.h"), os.path.join(CSRC, "sp2_ptx.cuh"), os.path.join(INCLUDE, "sp2.h")]
 
 
 def _nvcc():

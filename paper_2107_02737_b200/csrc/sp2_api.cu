@@ -482,6 +482,12 @@ sp2_status_t check_args(sp2_handle_t h, const void* H, const Pert& P, sp2_dtype_
 
 // One persistent launch for the whole stack?  Small problems: a layer is shorter than a launch and its tail.
 constexpr int kPersistMaxNpad = 2048;
+// The smallest problems: one CTA, iterate resident in shared memory (sp2_small.cu).  Automatic choice only.
+bool use_small(sp2_handle_t h) {
+  return h->opt.engine == SP2_ENGINE_TCGEN05 && h->opt.persistent == 0 && h->cur_n <= sp2_small_max_n() &&
+         h->cur_resp <= sp2_small_max_nb();
+}
+
 bool use_persistent(sp2_handle_t h) {
   if (h->opt.engine != SP2_ENGINE_TCGEN05 || h->opt.persistent == 2) return false;
   return h->opt.persistent == 1 || h->cur_npad <= kPersistMaxNpad;
@@ -489,6 +495,13 @@ bool use_persistent(sp2_handle_t h) {
 
 // enqueue layer launches [first, first + count) on `s`
 sp2_status_t enqueue_layers(sp2_handle_t h, int first, int count, cudaStream_t s, int* launches) {
+  if (use_small(h)) {
+    if (count <= 0) return SP2_OK;
+    cudaError_t e = sp2_launch_small(h->args[0], h->cur_npad, s);
+    if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
+    ++*launches;
+    return SP2_OK;
+  }
   if (use_persistent(h)) {       // the kernel loops until the device controller stops (it starts at layer ctrl->n)
     if (count <= 0) return SP2_OK;
     cudaError_t e = sp2_launch_layers_persistent(h->d_args(), h->cur_cg, h->n_active, s);
@@ -752,7 +765,9 @@ sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_work
   cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
   if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn) { delete h; return SP2_ERR_CUDA; }
   h->encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(fn);
-  if (sp2_layer_configure() != cudaSuccess || sp2_refine_configure() != cudaSuccess) { delete h; return SP2_ERR_CUDA; }
+  if (sp2_layer_configure() != cudaSuccess || sp2_refine_configure() != cudaSuccess || sp2_small_configure() != cudaSuccess) {
+    delete h; return SP2_ERR_CUDA;
+  }
   // The layer kernel is persistent and its last-wave units hand partial sums between CTAs, so every CTA(-pair) of a
   // launch must be able to run at once: size the grid by what the device can keep co-resident, fail here (not
   // with a device-side trap later) if the kernel does not fit at all.

@@ -86,7 +86,12 @@ struct Sp2Ctrl {
 
 // ----------------------------------------------------------------------------------------------
 // small device helpers
-__device__ __forceinline__ double sp2_exp2i(int k) { return scalbn(1.0, k); }
+// 2^k exactly: built from the exponent bits for normal results (every plane exponent lands here; the controller
+// runs in ONE thread on the critical path of each layer, and scalbn is a slow library call), scalbn otherwise
+__device__ __forceinline__ double sp2_exp2i(int k) {
+  if (k >= -1022 && k <= 1023) return __longlong_as_double((long long)(1023 + k) << 52);
+  return scalbn(1.0, k);
+}
 
 // largest k with bound * 2^k <= 2^SP2_FP16_TARGET_LOG2, clamped so that every epilogue
 // coefficient 2^(t'-2t) stays an fp32 normal.

@@ -52,3 +52,10 @@ cudaError_t sp2_layer_max_coresident(int cta_group, int num_sms, int* out);
 cudaError_t sp2_launch_layer(const Sp2LayerArgs& args, int engine, int cta_group, cudaStream_t s);
 size_t sp2_layer_scratch_slot_bytes(int cta_group);
 cudaError_t sp2_launch_layers_persistent(const Sp2LayerArgs* d_args, int cta_group, int grid_clusters, cudaStream_t s);
+
+// sp2_small.cu: the whole stack of a small problem (N <= sp2_small_max_n(), at most sp2_small_max_nb() perturbations) in
+// one launch of one CTA, iterate resident in shared memory.  args0 = the argument block of layer parity 0.
+int sp2_small_max_n();
+int sp2_small_max_nb();
+cudaError_t sp2_small_configure();
+cudaError_t sp2_launch_small(const Sp2LayerArgs& args0, int npad_g, cudaStream_t s);

@@ -91,7 +91,7 @@ def test_config2_n1024_response(sp2, torch_mod):
     assert np.abs(D1 - D1_pt).max() <= TOL_D1 * np.abs(D1_pt).max()
 
 
-@pytest.mark.parametrize("persistent", [1, 2])
+@pytest.mark.parametrize("persistent", [0, 1, 2])
 @pytest.mark.parametrize("cta_group", [1, 2])
 @pytest.mark.parametrize("n, base, response", [(300, 2, True), (77, 1, False), (520, 3, False), (641, 4, True)])
 def test_ragged_sizes_both_tile_shapes(sp2, torch_mod, n, base, response, cta_group, persistent):
