@@ -450,10 +450,12 @@ def run_ours(args):
     h = sp2.Sp2Handle(n, response=response, host_staging=True, refinement=args.refine > 0)
     if args.lanczos > 0:
         h.set_options(lanczos_steps=args.lanczos)
+    if args.max_ctas > 0 or args.persistent or args.seg_kb:
+        h.set_options(max_ctas=args.max_ctas, persistent=args.persistent, seg_kb=args.seg_kb)
     if args.refine > 0:
         if response:
             raise SystemExit("--refine goes with a density workload")
-        h.set_options(refine_layers=args.refine, lanczos_steps=args.lanczos)
+        h.set_options(refine_layers=args.refine)
 
     def step():
         if response:
@@ -822,6 +824,9 @@ def main(argv=None):
                     help="Lanczos steps for tighter spectral bounds (SURVEY 8(f) NEXT-3); extra, not the headline")
     ap.add_argument("--refine", type=int, default=0,
                     help="float64 refinement layers after the stack (PAPER.md:170; density workloads only); extra, not the headline")
+    ap.add_argument("--persistent", type=int, default=0, help="sp2_options_t.persistent (0 auto, 1 persistent kernel, 2 launch per layer)")
+    ap.add_argument("--seg-kb", type=int, default=0, help="sp2_options_t.seg_kb (0 = default)")
+    ap.add_argument("--max-ctas", type=int, default=0, help="sp2_options_t.max_ctas: use at most this many CTAs (0 = one per SM)")
     ap.add_argument("--stub-ms", type=float, default=0.0, help=argparse.SUPPRESS)   # test hook, see run_stub
     args = ap.parse_args(argv)
     if args.steps is None:
