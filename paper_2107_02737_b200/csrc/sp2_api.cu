@@ -518,8 +518,9 @@ sp2_status_t enqueue_layers(sp2_handle_t h, int first, int count, cudaStream_t s
 }
 
 sp2_status_t enqueue_finalise(sp2_handle_t h, const void* H, sp2_dtype_t in_dt, long ldh, int N, const Pert& P, void* D,
-                              sp2_dtype_t out_dt, long ldd, int ring_idx, cudaStream_t s, int* launches) {
-  for (int b = 0; b < (P.nb > 0 ? P.nb : 1); ++b) {   // D (+ D1_0), then D1_b alone for the rest of a batch
+                              sp2_dtype_t out_dt, long ldd, int ring_idx, cudaStream_t s, int* launches,
+                              bool refine_only = false) {
+  for (int b = 0; b < (P.nb > 0 ? P.nb : 1) && !refine_only; ++b) {   // D (+ D1_0), then D1_b alone for the rest of a batch
     const int zh = P.nb ? 2 + 2 * b : 0, zm = P.nb ? 3 + 2 * b : 1;
     __half* planes[8] = {h->plane(0, 0), h->plane(1, 0), h->plane(0, 1), h->plane(1, 1),
                          h->plane(zh, 0), h->plane(zm, 0), h->plane(zh, 1), h->plane(zm, 1)};
@@ -527,8 +528,10 @@ sp2_status_t enqueue_finalise(sp2_handle_t h, const void* H, sp2_dtype_t in_dt, 
                         ldd, N, b, h->fslots(), s);
     ++*launches;
   }
-  sp2_launch_finalise_reduce(h->ctrl(), N, h->fslots(), h->ring() + ring_idx, s);
-  ++*launches;
+  if (!refine_only) {
+    sp2_launch_finalise_reduce(h->ctrl(), N, h->fslots(), h->ring() + ring_idx, s);
+    ++*launches;
+  }
   const int nref = h->opt.refine_layers;
   if (nref > 0) {   // float64 refinement layers on the converged iterate; overwrites D, tr D, tr(DH)
     __half* yp[4] = {h->plane(0, 0), h->plane(1, 0), h->plane(0, 1), h->plane(1, 1)};
@@ -584,6 +587,25 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dty
         h->touch(h->L.r_refine_slots, refine_slot_doubles((size_t)npad) * sizeof(double));
       }
     }
+  }
+  if (use_small(h) && !lanczos_active(h, N, N_occ) && N_occ > 0 && N_occ < N) {
+    // the smallest problems: prologue, layer stack and finalise in ONE launch of one CTA (sp2_small.cu)
+    Sp2SmallProblem sp;
+    memset(&sp, 0, sizeof(sp));
+    sp.H = H; sp.D = D; sp.ldh = ldh; sp.ldd = ldd;
+    for (int b = 0; b < resp; ++b) { sp.H1[b] = P.H1[b]; sp.D1[b] = P.D1[b]; }
+    sp.N = N; sp.n_occ = N_occ; sp.max_layers = max_layers; sp.user_bounds = o.user_bounds;
+    sp.eps_min = o.eps_min; sp.eps_max = o.eps_max; sp.tol = tol; sp.forced_signs = o.forced_signs;
+    sp.forced_layers = forced; sp.no_recentre = o.no_recentre;
+    sp.in_f64 = in_dt == SP2_F64; sp.out_f64 = out_dt == SP2_F64; sp.ring_entry = h->ring() + ring_idx;
+    if (h->time_layers) SP2_CUDA(h, cudaEventRecord(h->evl0, s));
+    SP2_CUDA(h, sp2_launch_small_solve(h->args[0], npad, sp, s));
+    ++launches;
+    if (h->time_layers) SP2_CUDA(h, cudaEventRecord(h->evl1, s));
+    enqueue_finalise(h, H, in_dt, ldh, N, P, D, out_dt, ldd, ring_idx, s, &launches, true);   // float64 refinement, if asked for
+    h->launches += (unsigned long long)launches;
+    if (launches_out) *launches_out = launches;
+    return SP2_OK;
   }
   sp2_launch_init(c, N, N_occ, npad, resp, max_layers, o.user_bounds, o.eps_min, o.eps_max, tol, forced, o.forced_signs, o.no_recentre, s);
   ++launches;

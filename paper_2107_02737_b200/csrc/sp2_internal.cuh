@@ -108,6 +108,34 @@ __device__ __forceinline__ void sp2_split_f32(double a, float& hi, float& lo) {
   lo = (float)(a - (double)hi);
 }
 
+// The input layer from the reduced bounds (SURVEY 8(a) a1 -> a2): spectral interval, Delta, the first shift and the
+// first plane exponents.  One thread.  lo/hi: Gershgorin interval; tr: tr H; mx: max|H|; sum: sum of |H| (and |H1|):
+// the non-finite detector; c->maxabs_h1[b] already set for the nb perturbations.
+__device__ inline void sp2_setup_input_layer(Sp2Ctrl* c, double lo, double hi, double tr, double mx, double sum, int nb) {
+  c->tr_h = tr;
+  c->maxabs_h = mx;
+  double eps_min = lo, eps_max = hi;
+  if (c->lanczos_steps > 0 && isfinite(c->lz_min) && isfinite(c->lz_max) && c->lz_max > c->lz_min) {
+    // tighter bounds from k Lanczos steps, never wider than the Gershgorin discs
+    eps_min = fmax(eps_min, c->lz_min);
+    eps_max = fmin(eps_max, c->lz_max);
+  }
+  if (c->user_bounds) { eps_min = c->user_eps_min; eps_max = c->user_eps_max; }
+  c->eps_min = eps_min; c->eps_max = eps_max;
+  const double delta = eps_max - eps_min;
+  c->delta = delta;
+  if (!isfinite(sum) || !isfinite(eps_min) || !isfinite(eps_max)) {
+    c->done = 1; c->status = SP2_ERR_NONFINITE; return;
+  }
+  if (!(delta > 0.0)) { c->done = 1; c->status = SP2_ERR_DEGENERATE; return; }
+  // X_0 = (eps_max I - H)/Delta;  c_0 = tr(X_0)/N;  Y_0 = X_0 - c_0 I
+  const double N = (double)c->N;
+  c->c = (eps_max - c->tr_h / N) / delta;
+  // |Y0_ij| <= (max|H| + |tr H|/N) / Delta
+  c->t = sp2_pick_exponent((c->maxabs_h + fabs(c->tr_h) / N) / delta);
+  for (int b = 0; b < nb; ++b) c->u[b] = sp2_pick_exponent(c->maxabs_h1[b] / delta);
+}
+
 // Stop test at the top of layer n ("until all eigenvalues ... sufficiently close to
 // 1 or 0"; "idempotency conditions ... estimated from traces of intermediate
 // matrices").  DESIGN.md reading R4.  Returns a stop_reason (0 = continue).

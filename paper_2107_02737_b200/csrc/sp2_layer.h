@@ -55,7 +55,21 @@ cudaError_t sp2_launch_layers_persistent(const Sp2LayerArgs* d_args, int cta_gro
 
 // sp2_small.cu: the whole stack of a small problem (N <= sp2_small_max_n(), at most sp2_small_max_nb() perturbations) in
 // one launch of one CTA, iterate resident in shared memory.  args0 = the argument block of layer parity 0.
+struct Sp2SmallProblem {   // everything k_small_solve needs beyond the plane pointers: k_init's arguments, the caller's matrices
+  const void* H;
+  const void* H1[2];
+  void* D;
+  void* D1[2];
+  long ldh, ldd;
+  int N, n_occ, max_layers, user_bounds;
+  double eps_min, eps_max, tol;
+  unsigned long long forced_signs;
+  int forced_layers, no_recentre;
+  int in_f64, out_f64;
+  sp2_result_t* ring_entry;
+};
 int sp2_small_max_n();
 int sp2_small_max_nb();
 cudaError_t sp2_small_configure();
 cudaError_t sp2_launch_small(const Sp2LayerArgs& args0, int npad_g, cudaStream_t s);
+cudaError_t sp2_launch_small_solve(const Sp2LayerArgs& args0, int npad_g, const Sp2SmallProblem& p, cudaStream_t s);

@@ -129,28 +129,7 @@ __global__ void __launch_bounds__(256) k_setup(Sp2Ctrl* c, const Sp2BoundSlot* s
     __syncthreads();
   }
   if (tid != 0) return;
-  c->tr_h = red[2][0];
-  c->maxabs_h = red[3][0];
-  double eps_min = red[0][0], eps_max = red[1][0];
-  if (c->lanczos_steps > 0 && isfinite(c->lz_min) && isfinite(c->lz_max) && c->lz_max > c->lz_min) {
-    // tighter bounds from k Lanczos steps, never wider than the Gershgorin discs
-    eps_min = fmax(eps_min, c->lz_min);
-    eps_max = fmin(eps_max, c->lz_max);
-  }
-  if (c->user_bounds) { eps_min = c->user_eps_min; eps_max = c->user_eps_max; }
-  c->eps_min = eps_min; c->eps_max = eps_max;
-  const double delta = eps_max - eps_min;
-  c->delta = delta;
-  if (!isfinite(red[4][0]) || !isfinite(eps_min) || !isfinite(eps_max)) {
-    c->done = 1; c->status = SP2_ERR_NONFINITE; return;
-  }
-  if (!(delta > 0.0)) { c->done = 1; c->status = SP2_ERR_DEGENERATE; return; }
-  // X_0 = (eps_max I - H)/Delta;  c_0 = tr(X_0)/N;  Y_0 = X_0 - c_0 I
-  const double N = (double)c->N;
-  c->c = (eps_max - c->tr_h / N) / delta;
-  // |Y0_ij| <= (max|H| + |tr H|/N) / Delta
-  c->t = sp2_pick_exponent((c->maxabs_h + fabs(c->tr_h) / N) / delta);
-  for (int b = 0; b < nb; ++b) c->u[b] = sp2_pick_exponent(c->maxabs_h1[b] / delta);
+  sp2_setup_input_layer(c, red[0][0], red[1][0], red[2][0], red[3][0], red[4][0], nb);
 }
 
 // ------------------------------------------------------------------------------------------
