@@ -382,6 +382,57 @@ __device__ __forceinline__ void reduce_slots_fast(const Sp2Slot* slots, int coun
   named_bar_sync(1, kConsumerWarps * 32);
 }
 
+// The release half of the grid barrier, run by the consumer warps of the CTA that drew the layer's last ticket: slot
+// reduction, controller, new epoch.  Not inlined: its double-precision scalar code must not add to the register
+// pressure of the layer loop (the cta_group::2 instantiation spilled 750 bytes per thread with it inline).
+__device__ __noinline__ void persist_tail(const Sp2LayerArgs& a, SmemBarriers* bars, unsigned int epoch, int nb, int nblk) {
+  constexpr int NT = kConsumerWarps * 32;
+        __threadfence();
+  // The control block and the slots were last written by OTHER CTAs of this kernel, and this SM may hold stale
+  // copies of those lines in L1 from an earlier layer: read them past L1 (ld.cg), run the controller on a
+  // copy (below the ring's first stage would be busy with the next layer's loads: the copy lives next to the
+  // barriers) and write the changed part back.  Only the head of the block and the history entries of this
+  // layer move.
+  Sp2Ctrl* gctrl = a.ctrl;
+  Sp2Ctrl* ctrl = reinterpret_cast<Sp2Ctrl*>(bars->ctrl_copy);
+  {
+    const uint32_t* src = reinterpret_cast<const uint32_t*>(gctrl);
+    uint32_t* dst = reinterpret_cast<uint32_t*>(ctrl);
+    for (int i = threadIdx.x; i < (int)(SP2_CTRL_HEAD_BYTES / 4); i += NT) dst[i] = __ldcg(src + i);
+  }
+  for (int i = threadIdx.x; i < a.n_flags; i += NT) a.flags[i] = 0u;   // every split unit was consumed
+  named_bar_sync(1, NT);
+  double* redf = reinterpret_cast<double*>(bars->red);
+  double tr, fro, mx, tracc, unused;
+  reduce_slots_fast(a.slots + (size_t)nb * nblk, nblk, redf, tr, fro, mx, tracc);
+  for (int b = 0; b < nb; ++b) {
+    double trz, froz, mxz;
+    reduce_slots_fast(a.slots + (size_t)b * nblk, nblk, redf, trz, froz, mxz, unused);
+    if (threadIdx.x == 0) {
+      const double sz = sp2_exp2i(-ctrl->u[b]);
+      ctrl->tr_z[b] = trz * sz; ctrl->fro_z[b] = froz * sz * sz; ctrl->max_z[b] = mxz * sz;
+    }
+  }
+  if (threadIdx.x == 0) {
+    const int n = ctrl->n;                   // the controller reads e[n - 2] and writes tr_x[n], e[n]
+    if (n >= 2 && n < SP2_LAYER_CAP) ctrl->e[n - 2] = __ldcg(&gctrl->e[n - 2]);
+    sp2_trace_identity(ctrl, tracc);
+    const double sy = sp2_exp2i(-ctrl->t);
+    ctrl->tr_y = tr * sy; ctrl->fro_y = fro * sy * sy; ctrl->max_y = mx * sy;
+    sp2_controller(ctrl);
+    if (n < SP2_LAYER_CAP) { gctrl->tr_x[n] = ctrl->tr_x[n]; gctrl->e[n] = ctrl->e[n]; }
+  }
+  named_bar_sync(1, NT);
+  {
+    const uint32_t* src = reinterpret_cast<const uint32_t*>(ctrl);
+    uint32_t* dst = reinterpret_cast<uint32_t*>(gctrl);
+    for (int i = threadIdx.x; i < (int)(SP2_CTRL_HEAD_BYTES / 4); i += NT) dst[i] = src[i];   // (ticket, epoch: unchanged values)
+  }
+  __threadfence();
+  named_bar_sync(1, NT);
+  if (threadIdx.x == 0) st_release_u32(&gctrl->epoch, epoch);       // release half of the barrier
+}
+
 // ----------------------------------------------------------------------------------------------
 // Warp roles (384 threads): warps 0..7 consumers; warp 8 TMA producer, warp 9 MMA issuer, warp 10 TMEM
 // allocator, warp 11 idle.  The k range of a unit is cut into segments of seg_kb k-blocks; each
@@ -708,50 +759,7 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
       }
       named_bar_sync(1, NT);
       if (bars->is_last) {
-        __threadfence();
-        // The control block and the slots were last written by OTHER CTAs of this kernel, and this SM may hold stale
-        // copies of those lines in L1 from an earlier layer: read them past L1 (ld.cg), run the controller on a
-        // copy (below the ring's first stage would be busy with the next layer's loads: the copy lives next to the
-        // barriers) and write the changed part back.  Only the head of the block and the history entries of this
-        // layer move.
-        Sp2Ctrl* gctrl = a.ctrl;
-        Sp2Ctrl* ctrl = reinterpret_cast<Sp2Ctrl*>(bars->ctrl_copy);
-        {
-          const uint32_t* src = reinterpret_cast<const uint32_t*>(gctrl);
-          uint32_t* dst = reinterpret_cast<uint32_t*>(ctrl);
-          for (int i = threadIdx.x; i < (int)(SP2_CTRL_HEAD_BYTES / 4); i += NT) dst[i] = __ldcg(src + i);
-        }
-        for (int i = threadIdx.x; i < a.n_flags; i += NT) a.flags[i] = 0u;   // every split unit was consumed
-        named_bar_sync(1, NT);
-        double* redf = reinterpret_cast<double*>(bars->red);
-        double tr, fro, mx, tracc, unused;
-        reduce_slots_fast(a.slots + (size_t)nb * nblk, nblk, redf, tr, fro, mx, tracc);
-        for (int b = 0; b < nb; ++b) {
-          double trz, froz, mxz;
-          reduce_slots_fast(a.slots + (size_t)b * nblk, nblk, redf, trz, froz, mxz, unused);
-          if (threadIdx.x == 0) {
-            const double sz = sp2_exp2i(-ctrl->u[b]);
-            ctrl->tr_z[b] = trz * sz; ctrl->fro_z[b] = froz * sz * sz; ctrl->max_z[b] = mxz * sz;
-          }
-        }
-        if (threadIdx.x == 0) {
-          const int n = ctrl->n;                   // the controller reads e[n - 2] and writes tr_x[n], e[n]
-          if (n >= 2 && n < SP2_LAYER_CAP) ctrl->e[n - 2] = __ldcg(&gctrl->e[n - 2]);
-          sp2_trace_identity(ctrl, tracc);
-          const double sy = sp2_exp2i(-ctrl->t);
-          ctrl->tr_y = tr * sy; ctrl->fro_y = fro * sy * sy; ctrl->max_y = mx * sy;
-          sp2_controller(ctrl);
-          if (n < SP2_LAYER_CAP) { gctrl->tr_x[n] = ctrl->tr_x[n]; gctrl->e[n] = ctrl->e[n]; }
-        }
-        named_bar_sync(1, NT);
-        {
-          const uint32_t* src = reinterpret_cast<const uint32_t*>(ctrl);
-          uint32_t* dst = reinterpret_cast<uint32_t*>(gctrl);
-          for (int i = threadIdx.x; i < (int)(SP2_CTRL_HEAD_BYTES / 4); i += NT) dst[i] = src[i];   // (ticket, epoch: unchanged values)
-        }
-        __threadfence();
-        named_bar_sync(1, NT);
-        if (threadIdx.x == 0) st_release_u32(&gctrl->epoch, epoch);       // release half of the barrier
+        persist_tail(a, bars, epoch, nb, nblk);
       } else if (threadIdx.x == 0) {
         long long spins = 0;
         while ((int)(ld_acquire_u32(&a.ctrl->epoch) - epoch) < 0)
