@@ -547,8 +547,22 @@ def run_ours(args):
     e2e_s = max_over_ranks(my_e2e, world, dev)
     e2e_flops = sum_over_ranks(sum(logical_flops_per_layer(n, response) * r["layers"] for r in res_h), world, dev)
     mats = 2 if response else 1
+    # what the link alone costs: the same pinned buffers copied in and out with nothing in between (one stream, as
+    # in the call: the solve needs all of H and H1 before its first kernel and D, D1 exist only after its last)
+    scratch_dev = torch.empty_like(H)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for src in ([Hh, H1h] if response else [Hh]):
+        scratch_dev.copy_(src, non_blocking=True)
+    for dst in ([Dh, D1h] if response else [Dh]):
+        dst.copy_(scratch_dev, non_blocking=True)
+    torch.cuda.synchronize()
+    link_ms = 1e3 * (time.perf_counter() - t0)
+    del scratch_dev
     e2e = {"value": e2e_flops / e2e_s / 1e12, "unit": UNIT, "h2d_bytes_per_step": mats * n * n * esz,
-           "d2h_bytes_per_step": mats * n * n * esz + 96, "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps}
+           "d2h_bytes_per_step": mats * n * n * esz + 96, "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s / e2e_steps,
+           "link_ms_per_step": link_ms,
+           "note": "link_ms_per_step = the same host<->device copies alone; e2e - device time cannot go below it in a blocking call"}
 
     # ---- the oracle on this box's host cores (rank 0, N = 1 only)
     cpu_baseline = None
