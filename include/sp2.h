@@ -59,7 +59,8 @@ typedef enum {
   SP2_ERR_ARCH = 4,          /* device is not sm_100 */
   SP2_ERR_NONFINITE = 5,     /* H (or H1) holds NaN/Inf, or the iterate became non-finite */
   SP2_ERR_DEGENERATE = 6,    /* eps_max == eps_min (H = c*I): no spectral width to rescale */
-  SP2_WARN_NOT_CONVERGED = 7, /* max_layers reached; D (and D1) are still written */
+  SP2_WARN_NOT_CONVERGED = 7, /* max_layers reached, or the parameter-free stop fired away from N_occ (degenerate level at the
+                                Fermi energy); D (and D1) are still written */
   SP2_ERR_BOUNDS = 8         /* an eigenvalue of X left [0,1]: the spectral bounds (user_bounds, or a Lanczos estimate in a
                                 sequence step) do not enclose the spectrum of H; detected on the device from
                                 tr X - tr X^2 < 0 far from convergence; D is not written.  The blocking calls re-run a

@@ -191,7 +191,7 @@ def sp2_density(H, n_occ, H1=None, tol=0.0, max_layers=100, bounds=None):
         '+':  Z <- X Z + Z X            '-':  Z <- 2 Z - (X Z + Z X).
 
     Returns a dict with D, D1 (or None), layers, signs (str of '+'/'-'),
-    tr_x[n], e[n] (per evaluated layer), stop (reason), eps_min, eps_max,
+    tr_x[n], e[n] (per evaluated layer), stop (reason), converged, eps_min, eps_max,
     tr_d, tr_dh (= sum_ij D_ij H_ij, reading R6), tr_d1.
     """
     H = _as_f64_symmetric(H, "H")
@@ -244,7 +244,10 @@ def sp2_density(H, n_occ, H1=None, tol=0.0, max_layers=100, bounds=None):
         signs.append("+" if plus else "-")
         n += 1
 
-    return dict(D=X, D1=Z, layers=n, signs="".join(signs), tr_x=tr_hist, e=e_hist, stop=stop,
+    # converged: stopped by a rule other than the layer cap AND at the requested occupation (the floor rule can fire
+    # at a fractional occupation when a degenerate level sits at the Fermi energy); bookkeeping only, no arithmetic
+    converged = stop != "max_layers" and abs(float(np.trace(X)) - n_occ) < 0.5
+    return dict(D=X, D1=Z, layers=n, signs="".join(signs), tr_x=tr_hist, e=e_hist, stop=stop, converged=converged,
                 eps_min=eps_min, eps_max=eps_max, tr_d=float(np.trace(X)),
                 tr_dh=float(np.sum(X * H)),
                 tr_d1=None if Z is None else float(np.trace(Z)))

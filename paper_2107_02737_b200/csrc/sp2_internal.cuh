@@ -189,7 +189,11 @@ __device__ inline void sp2_controller(Sp2Ctrl* c) {
   const int stop = sp2_stop_rule(c, n, tr_x);
   if (stop) {
     c->done = 1; c->stop_reason = stop;
-    c->status = (stop == 4) ? SP2_WARN_NOT_CONVERGED : SP2_OK;
+    // the parameter-free floor rule (2) fires when the idempotency error stops improving; if the occupation is not
+    // N_occ by then (a degenerate level at the Fermi energy: fractional occupation), the result is not a converged
+    // projector and is reported like the layer cap: D is written, status says so
+    const bool off_occ = stop == 2 && !(fabs(tr_x - (double)c->n_occ) < 0.5);
+    c->status = (stop == 4 || off_occ) ? SP2_WARN_NOT_CONVERGED : SP2_OK;
     return;
   }
   const double nocc = (double)c->n_occ;

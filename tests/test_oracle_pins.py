@@ -378,6 +378,21 @@ def test_lanczos_bounds_enclose_the_spectrum_and_are_tighter(cfg1):
     assert np.abs(r_g["D"] - r_l["D"]).max() < 1e-12 and r_l["layers"] <= r_g["layers"] - 3
 
 
+def test_converged_flag_is_bookkeeping_only(cfg1):
+    """`converged` = a stop rule other than the cap fired AND the occupation is the requested one."""
+    r = oracle.sp2_density(cfg1["H"], cfg1["n_occ"])
+    assert r["converged"] and r["stop"] in ("floor", "idempotent") and abs(r["tr_d"] - cfg1["n_occ"]) < 1e-9
+    r5 = oracle.sp2_density(cfg1["H"], cfg1["n_occ"], max_layers=5)
+    assert not r5["converged"] and r5["stop"] == "max_layers"
+    # a degenerate level at the Fermi energy that N_occ splits: fractional occupation, never a converged projector
+    lam = np.array([-1.0, -0.5, 0.0, 0.0, 0.7, 1.2])
+    rng = np.random.default_rng(3)
+    Q, _ = np.linalg.qr(rng.standard_normal((6, 6)))
+    H = (Q * lam) @ Q.T
+    rd = oracle.sp2_density(0.5 * (H + H.T), 3)
+    assert not rd["converged"]
+
+
 def test_lanczos_bounds_are_a_heuristic_not_an_enclosure():
     """The other side of the pin above: the Lanczos interval is NOT rigorous.  With an extreme eigenvector exactly
     orthogonal to the start vector v_i = cos(0.7 i + 0.3), the Krylov space never contains it, the interval misses the
