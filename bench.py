@@ -450,8 +450,8 @@ def run_ours(args):
     h = sp2.Sp2Handle(n, response=response, host_staging=True, refinement=args.refine > 0)
     if args.lanczos > 0:
         h.set_options(lanczos_steps=args.lanczos)
-    if args.max_ctas > 0 or args.persistent or args.seg_kb:
-        h.set_options(max_ctas=args.max_ctas, persistent=args.persistent, seg_kb=args.seg_kb)
+    if args.max_ctas > 0 or args.persistent or args.seg_kb or args.cta_group:
+        h.set_options(max_ctas=args.max_ctas, persistent=args.persistent, seg_kb=args.seg_kb, cta_group=args.cta_group)
     if args.refine > 0:
         if response:
             raise SystemExit("--refine goes with a density workload")
@@ -840,6 +840,7 @@ def main(argv=None):
                     help="float64 refinement layers after the stack (PAPER.md:170; density workloads only); extra, not the headline")
     ap.add_argument("--persistent", type=int, default=0, help="sp2_options_t.persistent (0 auto, 1 persistent kernel, 2 launch per layer)")
     ap.add_argument("--seg-kb", type=int, default=0, help="sp2_options_t.seg_kb (0 = default)")
+    ap.add_argument("--cta-group", type=int, default=0, help="sp2_options_t.cta_group (0 = auto, 1 = 128x128 tiles, 2 = 256x256 on CTA pairs)")
     ap.add_argument("--max-ctas", type=int, default=0, help="sp2_options_t.max_ctas: use at most this many CTAs (0 = one per SM)")
     ap.add_argument("--stub-ms", type=float, default=0.0, help=argparse.SUPPRESS)   # test hook, see run_stub
     args = ap.parse_args(argv)

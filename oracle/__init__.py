@@ -12,6 +12,7 @@ the paper is silent and a reading had to be chosen.
 from .sp2_oracle import (  # noqa: F401
     gershgorin_bounds,
     lanczos_bounds,
+    power_trace_bounds,
     rescale_to_unit_interval,
     sp2_stop,
     sp2_density,

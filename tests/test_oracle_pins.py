@@ -378,6 +378,54 @@ def test_lanczos_bounds_enclose_the_spectrum_and_are_tighter(cfg1):
     assert np.abs(r_g["D"] - r_l["D"]).max() < 1e-12 and r_l["layers"] <= r_g["layers"] - 3
 
 
+def test_power_trace_bounds_are_a_rigorous_enclosure(cfg1):
+    """power_trace_bounds: [mu - r, mu + r] with r = (tr A^(2^(s+1)))^(1/2^(s+1)) must (i) enclose the LAPACK spectrum
+    on EVERY matrix, including the ones built against the Lanczos start vector, (ii) be sandwiched between the true
+    radius rho and N^(1/2^(s+1)) rho, (iii) tighten monotonically with s, (iv) reproduce the closed form on a diagonal
+    matrix, (v) never leave the Gershgorin interval, and (vi) give the same projector in fewer layers."""
+    n = 300
+    v0 = np.cos(0.7 * np.arange(n) + 0.3)
+    mats = [cfg1["H"], inputs.ssh_chain(200, 1.0, 0.6, onsite=0.3)[0], np.diag(np.linspace(-3.0, 5.0, 50)),
+            inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[3], 150))["H"].astype(np.float64),
+            inputs.hidden_eigenvector_problem(n, 40, -3.0, v0)[0], inputs.hidden_eigenvector_problem(n, 150, 3.0, v0)[0],
+            np.array([[2.0]]), 1e6 * cfg1["H"], 1e-6 * cfg1["H"] + 7.0 * np.eye(cfg1["H"].shape[0])]
+    for H in mats:
+        w = np.linalg.eigvalsh(H)
+        N = H.shape[0]
+        mu = np.trace(H) / N
+        rho = np.abs(w - mu).max()
+        g_lo, g_hi = oracle.gershgorin_bounds(H)
+        prev = None
+        for s in (0, 1, 2, 3, 4, 6):
+            lo, hi = oracle.power_trace_bounds(H, s)
+            tol = 1e-12 * max(1.0, np.abs(w).max())
+            assert lo <= w[0] + tol and hi >= w[-1] - tol, (N, s)                     # (i) enclosure, always
+            assert lo >= g_lo - tol and hi <= g_hi + tol                              # (v)
+            r_raw = rho * (np.sum((np.abs(w - mu) / rho) ** (2 ** (s + 1)))) ** (1.0 / 2 ** (s + 1)) if rho > 0 else 0.0   # the definition, from the eigenvalues
+            assert rho * (1 - 1e-12) <= r_raw <= N ** (1.0 / 2 ** (s + 1)) * rho * (1 + 1e-12)   # (ii)
+            if mu - r_raw >= g_lo and mu + r_raw <= g_hi:                              # not clipped by the discs: the formula itself
+                assert lo == pytest.approx(mu - r_raw, rel=1e-9, abs=1e-9 * rho) and hi == pytest.approx(mu + r_raw, rel=1e-9, abs=1e-9 * rho)
+            if prev is not None:
+                assert hi - lo <= prev * (1 + 1e-12)                                   # (iii)
+            prev = hi - lo
+    d = np.array([-2.0, 0.5, 1.5, 4.0])                                               # (iv) mu = 1, a = (-3, -.5, .5, 3)
+    lo, hi = oracle.power_trace_bounds(np.diag(d), 1)
+    r = (2 * 3.0 ** 4 + 2 * 0.5 ** 4) ** 0.25
+    assert (lo, hi) == (pytest.approx(max(-2.0, 1 - r)), pytest.approx(min(4.0, 1 + r)))
+    H, n_occ = cfg1["H"], cfg1["n_occ"]                                               # (vi)
+    lo, hi = oracle.power_trace_bounds(H, 4)
+    g_lo, g_hi = oracle.gershgorin_bounds(H)
+    assert (hi - lo) < 0.35 * (g_hi - g_lo)
+    r_g = oracle.sp2_density(H, n_occ)
+    r_p = oracle.sp2_density(H, n_occ, bounds=(lo, hi))
+    assert np.abs(r_g["D"] - r_p["D"]).max() < 1e-12 and r_p["layers"] <= r_g["layers"] - 3
+    # where Lanczos misses the hidden outlier and ruins the solve, this bound does not
+    Hh, _ = inputs.hidden_eigenvector_problem(n, 40, -3.0, v0)
+    D_eig, _ = oracle.density_eigh(Hh, 40)
+    r_h = oracle.sp2_density(Hh, 40, bounds=oracle.power_trace_bounds(Hh, 4))
+    assert np.abs(r_h["D"] - D_eig).max() < 1e-11
+
+
 def test_converged_flag_is_bookkeeping_only(cfg1):
     """`converged` = a stop rule other than the cap fired AND the occupation is the requested one."""
     r = oracle.sp2_density(cfg1["H"], cfg1["n_occ"])
