@@ -450,8 +450,9 @@ def run_ours(args):
     h = sp2.Sp2Handle(n, response=response, host_staging=True, refinement=args.refine > 0)
     if args.lanczos > 0:
         h.set_options(lanczos_steps=args.lanczos)
-    if args.max_ctas > 0 or args.persistent or args.seg_kb or args.cta_group:
-        h.set_options(max_ctas=args.max_ctas, persistent=args.persistent, seg_kb=args.seg_kb, cta_group=args.cta_group)
+    if args.max_ctas > 0 or args.persistent or args.seg_kb or args.cta_group or args.power:
+        h.set_options(max_ctas=args.max_ctas, persistent=args.persistent, seg_kb=args.seg_kb, cta_group=args.cta_group,
+                      power_squarings=args.power)
     if args.refine > 0:
         if response:
             raise SystemExit("--refine goes with a density workload")
@@ -576,7 +577,7 @@ def run_ours(args):
             "vs_baseline": None, "dtype": "f16", "data": "synthetic",
             "config": {"workload": config_text(cfg, call),
                        "precision": "FP16 hi + lo operand planes (22 bits), FP32 accumulation in k-segments, f64 scalars",
-                       "replicas": world, "layers_per_step": layers, "refine_layers": args.refine, "lanczos_steps": args.lanczos,
+                       "replicas": world, "layers_per_step": layers, "refine_layers": args.refine, "lanczos_steps": args.lanczos, "power_squarings": args.power,
                        "l2_policy": ("L2 flushed between steps (a 252 MiB buffer is overwritten; every step has its own pair of "
                                      "CUDA events, the flush is not counted)" if in_l2 else
                                      f"inputs larger than L2 (H {n * n * esz / 2 ** 20:.0f} MiB, each FP16 plane "
@@ -620,6 +621,8 @@ def run_sequence(args):
     h = sp2.Sp2Handle(n, host_staging=True)
     if args.lanczos > 0:
         h.set_options(lanczos_steps=args.lanczos)
+    if args.power > 0:
+        h.set_options(power_squarings=args.power)
 
     def barrier():
         if world > 1:
@@ -836,6 +839,8 @@ def main(argv=None):
     ap.add_argument("--cpu-eigh", action="store_true", help="also time numpy eigh + V_occ V_occ^T above N = 6000 (minutes)")
     ap.add_argument("--lanczos", type=int, default=0,
                     help="Lanczos steps for tighter spectral bounds (SURVEY 8(f) NEXT-3); extra, not the headline")
+    ap.add_argument("--power", type=int, default=0,
+                    help="sp2_options_t.power_squarings: rigorous power-trace spectral bounds (SURVEY 8(f) NEXT-3); extra, not the headline")
     ap.add_argument("--refine", type=int, default=0,
                     help="float64 refinement layers after the stack (PAPER.md:170; density workloads only); extra, not the headline")
     ap.add_argument("--persistent", type=int, default=0, help="sp2_options_t.persistent (0 auto, 1 persistent kernel, 2 launch per layer)")

@@ -110,6 +110,14 @@ typedef struct {
                        1 = the persistent multi-CTA kernel at any size; 2 = one launch per layer at any size */
   int max_ctas;     /* 0 = one CTA per SM (default); > 0: use at most this many CTAs for the layer kernel, e.g. to leave SMs
                        to other work on the same GPU (the layer grid must be co-resident, see "Conventions") */
+  int power_squarings; /* 0 = off (default: Gershgorin bounds only); 1..6: RIGOROUS tighter bounds from the trace of a
+                       matrix power.  Before the solve, A = (H - mu I)/r0 (mu = tr H/N) is squared s = power_squarings
+                       times on the same tensor kernel (density-only layers); since max_i |lambda_i - mu|^p <= tr (H - mu I)^p
+                       for even p, r = ||A^(2^s)||_F^(1/2^s) r0 bounds every eigenvalue's distance from mu, whatever the
+                       eigenvectors are (no start vector, unlike lanczos_steps), with r <= N^(1/2^(s+1)) rho.  The solve then
+                       uses [mu - r, mu + r] (widened by 1e-3 r, intersected with the Gershgorin discs).  Costs s density
+                       layers, saves ~2 log2(Gershgorin width / 2r) layers; takes precedence over lanczos_steps */
+  int reserved_pad;
 } sp2_options_t;
 
 typedef struct {

@@ -21,7 +21,8 @@
 // launchers defined in sp2_prologue.cu
 void sp2_launch_init(Sp2Ctrl* c, int N, int n_occ, int npad, int with_response, int max_layers, int user_bounds,
                      double eps_min, double eps_max, double tol, int forced_layers, unsigned long long forced_signs,
-                     int no_recentre, cudaStream_t s);
+                     int no_recentre, int power_squarings, cudaStream_t s);
+void sp2_launch_power_finish(Sp2Ctrl* c, cudaStream_t s);
 int sp2_bounds_blocks(int N);
 void sp2_launch_bounds(const void* H, sp2_dtype_t dt, long ld, int N, int mode, Sp2BoundSlot* slots, cudaStream_t s);
 void sp2_launch_setup(Sp2Ctrl* c, const Sp2BoundSlot* sh, int n_h, const Sp2BoundSlot* s1, int n_h1, cudaStream_t s);
@@ -78,13 +79,14 @@ struct Layout {
   size_t off_fslots;
   size_t off_tiles, tiles_count;
   size_t off_items, items_cap, off_item_begin, off_scratch, scratch_bytes, off_flags;
+  size_t off_items_pw, items_pw_cap, off_item_begin_pw;
   size_t off_ctrl, off_ring, off_args;
   size_t off_staging, staging_each;
   size_t off_refine, refine_each, off_refine_slots, refine_slots_count;
   size_t off_lanczos;
   size_t total;
   std::vector<Region> regions;
-  int r_plane0, r_slots, r_slots2, r_bslots, r_fslots, r_tiles, r_items, r_item_begin, r_scratch, r_flags, r_ctrl, r_args, r_ring,
+  int r_plane0, r_slots, r_slots2, r_bslots, r_fslots, r_tiles, r_items, r_item_begin, r_items_pw, r_item_begin_pw, r_scratch, r_flags, r_ctrl, r_args, r_ring,
       r_staging0, r_lanczos, r_refine0, r_refine_slots;
 };
 
@@ -148,13 +150,17 @@ Layout make_layout(int n_max, int flags) {
   L.items_cap = (1 + nb1) * L.tiles_count + 1024;
   L.r_items = carve("items", L.items_cap * sizeof(Sp2Item), &L.off_items);
   L.r_item_begin = carve("item_begin", (kMaxClusters + 1) * sizeof(int), &L.off_item_begin);
+  // density-only work lists for the power phase (sp2_options_t.power_squarings) of a solve that carries perturbations
+  L.items_pw_cap = resp ? L.tiles_count + 1024 : 0;
+  L.r_items_pw = carve("items_pw", L.items_pw_cap * sizeof(Sp2Item), &L.off_items_pw);
+  L.r_item_begin_pw = carve("item_begin_pw", (resp ? (kMaxClusters + 1) : 0) * sizeof(int), &L.off_item_begin_pw);
   L.scratch_bytes = 2 * (size_t)kMaxClusters * sp2_layer_scratch_slot_bytes(1);
   if (2 * (size_t)(kMaxClusters / 2) * sp2_layer_scratch_slot_bytes(2) > L.scratch_bytes)
     L.scratch_bytes = 2 * (size_t)(kMaxClusters / 2) * sp2_layer_scratch_slot_bytes(2);
   L.r_scratch = carve("scratch", L.scratch_bytes, &L.off_scratch);
   L.r_flags = carve("flags", 2 * kMaxClusters * sizeof(unsigned int), &L.off_flags);
   L.r_ctrl = carve("ctrl", sizeof(Sp2Ctrl), &L.off_ctrl);
-  L.r_args = carve("args", 2 * sizeof(Sp2LayerArgs), &L.off_args);
+  L.r_args = carve("args", 4 * sizeof(Sp2LayerArgs), &L.off_args);      // [0..1] the solve, [2..3] its power phase
   L.r_ring = carve("ring", (size_t)kRingCap * sizeof(sp2_result_t), &L.off_ring);
   L.r_staging0 = -1; L.staging_each = 0; L.off_staging = 0;
   if (flags & SP2_WITH_HOST_STAGING) {
@@ -204,6 +210,10 @@ struct sp2_handle_s {
   int cur_n, cur_npad, cur_cg, cur_resp, cur_seg, cur_lo, cur_maxctas;
   int n_active;                  // CTA(-pair)s whose work list is not empty (grid of the persistent multi-layer launch)
   Sp2LayerArgs args[2];          // parity 0: buffer 0 -> 1, parity 1: buffer 1 -> 0
+  Sp2LayerArgs args_pw[2];       // the same for the density-only power phase (= args when no perturbation is carried)
+  int n_flags_pw, n_active_pw, cur_pw;
+  std::vector<Sp2Item> items_pw_host;
+  std::vector<int> item_begin_pw_host;
   std::vector<int2> tiles_host;
   std::vector<Sp2Item> items_host;
   std::vector<int> item_begin_host;
@@ -232,6 +242,8 @@ struct sp2_handle_s {
   double* fslots() const { return reinterpret_cast<double*>(ws + L.off_fslots); }
   int2* tiles() const { return reinterpret_cast<int2*>(ws + L.off_tiles); }
   Sp2Item* items() const { return reinterpret_cast<Sp2Item*>(ws + L.off_items); }
+  Sp2Item* items_pw() const { return reinterpret_cast<Sp2Item*>(ws + L.off_items_pw); }
+  int* item_begin_pw() const { return reinterpret_cast<int*>(ws + L.off_item_begin_pw); }
   int* item_begin() const { return reinterpret_cast<int*>(ws + L.off_item_begin); }
   float* scratch() const { return reinterpret_cast<float*>(ws + L.off_scratch); }
   unsigned int* split_flags() const { return reinterpret_cast<unsigned int*>(ws + L.off_flags); }
@@ -396,7 +408,8 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = npad > 24576 ? 2 : (npad > 8192 ? 4 : 8);
   while ((npad / 64) % seg) seg >>= 1;
   if (h->cur_n == N && h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp && h->cur_seg == seg &&
-      h->cur_lo == h->opt.lo_bits && h->cur_maxctas == h->opt.max_ctas) return SP2_OK;
+      h->cur_lo == h->opt.lo_bits && h->cur_maxctas == h->opt.max_ctas && h->cur_pw == (h->opt.power_squarings > 0))
+    return SP2_OK;
   const int nt = npad / (128 * cg);
   build_tiles(nt, h->tiles_host);
   SP2_CUDA(h, cudaMemcpyAsync(h->tiles(), h->tiles_host.data(), h->tiles_host.size() * sizeof(int2),
@@ -423,6 +436,26 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   SP2_CUDA(h, cudaMemcpyAsync(h->item_begin(), h->item_begin_host.data(), h->item_begin_host.size() * sizeof(int),
                               cudaMemcpyHostToDevice, s));
   SP2_CUDA(h, cudaMemsetAsync(h->split_flags(), 0, 2 * kMaxClusters * sizeof(unsigned int), s));
+  // power phase of a solve that carries perturbations: the same tiles, density-only work lists of their own
+  const bool pw_lists = h->opt.power_squarings > 0 && resp > 0;
+  h->n_flags_pw = h->n_flags; h->n_active_pw = h->n_active;
+  if (pw_lists) {
+    int n_slots_pw = 0;
+    build_schedule((int)h->tiles_host.size(), 0, (npad / 64) / seg, nC, h->items_pw_host, h->item_begin_pw_host,
+                   &h->n_flags_pw, &n_slots_pw);
+    h->n_active_pw = 1;
+    for (int c = 0; c < nC; ++c) if (h->item_begin_pw_host[c + 1] > h->item_begin_pw_host[c]) h->n_active_pw = c + 1;
+    if (h->items_pw_host.size() > h->L.items_pw_cap || (size_t)n_slots_pw * sp2_layer_scratch_slot_bytes(cg) > h->L.scratch_bytes ||
+        h->n_flags_pw > 2 * kMaxClusters)
+      return SP2_ERR_WORKSPACE;
+    h->touch(h->L.r_items_pw, h->items_pw_host.size() * sizeof(Sp2Item));
+    h->touch(h->L.r_item_begin_pw, h->item_begin_pw_host.size() * sizeof(int));
+    h->touch(h->L.r_scratch, (size_t)n_slots_pw * sp2_layer_scratch_slot_bytes(cg));
+    SP2_CUDA(h, cudaMemcpyAsync(h->items_pw(), h->items_pw_host.data(), h->items_pw_host.size() * sizeof(Sp2Item),
+                                cudaMemcpyHostToDevice, s));
+    SP2_CUDA(h, cudaMemcpyAsync(h->item_begin_pw(), h->item_begin_pw_host.data(), h->item_begin_pw_host.size() * sizeof(int),
+                                cudaMemcpyHostToDevice, s));
+  }
   SP2_CUDA(h, cudaStreamSynchronize(s));     // host vectors may be rebuilt by the next prepare
   for (int par = 0; par < 2; ++par) {
     Sp2LayerArgs& a = h->args[par];
@@ -440,13 +473,18 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
     a.n_flags = h->n_flags; a.n_clusters = h->n_clusters;
     a.lo_bits = (h->opt.lo_bits >= 6 && h->opt.lo_bits <= 10) ? h->opt.lo_bits : 11;
     a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = resp; a.seg_kb = seg;
+    Sp2LayerArgs& q = h->args_pw[par];          // the power phase: Y planes only
+    q = a;
+    q.with_response = 0;
+    if (pw_lists) { q.items = h->items_pw(); q.item_begin = h->item_begin_pw(); q.n_flags = h->n_flags_pw; }
   }
   SP2_CUDA(h, cudaMemcpyAsync(h->d_args(), h->args, 2 * sizeof(Sp2LayerArgs), cudaMemcpyHostToDevice, s));
+  SP2_CUDA(h, cudaMemcpyAsync(h->d_args() + 2, h->args_pw, 2 * sizeof(Sp2LayerArgs), cudaMemcpyHostToDevice, s));
   SP2_CUDA(h, cudaStreamSynchronize(s));
-  h->touch(h->L.r_args, 2 * sizeof(Sp2LayerArgs));
+  h->touch(h->L.r_args, 4 * sizeof(Sp2LayerArgs));
   h->layers_hint = 0;
   h->cur_n = N; h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp; h->cur_seg = seg; h->cur_lo = h->opt.lo_bits;
-  h->cur_maxctas = h->opt.max_ctas;
+  h->cur_maxctas = h->opt.max_ctas; h->cur_pw = h->opt.power_squarings > 0;
   return SP2_OK;
 }
 
@@ -494,23 +532,25 @@ bool use_persistent(sp2_handle_t h) {
 }
 
 // enqueue layer launches [first, first + count) on `s`
-sp2_status_t enqueue_layers(sp2_handle_t h, int first, int count, cudaStream_t s, int* launches) {
+// pw: the density-only power phase (args_pw, its own work lists)
+sp2_status_t enqueue_layers(sp2_handle_t h, int first, int count, cudaStream_t s, int* launches, bool pw = false) {
+  const Sp2LayerArgs* A = pw ? h->args_pw : h->args;
   if (use_small(h)) {
     if (count <= 0) return SP2_OK;
-    cudaError_t e = sp2_launch_small(h->args[0], h->cur_npad, s);
+    cudaError_t e = sp2_launch_small(A[0], h->cur_npad, s);
     if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
     ++*launches;
     return SP2_OK;
   }
   if (use_persistent(h)) {       // the kernel loops until the device controller stops (it starts at layer ctrl->n)
     if (count <= 0) return SP2_OK;
-    cudaError_t e = sp2_launch_layers_persistent(h->d_args(), h->cur_cg, h->n_active, s);
+    cudaError_t e = sp2_launch_layers_persistent(h->d_args() + (pw ? 2 : 0), h->cur_cg, pw ? h->n_active_pw : h->n_active, s);
     if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
     ++*launches;
     return SP2_OK;
   }
   for (int n = first; n < first + count; ++n) {
-    cudaError_t e = sp2_launch_layer(h->args[n & 1], h->opt.engine, h->cur_cg, s);
+    cudaError_t e = sp2_launch_layer(A[n & 1], h->opt.engine, h->cur_cg, s);
     if (e != cudaSuccess) { h->last_cuda_error = (int)e; return SP2_ERR_CUDA; }
     ++*launches;
   }
@@ -542,9 +582,17 @@ sp2_status_t enqueue_finalise(sp2_handle_t h, const void* H, sp2_dtype_t in_dt, 
   return SP2_OK;
 }
 
+// rigorous bounds from the trace of a matrix power (sp2_options_t.power_squarings): a density-only phase of squarings
+// before the solve; takes precedence over the Lanczos estimate
+bool power_active(sp2_handle_t h, int N, int N_occ) {
+  const sp2_options_t& o = h->opt;
+  return o.power_squarings > 0 && !o.user_bounds && o.forced_layers <= 0 && N >= 2 && N_occ > 0 && N_occ < N;
+}
+
 bool lanczos_active(sp2_handle_t h, int N, int N_occ) {
   const sp2_options_t& o = h->opt;
-  return o.lanczos_steps > 0 && !o.user_bounds && !h->no_lanczos && N > 2 * o.lanczos_steps && N_occ > 0 && N_occ < N;
+  return o.lanczos_steps > 0 && !o.user_bounds && !h->no_lanczos && N > 2 * o.lanczos_steps && N_occ > 0 && N_occ < N &&
+         !power_active(h, N, N_occ);
 }
 
 int effective_max_layers(const sp2_options_t& o) {
@@ -588,7 +636,8 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dty
       }
     }
   }
-  if (use_small(h) && !lanczos_active(h, N, N_occ) && N_occ > 0 && N_occ < N) {
+  const bool power = power_active(h, N, N_occ);
+  if (use_small(h) && !lanczos_active(h, N, N_occ) && !power && N_occ > 0 && N_occ < N) {
     // the smallest problems: prologue, layer stack and finalise in ONE launch of one CTA (sp2_small.cu)
     Sp2SmallProblem sp;
     memset(&sp, 0, sizeof(sp));
@@ -607,7 +656,8 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dty
     if (launches_out) *launches_out = launches;
     return SP2_OK;
   }
-  sp2_launch_init(c, N, N_occ, npad, resp, max_layers, o.user_bounds, o.eps_min, o.eps_max, tol, forced, o.forced_signs, o.no_recentre, s);
+  sp2_launch_init(c, N, N_occ, npad, resp, max_layers, o.user_bounds, o.eps_min, o.eps_max, tol, forced, o.forced_signs, o.no_recentre,
+                  power ? o.power_squarings : 0, s);
   ++launches;
   sp2_launch_bounds(H, in_dt, ldh, N, 0, h->bslots(0), s); ++launches;
   for (int b = 0; b < resp; ++b) {    // one slot array of sp2_bounds_blocks(N) per perturbation, contiguous (k_setup)
@@ -619,6 +669,17 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dty
   if (lanczos_active(h, N, N_occ)) {
     sp2_launch_lanczos(c, H, in_dt, ldh, N, o.lanczos_steps, h->lanczos_vecs(), s);
     launches += 2 + 2 * o.lanczos_steps;
+  }
+  if (power) {
+    // power phase: A = (mu I - H)/r0 into the Y planes, power_squarings density-only layers Yhat <- gamma Yhat^2 on the
+    // same tensor kernel, then k_power_finish turns ||A^(2^s)||_F into an enclosing interval and hands it to the
+    // regular solve below as (device-side) user bounds
+    sp2_launch_setup(c, h->bslots(0), sp2_bounds_blocks(N), h->bslots(1), resp ? sp2_bounds_blocks(N) : 0, s); ++launches;
+    sp2_launch_rescale(H, in_dt, ldh, c, 0, h->plane(0, 0), h->plane(1, 0), npad, h->slots(), s); ++launches;
+    sp2_launch_ctrl0(c, h->slots(), h->slots2(), sp2_rescale_blocks(npad), s); ++launches;
+    st = enqueue_layers(h, 0, o.power_squarings, s, &launches, true);
+    if (st != SP2_OK) return st;
+    sp2_launch_power_finish(c, s); ++launches;
   }
   sp2_launch_setup(c, h->bslots(0), sp2_bounds_blocks(N), h->bslots(1), resp ? sp2_bounds_blocks(N) : 0, s); ++launches;
   if (N_occ == 0 || N_occ == N) {
@@ -780,7 +841,7 @@ sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_work
   h->n_max = n_max; h->flags = flags; h->device = dev; h->num_sms = prop.multiProcessorCount; h->nb_max = L.nb_max;
   h->ws = static_cast<uint8_t*>(d_workspace); h->ws_bytes = bytes; h->L = L;
   default_options(&h->opt);
-  h->cur_n = -1; h->cur_npad = -1; h->cur_cg = -1; h->cur_resp = -1; h->cur_seg = -1; h->cur_maxctas = -1; h->n_active = 1;
+  h->cur_n = -1; h->cur_npad = -1; h->cur_cg = -1; h->cur_resp = -1; h->cur_seg = -1; h->cur_maxctas = -1; h->n_active = 1; h->cur_pw = -1; h->n_active_pw = 1; h->n_flags_pw = 0;
   h->last_cuda_error = 0; h->launches = 0; h->seq_active = 0; h->layers_hint = 0; h->no_lanczos = 0;
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
@@ -835,6 +896,7 @@ sp2_status_t sp2_set_options(sp2_handle_t h, const sp2_options_t* opt) {
       opt->seg_kb != 16 && opt->seg_kb != 32) return SP2_ERR_INVALID_ARG;
   if (opt->user_bounds && !(opt->eps_max > opt->eps_min)) return SP2_ERR_INVALID_ARG;
   if (opt->persistent < 0 || opt->persistent > 2 || opt->max_ctas < 0) return SP2_ERR_INVALID_ARG;
+  if (opt->power_squarings < 0 || opt->power_squarings > 6) return SP2_ERR_INVALID_ARG;
   h->opt = *opt;
   h->layers_hint = 0;
   return SP2_OK;
@@ -993,7 +1055,7 @@ sp2_status_t sp2_congruence(sp2_handle_t h, const void* dZ, const void* dX, sp2_
   __half *Lh = h->plane(0, 0), *Lm = h->plane(1, 0), *Xh = h->plane(2, 0), *Xm = h->plane(3, 0), *Th = h->plane(2, 1),
          *Tm = h->plane(3, 1);
   // exponents, then planes: L = Z^T (C = Z^T X Z) or Z (C = Z X Z^T); X is symmetric
-  sp2_launch_init(c, N, 0, npad, 0, 1, 0, 0.0, 0.0, 0.0, 0, 0ull, 0, s);
+  sp2_launch_init(c, N, 0, npad, 0, 1, 0, 0.0, 0.0, 0.0, 0, 0ull, 0, 0, s);
   sp2_launch_bounds(dZ, in_dtype, ld, N, 1, h->bslots(0), s);
   sp2_launch_bounds(dX, in_dtype, ld, N, 1, h->bslots(1), s);
   sp2_launch_gsetup(c, h->bslots(0), h->bslots(1), sp2_bounds_blocks(N), N, h->ring(), s);

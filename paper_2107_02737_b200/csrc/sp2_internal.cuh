@@ -30,6 +30,7 @@ struct Sp2BoundSlot { // per block of the bounds kernel
   double tr;          // sum_i H_ii
   double mx;          // max |H_ij|
   double sum;         // sum |H_ij| (non-finite detector)
+  double sumsq;       // sum H_ij^2 = ||H||_F^2 (scale of the power-trace bounds)
 };
 
 struct Sp2Coef {      // epilogue coefficients of the layer about to run (scaled units)
@@ -72,6 +73,11 @@ struct Sp2Ctrl {
   int lanczos_steps, lanczos_pad;
   double lz_alpha[32], lz_beta[33];   // tridiagonal T_k; lz_beta[j] couples j-1 and j, lz_beta[k] is the residual norm
   double lz_min, lz_max;              // theta_min - beta_k, theta_max + beta_k
+  // Rigorous spectral bounds from the trace of a matrix power (sp2_options_t.power_squarings):
+  // a first, density-only phase squares A = (H - mu I)/r0 pw_total times; the iterate it stores is Yhat_s with
+  // A^(2^s) = 2^pw_log2scale * Yhat_s (renormalised by a power of two after every squaring)
+  int pw_total, pw_phase;             // squarings asked for; 1 while the power phase runs
+  double pw_mu, pw_r0, pw_log2scale;
   // float64 refinement layers (sp2_refine.cu)
   double ref_tr, ref_fro;   // tr X and ||X||_F^2 of the current float64 iterate
   int ref_plus, ref_done;   // branch of the next refinement layer; layers applied
@@ -111,9 +117,25 @@ __device__ __forceinline__ void sp2_split_f32(double a, float& hi, float& lo) {
 // The input layer from the reduced bounds (SURVEY 8(a) a1 -> a2): spectral interval, Delta, the first shift and the
 // first plane exponents.  One thread.  lo/hi: Gershgorin interval; tr: tr H; mx: max|H|; sum: sum of |H| (and |H1|):
 // the non-finite detector; c->maxabs_h1[b] already set for the nb perturbations.
-__device__ inline void sp2_setup_input_layer(Sp2Ctrl* c, double lo, double hi, double tr, double mx, double sum, int nb) {
+__device__ inline void sp2_setup_input_layer(Sp2Ctrl* c, double lo, double hi, double tr, double mx, double sum, int nb,
+                                             double sumsq = 0.0) {
   c->tr_h = tr;
   c->maxabs_h = mx;
+  if (c->pw_phase) {
+    // power phase: the iterate is A = (mu I - H)/r0 with mu = tr H/N and r0 = the RMS eigenvalue distance from mu
+    // (sqrt(||H||_F^2/N - mu^2) <= rho(H - mu I) <= sqrt(N) r0), no shift: c = 0 throughout
+    const double N = (double)c->N;
+    const double mu = tr / N;
+    const double r0 = sqrt(fmax(sumsq / N - mu * mu, 0.0));
+    c->pw_mu = mu; c->pw_r0 = r0; c->pw_log2scale = 0.0;
+    c->eps_min = lo; c->eps_max = hi;              // the Gershgorin interval, kept for the intersection
+    if (!isfinite(sum) || !isfinite(r0)) { c->done = 1; c->status = SP2_ERR_NONFINITE; return; }
+    if (!(r0 > 0.0) || !(hi > lo)) { c->done = 1; c->pw_total = 0; return; }   // H = mu I: nothing to tighten
+    c->delta = r0;
+    c->c = 0.0;
+    c->t = sp2_pick_exponent((mx + fabs(mu)) / r0);
+    return;
+  }
   double eps_min = lo, eps_max = hi;
   if (c->lanczos_steps > 0 && isfinite(c->lz_min) && isfinite(c->lz_max) && c->lz_max > c->lz_min) {
     // tighter bounds from k Lanczos steps, never wider than the Gershgorin discs
@@ -168,6 +190,25 @@ __device__ inline void sp2_controller(Sp2Ctrl* c) {
   const double cc = c->c;
   bool finite = isfinite(c->fro_y) && isfinite(c->tr_y) && isfinite(c->max_y);
   for (int b = 0; b < c->with_response; ++b) finite = finite && isfinite(c->fro_z[b]) && isfinite(c->max_z[b]);
+  if (c->pw_phase) {
+    // ---- power phase (no branches, no shift): Yhat' = gamma Yhat^2 with gamma = 2^-e the power of two that brings
+    // ||Yhat||_F^2 into [1, 2), so that ||Yhat'||_F <= 2 and >= 1/sqrt(N): no power ever over- or underflows
+    if (!(isfinite(c->fro_y) && isfinite(c->max_y))) { c->done = 1; c->status = SP2_ERR_NONFINITE; return; }
+    if (n >= c->pw_total || !(c->fro_y > 0.0)) { c->done = 1; c->stop_reason = 8; return; }   // k_power_finish takes over
+    int e;
+    frexp(c->fro_y, &e);                            // fro_y = m 2^e, m in [0.5, 1)
+    e -= 1;                                         // fro_y in [2^e, 2^(e+1))
+    c->pw_log2scale = 2.0 * c->pw_log2scale + (double)e;
+    const double gamma = sp2_exp2i(-e);
+    const int t = c->t;
+    const int t_next = sp2_pick_exponent(fmin(gamma * c->fro_y, 2.0));     // max|Yhat'| <= ||Yhat'||_F <= gamma ||Yhat||_F^2 < 2
+    c->coef.a1y_hi = 0.f; c->coef.a1y_lo = 0.f;
+    c->coef.a2y = (float)(gamma * sp2_exp2i(t_next - 2 * t));
+    c->coef.dsh_hi = 0.f; c->coef.dsh_lo = 0.f;
+    c->t_in = t; c->sigma_last = 0.0; c->fro_in = c->fro_y;
+    c->t = t_next; c->c = 0.0; c->n = n + 1;
+    return;
+  }
   if (!finite) {
     c->done = 1; c->status = SP2_ERR_NONFINITE; c->stop_reason = 0;
     return;

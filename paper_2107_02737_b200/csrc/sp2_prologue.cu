@@ -24,14 +24,16 @@ __device__ __forceinline__ double warp_max(double v) {
 }
 
 // 16-byte vector loads: float4 / double2
-__device__ __forceinline__ void abs_acc(const float4& x, double& s, double& m) {
+__device__ __forceinline__ void abs_acc(const float4& x, double& s, double& m, double& q) {
   const double a = fabs((double)x.x), b = fabs((double)x.y), c = fabs((double)x.z), d = fabs((double)x.w);
   s += (a + b) + (c + d);
+  q += (a * a + b * b) + (c * c + d * d);
   m = fmax(m, fmax(fmax(a, b), fmax(c, d)));
 }
-__device__ __forceinline__ void abs_acc(const double2& x, double& s, double& m) {
+__device__ __forceinline__ void abs_acc(const double2& x, double& s, double& m, double& q) {
   const double a = fabs(x.x), b = fabs(x.y);
   s += a + b;
+  q += a * a + b * b;
   m = fmax(m, fmax(a, b));
 }
 template <typename T> struct Vec16;
@@ -46,10 +48,10 @@ __global__ void __launch_bounds__(256) k_bounds(const T* __restrict__ H, long ld
                                                 Sp2BoundSlot* __restrict__ slots) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int row = blockIdx.x * 8 + warp;
-  double lo = INFINITY, hi = -INFINITY, tr = 0.0, mx = 0.0, sum = 0.0;
+  double lo = INFINITY, hi = -INFINITY, tr = 0.0, mx = 0.0, sum = 0.0, sumsq = 0.0;
   if (row < N) {
     const T* r = H + (size_t)row * ld;
-    double s = 0.0, m = 0.0;
+    double s = 0.0, m = 0.0, q = 0.0;
     const bool vec_ok = ((reinterpret_cast<uintptr_t>(r) & 15) == 0);
     int j0 = 0;
     if (vec_ok) {
@@ -57,29 +59,31 @@ __global__ void __launch_bounds__(256) k_bounds(const T* __restrict__ H, long ld
       constexpr int VN = Vec16<T>::n;
       const V* rv = reinterpret_cast<const V*>(r);
       const int nv = N / VN;
-      for (int v = lane; v < nv; v += 32) abs_acc(__ldg(rv + v), s, m);
+      for (int v = lane; v < nv; v += 32) abs_acc(__ldg(rv + v), s, m, q);
       j0 = nv * VN;
     }
     for (int j = j0 + lane; j < N; j += 32) {
       const double a = fabs((double)__ldg(r + j));
       s += a;
+      q += a * a;
       m = fmax(m, a);
     }
     s = warp_sum(s);
+    q = warp_sum(q);
     m = warp_max(m);
     const double d = (double)__ldg(r + row);
     const double rad = s - fabs(d);          // sum over j != i
-    lo = d - rad; hi = d + rad; tr = d; mx = m; sum = s;
+    lo = d - rad; hi = d + rad; tr = d; mx = m; sum = s; sumsq = q;
   }
-  __shared__ double sh[5][8];
-  if (lane == 0) { sh[0][warp] = lo; sh[1][warp] = hi; sh[2][warp] = tr; sh[3][warp] = mx; sh[4][warp] = sum; }
+  __shared__ double sh[6][8];
+  if (lane == 0) { sh[0][warp] = lo; sh[1][warp] = hi; sh[2][warp] = tr; sh[3][warp] = mx; sh[4][warp] = sum; sh[5][warp] = sumsq; }
   __syncthreads();
   if (threadIdx.x == 0) {
     Sp2BoundSlot o;
-    o.lo = sh[0][0]; o.hi = sh[1][0]; o.tr = sh[2][0]; o.mx = sh[3][0]; o.sum = sh[4][0];
+    o.lo = sh[0][0]; o.hi = sh[1][0]; o.tr = sh[2][0]; o.mx = sh[3][0]; o.sum = sh[4][0]; o.sumsq = sh[5][0];
     for (int w = 1; w < 8; ++w) {
       o.lo = fmin(o.lo, sh[0][w]); o.hi = fmax(o.hi, sh[1][w]);
-      o.tr += sh[2][w]; o.mx = fmax(o.mx, sh[3][w]); o.sum += sh[4][w];
+      o.tr += sh[2][w]; o.mx = fmax(o.mx, sh[3][w]); o.sum += sh[4][w]; o.sumsq += sh[5][w];
     }
     (void)mode;
     slots[blockIdx.x] = o;
@@ -90,12 +94,12 @@ __global__ void __launch_bounds__(256) k_bounds(const T* __restrict__ H, long ld
 // Reduce the bound slots, fix the input layer and the first plane exponents.  One block.
 __global__ void __launch_bounds__(256) k_setup(Sp2Ctrl* c, const Sp2BoundSlot* sh_slots, int n_h,
                                                const Sp2BoundSlot* s1_slots, int n_h1) {
-  __shared__ double red[5][256];
+  __shared__ double red[6][256];
   const int tid = threadIdx.x;
-  double lo = INFINITY, hi = -INFINITY, tr = 0.0, mx = 0.0, sum = 0.0, sum1 = 0.0;
+  double lo = INFINITY, hi = -INFINITY, tr = 0.0, mx = 0.0, sum = 0.0, sum1 = 0.0, sumsq = 0.0;
   for (int i = tid; i < n_h; i += 256) {
     lo = fmin(lo, sh_slots[i].lo); hi = fmax(hi, sh_slots[i].hi);
-    tr += sh_slots[i].tr; mx = fmax(mx, sh_slots[i].mx); sum += sh_slots[i].sum;
+    tr += sh_slots[i].tr; mx = fmax(mx, sh_slots[i].mx); sum += sh_slots[i].sum; sumsq += sh_slots[i].sumsq;
   }
   const int nb = n_h1 > 0 ? c->with_response : 0;     // s1_slots = nb arrays of n_h1 slots, one per perturbation
   double mx1[SP2_NB];
@@ -106,6 +110,7 @@ __global__ void __launch_bounds__(256) k_setup(Sp2Ctrl* c, const Sp2BoundSlot* s
       sum1 += s1_slots[(size_t)b * n_h1 + i].sum;
     }
   red[0][tid] = lo; red[1][tid] = hi; red[2][tid] = tr; red[3][tid] = fmax(mx, 0.0); red[4][tid] = sum + sum1;
+  red[5][tid] = sumsq;
   __syncthreads();
   for (int w = 128; w > 0; w >>= 1) {
     if (tid < w) {
@@ -114,6 +119,7 @@ __global__ void __launch_bounds__(256) k_setup(Sp2Ctrl* c, const Sp2BoundSlot* s
       red[2][tid] += red[2][tid + w];
       red[3][tid] = fmax(red[3][tid], red[3][tid + w]);
       red[4][tid] += red[4][tid + w];
+      red[5][tid] += red[5][tid + w];
     }
     __syncthreads();
   }
@@ -129,7 +135,7 @@ __global__ void __launch_bounds__(256) k_setup(Sp2Ctrl* c, const Sp2BoundSlot* s
     __syncthreads();
   }
   if (tid != 0) return;
-  sp2_setup_input_layer(c, red[0][0], red[1][0], red[2][0], red[3][0], red[4][0], nb);
+  sp2_setup_input_layer(c, red[0][0], red[1][0], red[2][0], red[3][0], red[4][0], nb, red[5][0]);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -230,7 +236,8 @@ __global__ void __launch_bounds__(256) k_ctrl0(Sp2Ctrl* c, const Sp2Slot* ys, co
   __shared__ double red[4 * 256];
   double tr, fro, mx, unused;
   sp2_reduce_slots(ys, count, red, tr, fro, mx, unused);
-  for (int b = 0; b < c->with_response; ++b) {       // zs = one slot array of `count` per perturbation
+  const int nbz = c->pw_phase ? 0 : c->with_response;   // the power phase carries no perturbation
+  for (int b = 0; b < nbz; ++b) {       // zs = one slot array of `count` per perturbation
     double trz, froz, mxz;
     sp2_reduce_slots(zs + (size_t)b * count, count, red, trz, froz, mxz, unused);
     if (threadIdx.x == 0) {
@@ -537,15 +544,41 @@ __global__ void k_close(Sp2Ctrl* c) {
   c->done = 1; c->status = SP2_WARN_NOT_CONVERGED; c->stop_reason = 7;
 }
 
+// End of the power phase (sp2_options_t.power_squarings): the rigorous radius r = ||A^(2^s)||_F^(1/2^s) r0 from the
+// Frobenius norm of the iterate the squarings left (PAPER.md:145 needs an interval that ENCLOSES the spectrum; this
+// one does whatever the eigenvectors are: max_i |lambda_i - mu|^p <= tr (H - mu I)^p for even p).  The interval
+// [mu - r, mu + r], widened by 1e-3 of r for the 22-bit arithmetic of the squarings and intersected with the
+// Gershgorin discs, is handed to the regular solve as user bounds; the control block is reset for it.
+__global__ void k_power_finish(Sp2Ctrl* c) {
+  const int s = c->n;                               // squarings actually applied
+  const bool have = c->pw_total > 0 && c->status == SP2_OK && c->fro_y > 0.0 && isfinite(c->fro_y);
+  double lo = c->eps_min, hi = c->eps_max;          // Gershgorin (k_setup of the power phase kept it)
+  if (have) {
+    // ||A^(2^s)||_F = 2^pw_log2scale sqrt(fro_y);  r = r0 * that^(1/2^s)
+    const double lg = (c->pw_log2scale + 0.5 * log2(c->fro_y)) / sp2_exp2i(s);
+    const double r = c->pw_r0 * exp2(lg) * (1.0 + 1e-3);
+    lo = fmax(lo, c->pw_mu - r);
+    hi = fmin(hi, c->pw_mu + r);
+  }
+  const int keep_status = (c->status == SP2_ERR_NONFINITE) ? c->status : SP2_OK;
+  c->pw_phase = 0;
+  if (have && hi > lo) { c->user_bounds = 1; c->user_eps_min = lo; c->user_eps_max = hi; }
+  c->n = 0; c->done = (keep_status != SP2_OK) ? 1 : 0; c->status = keep_status; c->stop_reason = 0;
+  c->sign_mask[0] = 0ull; c->sign_mask[1] = 0ull;
+  c->ticket = 0u; c->epoch = 0u;
+  c->c = 0.0; c->t = 0; c->sigma_last = 0.0; c->fro_in = 0.0; c->t_in = 0;
+}
+
 __global__ void k_init(Sp2Ctrl* c, int N, int n_occ, int npad, int with_response, int max_layers,
                        int user_bounds, double eps_min, double eps_max, double tol,
-                       int forced_layers, unsigned long long forced_signs, int no_recentre) {
+                       int forced_layers, unsigned long long forced_signs, int no_recentre, int power_squarings) {
   // one thread: reset the whole control block
   Sp2Ctrl z;
   memset(&z, 0, sizeof(z));
   z.N = N; z.n_occ = n_occ; z.npad = npad; z.with_response = with_response;
   z.max_layers = max_layers; z.user_bounds = user_bounds; z.user_eps_min = eps_min; z.user_eps_max = eps_max;
   z.tol = tol; z.forced_layers = forced_layers; z.forced_signs = forced_signs; z.no_recentre = no_recentre;
+  z.pw_total = power_squarings; z.pw_phase = power_squarings > 0 ? 1 : 0;
   *c = z;
 }
 
@@ -558,10 +591,12 @@ __global__ void k_init(Sp2Ctrl* c, int N, int n_occ, int npad, int with_response
 
 void sp2_launch_init(Sp2Ctrl* c, int N, int n_occ, int npad, int with_response, int max_layers,
                      int user_bounds, double eps_min, double eps_max, double tol, int forced_layers,
-                     unsigned long long forced_signs, int no_recentre, cudaStream_t s) {
+                     unsigned long long forced_signs, int no_recentre, int power_squarings, cudaStream_t s) {
   k_init<<<1, 1, 0, s>>>(c, N, n_occ, npad, with_response, max_layers, user_bounds, eps_min, eps_max, tol,
-                         forced_layers, forced_signs, no_recentre);
+                         forced_layers, forced_signs, no_recentre, power_squarings);
 }
+
+void sp2_launch_power_finish(Sp2Ctrl* c, cudaStream_t s) { k_power_finish<<<1, 1, 0, s>>>(c); }
 
 void sp2_launch_close(Sp2Ctrl* c, cudaStream_t s) { k_close<<<1, 1, 0, s>>>(c); }
 

@@ -55,7 +55,7 @@ class Sp2Options(C.Structure):
         ("engine", C.c_int), ("forced_layers", C.c_int),
         ("forced_signs", C.c_ulonglong), ("cta_group", C.c_int),
         ("lanczos_steps", C.c_int), ("refine_layers", C.c_int), ("seg_kb", C.c_int), ("lo_bits", C.c_int), ("no_recentre", C.c_int),
-        ("persistent", C.c_int), ("max_ctas", C.c_int),
+        ("persistent", C.c_int), ("max_ctas", C.c_int), ("power_squarings", C.c_int), ("reserved_pad", C.c_int),
     ]
 
 

@@ -43,7 +43,7 @@ def test_library_exports_every_declared_symbol(sp2):
 
 def test_struct_layouts_match_the_header(sp2):
     # sizes implied by the C declarations (natural alignment, LP64)
-    assert ctypes.sizeof(sp2.Sp2Options) == 72   # 2 int, 2 double, 2 int, u64, 8 int
+    assert ctypes.sizeof(sp2.Sp2Options) == 80   # 2 int, 2 double, 2 int, u64, 10 int
     assert ctypes.sizeof(sp2.Sp2Result) == 96
     assert sp2.Sp2Result.tr_d.offset == 32 and sp2.Sp2Result.gpu_ms.offset == 80
 

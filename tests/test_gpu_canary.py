@@ -8,7 +8,7 @@ geometry, not from the allocation formulas), and every other byte must still hol
 Sizes cover npad = 256 (where the round-1 slot array was 256 B short for a response solve: the layer kernel writes one
 slot per CTA and class, the layout had kept a per-tile formula), ragged sizes, several tiles, both cta_group code
 paths, and every entry point: density, response, batch(8), congruence, refinement, sequence, host buffers, the SIMT
-scaffold, Lanczos bounds and the trivial occupations.  Results are also checked (status, trace), so a kernel that
+scaffold, Lanczos and power-trace bounds and the trivial occupations.  Results are also checked (status, trace), so a kernel that
 stays in bounds by doing nothing does not pass.
 """
 import numpy as np
@@ -60,7 +60,11 @@ def test_workspace_canary_every_entry_point(torch_cuda, sp2, n):
         D, r = h.density(H, n_occ)
         assert r["status"] == 0 and abs(r["tr_d"] - n_occ) <= 1e-3, r
         _assert_clean(h, f"lanczos cta_group={cg}")
-        h.set_options(cta_group=cg, lanczos_steps=0)
+        h.set_options(cta_group=cg, lanczos_steps=0, power_squarings=3)
+        D, D1, r = h.response(H, H1s[0], n_occ)
+        assert r["status"] == 0 and abs(r["tr_d"] - n_occ) <= 1e-3, r
+        _assert_clean(h, f"power-trace bounds cta_group={cg}")
+        h.set_options(cta_group=cg, power_squarings=0)
         h.sequence_begin(n, n_occ, n_steps_hint=3)
         Ds = [torch.empty_like(H) for _ in range(3)]
         for Dt in Ds:

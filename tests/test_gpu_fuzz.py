@@ -1,6 +1,6 @@
 """Seeded random sweep of the GPU path against the oracle through the C ABI: N = 2..1500, any occupation, gaps
-0.02..1, f32 / f64 inputs, 0-3 perturbations (magnitudes up to 3 decades apart), every tile shape, with and without
-Lanczos bounds.  Tolerances [north_star]: max|dD| <= 1e-4, |tr D - N_occ| <= 1e-3, rel d tr(DH) <= 1e-5,
+0.02..1, f32 / f64 inputs, 0-3 perturbations (magnitudes up to 3 decades apart), every tile shape, with Gershgorin, Lanczos
+or power-trace bounds.  Tolerances [north_star]: max|dD| <= 1e-4, |tr D - N_occ| <= 1e-3, rel d tr(DH) <= 1e-5,
 max|dD1_b| <= 1e-3 max|D1_b|."""
 import numpy as np
 import pytest
@@ -25,21 +25,22 @@ def test_random_sweep_against_oracle(torch_cuda, sp2, seed0):
         cg = int(rng.choice([0, 1, 2]))
         lz = int(rng.choice([0, 0, 8]))
         lz = lz if n > lz else 0
+        pw = int(rng.choice([0, 0, 3])) if lz == 0 else 0          # rigorous power-trace bounds instead
         cfg = inputs.Sp2Config("sweep", 2, n, n_occ, (-1.5, -gap / 2), (gap / 2, 1.5), dt, False)
         p = inputs.make_problem(cfg, seed=seed0 * 1000 + it)
         H1s = inputs.perturbations(n, nb, seed=it, dtype=p["H"].dtype, decades=float(rng.choice([0.0, 1.0, 3.0])))
         H64 = p["H"].astype(np.float64)
-        bounds = oracle.lanczos_bounds(H64, lz) if lz else None
+        bounds = oracle.lanczos_bounds(H64, lz) if lz else (oracle.power_trace_bounds(H64, pw) if pw else None)
         ref = oracle.sp2_response_batch(H64, n_occ, [a.astype(np.float64) for a in H1s], bounds=bounds)
         h = sp2.Sp2Handle(n, batch=nb)
-        h.set_options(cta_group=cg, lanczos_steps=lz)
+        h.set_options(cta_group=cg, lanczos_steps=lz, power_squarings=pw)
         H = torch.from_numpy(p["H"]).cuda()
         if nb:
             D, D1s, _, r = h.response_batch(H, [torch.from_numpy(a).cuda() for a in H1s], n_occ)
         else:
             (D, r), D1s = h.density(H, n_occ), []
         h.close()
-        case = f"case {seed0}/{it}: n={n} n_occ={n_occ} gap={gap} {dt} nb={nb} cta_group={cg} lanczos={lz}"
+        case = f"case {seed0}/{it}: n={n} n_occ={n_occ} gap={gap} {dt} nb={nb} cta_group={cg} lanczos={lz} power={pw}"
         assert r["status"] == 0, case
         assert np.abs(D.cpu().numpy().astype(np.float64) - ref["D"]).max() <= 1e-4, case
         assert abs(r["tr_d"] - n_occ) <= 1e-3, case
