@@ -379,11 +379,12 @@ sp2_status_t encode_plane_map(sp2_handle_t h, CUtensorMap* map, const __half* ba
 }
 
 // Tile shape: CTA pairs on 256x256 tiles (cta_group::2) halve the operand traffic per flop and win at large N;
-// single CTAs on 128x128 tiles have 4x more units to balance and less launch / cluster overhead and win below
-// (measured cross-over on B200: ~5600 density-only, ~4600 with response).
+// single CTAs on 128x128 tiles have 4x more units to balance and less launch / cluster overhead and win below.
+// Measured cross-over on B200 (round 2, back-to-back solves, us per layer cg1 / cg2): density N = 4096 224 / 260,
+// 4608 300 / 288, 5120 424 / 426; with response N = 3072 281 / 281, 3584 434 / 415, 4096 636 / 568.
 int pick_cta_group(sp2_handle_t h, int npad, int resp) {
   if (h->opt.cta_group == 1 || h->opt.cta_group == 2) return h->opt.cta_group;
-  return npad >= (resp ? 4608 : 5632) ? 2 : 1;
+  return npad >= (resp ? 3584 : 4608) ? 2 : 1;
 }
 
 // CTA(-pair)s of one layer launch: one per SM (pair of SMs), bounded by what the device can keep co-resident
