@@ -280,6 +280,68 @@ def test_pitch_dtypes_user_bounds_and_tol(sp2, torch_mod):
     h.close()
 
 
+def test_one_cta_solve_pitch_dtypes_bounds_and_batch(sp2, torch_mod):
+    """The one-launch path (N <= 128: k_small_solve<TI,TO>) through every template instantiation and option it reads:
+    f32 / f64 input with ld > N, f32 / f64 output with ld > N, user bounds, tol, two perturbations of very different
+    size, NaN input, degenerate H, and the debug planes it leaves in the workspace."""
+    import oracle
+
+    torch = torch_mod
+    n = 100
+    p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[3], n))          # f32 input, 2/3 filling
+    n_occ = p["n_occ"]
+    H64 = p["H"].astype(np.float64)
+    ref = oracle.sp2_density(H64, n_occ)
+    h = sp2.Sp2Handle(128, batch=2)
+    for in_dt in (torch.float32, torch.float64):
+        for out_dt in (torch.float32, torch.float64):
+            big = torch.zeros(n, n + 12, dtype=in_dt, device="cuda")
+            big[:, :n] = torch.from_numpy(p["H"]).cuda().to(in_dt)
+            outbig = torch.full((n, n + 4), 7.0, dtype=out_dt, device="cuda")
+            D, r = h.density(big[:, :n], n_occ, out=outbig[:, :n])
+            assert r["status"] == 0 and r["kernel_launches"] == 1
+            assert np.abs(D.double().cpu().numpy() - ref["D"]).max() <= TOL_D
+            assert float(outbig[:, n:].min()) == 7.0                              # nothing written past N
+            assert abs(r["tr_d"] - n_occ) <= TOL_TR and abs(r["tr_dh"] - ref["tr_dh"]) <= TOL_E * abs(ref["tr_dh"])
+            assert r["eps_min"] == pytest.approx(ref["eps_min"], rel=1e-12) and r["eps_max"] == pytest.approx(ref["eps_max"], rel=1e-12)
+    H = torch.from_numpy(p["H"]).cuda()
+    lam = p["lam"]
+    h.set_options(user_bounds=(lam.min() - 1e-3, lam.max() + 1e-3))
+    D2, r2 = h.density(H, n_occ)
+    assert r2["layers"] < r["layers"] and np.abs(D2.double().cpu().numpy() - ref["D"]).max() <= TOL_D
+    h.set_options()
+    D3, r3 = h.density(H, n_occ, tol=1e-2)
+    assert r3["stop_reason"] == 1 and r3["layers"] <= r["layers"] and 0 <= r3["idem_est"] <= 1e-2
+    tr_x, e = h.debug_history()
+    assert len(e) == r3["layers"] + 1 and e[-1] == pytest.approx(r3["idem_est"])
+    # two perturbations, five decades apart, on the one-CTA path
+    H1s = inputs.perturbations(n, 2, seed=4, dtype=np.float32, decades=5.0)
+    refb = oracle.sp2_response_batch(H64, n_occ, [a.astype(np.float64) for a in H1s])
+    Db, D1b, tr1, rb = h.response_batch(H, [torch.from_numpy(a).cuda() for a in H1s], n_occ)
+    assert rb["status"] == 0 and rb["kernel_launches"] == 1
+    assert np.abs(Db.double().cpu().numpy() - refb["D"]).max() <= TOL_D
+    for b in range(2):
+        assert np.abs(D1b[b].double().cpu().numpy() - refb["D1"][b]).max() <= TOL_D1 * np.abs(refb["D1"][b]).max()
+        assert abs(tr1[b]) <= 1e-3 * np.abs(refb["D1"][b]).max() * n ** 0.5
+    Yh, ex, shift = h.debug_plane(0)
+    Ym = h.debug_plane(1)[0]
+    Y = (Yh.double() + Ym.double()).cpu().numpy() * 2.0 ** (-ex)
+    assert np.abs(shift * np.eye(n) + Y[:n, :n] - Db.double().cpu().numpy()).max() <= 1e-6     # the planes left behind are the final iterate
+    assert np.abs(Y[n:, :]).max() == 0.0 and np.abs(Y[:, n:]).max() == 0.0 and np.array_equal(Y, Y.T)
+    # error paths inside the one launch
+    Hn = H.clone()
+    Hn[3, 9] = float("nan")
+    with pytest.raises(sp2.Sp2Error) as ei:
+        h.density(Hn, n_occ)
+    assert ei.value.status == sp2.SP2_ERR_NONFINITE
+    with pytest.raises(sp2.Sp2Error) as ei:
+        h.density(2.5 * torch.eye(n, dtype=torch.float32, device="cuda"), n_occ)
+    assert ei.value.status == sp2.SP2_ERR_DEGENERATE
+    D4, r4 = h.density(H, n_occ)
+    assert r4["status"] == 0 and torch.equal(D4, h.density(H, n_occ)[0])          # still fine, and reproducible
+    h.close()
+
+
 def test_host_buffer_calls(sp2, torch_mod):
     import oracle
 
