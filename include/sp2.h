@@ -25,10 +25,14 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
  *   - The library allocates NO device memory: the caller passes a device workspace of at least
  *     sp2_workspace_bytes() bytes (e.g. a torch uint8 tensor), 1024-byte aligned, which the handle
- *     uses until sp2_destroy.  One handle = one call in flight (not re-entrant).  The layer kernel is persistent
- *     (one CTA per SM) and its last-wave units hand partial sums between CTAs, so run ONE solve per GPU at a
- *     time: two solves on different streams of the same GPU can starve each other's CTAs (a device-side
- *     watchdog then traps, SP2_ERR_CUDA, instead of hanging).
+ *     uses until sp2_destroy; nothing depends on its initial contents.  One handle = one call in flight (not
+ *     re-entrant).  The layer kernels are persistent (one CTA per SM): their last-wave units hand partial sums between
+ *     CTAs and, up to N = 2048, all layers of a solve run in one launch with a grid-wide barrier in between, so every
+ *     CTA of a launch must be resident at once.  sp2_create sizes the grid by what the device can keep co-resident
+ *     (cudaOccupancyMaxActiveClusters) and fails with SP2_ERR_CUDA if the kernel does not fit at all; at run time that
+ *     needs the SMs to be free, so run ONE solve per GPU at a time, or leave SMs to other work with
+ *     sp2_options_t.max_ctas: two solves on different streams of the same GPU can starve each other's CTAs (a
+ *     device-side watchdog then traps, SP2_ERR_CUDA, instead of hanging).
  *   - Every call returns an sp2_status_t; nothing throws, nothing prints.  The blocking calls
  *     enqueue all kernels on `stream`, synchronise that stream once, and fill *out (a HOST struct).
  *   - There is no CPU fallback: on a device that is not compute capability 10.x the calls return
