@@ -450,9 +450,9 @@ def run_ours(args):
     h = sp2.Sp2Handle(n, response=response, host_staging=True, refinement=args.refine > 0)
     if args.lanczos > 0:
         h.set_options(lanczos_steps=args.lanczos)
-    if args.max_ctas > 0 or args.persistent or args.seg_kb or args.cta_group or args.power:
+    if args.max_ctas > 0 or args.persistent or args.seg_kb or args.cta_group or args.power or args.lockstep:
         h.set_options(max_ctas=args.max_ctas, persistent=args.persistent, seg_kb=args.seg_kb, cta_group=args.cta_group,
-                      power_squarings=args.power)
+                      power_squarings=args.power, lockstep=args.lockstep)
     if args.refine > 0:
         if response:
             raise SystemExit("--refine goes with a density workload")
@@ -839,6 +839,7 @@ def main(argv=None):
     ap.add_argument("--cpu-eigh", action="store_true", help="also time numpy eigh + V_occ V_occ^T above N = 6000 (minutes)")
     ap.add_argument("--lanczos", type=int, default=0,
                     help="Lanczos steps for tighter spectral bounds (SURVEY 8(f) NEXT-3); extra, not the headline")
+    ap.add_argument("--lockstep", type=int, default=0, help="sp2_options_t.lockstep: 0 auto, 1 on, 2 off")
     ap.add_argument("--power", type=int, default=0,
                     help="sp2_options_t.power_squarings: rigorous power-trace spectral bounds (SURVEY 8(f) NEXT-3); extra, not the headline")
     ap.add_argument("--refine", type=int, default=0,

@@ -211,7 +211,7 @@ struct sp2_handle_s {
   int n_active;                  // CTA(-pair)s whose work list is not empty (grid of the persistent multi-layer launch)
   Sp2LayerArgs args[2];          // parity 0: buffer 0 -> 1, parity 1: buffer 1 -> 0
   Sp2LayerArgs args_pw[2];       // the same for the density-only power phase (= args when no perturbation is carried)
-  int n_flags_pw, n_active_pw, cur_pw;
+  int n_flags_pw, n_active_pw, cur_pw, cur_lock;
   std::vector<Sp2Item> items_pw_host;
   std::vector<int> item_begin_pw_host;
   std::vector<int2> tiles_host;
@@ -397,6 +397,8 @@ int layer_clusters(sp2_handle_t h, int cg) {
   return nC < 1 ? 1 : nC;
 }
 
+constexpr int kPersistMaxNpad = 2048;
+
 // (re)build the per-problem launch state: tile list, TMA descriptors, ping-pong argument blocks
 sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   const int npad = pad_n(N);
@@ -409,7 +411,8 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = npad > 24576 ? 2 : (npad > 8192 ? 4 : 8);
   while ((npad / 64) % seg) seg >>= 1;
   if (h->cur_n == N && h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp && h->cur_seg == seg &&
-      h->cur_lo == h->opt.lo_bits && h->cur_maxctas == h->opt.max_ctas && h->cur_pw == (h->opt.power_squarings > 0))
+      h->cur_lo == h->opt.lo_bits && h->cur_maxctas == h->opt.max_ctas && h->cur_pw == (h->opt.power_squarings > 0) &&
+      h->cur_lock == h->opt.lockstep)
     return SP2_OK;
   const int nt = npad / (128 * cg);
   build_tiles(nt, h->tiles_host);
@@ -458,6 +461,21 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
                                 cudaMemcpyHostToDevice, s));
   }
   SP2_CUDA(h, cudaStreamSynchronize(s));     // host vectors may be rebuilt by the next prepare
+  // soft lockstep of the producers over the leading whole units every CTA(-pair) has (launch-per-layer mode only;
+  // on by default where it was measured to pay: solves with response.  Density-only layers: no change in time.)
+  int lock_items = 0;
+  const bool lock_on = h->opt.lockstep == 1 || (h->opt.lockstep == 0 && resp > 0);
+  if (lock_on && npad > kPersistMaxNpad && h->n_active == nC) {
+    lock_items = 1 << 30;
+    for (int c = 0; c < nC; ++c) {
+      int whole = 0;
+      for (int i = h->item_begin_host[c]; i < h->item_begin_host[c + 1] && h->items_host[i].kind == 0; ++i) ++whole;
+      if (whole < lock_items) lock_items = whole;
+    }
+    if (lock_items > 0) --lock_items;          // counters sit between consecutive items
+    if (h->n_flags + lock_items > 2 * kMaxClusters) lock_items = 2 * kMaxClusters - h->n_flags;
+    if (lock_items < 0) lock_items = 0;
+  }
   for (int par = 0; par < 2; ++par) {
     Sp2LayerArgs& a = h->args[par];
     memset(&a, 0, sizeof(a));
@@ -472,12 +490,13 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
     a.ctrl = h->ctrl(); a.slots = h->slots(); a.tiles = h->tiles();
     a.items = h->items(); a.item_begin = h->item_begin(); a.scratch = h->scratch(); a.flags = h->split_flags();
     a.n_flags = h->n_flags; a.n_clusters = h->n_clusters;
+    a.lock_items = lock_items; a.lock_need = (cg * nC * 3) / 4;
     a.lo_bits = (h->opt.lo_bits >= 6 && h->opt.lo_bits <= 10) ? h->opt.lo_bits : 11;
     a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = resp; a.seg_kb = seg;
     Sp2LayerArgs& q = h->args_pw[par];          // the power phase: Y planes only
     q = a;
     q.with_response = 0;
-    if (pw_lists) { q.items = h->items_pw(); q.item_begin = h->item_begin_pw(); q.n_flags = h->n_flags_pw; }
+    if (pw_lists) { q.items = h->items_pw(); q.item_begin = h->item_begin_pw(); q.n_flags = h->n_flags_pw; q.lock_items = 0; }
   }
   SP2_CUDA(h, cudaMemcpyAsync(h->d_args(), h->args, 2 * sizeof(Sp2LayerArgs), cudaMemcpyHostToDevice, s));
   SP2_CUDA(h, cudaMemcpyAsync(h->d_args() + 2, h->args_pw, 2 * sizeof(Sp2LayerArgs), cudaMemcpyHostToDevice, s));
@@ -485,7 +504,7 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   h->touch(h->L.r_args, 4 * sizeof(Sp2LayerArgs));
   h->layers_hint = 0;
   h->cur_n = N; h->cur_npad = npad; h->cur_cg = cg; h->cur_resp = resp; h->cur_seg = seg; h->cur_lo = h->opt.lo_bits;
-  h->cur_maxctas = h->opt.max_ctas; h->cur_pw = h->opt.power_squarings > 0;
+  h->cur_maxctas = h->opt.max_ctas; h->cur_pw = h->opt.power_squarings > 0; h->cur_lock = h->opt.lockstep;
   return SP2_OK;
 }
 
@@ -520,7 +539,6 @@ sp2_status_t check_args(sp2_handle_t h, const void* H, const Pert& P, sp2_dtype_
 }
 
 // One persistent launch for the whole stack?  Small problems: a layer is shorter than a launch and its tail.
-constexpr int kPersistMaxNpad = 2048;
 // The smallest problems: one CTA, iterate resident in shared memory (sp2_small.cu).  Automatic choice only.
 bool use_small(sp2_handle_t h) {
   return h->opt.engine == SP2_ENGINE_TCGEN05 && h->opt.persistent == 0 && h->cur_n <= sp2_small_max_n() &&
@@ -842,7 +860,7 @@ sp2_status_t sp2_create(sp2_handle_t* handle, int n_max, int flags, void* d_work
   h->n_max = n_max; h->flags = flags; h->device = dev; h->num_sms = prop.multiProcessorCount; h->nb_max = L.nb_max;
   h->ws = static_cast<uint8_t*>(d_workspace); h->ws_bytes = bytes; h->L = L;
   default_options(&h->opt);
-  h->cur_n = -1; h->cur_npad = -1; h->cur_cg = -1; h->cur_resp = -1; h->cur_seg = -1; h->cur_maxctas = -1; h->n_active = 1; h->cur_pw = -1; h->n_active_pw = 1; h->n_flags_pw = 0;
+  h->cur_n = -1; h->cur_npad = -1; h->cur_cg = -1; h->cur_resp = -1; h->cur_seg = -1; h->cur_maxctas = -1; h->n_active = 1; h->cur_pw = -1; h->cur_lock = -1; h->n_active_pw = 1; h->n_flags_pw = 0;
   h->last_cuda_error = 0; h->launches = 0; h->seq_active = 0; h->layers_hint = 0; h->no_lanczos = 0;
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
@@ -898,6 +916,7 @@ sp2_status_t sp2_set_options(sp2_handle_t h, const sp2_options_t* opt) {
   if (opt->user_bounds && !(opt->eps_max > opt->eps_min)) return SP2_ERR_INVALID_ARG;
   if (opt->persistent < 0 || opt->persistent > 2 || opt->max_ctas < 0) return SP2_ERR_INVALID_ARG;
   if (opt->power_squarings < 0 || opt->power_squarings > 6) return SP2_ERR_INVALID_ARG;
+  if (opt->lockstep < 0 || opt->lockstep > 2) return SP2_ERR_INVALID_ARG;
   h->opt = *opt;
   h->layers_hint = 0;
   return SP2_OK;

@@ -104,7 +104,7 @@ __device__ inline void layer_tail(Sp2Ctrl* ctrl, const Sp2Slot* slots, int n_y, 
   __syncthreads();
   if (!*is_last_smem) return;
   __threadfence();
-  for (int i = threadIdx.x; i < n_flags; i += blockDim.x) flags[i] = 0u;   // every split unit was consumed
+  for (int i = threadIdx.x; i < n_flags; i += blockDim.x) flags[i] = 0u;   // every split unit was consumed (and the lockstep counters)
   double tr, fro, mx, tracc, unused;
   sp2_reduce_slots(slots + (size_t)nb * n_z, n_y, red, tr, fro, mx, tracc);
   for (int b = 0; b < nb; ++b) {
@@ -532,6 +532,18 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
             const int zpl = 2 + 2 * zb;                // planes of Z_b
             const int row_a = tij.x * TILE + (int)rank * kRows;
             const int row_b = tij.y * TILE + (int)rank * kRows;
+            // Soft lockstep at unit boundaries (launch-per-layer mode, large N): CTAs that run concurrently stream the
+            // same row / column panels, and a panel byte is fetched from DRAM once only while they stay coincident in
+            // L2.  A producer starts item k + 1 once lock_need of the grid's producers have issued all loads of item
+            // k; waiting for 3/4 of them rather than all keeps the stragglers of one item from stalling everybody
+            // (measured at N = 8192 with response: DRAM reads 6.2 -> 4.3 GB per launch, layer time -1 % under the
+            // power cap and -3 % outside it; waiting for all: 4.0 GB but +1 %).
+            const int kloc = iti - item_lo;
+            if (!PERSIST && kloc > 0 && kloc <= a.lock_items) {
+              const volatile unsigned int* cnt = a.flags + a.n_flags + (kloc - 1);
+              long long spins = 0;
+              while (*cnt < (unsigned)a.lock_need) if (++spins > kSpinLimit) __trap();
+            }
             for (int g = I.seg0 * seg_kb; g < I.seg1 * seg_kb; ++g) {
               // Y^2: A = (Yh, Ym), B = (Yh, Ym).  W pass 0: A = (Yh, Ym), B = (Zh, Zm).  W pass 1: A = (Zh, Zm), B = (Yh, Ym).
               const int p = (g >= KB) ? 1 : 0;
@@ -547,6 +559,7 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
               tma_load_2d<CG>(dst + 3 * kPlaneTileBytes, &a.tm[mb + 1], full_bar[stage], kb * kBK, row_b);
               if (++stage == kStages) { stage = 0; phase ^= 1u; }
             }
+            if (!PERSIST && kloc < a.lock_items) atomicAdd(a.flags + a.n_flags + kloc, 1u);   // this item's loads are issued
           }
           if (!PERSIST) break;
           // arrive half of the grid barrier: every CTA has stored its planes of the layer just loaded.  (When the
@@ -805,7 +818,7 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
     }
     __syncthreads();
     if (bars->is_last) {
-      for (int i = threadIdx.x; i < a.n_flags; i += blockDim.x) a.flags[i] = 0u;
+      for (int i = threadIdx.x; i < a.n_flags + a.lock_items; i += blockDim.x) a.flags[i] = 0u;
       if (threadIdx.x == 0) a.ctrl->ticket = 0u;
     }
     return;
@@ -822,7 +835,8 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
     }
     a.slots[(size_t)(cls == 0 ? a.with_response : cls - 1) * gridDim.x + blockIdx.x] = t;
   }
-  layer_tail(a.ctrl, a.slots, gridDim.x, gridDim.x, a.with_response, gridDim.x, &bars->is_last, red, a.flags, a.n_flags);
+  layer_tail(a.ctrl, a.slots, gridDim.x, gridDim.x, a.with_response, gridDim.x, &bars->is_last, red, a.flags,
+             a.n_flags + a.lock_items);
 }
 
 

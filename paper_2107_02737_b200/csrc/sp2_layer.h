@@ -30,6 +30,9 @@ struct alignas(64) Sp2LayerArgs {
   float* scratch;        // split-k partial sums
   unsigned int* flags;   // one arrival counter per split unit (zero between launches)
   int n_flags;
+  int lock_items;        // > 0: soft lockstep of the TMA producers over the first lock_items + 1 items of every work list
+                         // (arrival counters flags[n_flags .. n_flags + lock_items), zeroed with the split-k flags)
+  int lock_need;         // arrivals a producer waits for before it starts its next item (<= CTAs of the grid)
   int lo_bits;           // significant bits kept in the lo planes (11 = all)
   // plain-product mode (sp2_congruence): C = A B^T, A = tm[0..1], B = tm[2..3]
   int gemm_mode;         // 0: SP2 layer, 1: plain product

@@ -55,7 +55,7 @@ class Sp2Options(C.Structure):
         ("engine", C.c_int), ("forced_layers", C.c_int),
         ("forced_signs", C.c_ulonglong), ("cta_group", C.c_int),
         ("lanczos_steps", C.c_int), ("refine_layers", C.c_int), ("seg_kb", C.c_int), ("lo_bits", C.c_int), ("no_recentre", C.c_int),
-        ("persistent", C.c_int), ("max_ctas", C.c_int), ("power_squarings", C.c_int), ("reserved_pad", C.c_int),
+        ("persistent", C.c_int), ("max_ctas", C.c_int), ("power_squarings", C.c_int), ("lockstep", C.c_int),
     ]
 
 
@@ -237,8 +237,10 @@ class Sp2Handle:
             raise Sp2Error(st, status_string(st) + extra)
 
     def set_options(self, **kw):
-        """max_layers, user_bounds=(eps_min, eps_max) | None, engine, forced_layers, forced_signs, cta_group.
-        No keyword restores the defaults."""
+        """Fields of sp2_options_t (include/sp2.h) by name: max_layers, user_bounds=(eps_min, eps_max) | None, engine,
+        forced_layers, forced_signs, cta_group, seg_kb, lo_bits, refine_layers, lanczos_steps, persistent, max_ctas,
+        power_squarings, lockstep, ...  Keywords change the named fields and keep the others; no keyword restores the
+        defaults."""
         if not kw:
             self._raise(lib.sp2_set_options(self._h, None))
             return

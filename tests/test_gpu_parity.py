@@ -127,6 +127,33 @@ def test_persistent_stack_matches_per_layer_launches(sp2, torch_mod):
         assert np.array_equal(a[0], again[0]) and np.array_equal(a[1], again[1])
 
 
+def test_producer_lockstep_changes_timing_only(sp2, torch_mod):
+    """sp2_options_t.lockstep (launch-per-layer mode, N > 2048): the TMA producers wait for one another at unit
+    boundaries.  Same work lists, same reduction order: results are bitwise those of the free-running kernel, for both
+    tile shapes, a reduced grid, density-only lists (forced on) and a ragged size; one case goes to the oracle."""
+    import oracle
+
+    cases = ((2304, 2, True, dict()), (3100, 2, True, dict(cta_group=1)), (3100, 2, True, dict(cta_group=2, max_ctas=100)),
+             (2500, 3, False, dict()))
+    for n, base, response, opts in cases:
+        p = inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[base], n), device="cuda")
+        on = _solve(sp2, torch_mod, p, response=response, lockstep=1, **opts)
+        off = _solve(sp2, torch_mod, p, response=response, lockstep=2, **opts)
+        auto = _solve(sp2, torch_mod, p, response=response, **opts)
+        for x in (on, off, auto):
+            assert x[2]["status"] == 0 and abs(x[2]["tr_d"] - p["n_occ"]) <= TOL_TR
+        assert np.array_equal(on[0], off[0]) and np.array_equal(on[0], auto[0])
+        assert on[2]["signs"] == off[2]["signs"] and on[2]["tr_dh"] == off[2]["tr_dh"]
+        if response:
+            assert np.array_equal(on[1], off[1]) and np.array_equal(on[1], auto[1])
+        if n == 2304:
+            _check_against_oracle(p, on[0], on[1], on[2], oracle)
+    h = sp2.Sp2Handle(64)
+    with pytest.raises(Exception):
+        h.set_options(lockstep=3)
+    h.close()
+
+
 def test_segment_lengths_and_simt_scaffold_agree(sp2, torch_mod):
     import oracle
 
