@@ -124,8 +124,9 @@ typedef struct {
   int lockstep;     /* launch-per-layer mode (N > 2048): 0 = auto (on for solves with response), 1 = on, 2 = off.  On: the
                        TMA producer of a CTA starts its next work item only after 3/4 of the grid's producers have
                        issued the loads of the current one, so CTAs that stream the same panels stay coincident in L2
-                       (30 % fewer DRAM reads per layer at N = 8192).  Needs the grid co-resident, as the split-k
-                       hand-over does: never launch more CTAs than max_ctas allows on a shared device. */
+                       (30 % fewer DRAM reads per layer at N = 8192).  A hint only: a producer that
+                       waits longer than about half a work item free-runs for the rest of the launch, so sharing the
+                       device with other streams costs the saving, not progress.  Results are bitwise the same. */
 } sp2_options_t;
 
 typedef struct {

@@ -491,6 +491,7 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
     a.items = h->items(); a.item_begin = h->item_begin(); a.scratch = h->scratch(); a.flags = h->split_flags();
     a.n_flags = h->n_flags; a.n_clusters = h->n_clusters;
     a.lock_items = lock_items; a.lock_need = (cg * nC * 3) / 4;
+    a.lock_polls = 16 + npad / 64;             // ~ half the duration of a whole unit (k-blocks x 1.2 us at the capped clock)
     a.lo_bits = (h->opt.lo_bits >= 6 && h->opt.lo_bits <= 10) ? h->opt.lo_bits : 11;
     a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = resp; a.seg_kb = seg;
     Sp2LayerArgs& q = h->args_pw[par];          // the power phase: Y planes only

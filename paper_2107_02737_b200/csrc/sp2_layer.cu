@@ -516,6 +516,7 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
       if (elect_one()) {
         int stage = 0; uint32_t phase = 0;
         unsigned int layers_loaded = 0;
+        bool lock_live = true;
         uint32_t full_bar[kStages];
         for (int s = 0; s < kStages; ++s) {
           full_bar[s] = smem_u32(&bars->full[s]);
@@ -538,11 +539,17 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
             // k; waiting for 3/4 of them rather than all keeps the stragglers of one item from stalling everybody
             // (measured at N = 8192 with response: DRAM reads 6.2 -> 4.3 GB per launch, layer time -1 % under the
             // power cap and -3 % outside it; waiting for all: 4.0 GB but +1 %).
+            // The wait is a hint, not a dependency: it gives up after lock_polls polls (about half an item) and this CTA
+            // then free-runs for the rest of the launch, so a grid that is not fully resident (another stream's
+            // kernels on the same SMs) loses the traffic saving, never its progress.
             const int kloc = iti - item_lo;
-            if (!PERSIST && kloc > 0 && kloc <= a.lock_items) {
+            if (!PERSIST && lock_live && kloc > 0 && kloc <= a.lock_items) {
               const volatile unsigned int* cnt = a.flags + a.n_flags + (kloc - 1);
-              long long spins = 0;
-              while (*cnt < (unsigned)a.lock_need) if (++spins > kSpinLimit) __trap();
+              int polls = 0;
+              while (*cnt < (unsigned)a.lock_need) {
+                if (++polls > a.lock_polls) { lock_live = false; break; }
+                __nanosleep(256);
+              }
             }
             for (int g = I.seg0 * seg_kb; g < I.seg1 * seg_kb; ++g) {
               // Y^2: A = (Yh, Ym), B = (Yh, Ym).  W pass 0: A = (Yh, Ym), B = (Zh, Zm).  W pass 1: A = (Zh, Zm), B = (Yh, Ym).

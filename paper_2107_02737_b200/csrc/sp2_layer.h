@@ -32,6 +32,7 @@ struct alignas(64) Sp2LayerArgs {
   int n_flags;
   int lock_items;        // > 0: soft lockstep of the TMA producers over the first lock_items + 1 items of every work list
                          // (arrival counters flags[n_flags .. n_flags + lock_items), zeroed with the split-k flags)
+  int lock_polls;        // polls (256 ns apart) after which a producer gives the lockstep up for the rest of the launch
   int lock_need;         // arrivals a producer waits for before it starts its next item (<= CTAs of the grid)
   int lo_bits;           // significant bits kept in the lo planes (11 = all)
   // plain-product mode (sp2_congruence): C = A B^T, A = tm[0..1], B = tm[2..3]

@@ -154,6 +154,49 @@ def test_producer_lockstep_changes_timing_only(sp2, torch_mod):
     h.close()
 
 
+@pytest.mark.parametrize("max_ctas", [0, 74])
+def test_two_handles_on_two_streams_at_once(sp2, torch_mod, max_ctas):
+    """Two large response solves in flight on one device (two handles, two streams, two host threads): with the SMs
+    partitioned by max_ctas, and with both grids competing for all of them -- the producers' lockstep then times out and
+    free-runs.  Either way the results are bitwise those of the same solves run alone."""
+    import threading
+
+    torch = torch_mod
+    n = 2304
+    ps = [inputs.make_problem(inputs.scaled_config(inputs.CONFIGS[2], n), seed=s, device="cuda") for s in (1, 2)]
+    Hs = [torch.from_numpy(p["H"]).cuda() for p in ps]
+    H1s = [torch.from_numpy(p["H1"]).cuda() for p in ps]
+    hs = [sp2.Sp2Handle(n, response=True) for _ in ps]
+    alone = []
+    for h, H, H1, p in zip(hs, Hs, H1s, ps):
+        h.set_options(max_ctas=max_ctas)
+        D, D1, r = h.response(H, H1, p["n_occ"])
+        assert r["status"] == 0 and abs(r["tr_d"] - p["n_occ"]) <= TOL_TR
+        alone.append((D.clone(), D1.clone(), r["signs"]))
+    torch.cuda.synchronize()
+    got = [None, None]
+
+    def run(i):
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            for _ in range(4):
+                D, D1, r = hs[i].response(Hs[i], H1s[i], ps[i]["n_occ"])
+            got[i] = (D.clone(), D1.clone(), r["signs"], r["status"])
+        s.synchronize()
+
+    ts = [threading.Thread(target=run, args=(i,)) for i in range(2)]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+    torch.cuda.synchronize()
+    for i in range(2):
+        assert got[i] is not None and got[i][3] == 0
+        assert torch.equal(got[i][0], alone[i][0]) and torch.equal(got[i][1], alone[i][1]) and got[i][2] == alone[i][2]
+    for h in hs:
+        h.close()
+
+
 def test_segment_lengths_and_simt_scaffold_agree(sp2, torch_mod):
     import oracle
 
