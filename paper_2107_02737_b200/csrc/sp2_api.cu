@@ -398,6 +398,7 @@ int layer_clusters(sp2_handle_t h, int cg) {
 }
 
 constexpr int kPersistMaxNpad = 2048;
+constexpr int kLockstepMinNpad = 7168;
 
 // (re)build the per-problem launch state: tile list, TMA descriptors, ping-pong argument blocks
 sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
@@ -461,10 +462,11 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
                                 cudaMemcpyHostToDevice, s));
   }
   SP2_CUDA(h, cudaStreamSynchronize(s));     // host vectors may be rebuilt by the next prepare
-  // soft lockstep of the producers over the leading whole units every CTA(-pair) has (launch-per-layer mode only;
-  // on by default where it was measured to pay: solves with response.  Density-only layers: no change in time.)
+  // soft lockstep of the producers over the leading whole units every CTA(-pair) has (launch-per-layer mode only).
+  // On by default from N = 7168: measured per-layer gain 1-3 % at N = 8192 (D + D1 .. four perturbations; density-only
+  // unchanged), 1.3 % / 5-7 % at N = 12288 (density / response), 2.8 % / 7.7 % at N = 16384; no gain below.
   int lock_items = 0;
-  const bool lock_on = h->opt.lockstep == 1 || (h->opt.lockstep == 0 && resp > 0);
+  const bool lock_on = h->opt.lockstep == 1 || (h->opt.lockstep == 0 && npad >= kLockstepMinNpad);
   if (lock_on && npad > kPersistMaxNpad && h->n_active == nC) {
     lock_items = 1 << 30;
     for (int c = 0; c < nC; ++c) {
