@@ -121,12 +121,13 @@ typedef struct {
                        eigenvectors are (no start vector, unlike lanczos_steps), with r <= N^(1/2^(s+1)) rho.  The solve then
                        uses [mu - r, mu + r] (widened by 1e-3 r, intersected with the Gershgorin discs).  Costs s density
                        layers, saves ~2 log2(Gershgorin width / 2r) layers; takes precedence over lanczos_steps */
-  int lockstep;     /* launch-per-layer mode (N > 2048): 0 = auto (on from N = 7168), 1 = on, 2 = off.  On: the
-                       TMA producer of a CTA starts its next work item only after 3/4 of the grid's producers have
-                       issued the loads of the current one, so CTAs that stream the same panels stay coincident in L2
-                       (30 % fewer DRAM reads per layer at N = 8192).  A hint only: a producer that
-                       waits longer than about half a work item free-runs for the rest of the launch, so sharing the
-                       device with other streams costs the saving, not progress.  Results are bitwise the same. */
+  int lockstep;     /* launch-per-layer mode (N > 2048): 0 = auto (on from N = 7168), 1 = on, 2 = off.  On: the TMA producer
+                       of a CTA checks in every 16 k-blocks and runs ahead only when 7/8 of the grid's producers have
+                       reached the same point, so CTAs that stream the same panels stay coincident in L2 (a third
+                       fewer DRAM reads per layer at N = 8192, a third of them left at N = 16384).  A hint only: a
+                       producer that waits longer than about half a work item free-runs for the rest of the launch,
+                       so sharing the device with other streams costs the saving, not progress.  Results are bitwise
+                       the same either way. */
 } sp2_options_t;
 
 typedef struct {

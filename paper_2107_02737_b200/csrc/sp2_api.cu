@@ -55,6 +55,7 @@ constexpr int kRingCap = 4096;
 constexpr int kPadTo = 256;          // npad is a multiple of the largest tile edge
 constexpr int kSimtMaxN = 4096;
 constexpr int kMaxClusters = 256;   // >= SM count of any sm_100 part
+constexpr int kFlagWords = 2 * kMaxClusters + 32768;   // split-k flags, then the checkpoint counters of the producers' lockstep
 constexpr int kSeqSlack = 8;        // extra layer launches per sequence step on top of the last finished step's count
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -158,7 +159,7 @@ Layout make_layout(int n_max, int flags) {
   if (2 * (size_t)(kMaxClusters / 2) * sp2_layer_scratch_slot_bytes(2) > L.scratch_bytes)
     L.scratch_bytes = 2 * (size_t)(kMaxClusters / 2) * sp2_layer_scratch_slot_bytes(2);
   L.r_scratch = carve("scratch", L.scratch_bytes, &L.off_scratch);
-  L.r_flags = carve("flags", 2 * kMaxClusters * sizeof(unsigned int), &L.off_flags);
+  L.r_flags = carve("flags", kFlagWords * sizeof(unsigned int), &L.off_flags);
   L.r_ctrl = carve("ctrl", sizeof(Sp2Ctrl), &L.off_ctrl);
   L.r_args = carve("args", 4 * sizeof(Sp2LayerArgs), &L.off_args);      // [0..1] the solve, [2..3] its power phase
   L.r_ring = carve("ring", (size_t)kRingCap * sizeof(sp2_result_t), &L.off_ring);
@@ -434,13 +435,13 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   h->touch(h->L.r_tiles, h->tiles_host.size() * sizeof(int2));
   h->touch(h->L.r_items, h->items_host.size() * sizeof(Sp2Item));
   h->touch(h->L.r_item_begin, h->item_begin_host.size() * sizeof(int));
-  h->touch(h->L.r_flags, 2 * kMaxClusters * sizeof(unsigned int));
+  h->touch(h->L.r_flags, kFlagWords * sizeof(unsigned int));
   h->touch(h->L.r_scratch, (size_t)n_slots * sp2_layer_scratch_slot_bytes(cg));
   SP2_CUDA(h, cudaMemcpyAsync(h->items(), h->items_host.data(), h->items_host.size() * sizeof(Sp2Item),
                               cudaMemcpyHostToDevice, s));
   SP2_CUDA(h, cudaMemcpyAsync(h->item_begin(), h->item_begin_host.data(), h->item_begin_host.size() * sizeof(int),
                               cudaMemcpyHostToDevice, s));
-  SP2_CUDA(h, cudaMemsetAsync(h->split_flags(), 0, 2 * kMaxClusters * sizeof(unsigned int), s));
+  SP2_CUDA(h, cudaMemsetAsync(h->split_flags(), 0, kFlagWords * sizeof(unsigned int), s));
   // power phase of a solve that carries perturbations: the same tiles, density-only work lists of their own
   const bool pw_lists = h->opt.power_squarings > 0 && resp > 0;
   h->n_flags_pw = h->n_flags; h->n_active_pw = h->n_active;
@@ -463,20 +464,21 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   }
   SP2_CUDA(h, cudaStreamSynchronize(s));     // host vectors may be rebuilt by the next prepare
   // soft lockstep of the producers over the leading whole units every CTA(-pair) has (launch-per-layer mode only).
-  // On by default from N = 7168: measured per-layer gain 1-3 % at N = 8192 (D + D1 .. four perturbations; density-only
-  // unchanged), 1.3 % / 5-7 % at N = 12288 (density / response), 2.8 % / 7.7 % at N = 16384; no gain below.
-  int lock_items = 0;
+  // On by default from N = 7168: measured per-layer gain 2-3 % at N = 8192 with response (density-only unchanged),
+  // 9 % at N = 12288, 11 % (D + D1) and 4 % (density) at N = 16384; no gain below.
+  int lock_kb = 0;
   const bool lock_on = h->opt.lockstep == 1 || (h->opt.lockstep == 0 && npad >= kLockstepMinNpad);
   if (lock_on && npad > kPersistMaxNpad && h->n_active == nC) {
-    lock_items = 1 << 30;
+    lock_kb = 1 << 30;
     for (int c = 0; c < nC; ++c) {
       int whole = 0;
-      for (int i = h->item_begin_host[c]; i < h->item_begin_host[c + 1] && h->items_host[i].kind == 0; ++i) ++whole;
-      if (whole < lock_items) lock_items = whole;
+      for (int i = h->item_begin_host[c]; i < h->item_begin_host[c + 1] && h->items_host[i].kind == 0; ++i)
+        whole += (h->items_host[i].seg1 - h->items_host[i].seg0) * seg;
+      if (whole < lock_kb) lock_kb = whole;
     }
-    if (lock_items > 0) --lock_items;          // counters sit between consecutive items
-    if (h->n_flags + lock_items > 2 * kMaxClusters) lock_items = 2 * kMaxClusters - h->n_flags;
-    if (lock_items < 0) lock_items = 0;
+    lock_kb -= lock_kb % kLockEvery;
+    const int room = (kFlagWords - h->n_flags) * kLockEvery;   // beyond it the producers free-run
+    if (lock_kb > room) lock_kb = room;
   }
   for (int par = 0; par < 2; ++par) {
     Sp2LayerArgs& a = h->args[par];
@@ -492,14 +494,14 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
     a.ctrl = h->ctrl(); a.slots = h->slots(); a.tiles = h->tiles();
     a.items = h->items(); a.item_begin = h->item_begin(); a.scratch = h->scratch(); a.flags = h->split_flags();
     a.n_flags = h->n_flags; a.n_clusters = h->n_clusters;
-    a.lock_items = lock_items; a.lock_need = (cg * nC * 3) / 4;
+    a.lock_kb = lock_kb; a.lock_need = (cg * nC * 7) / 8;
     a.lock_polls = 16 + npad / 64;             // ~ half the duration of a whole unit (k-blocks x 1.2 us at the capped clock)
     a.lo_bits = (h->opt.lo_bits >= 6 && h->opt.lo_bits <= 10) ? h->opt.lo_bits : 11;
     a.n = N; a.npad = npad; a.n_tiles = (int)h->tiles_host.size(); a.with_response = resp; a.seg_kb = seg;
     Sp2LayerArgs& q = h->args_pw[par];          // the power phase: Y planes only
     q = a;
     q.with_response = 0;
-    if (pw_lists) { q.items = h->items_pw(); q.item_begin = h->item_begin_pw(); q.n_flags = h->n_flags_pw; q.lock_items = 0; }
+    if (pw_lists) { q.items = h->items_pw(); q.item_begin = h->item_begin_pw(); q.n_flags = h->n_flags_pw; q.lock_kb = 0; }
   }
   SP2_CUDA(h, cudaMemcpyAsync(h->d_args(), h->args, 2 * sizeof(Sp2LayerArgs), cudaMemcpyHostToDevice, s));
   SP2_CUDA(h, cudaMemcpyAsync(h->d_args() + 2, h->args_pw, 2 * sizeof(Sp2LayerArgs), cudaMemcpyHostToDevice, s));
@@ -1061,7 +1063,7 @@ sp2_status_t sp2_congruence(sp2_handle_t h, const void* dZ, const void* dX, sp2_
   h->touch(h->L.r_tiles, h->tiles_host.size() * sizeof(int2));
   h->touch(h->L.r_items, h->items_host.size() * sizeof(Sp2Item));
   h->touch(h->L.r_item_begin, h->item_begin_host.size() * sizeof(int));
-  h->touch(h->L.r_flags, 2 * kMaxClusters * sizeof(unsigned int));
+  h->touch(h->L.r_flags, kFlagWords * sizeof(unsigned int));
   h->touch(h->L.r_scratch, (size_t)n_slots * sp2_layer_scratch_slot_bytes(cg));
   h->touch(h->L.r_ctrl, sizeof(Sp2Ctrl));
   h->touch(h->L.r_ring, sizeof(sp2_result_t));
@@ -1072,7 +1074,7 @@ sp2_status_t sp2_congruence(sp2_handle_t h, const void* dZ, const void* dX, sp2_
   SP2_CUDA(h, cudaMemcpyAsync(h->items(), h->items_host.data(), h->items_host.size() * sizeof(Sp2Item), cudaMemcpyHostToDevice, s));
   SP2_CUDA(h, cudaMemcpyAsync(h->item_begin(), h->item_begin_host.data(), h->item_begin_host.size() * sizeof(int),
                               cudaMemcpyHostToDevice, s));
-  SP2_CUDA(h, cudaMemsetAsync(h->split_flags(), 0, 2 * kMaxClusters * sizeof(unsigned int), s));
+  SP2_CUDA(h, cudaMemsetAsync(h->split_flags(), 0, kFlagWords * sizeof(unsigned int), s));
   SP2_CUDA(h, cudaStreamSynchronize(s));
   Sp2Ctrl* c = h->ctrl();
   __half *Lh = h->plane(0, 0), *Lm = h->plane(1, 0), *Xh = h->plane(2, 0), *Xm = h->plane(3, 0), *Th = h->plane(2, 1),

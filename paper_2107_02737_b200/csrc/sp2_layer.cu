@@ -517,6 +517,7 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
         int stage = 0; uint32_t phase = 0;
         unsigned int layers_loaded = 0;
         bool lock_live = true;
+        int cum = 0;                       // k-blocks issued inside the lockstep region of this launch
         uint32_t full_bar[kStages];
         for (int s = 0; s < kStages; ++s) {
           full_bar[s] = smem_u32(&bars->full[s]);
@@ -533,30 +534,28 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
             const int zpl = 2 + 2 * zb;                // planes of Z_b
             const int row_a = tij.x * TILE + (int)rank * kRows;
             const int row_b = tij.y * TILE + (int)rank * kRows;
-            // Soft lockstep at unit boundaries (launch-per-layer mode, large N): CTAs that run concurrently stream the
-            // same row / column panels, and a panel byte is fetched from DRAM once only while they stay coincident in
-            // L2.  A producer starts item k + 1 once lock_need of the grid's producers have issued all loads of item
-            // k; waiting for 3/4 of them rather than all keeps the stragglers of one item from stalling everybody
-            // (measured at N = 8192 with response: DRAM reads 6.2 -> 4.3 GB per launch, layer time -1 % under the
-            // power cap and -3 % outside it; waiting for all: 4.0 GB but +1 %).
-            // The wait is a hint, not a dependency: it gives up after lock_polls polls (about half an item) and this CTA
-            // then free-runs for the rest of the launch, so a grid that is not fully resident (another stream's
-            // kernels on the same SMs) loses the traffic saving, never its progress.
-            const int kloc = iti - item_lo;
-            if (!PERSIST && lock_live && kloc > 0 && kloc <= a.lock_items) {
-              const volatile unsigned int* cnt = a.flags + a.n_flags + (kloc - 1);
-              int polls = 0;
-              while (*cnt < (unsigned)a.lock_need) {
-                if (++polls > a.lock_polls) { lock_live = false; break; }
-                __nanosleep(256);
-              }
-            }
             for (int g = I.seg0 * seg_kb; g < I.seg1 * seg_kb; ++g) {
               // Y^2: A = (Yh, Ym), B = (Yh, Ym).  W pass 0: A = (Yh, Ym), B = (Zh, Zm).  W pass 1: A = (Zh, Zm), B = (Yh, Ym).
               const int p = (g >= KB) ? 1 : 0;
               const int kb = g - p * KB;
               const int ma = (wunit && p == 1) ? zpl : 0;
               const int mb = (MODE == 1 || (wunit && p == 0)) ? zpl : 0;
+              // Soft lockstep (launch-per-layer mode, large N): CTAs that run concurrently stream the same row / column
+              // panels, and a panel byte is fetched from DRAM once only while they stay within an L2's worth of
+              // k-blocks of one another.  Every kLockEvery k-blocks of its leading whole units a producer arrives on a
+              // checkpoint counter and starts the next chunk only when lock_need of the grid's producers have arrived
+              // there too (7/8 of them: one slow CTA does not stall the rest; the 3-stage ring hides short waits).
+              // The wait is a hint, not a dependency: it gives up after lock_polls polls and this CTA then free-runs
+              // for the rest of the launch, so a grid that is not fully resident (another stream's kernels on the same
+              // SMs) loses the traffic saving, not its progress.
+              if (!PERSIST && lock_live && cum < a.lock_kb && cum > 0 && (cum & (kLockEvery - 1)) == 0) {
+                const volatile unsigned int* cnt = a.flags + a.n_flags + (cum / kLockEvery - 1);
+                int polls = 0;
+                while (*cnt < (unsigned)a.lock_need) {
+                  if (++polls > a.lock_polls) { lock_live = false; break; }
+                  __nanosleep(256);
+                }
+              }
               mbar_wait(smem_u32(&bars->empty[stage]), phase ^ 1u);
               const uint32_t dst = smem_u32(smem + stage * kStageBytes);
               if (CG == 1 || leader) mbar_expect_tx(smem_u32(&bars->full[stage]), (uint32_t)(CG * kStageBytes));
@@ -565,8 +564,11 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
               tma_load_2d<CG>(dst + 2 * kPlaneTileBytes, &a.tm[mb + 0], full_bar[stage], kb * kBK, row_b);
               tma_load_2d<CG>(dst + 3 * kPlaneTileBytes, &a.tm[mb + 1], full_bar[stage], kb * kBK, row_b);
               if (++stage == kStages) { stage = 0; phase ^= 1u; }
+              if (!PERSIST && cum < a.lock_kb) {
+                ++cum;
+                if ((cum & (kLockEvery - 1)) == 0) atomicAdd(a.flags + a.n_flags + (cum / kLockEvery - 1), 1u);
+              }
             }
-            if (!PERSIST && kloc < a.lock_items) atomicAdd(a.flags + a.n_flags + kloc, 1u);   // this item's loads are issued
           }
           if (!PERSIST) break;
           // arrive half of the grid barrier: every CTA has stored its planes of the layer just loaded.  (When the
@@ -825,7 +827,7 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
     }
     __syncthreads();
     if (bars->is_last) {
-      for (int i = threadIdx.x; i < a.n_flags + a.lock_items; i += blockDim.x) a.flags[i] = 0u;
+      for (int i = threadIdx.x; i < a.n_flags + a.lock_kb / kLockEvery; i += blockDim.x) a.flags[i] = 0u;
       if (threadIdx.x == 0) a.ctrl->ticket = 0u;
     }
     return;
@@ -843,7 +845,7 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
     a.slots[(size_t)(cls == 0 ? a.with_response : cls - 1) * gridDim.x + blockIdx.x] = t;
   }
   layer_tail(a.ctrl, a.slots, gridDim.x, gridDim.x, a.with_response, gridDim.x, &bars->is_last, red, a.flags,
-             a.n_flags + a.lock_items);
+             a.n_flags + a.lock_kb / kLockEvery);
 }
 
 

@@ -15,6 +15,8 @@ struct Sp2Item {
   int slot, nparts, flag_id, pad;
 };
 
+constexpr int kLockEvery = 16;   // k-blocks between two checkpoints of the producers' lockstep
+
 // Arguments of one layer launch.  tm[] are TMA descriptors of the INPUT planes (Yh, Ym, then Zh, Zm of every
 // perturbation b at 2 + 2b): 2-D FP16 tensors npad x npad, box sp2_layer_box_k() (k) x 128 (rows), swizzle = box row bytes.
 #define SP2_LAYER_PLANES (2 + 2 * SP2_NB)
@@ -30,10 +32,11 @@ struct alignas(64) Sp2LayerArgs {
   float* scratch;        // split-k partial sums
   unsigned int* flags;   // one arrival counter per split unit (zero between launches)
   int n_flags;
-  int lock_items;        // > 0: soft lockstep of the TMA producers over the first lock_items + 1 items of every work list
-                         // (arrival counters flags[n_flags .. n_flags + lock_items), zeroed with the split-k flags)
+  // soft lockstep of the TMA producers over the leading whole units of every work list; checkpoint counters
+  // flags[n_flags .. n_flags + lock_kb / kLockEvery), zeroed with the split-k flags
+  int lock_kb;           // k-blocks of the lockstep region (a multiple of kLockEvery, the same for every CTA; 0 = off)
+  int lock_need;         // arrivals a producer waits for at a checkpoint (<= CTAs of the grid)
   int lock_polls;        // polls (256 ns apart) after which a producer gives the lockstep up for the rest of the launch
-  int lock_need;         // arrivals a producer waits for before it starts its next item (<= CTAs of the grid)
   int lo_bits;           // significant bits kept in the lo planes (11 = all)
   // plain-product mode (sp2_congruence): C = A B^T, A = tm[0..1], B = tm[2..3]
   int gemm_mode;         // 0: SP2 layer, 1: plain product
