@@ -398,6 +398,15 @@ def run_stub(args):
     return 0
 
 
+def apply_knobs(h, args):
+    """The library options the command line exposes (all default to the library's own defaults), for every workload."""
+    if args.lanczos > 0:
+        h.set_options(lanczos_steps=args.lanczos)
+    if args.max_ctas > 0 or args.persistent or args.seg_kb or args.cta_group or args.power or args.lockstep:
+        h.set_options(max_ctas=args.max_ctas, persistent=args.persistent, seg_kb=args.seg_kb, cta_group=args.cta_group,
+                      power_squarings=args.power, lockstep=args.lockstep)
+
+
 def timed_steps(torch, step, k, flush_buf, barrier):
     """Time exactly k steps with CUDA events on the launching stream.  Inputs larger than L2 (flush_buf None): one
     pair of events brackets the k steps.  Inputs that fit in L2: a buffer larger than L2 is overwritten between steps
@@ -448,11 +457,7 @@ def run_ours(args):
     D = torch.empty_like(H)
     D1 = torch.empty_like(H) if response else None
     h = sp2.Sp2Handle(n, response=response, host_staging=True, refinement=args.refine > 0)
-    if args.lanczos > 0:
-        h.set_options(lanczos_steps=args.lanczos)
-    if args.max_ctas > 0 or args.persistent or args.seg_kb or args.cta_group or args.power or args.lockstep:
-        h.set_options(max_ctas=args.max_ctas, persistent=args.persistent, seg_kb=args.seg_kb, cta_group=args.cta_group,
-                      power_squarings=args.power, lockstep=args.lockstep)
+    apply_knobs(h, args)
     if args.refine > 0:
         if response:
             raise SystemExit("--refine goes with a density workload")
@@ -619,10 +624,7 @@ def run_sequence(args):
     D = torch.empty_like(H0)
     D_first = torch.empty_like(H0)
     h = sp2.Sp2Handle(n, host_staging=True)
-    if args.lanczos > 0:
-        h.set_options(lanczos_steps=args.lanczos)
-    if args.power > 0:
-        h.set_options(power_squarings=args.power)
+    apply_knobs(h, args)
 
     def barrier():
         if world > 1:
@@ -779,8 +781,7 @@ def run_batch(args):
     D = torch.empty_like(H)
     D1s = [torch.empty_like(H) for _ in range(B)]
     h = sp2.Sp2Handle(n, batch=B)
-    if args.lanczos > 0:
-        h.set_options(lanczos_steps=args.lanczos)
+    apply_knobs(h, args)
     for _ in range(max(args.warmup, 3)):
         h.response_batch(H, H1s, n_occ, out=D, out1s=D1s)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
