@@ -65,10 +65,12 @@ typedef enum {
   SP2_ERR_DEGENERATE = 6,    /* eps_max == eps_min (H = c*I): no spectral width to rescale */
   SP2_WARN_NOT_CONVERGED = 7, /* max_layers reached, or the parameter-free stop fired away from N_occ (degenerate level at the
                                 Fermi energy); D (and D1) are still written */
-  SP2_ERR_BOUNDS = 8         /* an eigenvalue of X left [0,1]: the spectral bounds (user_bounds, or a Lanczos estimate in a
+  SP2_ERR_BOUNDS = 8,        /* an eigenvalue of X left [0,1]: the spectral bounds (user_bounds, or a Lanczos estimate in a
                                 sequence step) do not enclose the spectrum of H; detected on the device from
                                 tr X - tr X^2 < 0 far from convergence; D is not written.  The blocking calls re-run a
                                 solve whose LANCZOS bounds fail this check with Gershgorin discs (result.bounds_fallback) */
+  SP2_ERR_TOO_LARGE = 9      /* sp2_density_noalloc only: N exceeds sp2_noalloc_max_n() (the library's static scratch);
+                                nothing was launched -- use a handle with a workspace for larger problems */
 } sp2_status_t;
 
 typedef enum { SP2_F32 = 0, SP2_F64 = 1 } sp2_dtype_t;
@@ -218,6 +220,33 @@ SP2_API sp2_status_t sp2_congruence(sp2_handle_t handle, const void* dZ, const v
                                     int transpose_first, void* dC, sp2_dtype_t out_dtype, long ldc, void* stream);
 
 /* Diagnostics. */
+/* ---- no-allocation entry point ------------------------------------------------------------------------------------
+ * sp2_density_noalloc: the density matrix of a SMALL problem (2 <= N <= sp2_noalloc_max_n() = 128, 0 < N_occ < N) without
+ * a handle, a workspace or any allocation: for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  Same operation as sp2_density with default options (Gershgorin
+ * rescale, SP2 layers with the trace rule and the parameter-free stop): ONE launch of the one-CTA
+ * kernel that keeps the iterate in shared memory.  The global scratch that kernel needs (final hi/lo planes of both
+ * ping-pong buffers, control block, result entry: sp2_noalloc_scratch_bytes() = 134 912 bytes, 132 KB) is a file-scope
+ * `static __device__` array inside the library, which every GPU that loads the library holds until the process exits.
+ *   dH, dD      device pointers, row-major, pitches ldh / ldd >= N in elements, dtypes as given; owned by the caller
+ *   d_result    optional DEVICE pointer: the kernel writes the result struct there (else into the static scratch)
+ *   out         optional HOST pointer: if non-NULL the call copies the result struct back and synchronises `stream`
+ *               before it returns (return value = out->status); if NULL the call only enqueues (returns SP2_OK when
+ *               the launch was accepted; the solve's status is in *d_result once the stream reaches that point)
+ *   stream      cudaStream_t, NULL = default stream; the device is the calling thread's current device
+ * Errors: SP2_ERR_TOO_LARGE for N > sp2_noalloc_max_n() (nothing launched), SP2_ERR_INVALID_ARG (null pointer, N < 2,
+ * N_occ outside (0, N), pitch < N, bad dtype, tol < 0), SP2_ERR_ARCH off sm_100, SP2_ERR_CUDA, and the solve's own
+ * statuses.  Calls no cudaMalloc / cudaFree / allocating library routine.  The first call on each device does a
+ * one-time set-up (cudaFuncSetAttribute, cudaGetSymbolAddress): make it outside stream capture.
+ * EVERY call on a device shares the one scratch array, which keeps the last call's contents (the kernel overwrites all
+ * of it and needs none of it zeroed): calls that overlap on the GPU (two streams, two host threads) RACE on the
+ * control block and the result entry -- serialise them on one stream, or use handles. */
+SP2_API sp2_status_t sp2_density_noalloc(const void* dH, sp2_dtype_t in_dtype, long ldh, int N, int N_occ, double tol,
+                                         void* dD, sp2_dtype_t out_dtype, long ldd, sp2_result_t* d_result,
+                                         sp2_result_t* out, void* stream);
+SP2_API int sp2_noalloc_max_n(void);             /* 128 */
+SP2_API size_t sp2_noalloc_scratch_bytes(void);  /* bytes of static device memory per GPU */
+
 SP2_API const char* sp2_status_string(sp2_status_t status);
 SP2_API int sp2_last_cuda_error(sp2_handle_t handle);            /* cudaError_t of the last failing CUDA call, 0 if none */
 SP2_API unsigned long long sp2_launch_count(sp2_handle_t handle); /* kernels launched through this handle so far */

@@ -1127,6 +1127,7 @@ const char* sp2_status_string(sp2_status_t s) {
     case SP2_ERR_DEGENERATE: return "degenerate spectral bounds (eps_max == eps_min)";
     case SP2_WARN_NOT_CONVERGED: return "not converged within max_layers";
     case SP2_ERR_BOUNDS: return "spectral bounds do not enclose the spectrum";
+    case SP2_ERR_TOO_LARGE: return "N exceeds the static scratch of the no-allocation entry point (sp2_noalloc_max_n)";
   }
   return "unknown status";
 }

@@ -26,6 +26,8 @@
 // Both leave the final planes and the control block in the workspace, where the debug hooks and the float64
 // refinement expect them.
 #include <cuda.h>
+#include <cstring>
+#include <mutex>
 #include "sp2_internal.cuh"
 #include "sp2_layer.h"
 #include "sp2_ptx.cuh"
@@ -552,4 +554,112 @@ cudaError_t sp2_launch_small_solve(const Sp2LayerArgs& args0, int npad_g, const 
   else if (p.out_f64) k_small_solve<float, double><<<1, kThreadsS, smem, s>>>(args0, npad_g, p);
   else k_small_solve<float, float><<<1, kThreadsS, smem, s>>>(args0, npad_g, p);
   return cudaGetLastError();
+}
+
+// ================================================================================================
+// sp2_density_noalloc (include/sp2.h): the one-CTA solve for callers that may not allocate.
+//
+// k_small_solve keeps the iterate in shared memory, but it still has global scratch: the final hi/lo planes of both
+// ping-pong buffers (small_store_state: what the handle's debug hooks and the refinement read), the control block
+// and the result entry.  A handle carves those out of the caller's workspace; here they live in ONE file-scope device
+// array that every GPU which loads the library holds until the process exits.  The kernel is the same k_small_solve
+// (density only), the library options are the defaults, and the matrices are the caller's.
+//
+// In host code `g_noalloc_scratch` is a host-side stand-in for the symbol, NOT a device address: the address the kernel
+// gets comes from cudaGetSymbolAddress, asked once per device with that device current.
+namespace {
+
+constexpr int kNoAllocMaxN = kNs;                                                  // 128
+constexpr size_t kNoAllocPlaneBytes = (size_t)kNs * kNs * sizeof(__half);          // one global plane, pitch kNs
+constexpr size_t kNoAllocCtrlOff = 4 * kNoAllocPlaneBytes;                         // Yh, Ym of buffers 0 and 1
+constexpr size_t kNoAllocResultOff = kNoAllocCtrlOff + ((sizeof(Sp2Ctrl) + 255) / 256) * 256;
+constexpr size_t kNoAllocBytes = kNoAllocResultOff + 256;
+
+constexpr int kNoAllocMaxDevices = 64;
+struct NoAllocDevice {
+  int state;               // 0: not set up, 1: ready, < 0: -(sp2_status_t) of the failed set-up
+  int cuda_error;
+  unsigned char* scratch;  // DEVICE address of g_noalloc_scratch on this device
+};
+NoAllocDevice g_noalloc_dev[kNoAllocMaxDevices];
+std::mutex g_noalloc_mutex;
+
+}  // namespace
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+static_assert(kNoAllocBytes <= 160 * 1024, "sp2_density_noalloc: the static scratch is documented as <= 160 KB per GPU");
+static_assert(sizeof(sp2_result_t) <= 256, "result entry");
+
+namespace {
+
+// once per device, with that device current: architecture check, shared-memory opt-in of the kernel, symbol address
+sp2_status_t noalloc_setup(int dev, NoAllocDevice** out) {
+  if (dev < 0 || dev >= kNoAllocMaxDevices) return SP2_ERR_INVALID_ARG;
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  NoAllocDevice& d = g_noalloc_dev[dev];
+  if (d.state == 0) {
+    int major = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) { d.state = -(int)SP2_ERR_CUDA; d.cuda_error = (int)e; }
+    else if (major != 10) { d.state = -(int)SP2_ERR_ARCH; }
+    else {
+      e = sp2_small_configure();
+      void* ptr = nullptr;
+      if (e == cudaSuccess) e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+      if (e != cudaSuccess || !ptr) { d.state = -(int)SP2_ERR_CUDA; d.cuda_error = (int)e; (void)cudaGetLastError(); }
+      else { d.scratch = static_cast<unsigned char*>(ptr); d.state = 1; }
+    }
+  }
+  if (d.state < 0) return (sp2_status_t)(-d.state);
+  *out = &d;
+  return SP2_OK;
+}
+
+}  // namespace
+
+extern "C" size_t sp2_noalloc_scratch_bytes(void) { return kNoAllocBytes; }
+extern "C" int sp2_noalloc_max_n(void) { return kNoAllocMaxN; }
+
+extern "C" sp2_status_t sp2_density_noalloc(const void* dH, sp2_dtype_t in_dtype, long ldh, int N, int N_occ, double tol,
+                                            void* dD, sp2_dtype_t out_dtype, long ldd, sp2_result_t* d_result,
+                                            sp2_result_t* out, void* stream) {
+  if (N > kNoAllocMaxN) return SP2_ERR_TOO_LARGE;                    // beyond the static scratch: use a handle
+  if (!dH || !dD || N < 2 || N_occ < 1 || N_occ >= N || ldh < N || ldd < N) return SP2_ERR_INVALID_ARG;
+  if ((in_dtype != SP2_F32 && in_dtype != SP2_F64) || (out_dtype != SP2_F32 && out_dtype != SP2_F64)) return SP2_ERR_INVALID_ARG;
+  if (!(tol >= 0.0)) return SP2_ERR_INVALID_ARG;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return SP2_ERR_CUDA;
+  NoAllocDevice* d = nullptr;
+  sp2_status_t st = noalloc_setup(dev, &d);
+  if (st != SP2_OK) return st;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+
+  // the argument block of layer parity 0, as a handle's prepare() fills it for a density-only problem of pitch kNs;
+  // k_small_solve reads in[] / out[] (state write-back), ctrl, with_response and lo_bits only (no TMA descriptors)
+  Sp2LayerArgs a;
+  memset(&a, 0, sizeof(a));
+  __half* planes = reinterpret_cast<__half*>(d->scratch);
+  const size_t pe = kNoAllocPlaneBytes / sizeof(__half);
+  a.in[0] = planes;           a.in[1] = planes + pe;                 // buffer 0: Yh, Ym
+  a.out[0] = planes + 2 * pe; a.out[1] = planes + 3 * pe;            // buffer 1
+  a.ctrl = reinterpret_cast<Sp2Ctrl*>(d->scratch + kNoAllocCtrlOff);
+  a.lo_bits = 11;
+  a.n = N; a.npad = kNs; a.with_response = 0;
+  sp2_result_t* entry = d_result ? d_result : reinterpret_cast<sp2_result_t*>(d->scratch + kNoAllocResultOff);
+
+  Sp2SmallProblem p;
+  memset(&p, 0, sizeof(p));
+  p.H = dH; p.D = dD; p.ldh = ldh; p.ldd = ldd;
+  p.N = N; p.n_occ = N_occ; p.max_layers = 100; p.user_bounds = 0; p.tol = tol;
+  p.in_f64 = in_dtype == SP2_F64; p.out_f64 = out_dtype == SP2_F64; p.ring_entry = entry;
+  // Nothing in the scratch has to start at zero: the kernel builds its control block and planes in shared memory and
+  // only WRITES the global copies, in full, at its end.  The array keeps the last call's contents in between.
+  cudaError_t e = sp2_launch_small_solve(a, kNs, p, s);
+  if (e != cudaSuccess) return SP2_ERR_CUDA;
+  if (!out) return SP2_OK;                                           // asynchronous: the status is in *d_result
+  e = cudaMemcpyAsync(out, entry, sizeof(sp2_result_t), cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) return SP2_ERR_CUDA;
+  out->kernel_launches = 1;
+  return (sp2_status_t)out->status;
 }

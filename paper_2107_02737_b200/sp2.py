@@ -28,6 +28,7 @@ SP2_ERR_NONFINITE = 5
 SP2_ERR_DEGENERATE = 6
 SP2_WARN_NOT_CONVERGED = 7
 SP2_ERR_BOUNDS = 8
+SP2_ERR_TOO_LARGE = 9
 
 SP2_F32, SP2_F64 = 0, 1
 SP2_WITH_RESPONSE, SP2_WITH_HOST_STAGING, SP2_WITH_REFINEMENT = 1, 2, 4
@@ -44,6 +45,7 @@ EXPORTS = [
     "sp2_density", "sp2_response", "sp2_response_batch", "sp2_density_host", "sp2_response_host",
     "sp2_sequence_begin", "sp2_sequence_step", "sp2_sequence_end", "sp2_congruence",
     "sp2_status_string", "sp2_last_cuda_error", "sp2_launch_count",
+    "sp2_density_noalloc", "sp2_noalloc_max_n", "sp2_noalloc_scratch_bytes",
     "sp2_debug_history", "sp2_debug_plane", "sp2_debug_schedule", "sp2_debug_layout",
 ]
 
@@ -119,6 +121,12 @@ def _load():
     lib.sp2_sequence_end.argtypes = [vp, C.POINTER(Sp2Result), C.POINTER(i)]
     lib.sp2_congruence.restype = i
     lib.sp2_congruence.argtypes = [vp, vp, vp, i, l, i, i, vp, i, l, vp]
+    lib.sp2_density_noalloc.restype = i
+    lib.sp2_density_noalloc.argtypes = [vp, i, l, i, i, d, vp, i, l, vp, C.POINTER(Sp2Result), vp]
+    lib.sp2_noalloc_max_n.restype = i
+    lib.sp2_noalloc_max_n.argtypes = []
+    lib.sp2_noalloc_scratch_bytes.restype = sz
+    lib.sp2_noalloc_scratch_bytes.argtypes = []
     lib.sp2_status_string.restype = C.c_char_p
     lib.sp2_status_string.argtypes = [i]
     lib.sp2_last_cuda_error.restype = i
@@ -158,6 +166,38 @@ def status_string(status: int) -> str:
 
 def workspace_bytes(n_max: int, flags: int = 0) -> int:
     return int(lib.sp2_workspace_bytes(int(n_max), int(flags)))
+
+
+def noalloc_max_n() -> int:
+    return int(lib.sp2_noalloc_max_n())
+
+
+def noalloc_scratch_bytes() -> int:
+    return int(lib.sp2_noalloc_scratch_bytes())
+
+
+def density_noalloc(H, n_occ: int, out, tol: float = 0.0, d_result=None, blocking: bool = True):
+    """sp2_density_noalloc: H (CUDA tensor, N <= noalloc_max_n()) -> `out` (CUDA tensor the CALLER allocated) with no
+    handle and no workspace; scratch is the library's static device array.  Runs on H's device and torch's current
+    stream there.  blocking=False only enqueues (pass d_result, a CUDA uint8 tensor of >= 96 bytes, to get the status)."""
+    import torch
+
+    n = H.shape[0]
+    for t in (H, out):
+        if not t.is_cuda or t.dim() != 2 or t.shape[0] != n or t.shape[1] != n or t.stride(1) != 1:
+            raise ValueError("expected N x N CUDA tensors with unit column stride")
+    if out.device != H.device:
+        raise ValueError("H and out must be on the same device")
+    r = Sp2Result()
+    dres = C.c_void_p(d_result.data_ptr()) if d_result is not None else None
+    with torch.cuda.device(H.device):
+        stream = C.c_void_p(torch.cuda.current_stream(H.device).cuda_stream)
+        st = lib.sp2_density_noalloc(C.c_void_p(H.data_ptr()), _dtype_code(H), H.stride(0), n, int(n_occ), float(tol),
+                                     C.c_void_p(out.data_ptr()), _dtype_code(out), out.stride(0), dres,
+                                     C.byref(r) if blocking else None, stream)
+    if st not in (SP2_OK, SP2_WARN_NOT_CONVERGED):
+        raise Sp2Error(st, status_string(st))
+    return out, (r.as_dict() if blocking else None)
 
 
 def _dtype_code(t):
