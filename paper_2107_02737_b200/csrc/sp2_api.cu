@@ -45,8 +45,9 @@ void sp2_launch_close(Sp2Ctrl* c, cudaStream_t s);
 void sp2_launch_lanczos(Sp2Ctrl* c, const void* H, sp2_dtype_t dt, long ld, int N, int steps, double* vecs, cudaStream_t s);
 // sp2_refine.cu
 cudaError_t sp2_refine_configure();
+void sp2_refine_box(int* box_k, int* box_rows);
 int sp2_launch_refine(Sp2Ctrl* c, __half* const planes[4], int npad, int N, int n_layers, double* Xa, double* Xb,
-                      double* slots, const void* H, sp2_dtype_t in_dt, long ldh, void* D,
+                      const CUtensorMap* maps, double* slots, const void* H, sp2_dtype_t in_dt, long ldh, void* D,
                       sp2_dtype_t out_dt, long ldo, sp2_result_t* ring_entry, cudaStream_t s);
 
 namespace {
@@ -599,7 +600,20 @@ sp2_status_t enqueue_finalise(sp2_handle_t h, const void* H, sp2_dtype_t in_dt, 
   const int nref = h->opt.refine_layers;
   if (nref > 0) {   // float64 refinement layers on the converged iterate; overwrites D, tr D, tr(DH)
     __half* yp[4] = {h->plane(0, 0), h->plane(1, 0), h->plane(0, 1), h->plane(1, 1)};
-    const int k = sp2_launch_refine(h->ctrl(), yp, h->cur_npad, N, nref, h->refine_x(0), h->refine_x(1), h->refine_slots(),
+    CUtensorMap maps[2];                          // the two float64 iterates as TMA tensors (sp2_refine.cu)
+    for (int w = 0; w < 2; ++w) {
+      int bk = 0, br = 0;
+      sp2_refine_box(&bk, &br);
+      cuuint64_t gdim[2] = {(cuuint64_t)h->cur_npad, (cuuint64_t)h->cur_npad};
+      cuuint64_t gstride[1] = {(cuuint64_t)h->cur_npad * sizeof(double)};
+      cuuint32_t box[2] = {(cuuint32_t)bk, (cuuint32_t)br};
+      cuuint32_t estr[2] = {1, 1};
+      CUresult r = h->encode(&maps[w], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, h->refine_x(w), gdim, gstride, box, estr,
+                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      if (r != CUDA_SUCCESS) { h->last_cuda_error = 100000 + (int)r; return SP2_ERR_CUDA; }
+    }
+    const int k = sp2_launch_refine(h->ctrl(), yp, h->cur_npad, N, nref, h->refine_x(0), h->refine_x(1), maps, h->refine_slots(),
                                     H, in_dt, ldh, D, out_dt, ldd, h->ring() + ring_idx, s);
     *launches += k;
   }

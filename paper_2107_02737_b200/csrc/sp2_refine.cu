@@ -10,29 +10,23 @@
 // the diagonal are computed and mirrored, and B[k][j] = X[j][k] makes both operands row panels of X.
 //
 //   k_refine_expand    planes -> X (float64, npad x npad, zero padding), partial tr X and ||X||_F^2
-//   k_refine_layer     one layer: 128x128 tiles, 3-stage cp.async ring, DMMA, fused update + mirrored store +
-//                      partials; the last block reduces them and fixes the next branch
+//   k_refine_layer     one layer: persistent blocks, 128x128 tiles, producer warp + mbarrier ring, DMMA consumers, fused
+//                      update + mirrored store + partials; the last block reduces them and fixes the next branch
 //   k_refine_finalise  X -> D in the caller's dtype, tr(DH); result struct
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cuda_fp16.h>
 #include <stdint.h>
 #include "sp2_internal.cuh"
+#include "sp2_ptx.cuh"
 
 namespace {
 
 constexpr int kT = 128;          // tile edge
 constexpr int kK = 16;           // k doubles per stage
 constexpr int kLd = 20;          // padded row pitch of a stage tile in doubles (160 B: 16-B aligned, conflict-free LDS.64)
-constexpr int kRStages = 3;
+constexpr int kRStages = 5;
 constexpr int kTileDoubles = kT * kLd;
-
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-  const uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
@@ -40,7 +34,7 @@ __device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b)
                : "d"(a), "d"(b));
 }
 
-__device__ __forceinline__ double block_sum(double v, double* sh /* 8 */) {
+__device__ __forceinline__ double block_sum(double v, double* sh /* one per warp */) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -103,86 +97,142 @@ __global__ void __launch_bounds__(256) k_refine_reduce(Sp2Ctrl* c, const double*
 }
 
 // ------------------------------------------------------------------------------------------
-// One float64 layer.  Block = one upper-triangular 128x128 tile; 8 warps as 2 (rows) x 4 (cols), warp tile 64x32 =
-// 8 x 4 DMMA tiles of 8x8 (64 accumulator doubles per thread).
-__global__ void __launch_bounds__(256, 1) k_refine_layer(Sp2Ctrl* c, const double* __restrict__ Xin, double* __restrict__ Xout,
-                                                         int npad, double* __restrict__ slots, unsigned int* ticket) {
+// One float64 layer.  Persistent blocks (one per SM) walk the upper-triangular 128x128 tiles in supertiles of
+// kRGroup x kRGroup, so that the ~148 tiles in flight share ~2 x kRGroup row panels of X (8 MB each at N = 8192) and stream
+// them through L2 together.  Warp-specialised: warp 8 is the producer (one TMA box of 128 rows x kLd doubles per operand
+// and k-slice, completion on the stage's `full` mbarrier), warps 0-7 are the DMMA consumers, 2 (rows)
+// x 4 (cols), warp tile 64x32 = 8 x 4 DMMA tiles of 8x8 (64 accumulator doubles per thread); they hand a stage back by
+// arriving on its `empty` mbarrier.  No block-wide barrier and no per-thread copy instructions in the consumers: the
+// first version (every thread issued cp.async, __syncthreads per k-slice) kept the DMMA pipe only 80 % busy, 15 % of the
+// warp samples sat at the slice boundary (barrier, and the copies' address registers being recycled).  The ring runs
+// on across tile boundaries, so the next tile's operands arrive during this tile's epilogue.
+constexpr int kRConsumerWarps = 8;
+constexpr int kRThreads = (kRConsumerWarps + 1) * 32;
+constexpr int kRGroup = 12;
+
+// tile t of the grouped order -> (bi, bj), bi <= bj.  Supertiles (I <= J) row-major; inside, rows then columns.
+__device__ __forceinline__ void refine_tile(int t, int nb, int& bi, int& bj) {
+  const int ng = (nb + kRGroup - 1) / kRGroup;
+  for (int I = 0; I < ng; ++I) {
+    const int h = min(kRGroup, nb - I * kRGroup);
+    for (int J = I; J < ng; ++J) {
+      const int w = min(kRGroup, nb - J * kRGroup);
+      const int cnt = (I == J) ? h * (h + 1) / 2 : h * w;
+      if (t < cnt) {
+        int r = 0, cidx = t;
+        if (I == J) { while (cidx >= h - r) { cidx -= h - r; ++r; } cidx += r; }
+        else { r = t / w; cidx = t - r * w; }
+        bi = I * kRGroup + r; bj = J * kRGroup + cidx;
+        return;
+      }
+      t -= cnt;
+    }
+  }
+  bi = bj = 0;   // not reached for t < nb (nb + 1) / 2
+}
+
+__global__ void __launch_bounds__(kRThreads, 1) k_refine_layer(Sp2Ctrl* c, const __grid_constant__ CUtensorMap tm_in,
+                                                               const double* __restrict__ Xin, double* __restrict__ Xout,
+                                                               int npad, double* __restrict__ slots, unsigned int* ticket) {
   if (!refine_active(c)) return;
-  extern __shared__ double rsm[];
+  extern __shared__ __align__(1024) uint8_t rsm_raw[];
+  double* rsm = reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(rsm_raw) + 127) & ~(uintptr_t)127);   // TMA destinations
+  __shared__ uint64_t bar_full[kRStages], bar_empty[kRStages];
   const int nb = npad / kT;
-  int bi = 0, rem = blockIdx.x;
-  while (rem >= nb - bi) { rem -= nb - bi; ++bi; }
-  const int bj = bi + rem;
-  const int i0 = bi * kT, j0 = bj * kT;
+  const int n_tiles = nb * (nb + 1) / 2;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int wm = warp >> 2, wn = warp & 3;                 // 2 x 4 warps
-  const int g = lane >> 2, q = lane & 3;                   // DMMA fragment coordinates
+  const bool plus = c->ref_plus != 0;
+  const int KB = npad / kK;
+  double tr = 0.0, fro = 0.0;
 
   auto stage_a = [&](int s) { return rsm + (size_t)s * 2 * kTileDoubles; };
   auto stage_b = [&](int s) { return rsm + (size_t)s * 2 * kTileDoubles + kTileDoubles; };
-  auto load_stage = [&](int s, int kb) {
-    // 128 rows x 16 doubles per operand = 1024 chunks of 16 B; 4 + 4 per thread
-#pragma unroll
-    for (int t = 0; t < 4; ++t) {
-      const int ch = tid + t * 256;
-      const int r = ch >> 3, cc = (ch & 7) * 2;
-      cp_async16(stage_a(s) + r * kLd + cc, Xin + (size_t)(i0 + r) * npad + kb * kK + cc);
-      cp_async16(stage_b(s) + r * kLd + cc, Xin + (size_t)(j0 + r) * npad + kb * kK + cc);
+
+  if (tid == 0) {
+    for (int s = 0; s < kRStages; ++s) {
+      sp2ptx::mbar_init(sp2ptx::smem_u32(&bar_full[s]), 1);
+      sp2ptx::mbar_init(sp2ptx::smem_u32(&bar_empty[s]), kRConsumerWarps);
     }
-    cp_async_commit();
-  };
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
 
-  double acc[8][4][2];
-#pragma unroll
-  for (int a = 0; a < 8; ++a)
-#pragma unroll
-    for (int b = 0; b < 4; ++b) { acc[a][b][0] = 0.0; acc[a][b][1] = 0.0; }
-
-  const int KB = npad / kK;
-  load_stage(0, 0);
-  if (KB > 1) load_stage(1, 1); else cp_async_commit();
-  for (int kb = 0; kb < KB; ++kb) {
-    cp_async_wait<1>();
-    __syncthreads();
-    if (kb + 2 < KB) load_stage((kb + 2) % kRStages, kb + 2); else cp_async_commit();
-    const double* A = stage_a(kb % kRStages) + (wm * 64) * kLd;
-    const double* B = stage_b(kb % kRStages) + (wn * 32) * kLd;
-#pragma unroll
-    for (int k4 = 0; k4 < kK / 4; ++k4) {
-      double af[8], bf[4];
-#pragma unroll
-      for (int a = 0; a < 8; ++a) af[a] = A[(a * 8 + g) * kLd + k4 * 4 + q];
-#pragma unroll
-      for (int b = 0; b < 4; ++b) bf[b] = B[(b * 8 + g) * kLd + k4 * 4 + q];
+  if (warp == kRConsumerWarps) {
+    // ------------------------------------------------ producer (one lane): per k-slice one TMA box per operand,
+    // kLd (= kK + 4) doubles wide so that the rows land in shared memory with the padded pitch the fragment loads want
+    if (sp2ptx::elect_one()) {
+      int stage = 0; uint32_t phase = 0;
+      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+        int bi, bj;
+        refine_tile(t, nb, bi, bj);
+        for (int kb = 0; kb < KB; ++kb) {
+          sp2ptx::mbar_wait(sp2ptx::smem_u32(&bar_empty[stage]), phase ^ 1u);
+          const uint32_t full = sp2ptx::smem_u32(&bar_full[stage]);
+          sp2ptx::mbar_expect_tx(full, 2u * kTileDoubles * (uint32_t)sizeof(double));
+          sp2ptx::tma_load_2d<1>(sp2ptx::smem_u32(stage_a(stage)), &tm_in, full, kb * kK, bi * kT);
+          sp2ptx::tma_load_2d<1>(sp2ptx::smem_u32(stage_b(stage)), &tm_in, full, kb * kK, bj * kT);
+          if (++stage == kRStages) { stage = 0; phase ^= 1u; }
+        }
+      }
+    }
+  } else {
+    // ------------------------------------------------ DMMA consumers
+    const int wm = warp >> 2, wn = warp & 3;                 // 2 x 4 warps
+    const int g = lane >> 2, q = lane & 3;                   // DMMA fragment coordinates
+    int stage = 0; uint32_t phase = 0;
+    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+      int bi, bj;
+      refine_tile(t, nb, bi, bj);
+      const int i0 = bi * kT, j0 = bj * kT;
+      double acc[8][4][2];
 #pragma unroll
       for (int a = 0; a < 8; ++a)
 #pragma unroll
-        for (int b = 0; b < 4; ++b) dmma(acc[a][b][0], acc[a][b][1], af[a], bf[b]);
-    }
-  }
-  cp_async_wait<0>();
+        for (int b = 0; b < 4; ++b) { acc[a][b][0] = 0.0; acc[a][b][1] = 0.0; }
 
-  // epilogue: X' = X^2 or 2X - X^2; elements with gj >= gi only, mirrored; partials
-  const bool plus = c->ref_plus != 0;
-  double tr = 0.0, fro = 0.0;
+      for (int kb = 0; kb < KB; ++kb) {
+        sp2ptx::mbar_wait(sp2ptx::smem_u32(&bar_full[stage]), phase);
+        const double* A = stage_a(stage) + (wm * 64 + g) * kLd + q;
+        const double* B = stage_b(stage) + (wn * 32 + g) * kLd + q;
 #pragma unroll
-  for (int a = 0; a < 8; ++a) {
-    const int gi = i0 + wm * 64 + a * 8 + g;
+        for (int k4 = 0; k4 < kK / 4; ++k4) {
+          double af[8], bf[4];
 #pragma unroll
-    for (int b = 0; b < 4; ++b) {
+          for (int a = 0; a < 8; ++a) af[a] = A[a * 8 * kLd + k4 * 4];
 #pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        const int gj = j0 + wn * 32 + b * 8 + 2 * q + e;
-        if (gj < gi) continue;
-        double v = acc[a][b][e];
-        if (!plus) v = 2.0 * Xin[(size_t)gi * npad + gj] - v;
-        Xout[(size_t)gi * npad + gj] = v;
-        if (gj > gi) { Xout[(size_t)gj * npad + gi] = v; fro += 2.0 * v * v; }
-        else { tr += v; fro += v * v; }
+          for (int b = 0; b < 4; ++b) bf[b] = B[b * 8 * kLd + k4 * 4];
+#pragma unroll
+          for (int a = 0; a < 8; ++a)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) dmma(acc[a][b][0], acc[a][b][1], af[a], bf[b]);
+        }
+        __syncwarp();
+        if (lane == 0) sp2ptx::mbar_arrive(sp2ptx::smem_u32(&bar_empty[stage]));
+        if (++stage == kRStages) { stage = 0; phase ^= 1u; }
+      }
+
+      // epilogue: X' = X^2 or 2X - X^2; elements with gj >= gi only, mirrored; partials
+#pragma unroll
+      for (int a = 0; a < 8; ++a) {
+        const int gi = i0 + wm * 64 + a * 8 + g;
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const int gj = j0 + wn * 32 + b * 8 + 2 * q + e;
+            if (gj < gi) continue;
+            double v = acc[a][b][e];
+            if (!plus) v = 2.0 * Xin[(size_t)gi * npad + gj] - v;
+            Xout[(size_t)gi * npad + gj] = v;
+            if (gj > gi) { Xout[(size_t)gj * npad + gi] = v; fro += 2.0 * v * v; }
+            else { tr += v; fro += v * v; }
+          }
+        }
       }
     }
   }
-  __shared__ double sh[8];
+
+  __shared__ double sh[kRThreads / 32];
   __shared__ unsigned int is_last;
   tr = block_sum(tr, sh);
   fro = block_sum(fro, sh);
@@ -195,7 +245,7 @@ __global__ void __launch_bounds__(256, 1) k_refine_layer(Sp2Ctrl* c, const doubl
   if (!is_last) return;
   __threadfence();
   double a = 0.0, b = 0.0;
-  for (int i = tid; i < (int)gridDim.x; i += 256) { a += __ldcg(slots + 2 * i); b += __ldcg(slots + 2 * i + 1); }
+  for (int i = tid; i < (int)gridDim.x; i += kRThreads) { a += __ldcg(slots + 2 * i); b += __ldcg(slots + 2 * i + 1); }
   a = block_sum(a, sh);
   b = block_sum(b, sh);
   if (tid == 0) { *ticket = 0u; refine_decide(c, a, b); c->ref_done += 1; }
@@ -236,7 +286,16 @@ __global__ void __launch_bounds__(256) k_refine_result(Sp2Ctrl* c, const double*
 }  // namespace
 
 // ------------------------------------------------------------------------------------------
-size_t sp2_refine_smem_bytes() { return (size_t)kRStages * 2 * kTileDoubles * sizeof(double); }
+size_t sp2_refine_smem_bytes() { return (size_t)kRStages * 2 * kTileDoubles * sizeof(double) + 1024; }
+// TMA box of the float64 iterates: {k extent, rows} in doubles
+void sp2_refine_box(int* box_k, int* box_rows) { *box_k = kLd; *box_rows = kT; }
+
+static int refine_sm_count() {
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1)
+    sms = 148;
+  return sms;
+}
 
 cudaError_t sp2_refine_configure() {
   return cudaFuncSetAttribute(k_refine_layer, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp2_refine_smem_bytes());
@@ -244,16 +303,17 @@ cudaError_t sp2_refine_configure() {
 
 // enqueue expand + n_layers float64 layers + finalise; returns the number of kernels launched
 int sp2_launch_refine(Sp2Ctrl* c, __half* const planes[4] /* Yh0, Ym0, Yh1, Ym1 */, int npad, int N, int n_layers,
-                      double* Xa, double* Xb, double* slots, const void* H, sp2_dtype_t in_dt, long ldh,
+                      double* Xa, double* Xb, const CUtensorMap* maps /* of Xa, Xb: sp2_refine_box() */, double* slots, const void* H, sp2_dtype_t in_dt, long ldh,
                       void* D, sp2_dtype_t out_dt, long ldo, sp2_result_t* ring_entry, cudaStream_t s) {
   int launches = 0;
   k_refine_expand<<<npad, 256, 0, s>>>(c, planes[0], planes[1], planes[2], planes[3], npad, Xa, slots); ++launches;
   k_refine_reduce<<<1, 256, 0, s>>>(c, slots, npad); ++launches;
   const int nb = npad / kT;
-  const int grid = nb * (nb + 1) / 2;
+  const int n_tiles = nb * (nb + 1) / 2;
+  const int grid = n_tiles < refine_sm_count() ? n_tiles : refine_sm_count();   // persistent: one block per SM
   double* in = Xa; double* out = Xb;
   for (int r = 0; r < n_layers; ++r) {
-    k_refine_layer<<<grid, 256, sp2_refine_smem_bytes(), s>>>(c, in, out, npad, slots, &c->ref_ticket); ++launches;
+    k_refine_layer<<<grid, kRThreads, sp2_refine_smem_bytes(), s>>>(c, maps[r & 1], in, out, npad, slots, &c->ref_ticket); ++launches;
     double* t = in; in = out; out = t;
   }
 #define SP2_RFIN(TI, TO) k_refine_finalise<TI, TO><<<N, 256, 0, s>>>(c, in, npad, (const TI*)H, ldh, (TO*)D, ldo, slots)
