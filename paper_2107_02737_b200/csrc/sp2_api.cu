@@ -46,8 +46,11 @@ void sp2_launch_lanczos(Sp2Ctrl* c, const void* H, sp2_dtype_t dt, long ld, int 
 // sp2_refine.cu
 cudaError_t sp2_refine_configure();
 void sp2_refine_box(int* box_k, int* box_rows);
+int sp2_refine_max_blocks();
+size_t sp2_refine_parts_bytes(int blocks);
+int sp2_refine_grid(int npad, int max_blocks);
 int sp2_launch_refine(Sp2Ctrl* c, __half* const planes[4], int npad, int N, int n_layers, double* Xa, double* Xb,
-                      const CUtensorMap* maps, double* slots, const void* H, sp2_dtype_t in_dt, long ldh, void* D,
+                      const CUtensorMap* maps, double* slots, void* parts_region, int max_blocks, const void* H, sp2_dtype_t in_dt, long ldh, void* D,
                       sp2_dtype_t out_dt, long ldo, sp2_result_t* ring_entry, cudaStream_t s);
 
 namespace {
@@ -84,12 +87,12 @@ struct Layout {
   size_t off_items_pw, items_pw_cap, off_item_begin_pw;
   size_t off_ctrl, off_ring, off_args;
   size_t off_staging, staging_each;
-  size_t off_refine, refine_each, off_refine_slots, refine_slots_count;
+  size_t off_refine, refine_each, off_refine_slots, refine_slots_count, off_refine_parts;
   size_t off_lanczos;
   size_t total;
   std::vector<Region> regions;
   int r_plane0, r_slots, r_slots2, r_bslots, r_fslots, r_tiles, r_items, r_item_begin, r_items_pw, r_item_begin_pw, r_scratch, r_flags, r_ctrl, r_args, r_ring,
-      r_staging0, r_lanczos, r_refine0, r_refine_slots;
+      r_staging0, r_lanczos, r_refine0, r_refine_slots, r_refine_parts;
 };
 
 int add_region(Layout& L, const char* name, size_t off, size_t reserved) {
@@ -177,7 +180,7 @@ Layout make_layout(int n_max, int flags) {
     }
   }
   L.r_lanczos = carve("lanczos", 3 * (size_t)n_max * sizeof(double), &L.off_lanczos);
-  L.r_refine0 = -1; L.r_refine_slots = -1; L.refine_each = 0; L.off_refine = 0; L.off_refine_slots = 0;
+  L.r_refine0 = -1; L.r_refine_slots = -1; L.r_refine_parts = -1; L.off_refine_parts = 0; L.refine_each = 0; L.off_refine = 0; L.off_refine_slots = 0;
   L.refine_slots_count = 0;
   if (flags & SP2_WITH_REFINEMENT) {
     L.refine_each = align_up(npad * npad * sizeof(double), 1024);
@@ -186,6 +189,7 @@ Layout make_layout(int n_max, int flags) {
     add_region(L, "refine1", off, L.refine_each); off += L.refine_each;
     L.refine_slots_count = refine_slot_doubles(npad);
     L.r_refine_slots = carve("refine_slots", L.refine_slots_count * sizeof(double), &L.off_refine_slots);
+    L.r_refine_parts = carve("refine_parts", sp2_refine_parts_bytes(sp2_refine_max_blocks()), &L.off_refine_parts);
   }
   L.total = off;
   return L;
@@ -256,6 +260,7 @@ struct sp2_handle_s {
   double* lanczos_vecs() const { return reinterpret_cast<double*>(ws + L.off_lanczos); }
   double* refine_x(int i) const { return reinterpret_cast<double*>(ws + L.off_refine + (size_t)i * L.refine_each); }
   double* refine_slots() const { return reinterpret_cast<double*>(ws + L.off_refine_slots); }
+  void* refine_parts() const { return ws + L.off_refine_parts; }
   // bookkeeping for sp2_debug_layout: this call may write [off, off + bytes) of region `id`
   void touch(int id, size_t bytes) {
     if (id >= 0 && id < (int)L.regions.size() && bytes > L.regions[id].used) L.regions[id].used = bytes;
@@ -614,6 +619,7 @@ sp2_status_t enqueue_finalise(sp2_handle_t h, const void* H, sp2_dtype_t in_dt, 
       if (r != CUDA_SUCCESS) { h->last_cuda_error = 100000 + (int)r; return SP2_ERR_CUDA; }
     }
     const int k = sp2_launch_refine(h->ctrl(), yp, h->cur_npad, N, nref, h->refine_x(0), h->refine_x(1), maps, h->refine_slots(),
+                                    h->refine_parts(), h->opt.max_ctas,
                                     H, in_dt, ldh, D, out_dt, ldd, h->ring() + ring_idx, s);
     *launches += k;
   }
@@ -671,6 +677,7 @@ sp2_status_t enqueue_solve(sp2_handle_t h, const void* H, const Pert& P, sp2_dty
         h->touch(h->L.r_refine0, (size_t)npad * npad * sizeof(double));
         h->touch(h->L.r_refine0 + 1, (size_t)npad * npad * sizeof(double));
         h->touch(h->L.r_refine_slots, refine_slot_doubles((size_t)npad) * sizeof(double));
+        h->touch(h->L.r_refine_parts, sp2_refine_parts_bytes(sp2_refine_grid(npad, o.max_ctas)));
       }
     }
   }

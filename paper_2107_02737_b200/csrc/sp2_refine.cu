@@ -86,7 +86,9 @@ __global__ void __launch_bounds__(256) k_refine_expand(Sp2Ctrl* c, const __half*
 }
 
 // reduce `count` (tr, fro) slot pairs in index order, one block
-__global__ void __launch_bounds__(256) k_refine_reduce(Sp2Ctrl* c, const double* slots, int count) {
+__global__ void __launch_bounds__(256) k_refine_reduce(Sp2Ctrl* c, const double* slots, int count, unsigned int* part_flags,
+                                                       int n_flags) {
+  for (int i = threadIdx.x; i < n_flags; i += 256) part_flags[i] = 0u;   // the workspace starts with arbitrary contents
   if (!refine_active(c)) return;
   __shared__ double sh[8];
   double a = 0.0, b = 0.0;
@@ -109,6 +111,7 @@ __global__ void __launch_bounds__(256) k_refine_reduce(Sp2Ctrl* c, const double*
 constexpr int kRConsumerWarps = 8;
 constexpr int kRThreads = (kRConsumerWarps + 1) * 32;
 constexpr int kRGroup = 12;
+constexpr int kRMaxBlocks = 256;  // >= SM count of any sm_100 part (flags fit the 1 KB header of the parts region)
 
 // tile t of the grouped order -> (bi, bj), bi <= bj.  Supertiles (I <= J) row-major; inside, rows then columns.
 __device__ __forceinline__ void refine_tile(int t, int nb, int& bi, int& bj) {
@@ -133,7 +136,8 @@ __device__ __forceinline__ void refine_tile(int t, int nb, int& bi, int& bj) {
 
 __global__ void __launch_bounds__(kRThreads, 1) k_refine_layer(Sp2Ctrl* c, const __grid_constant__ CUtensorMap tm_in,
                                                                const double* __restrict__ Xin, double* __restrict__ Xout,
-                                                               int npad, double* __restrict__ slots, unsigned int* ticket) {
+                                                               int npad, double* __restrict__ slots, unsigned int* ticket,
+                                                               double* __restrict__ parts, unsigned int* __restrict__ part_flags) {
   if (!refine_active(c)) return;
   extern __shared__ __align__(1024) uint8_t rsm_raw[];
   double* rsm = reinterpret_cast<double*>((reinterpret_cast<uintptr_t>(rsm_raw) + 127) & ~(uintptr_t)127);   // TMA destinations
@@ -144,6 +148,28 @@ __global__ void __launch_bounds__(kRThreads, 1) k_refine_layer(Sp2Ctrl* c, const
   const bool plus = c->ref_plus != 0;
   const int KB = npad / kK;
   double tr = 0.0, fro = 0.0;
+  // Work split (deterministic): whole tiles round-robin while there are gridDim.x of them left (tile r * grid + b in round
+  // r: the blocks of a round share panels and stream them at the same k, which keeps them coincident in L2), then the
+  // k-slices of the remaining rem < gridDim.x tiles are cut into gridDim.x equal contiguous ranges, so every block gets
+  // the same amount of work whatever the tile count (2080 tiles on 148 SMs otherwise run as 15 rounds of 14.05; the 36
+  // tiles of N = 1024 would use 36 SMs).  In that last phase a block whose range starts inside a tile computes that part
+  // first and leaves its accumulators in parts[blockIdx.x] (flag set with release); the block whose range starts the
+  // tile computes its own part, adds the other blocks' parts in block order and runs the epilogue.
+  const int G = (int)gridDim.x;
+  const int R = n_tiles / G, rem = n_tiles - R * G;
+  const long long rtotal = (long long)rem * KB;
+  const long long r_begin = rtotal * blockIdx.x / G, r_end = rtotal * (blockIdx.x + 1) / G;
+  // item `it` of this block -> (tile, k-slice range); returns false when the block is done.  rs: cursor of the last phase
+  auto next_item = [&](int it, long long& rs, int& t, int& kb_lo, int& kb_hi) -> bool {
+    if (it < R) { t = it * G + (int)blockIdx.x; kb_lo = 0; kb_hi = KB; return true; }
+    if (rs >= r_end) return false;
+    const int tr = (int)(rs / KB);
+    kb_lo = (int)(rs - (long long)tr * KB);
+    kb_hi = (int)((r_end - (long long)tr * KB) < KB ? (r_end - (long long)tr * KB) : KB);
+    t = R * G + tr;
+    rs = (long long)tr * KB + kb_hi;
+    return true;
+  };
 
   auto stage_a = [&](int s) { return rsm + (size_t)s * 2 * kTileDoubles; };
   auto stage_b = [&](int s) { return rsm + (size_t)s * 2 * kTileDoubles + kTileDoubles; };
@@ -162,10 +188,12 @@ __global__ void __launch_bounds__(kRThreads, 1) k_refine_layer(Sp2Ctrl* c, const
     // kLd (= kK + 4) doubles wide so that the rows land in shared memory with the padded pitch the fragment loads want
     if (sp2ptx::elect_one()) {
       int stage = 0; uint32_t phase = 0;
-      for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+      long long rs = r_begin;
+      int t, kb_lo, kb_hi;
+      for (int it = 0; next_item(it, rs, t, kb_lo, kb_hi); ++it) {
         int bi, bj;
         refine_tile(t, nb, bi, bj);
-        for (int kb = 0; kb < KB; ++kb) {
+        for (int kb = kb_lo; kb < kb_hi; ++kb) {
           sp2ptx::mbar_wait(sp2ptx::smem_u32(&bar_empty[stage]), phase ^ 1u);
           const uint32_t full = sp2ptx::smem_u32(&bar_full[stage]);
           sp2ptx::mbar_expect_tx(full, 2u * kTileDoubles * (uint32_t)sizeof(double));
@@ -180,7 +208,9 @@ __global__ void __launch_bounds__(kRThreads, 1) k_refine_layer(Sp2Ctrl* c, const
     const int wm = warp >> 2, wn = warp & 3;                 // 2 x 4 warps
     const int g = lane >> 2, q = lane & 3;                   // DMMA fragment coordinates
     int stage = 0; uint32_t phase = 0;
-    for (int t = blockIdx.x; t < n_tiles; t += gridDim.x) {
+    long long rs = r_begin;
+    int t, kb_lo, kb_hi;
+    for (int it = 0; next_item(it, rs, t, kb_lo, kb_hi); ++it) {
       int bi, bj;
       refine_tile(t, nb, bi, bj);
       const int i0 = bi * kT, j0 = bj * kT;
@@ -190,7 +220,7 @@ __global__ void __launch_bounds__(kRThreads, 1) k_refine_layer(Sp2Ctrl* c, const
 #pragma unroll
         for (int b = 0; b < 4; ++b) { acc[a][b][0] = 0.0; acc[a][b][1] = 0.0; }
 
-      for (int kb = 0; kb < KB; ++kb) {
+      for (int kb = kb_lo; kb < kb_hi; ++kb) {
         sp2ptx::mbar_wait(sp2ptx::smem_u32(&bar_full[stage]), phase);
         const double* A = stage_a(stage) + (wm * 64 + g) * kLd + q;
         const double* B = stage_b(stage) + (wn * 32 + g) * kLd + q;
@@ -209,6 +239,44 @@ __global__ void __launch_bounds__(kRThreads, 1) k_refine_layer(Sp2Ctrl* c, const
         __syncwarp();
         if (lane == 0) sp2ptx::mbar_arrive(sp2ptx::smem_u32(&bar_empty[stage]));
         if (++stage == kRStages) { stage = 0; phase ^= 1u; }
+      }
+
+      if (kb_lo > 0) {
+        // a later part of a tile that another block started: park the accumulators (thread-private order, coalesced)
+        double* mine = parts + (size_t)blockIdx.x * (kT * kT) + tid;
+#pragma unroll
+        for (int a = 0; a < 8; ++a)
+#pragma unroll
+          for (int b = 0; b < 4; ++b) {
+            __stcg(mine + (size_t)((a * 4 + b) * 2 + 0) * (kRConsumerWarps * 32), acc[a][b][0]);
+            __stcg(mine + (size_t)((a * 4 + b) * 2 + 1) * (kRConsumerWarps * 32), acc[a][b][1]);
+          }
+        __threadfence();
+        asm volatile("bar.sync 1, %0;" ::"n"(kRConsumerWarps * 32) : "memory");
+        if (tid == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(part_flags + blockIdx.x), "r"(1u) : "memory");
+        continue;
+      }
+      if (kb_hi < KB) {
+        // this block started the tile: add the parts of the blocks that continue it, in block order
+        for (int j = blockIdx.x + 1; j < G && rtotal * j / G < (long long)(t - R * G + 1) * KB; ++j) {
+          if (tid == 0) {
+            unsigned int v = 0;
+            long long spins = 0;
+            do {
+              asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(part_flags + j) : "memory");
+              if (++spins > sp2ptx::kSpinLimit) __trap();
+            } while (v == 0u);
+          }
+          asm volatile("bar.sync 1, %0;" ::"n"(kRConsumerWarps * 32) : "memory");
+          const double* theirs = parts + (size_t)j * (kT * kT) + tid;
+#pragma unroll
+          for (int a = 0; a < 8; ++a)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+              acc[a][b][0] += __ldcg(theirs + (size_t)((a * 4 + b) * 2 + 0) * (kRConsumerWarps * 32));
+              acc[a][b][1] += __ldcg(theirs + (size_t)((a * 4 + b) * 2 + 1) * (kRConsumerWarps * 32));
+            }
+        }
       }
 
       // epilogue: X' = X^2 or 2X - X^2; elements with gj >= gi only, mirrored; partials
@@ -248,6 +316,7 @@ __global__ void __launch_bounds__(kRThreads, 1) k_refine_layer(Sp2Ctrl* c, const
   for (int i = tid; i < (int)gridDim.x; i += kRThreads) { a += __ldcg(slots + 2 * i); b += __ldcg(slots + 2 * i + 1); }
   a = block_sum(a, sh);
   b = block_sum(b, sh);
+  for (int i = tid; i < (int)gridDim.x; i += kRThreads) part_flags[i] = 0u;     // every part was consumed
   if (tid == 0) { *ticket = 0u; refine_decide(c, a, b); c->ref_done += 1; }
 }
 
@@ -302,18 +371,36 @@ cudaError_t sp2_refine_configure() {
 }
 
 // enqueue expand + n_layers float64 layers + finalise; returns the number of kernels launched
+// scratch of the split tiles: one flag and one 128x128 accumulator image per block
+int sp2_refine_max_blocks() { return kRMaxBlocks; }
+size_t sp2_refine_parts_bytes(int blocks) { return 1024 + (size_t)blocks * kT * kT * sizeof(double); }
+int sp2_refine_grid(int npad, int max_blocks) {
+  const int nb = npad / kT;
+  const long long total = (long long)(nb * (nb + 1) / 2) * (npad / kK);   // k-slices of a layer
+  int grid = refine_sm_count();
+  if (max_blocks > 0 && grid > max_blocks) grid = max_blocks;
+  if (grid > kRMaxBlocks) grid = kRMaxBlocks;
+  if ((long long)grid * 4 > total) grid = (int)(total / 4);           // at least four k-slices per block
+  return grid < 1 ? 1 : grid;
+}
+
+// enqueue expand + n_layers float64 layers + finalise; returns the number of kernels launched.  The blocks of a layer
+// hand partial tiles to one another (see k_refine_layer), so its grid (sp2_refine_grid) must be co-resident: one block per
+// SM, at most max_blocks of them (sp2_options_t.max_ctas).
 int sp2_launch_refine(Sp2Ctrl* c, __half* const planes[4] /* Yh0, Ym0, Yh1, Ym1 */, int npad, int N, int n_layers,
-                      double* Xa, double* Xb, const CUtensorMap* maps /* of Xa, Xb: sp2_refine_box() */, double* slots, const void* H, sp2_dtype_t in_dt, long ldh,
+                      double* Xa, double* Xb, const CUtensorMap* maps /* of Xa, Xb: sp2_refine_box() */, double* slots,
+                      void* parts_region, int max_blocks, const void* H, sp2_dtype_t in_dt, long ldh,
                       void* D, sp2_dtype_t out_dt, long ldo, sp2_result_t* ring_entry, cudaStream_t s) {
   int launches = 0;
+  unsigned int* part_flags = static_cast<unsigned int*>(parts_region);
+  double* parts = reinterpret_cast<double*>(static_cast<uint8_t*>(parts_region) + 1024);
+  const int grid = sp2_refine_grid(npad, max_blocks);
   k_refine_expand<<<npad, 256, 0, s>>>(c, planes[0], planes[1], planes[2], planes[3], npad, Xa, slots); ++launches;
-  k_refine_reduce<<<1, 256, 0, s>>>(c, slots, npad); ++launches;
-  const int nb = npad / kT;
-  const int n_tiles = nb * (nb + 1) / 2;
-  const int grid = n_tiles < refine_sm_count() ? n_tiles : refine_sm_count();   // persistent: one block per SM
+  k_refine_reduce<<<1, 256, 0, s>>>(c, slots, npad, part_flags, grid); ++launches;
   double* in = Xa; double* out = Xb;
   for (int r = 0; r < n_layers; ++r) {
-    k_refine_layer<<<grid, kRThreads, sp2_refine_smem_bytes(), s>>>(c, maps[r & 1], in, out, npad, slots, &c->ref_ticket); ++launches;
+    k_refine_layer<<<grid, kRThreads, sp2_refine_smem_bytes(), s>>>(c, maps[r & 1], in, out, npad, slots, &c->ref_ticket, parts,
+                                                                     part_flags); ++launches;
     double* t = in; in = out; out = t;
   }
 #define SP2_RFIN(TI, TO) k_refine_finalise<TI, TO><<<N, 256, 0, s>>>(c, in, npad, (const TI*)H, ldh, (TO*)D, ldo, slots)
