@@ -32,7 +32,8 @@
  *     (cudaOccupancyMaxActiveClusters) and fails with SP2_ERR_CUDA if the kernel does not fit at all; at run time that
  *     needs the SMs to be free, so run ONE solve per GPU at a time, or leave SMs to other work with
  *     sp2_options_t.max_ctas: two solves on different streams of the same GPU can starve each other's CTAs (a
- *     device-side watchdog then traps, SP2_ERR_CUDA, instead of hanging).
+ *     device-side watchdog then traps, SP2_ERR_CUDA, instead of hanging).  The float64 refinement layers follow the
+ *     same rule (one block per SM, at most max_ctas of them; their last tiles are split between blocks).
  *   - Every call returns an sp2_status_t; nothing throws, nothing prints.  The blocking calls
  *     enqueue all kernels on `stream`, synchronise that stream once, and fill *out (a HOST struct).
  *   - There is no CPU fallback: on a device that is not compute capability 10.x the calls return
