@@ -9,8 +9,10 @@ from paper_2107_02737_b200 import inputs
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("n, base", [(384, 2), (700, 3), (1300, 4)])
-def test_refinement_matches_oracle_layers(torch_cuda, sp2, n, base):
+# sizes: 6, 21 and 66 tiles (every tile split along k between the blocks), 171 tiles (one round of whole tiles on 148
+# SMs, then the remaining 23 split), and a reduced grid (max_ctas: other split points, same result)
+@pytest.mark.parametrize("n, base, max_ctas", [(384, 2, 0), (700, 3, 0), (700, 3, 40), (1300, 4, 0), (2304, 2, 0), (2304, 2, 100)])
+def test_refinement_matches_oracle_layers(torch_cuda, sp2, n, base, max_ctas):
     import oracle
 
     torch = torch_cuda
@@ -18,6 +20,7 @@ def test_refinement_matches_oracle_layers(torch_cuda, sp2, n, base):
     n_occ = p["n_occ"]
     H = torch.from_numpy(p["H"].astype(np.float64)).cuda()
     h = sp2.Sp2Handle(n, refinement=True)
+    h.set_options(max_ctas=max_ctas)
     D0, r0 = h.density(H, n_occ)                          # unrefined: exactly the iterate the refinement starts from
     h.set_options(refine_layers=2)
     D2, r2 = h.density(H, n_occ)
