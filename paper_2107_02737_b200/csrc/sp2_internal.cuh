@@ -160,20 +160,18 @@ __device__ inline void sp2_setup_input_layer(Sp2Ctrl* c, double lo, double hi, d
 
 // Stop test at the top of layer n ("until all eigenvalues ... sufficiently close to
 // 1 or 0"; "idempotency conditions ... estimated from traces of intermediate
-// matrices").  DESIGN.md reading R4.  Returns a stop_reason (0 = continue).
-__device__ inline int sp2_stop_rule(const Sp2Ctrl* c, int n, double tr_x) {
-  const double e_n = c->e[n];
-  const bool near_occ = fabs(tr_x - (double)c->n_occ) < 0.5;
-  if (c->forced_layers > 0) return n >= c->forced_layers ? 6 : 0;
-  if (c->tol > 0.0 && e_n >= 0.0 && e_n <= c->tol && near_occ) return 1;
+// matrices").  DESIGN.md reading R4.  Returns a stop_reason (0 = continue).  All inputs by value: the caller has read
+// them from the control block in one batch (see sp2_controller).
+__device__ __forceinline__ int sp2_stop_rule(int n, double tr_x, double e_n, double e_nm2, int s1, int s2, double n_occ,
+                                             int forced_layers, double tol, int max_layers) {
+  const bool near_occ = fabs(tr_x - n_occ) < 0.5;
+  if (forced_layers > 0) return n >= forced_layers ? 6 : 0;
+  if (tol > 0.0 && e_n >= 0.0 && e_n <= tol && near_occ) return 1;
   if (n >= 3) {
-    const int s1 = (int)((c->sign_mask[(n - 1) >> 6] >> ((n - 1) & 63)) & 1ull);
-    const int s2 = (int)((c->sign_mask[(n - 2) >> 6] >> ((n - 2) & 63)) & 1ull);
-    const double e2 = c->e[n - 2];
-    if (s1 != s2 && e2 < 1.0 && (e_n <= 0.0 || e_n > 4.5 * e2 * e2)) return 2;
+    if (s1 != s2 && e_nm2 < 1.0 && (e_n <= 0.0 || e_n > 4.5 * e_nm2 * e_nm2)) return 2;
   }
   if (e_n <= 0.0 && near_occ) return 3;
-  if (n >= c->max_layers) return 4;
+  if (n >= max_layers) return 4;
   return 0;
 }
 
@@ -184,28 +182,41 @@ __device__ inline int sp2_stop_rule(const Sp2Ctrl* c, int n, double tr_x) {
 //   tr X^2 = N c^2 + 2 c tr Y + ||Y||_F^2        (X symmetric => tr X^2 = ||X||_F^2)
 // so the branch of layer n is known before its GEMM runs (no host round trip, PAPER.md:186 does
 // this on the CPU).
+// Shape: every input is read from *c up front, the arithmetic runs in registers, the results are stored at the end.
+// The thread sits on the critical path of every layer of the one-launch kernels, and with loads and stores
+// interleaved (*c is reached through a generic pointer into shared or global memory) each access waited for the
+// one before it: 4.6 us per layer in the persistent kernel, most of it memory latency.
 __device__ inline void sp2_controller(Sp2Ctrl* c) {
   const int n = c->n;
+  const int nb = c->with_response;
   const double N = (double)c->N;
   const double cc = c->c;
-  bool finite = isfinite(c->fro_y) && isfinite(c->tr_y) && isfinite(c->max_y);
-  for (int b = 0; b < c->with_response; ++b) finite = finite && isfinite(c->fro_z[b]) && isfinite(c->max_z[b]);
-  if (c->pw_phase) {
+  const double fro_y = c->fro_y, tr_y = c->tr_y, max_y = c->max_y;
+  const int pw_phase = c->pw_phase;
+  const int forced_layers = c->forced_layers, no_recentre = c->no_recentre, max_layers = c->max_layers;
+  const unsigned long long forced_signs = c->forced_signs;
+  const double nocc = (double)c->n_occ;
+  const double tol = c->tol;
+  const int t = c->t;
+  const unsigned long long mask0 = c->sign_mask[0], mask1 = c->sign_mask[1];
+  const double e_nm2 = (n >= 2 && n - 2 < SP2_LAYER_CAP) ? c->e[n - 2] : 0.0;
+  bool finite = isfinite(fro_y) && isfinite(tr_y) && isfinite(max_y);
+  for (int b = 0; b < nb; ++b) finite = finite && isfinite(c->fro_z[b]) && isfinite(c->max_z[b]);
+  if (pw_phase) {
     // ---- power phase (no branches, no shift): Yhat' = gamma Yhat^2 with gamma = 2^-e the power of two that brings
     // ||Yhat||_F^2 into [1, 2), so that ||Yhat'||_F <= 2 and >= 1/sqrt(N): no power ever over- or underflows
-    if (!(isfinite(c->fro_y) && isfinite(c->max_y))) { c->done = 1; c->status = SP2_ERR_NONFINITE; return; }
-    if (n >= c->pw_total || !(c->fro_y > 0.0)) { c->done = 1; c->stop_reason = 8; return; }   // k_power_finish takes over
+    if (!(isfinite(fro_y) && isfinite(max_y))) { c->done = 1; c->status = SP2_ERR_NONFINITE; return; }
+    if (n >= c->pw_total || !(fro_y > 0.0)) { c->done = 1; c->stop_reason = 8; return; }   // k_power_finish takes over
     int e;
-    frexp(c->fro_y, &e);                            // fro_y = m 2^e, m in [0.5, 1)
+    frexp(fro_y, &e);                               // fro_y = m 2^e, m in [0.5, 1)
     e -= 1;                                         // fro_y in [2^e, 2^(e+1))
     c->pw_log2scale = 2.0 * c->pw_log2scale + (double)e;
     const double gamma = sp2_exp2i(-e);
-    const int t = c->t;
-    const int t_next = sp2_pick_exponent(fmin(gamma * c->fro_y, 2.0));     // max|Yhat'| <= ||Yhat'||_F <= gamma ||Yhat||_F^2 < 2
+    const int t_next = sp2_pick_exponent(fmin(gamma * fro_y, 2.0));     // max|Yhat'| <= ||Yhat'||_F <= gamma ||Yhat||_F^2 < 2
     c->coef.a1y_hi = 0.f; c->coef.a1y_lo = 0.f;
     c->coef.a2y = (float)(gamma * sp2_exp2i(t_next - 2 * t));
     c->coef.dsh_hi = 0.f; c->coef.dsh_lo = 0.f;
-    c->t_in = t; c->sigma_last = 0.0; c->fro_in = c->fro_y;
+    c->t_in = t; c->sigma_last = 0.0; c->fro_in = fro_y;
     c->t = t_next; c->c = 0.0; c->n = n + 1;
     return;
   }
@@ -213,34 +224,34 @@ __device__ inline void sp2_controller(Sp2Ctrl* c) {
     c->done = 1; c->status = SP2_ERR_NONFINITE; c->stop_reason = 0;
     return;
   }
-  const double tr_x = N * cc + c->tr_y;
-  const double tr_x2 = N * cc * cc + 2.0 * cc * c->tr_y + c->fro_y;
-  c->tr_x[n] = tr_x;
-  c->e[n] = tr_x - tr_x2;
+  const double tr_x = N * cc + tr_y;
+  const double tr_x2 = N * cc * cc + 2.0 * cc * tr_y + fro_y;
+  const double e_n = tr_x - tr_x2;
+  if (n < SP2_LAYER_CAP) { c->tr_x[n] = tr_x; c->e[n] = e_n; }
   // Guard on the spectral bounds: spec(X) inside [0, 1] gives tr X^2 <= tr X and 0 <= tr X <= N.  An eigenvalue outside
   // [0, 1] (bounds that miss part of the spectrum: user_bounds, or the Lanczos estimate) is driven away from the
   // interval by one of the two branches, doubly exponentially, so e_n turns negative far beyond rounding (which
   // is ~1e-7 N at convergence) within a few layers.  Every assumption downstream (plane exponents, convergence)
   // rests on [0, 1], so the solve stops here.
   const double guard = 1e-2 + 1e-5 * N;
-  if (c->forced_layers <= 0 && (c->e[n] < -guard || tr_x < -guard || tr_x > N + guard)) {
+  if (forced_layers <= 0 && (e_n < -guard || tr_x < -guard || tr_x > N + guard)) {
     c->done = 1; c->status = SP2_ERR_BOUNDS; c->stop_reason = 0;
     return;
   }
-  const int stop = sp2_stop_rule(c, n, tr_x);
+  const int s1 = n >= 1 ? (int)((((n - 1) >> 6) ? mask1 : mask0) >> ((n - 1) & 63) & 1ull) : 0;
+  const int s2 = n >= 2 ? (int)((((n - 2) >> 6) ? mask1 : mask0) >> ((n - 2) & 63) & 1ull) : 0;
+  const int stop = sp2_stop_rule(n, tr_x, e_n, e_nm2, s1, s2, nocc, forced_layers, tol, max_layers);
   if (stop) {
     c->done = 1; c->stop_reason = stop;
     // the parameter-free floor rule (2) fires when the idempotency error stops improving; if the occupation is not
     // N_occ by then (a degenerate level at the Fermi energy: fractional occupation), the result is not a converged
     // projector and is reported like the layer cap: D is written, status says so
-    const bool off_occ = stop == 2 && !(fabs(tr_x - (double)c->n_occ) < 0.5);
+    const bool off_occ = stop == 2 && !(fabs(tr_x - nocc) < 0.5);
     c->status = (stop == 4 || off_occ) ? SP2_WARN_NOT_CONVERGED : SP2_OK;
     return;
   }
-  const double nocc = (double)c->n_occ;
   bool plus = fabs(tr_x2 - nocc) < fabs(2.0 * tr_x - tr_x2 - nocc);   // ties -> '-' (reading R3)
-  if (c->forced_layers > 0) plus = (c->forced_signs >> n) & 1ull;
-  if (plus) c->sign_mask[n >> 6] |= (1ull << (n & 63));
+  if (forced_layers > 0) plus = (forced_signs >> n) & 1ull;
   const double alpha = plus ? 2.0 * cc : 2.0 - 2.0 * cc;    // X^2     = c^2 I + 2c Y + Y^2
   const double sigma = plus ? 1.0 : -1.0;                   // 2X - X^2 = (2c-c^2) I + (2-2c) Y - Y^2
   const double c_map = plus ? cc * cc : 2.0 * cc - cc * cc;
@@ -257,29 +268,40 @@ __device__ inline void sp2_controller(Sp2Ctrl* c) {
   const double f_occ = nocc / N;
   const double var_x = fmax(tr_x2 / N - (tr_x / N) * (tr_x / N), 0.0);
   const double c_mid = tr_next / N + sqrt(var_x) * (0.5 - f_occ) / sqrt(f_occ * (1.0 - f_occ));
-  const double c_next = (c->forced_layers > 0 && c->no_recentre) ? c_map : fmin(fmax(c_mid, 0.0), 1.0);
+  const double c_next = (forced_layers > 0 && no_recentre) ? c_map : fmin(fmax(c_mid, 0.0), 1.0);
   const double dshift = c_map - c_next;
   // bounds on max|Y'|, max|Z'|: |(Y^2)_ij| <= ||Y||_2^2 and
   // ||Y||_2 <= min(||Y||_F, s) with s = max(c, 1-c) because spec(X) is inside [0,1].
   const double s = fmax(cc, 1.0 - cc) * 1.001 + 1e-6;
-  const double y2 = fmin(c->fro_y, s * s);
-  const double by = fabs(alpha) * c->max_y + y2 + fabs(dshift);
+  const double y2 = fmin(fro_y, s * s);
+  const double by = fabs(alpha) * max_y + y2 + fabs(dshift);
   const int t_next = sp2_pick_exponent(by);
-  const int t = c->t;
-  sp2_split_f32(alpha * sp2_exp2i(t_next - t), c->coef.a1y_hi, c->coef.a1y_lo);
-  c->coef.a2y = (float)(sigma * sp2_exp2i(t_next - 2 * t));
-  sp2_split_f32(dshift * sp2_exp2i(t_next), c->coef.dsh_hi, c->coef.dsh_lo);
-  for (int b = 0; b < c->with_response; ++b) {   // every perturbation keeps its own exponent
-    const double bz = fabs(alpha) * c->max_z[b] + 2.0 * sqrt(y2) * sqrt(c->fro_z[b]);
-    const int u_next = sp2_pick_exponent(bz);
+  float a1y_hi, a1y_lo, dsh_hi, dsh_lo;
+  sp2_split_f32(alpha * sp2_exp2i(t_next - t), a1y_hi, a1y_lo);
+  const float a2y = (float)(sigma * sp2_exp2i(t_next - 2 * t));
+  sp2_split_f32(dshift * sp2_exp2i(t_next), dsh_hi, dsh_lo);
+  const double sq_y2 = sqrt(y2);
+  for (int b = 0; b < nb; ++b) {   // every perturbation keeps its own exponent
+    const double max_zb = c->max_z[b], fro_zb = c->fro_z[b];
     const int u = c->u[b];
-    sp2_split_f32(alpha * sp2_exp2i(u_next - u), c->coef.a1z_hi[b], c->coef.a1z_lo[b]);
+    const double bz = fabs(alpha) * max_zb + 2.0 * sq_y2 * sqrt(fro_zb);
+    const int u_next = sp2_pick_exponent(bz);
+    float hi, lo;
+    sp2_split_f32(alpha * sp2_exp2i(u_next - u), hi, lo);
+    c->coef.a1z_hi[b] = hi; c->coef.a1z_lo[b] = lo;
     c->coef.a2z[b] = (float)(sigma * sp2_exp2i(u_next - t - u));
-    c->u[b] = u_next; // exponents describe the iterate the layer WRITES; the layer itself only
-  }                   // needs coef, so they can be advanced here
+    c->u[b] = u_next; // exponents describe the iterate the layer WRITES; the layer itself only needs coef
+  }
+  // ---- results
+  if (plus) {
+    if (n >> 6) c->sign_mask[1] = mask1 | (1ull << (n & 63));
+    else c->sign_mask[0] = mask0 | (1ull << (n & 63));
+  }
+  c->coef.a1y_hi = a1y_hi; c->coef.a1y_lo = a1y_lo; c->coef.a2y = a2y;
+  c->coef.dsh_hi = dsh_hi; c->coef.dsh_lo = dsh_lo;
   c->t_in = t;
   c->sigma_last = sigma;
-  c->fro_in = c->fro_y;
+  c->fro_in = fro_y;
   c->t = t_next;
   c->c = c_next;
   c->n = n + 1;

@@ -58,7 +58,7 @@ struct alignas(8) SmemBarriers {
   // started; prod_final = it will start no more (the MMA issuer follows the producer)
   uint32_t stop, prod_layers, prod_final, pad0;
   double red[32];         // persistent mode: warp partials of the slot reduction
-  // persistent mode: the last CTA's working copy of the control block (head + the history entries it touches)
+  // persistent mode: this CTA's own copy of the control block (every CTA runs the controller, see persist_control)
   alignas(8) uint8_t ctrl_copy[sizeof(Sp2Ctrl)];
   // 32x32 diagonal blocks in flight, one per TMEM lane quarter (of the two warps of a quarter only one holds the
   // diagonal): packed hi | lo << 16 per element, rows padded to 33 words (conflict-free row and column reads)
@@ -89,6 +89,16 @@ __device__ __forceinline__ uint32_t u4_word(const uint4& v, int i) {
   return i == 0 ? v.x : (i == 1 ? v.y : (i == 2 ? v.z : v.w));
 }
 
+// The scalar part of a layer boundary in one thread: trace identity, rescaled sums, controller.  Not inlined: its
+// float64 code (a batch of loads, arithmetic in registers, a batch of stores) must not add to the register pressure
+// of the kernels around it.
+__device__ __noinline__ void layer_scalar_control(Sp2Ctrl* ctrl, double tr, double fro, double mx, double tracc) {
+  sp2_trace_identity(ctrl, tracc);
+  const double sy = sp2_exp2i(-ctrl->t);
+  ctrl->tr_y = tr * sy; ctrl->fro_y = fro * sy * sy; ctrl->max_y = mx * sy;
+  sp2_controller(ctrl);
+}
+
 // ----------------------------------------------------------------------------------------------
 // shared tail of both engines: last block reduces the slots (index order) and runs the controller
 // slot array: [z slots of perturbation 0 (n_z)] ... [z slots of perturbation nb - 1][y slots (n_y)]
@@ -116,11 +126,8 @@ __device__ inline void layer_tail(Sp2Ctrl* ctrl, const Sp2Slot* slots, int n_y, 
     }
   }
   if (threadIdx.x == 0) {
-    sp2_trace_identity(ctrl, tracc);
-    const double sy = sp2_exp2i(-ctrl->t);
-    ctrl->tr_y = tr * sy; ctrl->fro_y = fro * sy * sy; ctrl->max_y = mx * sy;
     ctrl->ticket = 0;
-    sp2_controller(ctrl);
+    layer_scalar_control(ctrl, tr, fro, mx, tracc);
   }
 }
 
@@ -382,55 +389,31 @@ __device__ __forceinline__ void reduce_slots_fast(const Sp2Slot* slots, int coun
   named_bar_sync(1, kConsumerWarps * 32);
 }
 
-// The release half of the grid barrier, run by the consumer warps of the CTA that drew the layer's last ticket: slot
-// reduction, controller, new epoch.  Not inlined: its double-precision scalar code must not add to the register
-// pressure of the layer loop (the cta_group::2 instantiation spilled 750 bytes per thread with it inline).
-__device__ __noinline__ void persist_tail(const Sp2LayerArgs& a, SmemBarriers* bars, unsigned int epoch, int nb, int nblk) {
-  constexpr int NT = kConsumerWarps * 32;
-        __threadfence();
-  // The control block and the slots were last written by OTHER CTAs of this kernel, and this SM may hold stale
-  // copies of those lines in L1 from an earlier layer: read them past L1 (ld.cg), run the controller on a
-  // copy (below the ring's first stage would be busy with the next layer's loads: the copy lives next to the
-  // barriers) and write the changed part back.  Only the head of the block and the history entries of this
-  // layer move.
-  Sp2Ctrl* gctrl = a.ctrl;
+// Persistent mode, after the grid barrier of a layer (every CTA has drawn its ticket): the controller, REPLICATED.
+// Every CTA reduces the per-CTA slots of the layer in the same fixed order and runs the same scalar controller on its own
+// shared-memory copy of the control block, so all of them hold the same coefficients, branch and stop decision without
+// a second, release half of the barrier (one CTA computing, writing back, fencing, releasing, everybody else polling and
+// re-reading: 5 us of the ~9 us that serial tail took per layer).  Block 0 alone writes the history entries to global
+// memory.  Not inlined: its double-precision scalar code must not add to the register pressure of the layer loop.
+__device__ __noinline__ void persist_control(const Sp2LayerArgs& a, SmemBarriers* bars, const Sp2Slot* slots, int nb, int nblk) {
   Sp2Ctrl* ctrl = reinterpret_cast<Sp2Ctrl*>(bars->ctrl_copy);
-  {
-    const uint32_t* src = reinterpret_cast<const uint32_t*>(gctrl);
-    uint32_t* dst = reinterpret_cast<uint32_t*>(ctrl);
-    for (int i = threadIdx.x; i < (int)(SP2_CTRL_HEAD_BYTES / 4); i += NT) dst[i] = __ldcg(src + i);
-  }
-  for (int i = threadIdx.x; i < a.n_flags; i += NT) a.flags[i] = 0u;   // every split unit was consumed
-  named_bar_sync(1, NT);
   double* redf = reinterpret_cast<double*>(bars->red);
   double tr, fro, mx, tracc, unused;
-  reduce_slots_fast(a.slots + (size_t)nb * nblk, nblk, redf, tr, fro, mx, tracc);
+  reduce_slots_fast(slots + (size_t)nb * nblk, nblk, redf, tr, fro, mx, tracc);
   for (int b = 0; b < nb; ++b) {
     double trz, froz, mxz;
-    reduce_slots_fast(a.slots + (size_t)b * nblk, nblk, redf, trz, froz, mxz, unused);
+    reduce_slots_fast(slots + (size_t)b * nblk, nblk, redf, trz, froz, mxz, unused);
     if (threadIdx.x == 0) {
       const double sz = sp2_exp2i(-ctrl->u[b]);
       ctrl->tr_z[b] = trz * sz; ctrl->fro_z[b] = froz * sz * sz; ctrl->max_z[b] = mxz * sz;
     }
   }
   if (threadIdx.x == 0) {
-    const int n = ctrl->n;                   // the controller reads e[n - 2] and writes tr_x[n], e[n]
-    if (n >= 2 && n < SP2_LAYER_CAP) ctrl->e[n - 2] = __ldcg(&gctrl->e[n - 2]);
-    sp2_trace_identity(ctrl, tracc);
-    const double sy = sp2_exp2i(-ctrl->t);
-    ctrl->tr_y = tr * sy; ctrl->fro_y = fro * sy * sy; ctrl->max_y = mx * sy;
-    sp2_controller(ctrl);
-    if (n < SP2_LAYER_CAP) { gctrl->tr_x[n] = ctrl->tr_x[n]; gctrl->e[n] = ctrl->e[n]; }
+    const int n = ctrl->n;                   // the controller reads e[n - 2] and writes tr_x[n], e[n] (local history)
+    layer_scalar_control(ctrl, tr, fro, mx, tracc);
+    if (blockIdx.x == 0 && n < SP2_LAYER_CAP) { a.ctrl->tr_x[n] = ctrl->tr_x[n]; a.ctrl->e[n] = ctrl->e[n]; }
   }
-  named_bar_sync(1, NT);
-  {
-    const uint32_t* src = reinterpret_cast<const uint32_t*>(ctrl);
-    uint32_t* dst = reinterpret_cast<uint32_t*>(gctrl);
-    for (int i = threadIdx.x; i < (int)(SP2_CTRL_HEAD_BYTES / 4); i += NT) dst[i] = src[i];   // (ticket, epoch: unchanged values)
-  }
-  __threadfence();
-  named_bar_sync(1, NT);
-  if (threadIdx.x == 0) st_release_u32(&gctrl->epoch, epoch);       // release half of the barrier
+  named_bar_sync(1, kConsumerWarps * 32);
 }
 
 // ----------------------------------------------------------------------------------------------
@@ -580,6 +563,7 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
             if (ld_acquire_u32(&a.ctrl->ticket) >= (epoch0 + layers_loaded) * gridDim.x) { more = true; break; }
             if (*reinterpret_cast<volatile const uint32_t*>(&bars->stop)) break;
             if (spins > kSpinLimit) __trap();
+            __nanosleep(200);       // this warp shares a scheduler with two consumer warps (epilogue, controller)
           }
           if (!more) { *reinterpret_cast<volatile uint32_t*>(&bars->prod_final) = 1u; break; }
           fence_proxy_async_global();
@@ -631,6 +615,7 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
             if (*reinterpret_cast<volatile const uint32_t*>(&bars->prod_layers) > layers_issued) { more = true; break; }
             if (*reinterpret_cast<volatile const uint32_t*>(&bars->prod_final)) break;
             if (spins > kSpinLimit) __trap();
+            __nanosleep(100);
           }
           if (!more) break;
         }
@@ -649,9 +634,16 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
     const uint32_t lo_round = drop > 0 ? (1u << (drop - 1)) * 0x00010001u : 0u;
     int as = 0; uint32_t aphase = 0;
     unsigned int epoch = epoch0;
+    if constexpr (PERSIST) {                      // this CTA's working copy of the control block (history included)
+      const uint32_t* src = reinterpret_cast<const uint32_t*>(a0.ctrl);
+      uint32_t* dst = reinterpret_cast<uint32_t*>(bars->ctrl_copy);
+      for (int i = threadIdx.x; i < (int)(sizeof(Sp2Ctrl) / 4); i += kConsumerWarps * 32) dst[i] = __ldcg(src + i);
+      named_bar_sync(1, kConsumerWarps * 32);
+    }
     for (;;) {
     const Sp2LayerArgs& a = args[par];
-    const volatile Sp2Coef* cz = &a.ctrl->coef;   // volatile: rewritten by another CTA between layers (persistent mode)
+    // persistent mode: the coefficients come from this CTA's copy, rewritten by its thread 0 between layers
+    const volatile Sp2Coef* cz = PERSIST ? &reinterpret_cast<const volatile Sp2Ctrl*>(bars->ctrl_copy)->coef : &a.ctrl->coef;
     const float cf_a1y_hi = cz->a1y_hi, cf_a1y_lo = cz->a1y_lo, cf_a2y = cz->a2y;
     const float cf_dsh_hi = cz->dsh_hi, cf_dsh_lo = cz->dsh_lo;
     for (int iti = item_lo; iti < item_hi; ++iti) {
@@ -704,14 +696,16 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
 #pragma unroll
         for (int c = 0; c < WCOLS; ++c) dst[c * 32] = sums[c];       // lanes contiguous: 128 B per store
         __syncwarp();
-        if (lane == 0) { __threadfence(); atomicAdd(a.flags + I.flag_id, 1u); }
+        // (split-k flags: two sets in persistent mode, used by alternate layers; block 0 re-arms the set just consumed)
+        if (lane == 0) { __threadfence(); atomicAdd(a.flags + (PERSIST ? (epoch & 1u) * (unsigned int)a.n_flags : 0u) + I.flag_id, 1u); }
         continue;
       }
       if (I.kind == 2) {
         if (lane == 0) {
           const unsigned int target = (unsigned int)(I.nparts * kConsumerWarps * CG);
           long long spins = 0;
-          while (*reinterpret_cast<volatile unsigned int*>(a.flags + I.flag_id) < target)
+          const volatile unsigned int* fl = a.flags + (PERSIST ? (epoch & 1u) * (unsigned int)a.n_flags : 0u) + I.flag_id;
+          while (*fl < target)
             if (++spins > kSpinLimit) __trap();
           __threadfence();
         }
@@ -760,7 +754,10 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
       fence_proxy_async_global();                  // this thread's plane stores -> visible to the next layer's TMA loads
       __threadfence();
       named_bar_sync(1, NT);
-      if ((int)threadIdx.x < 1 + nb) {             // one slot per CTA and class: [z_0 .. z_{nb-1}][y], gridDim.x each
+      // one slot per CTA and class: [z_0 .. z_{nb-1}][y], gridDim.x each; two sets, used by alternate layers (a fast
+      // CTA may write the next layer's slots while a slow one still reads this layer's)
+      Sp2Slot* const lslots = a.slots + (size_t)(epoch & 1u) * (size_t)(1 + nb) * nblk;
+      if ((int)threadIdx.x < 1 + nb) {
         const int cls = threadIdx.x;
         Sp2Slot t = bars->acc[0][cls];
         for (int w = 1; w < kConsumerWarps; ++w) {
@@ -768,28 +765,38 @@ __device__ __forceinline__ void layer_body(const Sp2LayerArgs* __restrict__ args
           t.tr += o.tr; t.fro += o.fro; t.tracc += o.tracc;
           t.mx = (o.mx > t.mx || o.mx != o.mx) ? o.mx : t.mx;
         }
-        a.slots[(size_t)(cls == 0 ? nb : cls - 1) * nblk + blockIdx.x] = t;
+        lslots[(size_t)(cls == 0 ? nb : cls - 1) * nblk + blockIdx.x] = t;
         Sp2Slot z; z.tr = 0.0; z.fro = 0.0; z.tracc = 0.0; z.mx = 0.f; z.pad = 0.f;
         for (int w = 0; w < kConsumerWarps; ++w) bars->acc[w][cls] = z;
         __threadfence();
       }
       named_bar_sync(1, NT);
       ++epoch;
-      if (threadIdx.x == 0) {                      // arrive: the ticket only grows, epoch * nblk tickets end layer `epoch`
-        const unsigned int old_t = atomicAdd(&a.ctrl->ticket, 1u);
-        bars->is_last = (old_t == epoch * (unsigned int)nblk - 1u) ? 1u : 0u;
-      }
-      named_bar_sync(1, NT);
-      if (bars->is_last) {
-        persist_tail(a, bars, epoch, nb, nblk);
-      } else if (threadIdx.x == 0) {
+      if (threadIdx.x == 0) {                      // the ticket only grows: epoch * nblk tickets end layer `epoch`
+        atomicAdd(&a.ctrl->ticket, 1u);
         long long spins = 0;
-        while ((int)(ld_acquire_u32(&a.ctrl->epoch) - epoch) < 0)
+        while ((int)(ld_acquire_u32(&a.ctrl->ticket) - epoch * (unsigned int)nblk) < 0)
           if (++spins > kSpinLimit) __trap();
+        __threadfence();
       }
       named_bar_sync(1, NT);
-      const int done = *reinterpret_cast<volatile const int*>(&a.ctrl->done);
+      if (blockIdx.x == 0) {                       // every split unit of the layer was consumed: re-arm its flag set
+        unsigned int* const used_flags = a.flags + ((epoch - 1u) & 1u) * (unsigned int)a.n_flags;
+        for (int i = threadIdx.x; i < a.n_flags; i += NT) used_flags[i] = 0u;
+        __threadfence();                           // ordered before this CTA's next ticket, which gates the set's next use
+      }
+      persist_control(a, bars, a.slots + (size_t)((epoch - 1u) & 1u) * (size_t)(1 + nb) * nblk, nb, nblk);
+      Sp2Ctrl* const lctrl = reinterpret_cast<Sp2Ctrl*>(bars->ctrl_copy);
+      const int done = *reinterpret_cast<volatile const int*>(&lctrl->done);
       if (done) {
+        if (blockIdx.x == 0) {                     // the final control block -> global memory (read by the finalise kernels)
+          if (threadIdx.x == 0) { lctrl->epoch = epoch; lctrl->ticket = epoch * (unsigned int)nblk; }
+          named_bar_sync(1, NT);
+          const uint32_t* src = reinterpret_cast<const uint32_t*>(lctrl);
+          uint32_t* dst = reinterpret_cast<uint32_t*>(a.ctrl);
+          for (int i = threadIdx.x; i < (int)(SP2_CTRL_HEAD_BYTES / 4); i += NT) dst[i] = src[i];
+          __threadfence();
+        }
         // the producer and the tensor core have started one more layer (see above): drain it, no epilogue
         if (threadIdx.x == 0) *reinterpret_cast<volatile uint32_t*>(&bars->stop) = 1u;
         for (int iti = item_lo; iti < item_hi; ++iti) {
@@ -949,7 +956,7 @@ int sp2_layer_slots(int npad, int grid_ctas, int with_response, int engine) {
     const int nb = npad / 16;
     return nb * (nb + 1) / 2 * (1 + with_response);
   }
-  return grid_ctas * (1 + with_response);
+  return 2 * grid_ctas * (1 + with_response);   // two sets: the persistent mode alternates them between layers
 }
 
 cudaError_t sp2_layer_configure() {
