@@ -416,8 +416,17 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   // (measured at 2/3 filling, the worst case: 3.8e-4 at N = 24000, 6.1e-4 at N = 32768 against the 1e-3 bar), so the
   // largest problems take shorter segments (1.5e-4 at N = 32768, at 15 % lower throughput) and problems up to
   // N = 8192 longer ones (8 k-blocks: 8e-5 at N = 8192, 2 % faster than 4)
-  if (seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32) seg = npad > 24576 ? 2 : (npad > 8192 ? 4 : 8);
+  const bool seg_auto = seg != 1 && seg != 2 && seg != 4 && seg != 8 && seg != 16 && seg != 32;
+  if (seg_auto) seg = npad > 24576 ? 2 : (npad > 8192 ? 4 : 8);
   while ((npad / 64) % seg) seg >>= 1;
+  // Up to N = 2048 (the latency-bound, one-launch regime) the work lists are built at the granularity of a whole k sweep
+  // and never cut a pass along k: the accumulation segments stay as above (they set the rounding error), but a unit
+  // cut into three or four parts that are handed over through scratch one after the other is what made sizes whose
+  // k-block count has no large power-of-two divisor slow (N = 1152: 9 segments of 2 k-blocks per sweep, 41 us per
+  // density layer; N = 1664: 13 of 2, 73 us; N = 1024: 24 us).  Now 28 and 35 us.
+  const bool small_regime = seg_auto && npad <= kPersistMaxNpad;
+  const int segs_pass = (npad / 64) / seg;                 // accumulation segments per k sweep
+  const int sched_segs = small_regime ? 1 : segs_pass;     // granularity of the work lists
   if (h->cur_n == N && h->cur_npad == npad && h->cur_cg == cg && h->cur_resp == resp && h->cur_seg == seg &&
       h->cur_lo == h->opt.lo_bits && h->cur_maxctas == h->opt.max_ctas && h->cur_pw == (h->opt.power_squarings > 0) &&
       h->cur_lock == h->opt.lockstep)
@@ -429,8 +438,10 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   const int nC = layer_clusters(h, cg);
   // (fewer units than CTA(-pair)s is fine: the schedule splits them along k, every SM gets work)
   int n_slots = 0;
-  build_schedule((int)h->tiles_host.size(), resp, (npad / 64) / seg, nC, h->items_host, h->item_begin_host,
+  build_schedule((int)h->tiles_host.size(), resp, sched_segs, nC, h->items_host, h->item_begin_host,
                  &h->n_flags, &n_slots);
+  if (sched_segs != segs_pass)
+    for (Sp2Item& it : h->items_host) { it.seg0 *= segs_pass; it.seg1 *= segs_pass; }
   h->n_clusters = nC;
   h->n_active = 1;
   for (int c = 0; c < nC; ++c) if (h->item_begin_host[c + 1] > h->item_begin_host[c]) h->n_active = c + 1;
@@ -453,8 +464,10 @@ sp2_status_t prepare(sp2_handle_t h, int N, int resp, cudaStream_t s) {
   h->n_flags_pw = h->n_flags; h->n_active_pw = h->n_active;
   if (pw_lists) {
     int n_slots_pw = 0;
-    build_schedule((int)h->tiles_host.size(), 0, (npad / 64) / seg, nC, h->items_pw_host, h->item_begin_pw_host,
+    build_schedule((int)h->tiles_host.size(), 0, sched_segs, nC, h->items_pw_host, h->item_begin_pw_host,
                    &h->n_flags_pw, &n_slots_pw);
+    if (sched_segs != segs_pass)
+      for (Sp2Item& it : h->items_pw_host) { it.seg0 *= segs_pass; it.seg1 *= segs_pass; }
     h->n_active_pw = 1;
     for (int c = 0; c < nC; ++c) if (h->item_begin_pw_host[c + 1] > h->item_begin_pw_host[c]) h->n_active_pw = c + 1;
     if (h->items_pw_host.size() > h->L.items_pw_cap || (size_t)n_slots_pw * sp2_layer_scratch_slot_bytes(cg) > h->L.scratch_bytes ||
